@@ -1,0 +1,164 @@
+/*
+ * sw.h -- C ABI of the B200 Swendsen-Wang library (libsw_b200.so).
+ *
+ * One thing is built here: the full Swendsen-Wang sweep on the 2D square-lattice Ising model with
+ * periodic boundaries (arxiv 2302.14720, Protzman & Giedt; "five steps ... of which
+ * three require computation"), as hand-written CUDA for sm_100a.  There is no CPU fallback: every
+ * entry point that needs the GPU fails with SW_ECUDA when no usable device is present.
+ *
+ * Conventions:
+ *   site i = y*L + x, 0 <= x,y < L; East(i) = y*L + (x+1) mod L; South(i) = ((y+1) mod L)*L + x;
+ *   N = L*L; spins are int8 +1 / -1; J = 1, k_B = 1;
+ *   bond probability  p = 1 - exp(-2/T)  -- the paper prints p = 1 - exp(-1/k_B T)
+ *   in its own units; with H = -sum s_i s_j and the critical point its figures show
+ *   near k_B T ~ 2.25 this is 1 - exp(-2J/T) with J = 1.  T_c = 2/ln(1+sqrt 2).
+ *
+ * One sweep with sweep index t (the k-th sweep since creation uses t = k, from 0):
+ *   1 bonds   (section 2.1)  w = Philox4x32-10(ctr = (i>>1, t_lo, t_hi, 1), key = seed);
+ *             bondE[i] = spins[i]==spins[East(i)]  && w[2*(i&1)]   < thr
+ *             bondS[i] = spins[i]==spins[South(i)] && w[2*(i&1)+1] < thr,  thr = floor(p * 2^32) (<= 2^32-1)
+ *   2 labels  (section 2.3)  label[i] = minimum site index of i's connected component
+ *             of the bond graph ("lowest value label", labels "incrementing from zero")
+ *   3 assign  (section 2.4)     spins[i] = bit(label[i]) ? +1 : -1, where
+ *             bit(r) = (Philox(ctr = (r>>7, t_lo, t_hi, 2), key = seed)[(r>>5)&3] >> (r&31)) & 1
+ *   observables (section 2.5)   E = -sum_i s_i (s_East(i) + s_South(i)), M = sum_i s_i.
+ * The random start is spins[i] = bit_INIT(i) ? +1 : -1 with tag 0 and t = 0.
+ *
+ * Memory: the handle owns its device buffers (or carves them from a caller-supplied workspace,
+ * sw_create_in).  Pointers returned by sw_spins / sw_labels / sw_bonds are DEVICE pointers,
+ * borrowed: valid until the next sw_sweep, sw_set_* or sw_destroy on that handle.  All `out`
+ * arguments are HOST memory owned by the caller unless stated.
+ *
+ * Streams: all work of a handle is issued on one CUDA stream (default: the legacy default stream;
+ * sw_set_stream installs another, e.g. torch.cuda.current_stream().cuda_stream).  sw_sweep is
+ * asynchronous; sw_observables / sw_series / sw_stage_ms / sw_get_spins synchronise that stream.
+ *
+ * Errors: no exceptions, no abort.  int functions return SW_OK (0) or a negative code; pointer
+ * functions return NULL; sw_last_error() gives the text for the calling thread.
+ */
+#ifndef SW_B200_H
+#define SW_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SW_OK       0
+#define SW_EINVAL  -1   /* L < 2, L > 32768, T <= 0 or not finite, n < 0, nb < 1, null pointer, bad size */
+#define SW_ENOMEM  -2   /* host or device allocation failed / workspace too small */
+#define SW_ECUDA   -3   /* CUDA error (sticky); text in sw_last_error() */
+#define SW_ESTATE  -4   /* labels / bonds asked for before the first sweep, etc. */
+
+#define SW_MAX_L   32768      /* int32 labels: N <= 2^30 */
+
+typedef struct sw_handle sw_handle;   /* opaque */
+
+/* Observables of one lattice.  E and M are of the CURRENT spins; n_clusters / largest_cluster are of
+ * the LAST sweep's bond graph (0 before any sweep); `sweep` = number of sweeps completed.
+ * e_per_site = energy / N, abs_m_per_site = |magnetisation| / N, in double. */
+typedef struct {
+    int64_t  energy;
+    int64_t  magnetisation;
+    int64_t  n_clusters;
+    int64_t  largest_cluster;
+    uint64_t sweep;
+    double   e_per_site;
+    double   abs_m_per_site;
+} sw_obs;
+
+/* ---- creation (Fig. 1: the first configuration assigns a random spin to each site) ---- */
+
+/* One L x L lattice at temperature T, random start from `seed` (Philox tag 0).  NULL on error. */
+sw_handle* sw_create(int32_t L, double T, uint64_t seed);
+
+/* nb independent L x L lattices (BASELINE config 5: temperature scan), lattice b at T[b] with seed[b];
+ * every stage is ONE launch for the whole batch.  T, seed: HOST arrays of nb entries. */
+sw_handle* sw_create_batch(int32_t L, int32_t nb, const double* T, const uint64_t* seed);
+
+/* Bytes of device workspace a handle for (L, nb) needs; 0 on invalid arguments. */
+uint64_t   sw_workspace_bytes(int32_t L, int32_t nb);
+
+/* As sw_create_batch, but every device buffer is carved from `workspace` (DEVICE pointer, 256-byte
+ * aligned, >= sw_workspace_bytes(L, nb) bytes, owned by the caller and kept alive until sw_destroy).
+ * This is how the Python binding lets PyTorch own the memory. */
+sw_handle* sw_create_in(void* workspace, uint64_t workspace_bytes,
+                        int32_t L, int32_t nb, const double* T, const uint64_t* seed);
+
+void       sw_destroy(sw_handle* h);                       /* NULL is a no-op */
+
+/* ---- the hot path ---- */
+
+/* n >= 0 full sweeps (bonds -> labels -> assignment -> observables) on the handle's stream;
+ * asynchronous.  PAPER.md:33 (the five-step iteration). */
+int        sw_sweep(sw_handle* h, int64_t n);
+
+/* DEVICE pointer to nb*N int32: flat minimum-index labels of the last sweep, each lattice indexed
+ * within itself.  Flattens lazily if the last sweep left a parent forest.  NULL + SW_ESTATE text
+ * before the first sweep.  PAPER.md:51. */
+const int32_t* sw_labels(sw_handle* h);
+
+/* Synchronises; fills out[0..nb-1] (HOST).  PAPER.md:63. */
+int        sw_observables(sw_handle* h, sw_obs* out);
+
+/* ---- extras the configurations and the parity tests need ---- */
+
+const int8_t* sw_spins(sw_handle* h);                      /* DEVICE ptr, nb*N int8 (+1/-1) */
+
+/* DEVICE pointers to the canonical bond bit-planes of the last sweep: bit (i&31) of uint32 word
+ * (i>>5), i the site index; lattice b starts at word b*words_per_lattice, words_per_lattice =
+ * ceil(N/32).  SW_ESTATE before the first sweep.  PAPER.md:39, Fig. 2. */
+int        sw_bonds(sw_handle* h, const uint32_t** bondE, const uint32_t** bondS);
+
+/* Replace the spins (cold start, injected states).  `spins`: nb*N int8 of +1/-1, on the device
+ * (is_host = 0) or on the host (is_host = 1).  Values are not validated. */
+int        sw_set_spins(sw_handle* h, const int8_t* spins, int is_host);
+int        sw_set_cold(sw_handle* h);                      /* all +1 (BASELINE config 3) */
+int        sw_get_spins(sw_handle* h, int8_t* out_host);   /* synchronising copy, nb*N bytes */
+int        sw_get_labels(sw_handle* h, int32_t* out_host); /* synchronising copy, nb*N int32 */
+
+/* Next sweep uses sweep index t (checkpoint / resume, one-step parity at large L). */
+int        sw_set_sweep_index(sw_handle* h, uint64_t t);
+uint64_t   sw_sweep_index(const sw_handle* h);
+
+int        sw_set_stream(sw_handle* h, void* cuda_stream); /* a cudaStream_t; NULL = default stream */
+
+/* Per-sweep history of the LAST sw_sweep call, oldest first: entry (k*nb + b) is lattice b after the
+ * k-th retained sweep.  At most `cap` entries are written; returns the number of sweeps retained
+ * (<= the series capacity, default 4096 sweeps, see sw_set_series_capacity) or a negative code. */
+int64_t    sw_series(sw_handle* h, sw_obs* out, int64_t cap);
+int        sw_set_series_capacity(sw_handle* h, int64_t sweeps);
+
+/* Per-stage device time in ms, summed over the sweeps of the last sw_sweep call that ran with stage
+ * timing on: out = {bond, label, flip, observe}.  Stage timing brackets each stage with CUDA events
+ * (it serialises nothing but adds event records; off by default).  BASELINE config 3. */
+int        sw_set_stage_timing(sw_handle* h, int on);
+int        sw_stage_ms(sw_handle* h, float out[4]);
+
+/* Select the kernel path: 0 = automatic (tiled path when L is a multiple of 64, generic otherwise),
+ * 1 = force the generic any-L path (global union-find, no tiles).  Results are identical. */
+int        sw_set_path(sw_handle* h, int path);
+
+/* Number of kernel launches issued by the last sw_sweep call (for bench.py's gpu_launches). */
+int64_t    sw_last_launch_count(const sw_handle* h);
+
+uint32_t   sw_threshold(const sw_handle* h, int32_t b);    /* integer bond threshold of lattice b */
+int32_t    sw_L(const sw_handle* h);
+int32_t    sw_batch(const sw_handle* h);
+
+/* Stand-alone pieces for tests (device work on the default stream, synchronising):
+ * Philox4x32-10 of n (ctr, key) pairs, HOST arrays ctr[4n], key[2n] -> out[4n], computed ON THE GPU
+ * by the same device function the kernels use. */
+int        sw_test_philox(const uint32_t* ctr, const uint32_t* key, uint32_t* out, int64_t n);
+/* Label injected bond planes: bondE/bondS HOST canonical bit-planes of one L x L lattice ->
+ * labels_out[N] (HOST), through the handle's labelling kernels (h must have the same L, nb = 1). */
+int        sw_test_label(sw_handle* h, const uint32_t* bondE, const uint32_t* bondS, int32_t* labels_out);
+
+const char* sw_last_error(void);                           /* thread-local text, never NULL */
+const char* sw_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SW_B200_H */

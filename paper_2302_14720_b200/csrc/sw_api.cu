@@ -1,0 +1,530 @@
+// sw_api.cu -- host logic and the extern "C" boundary of libsw_b200.so (see include/sw.h).
+// Product code (CUDA path).  No CPU fallback: every compute entry point needs a CUDA device.
+#include "../../include/sw.h"
+#include "sw_common.cuh"
+#include "sw_generic.cuh"
+#include "sw_tiled.cuh"
+
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+using namespace sw;
+
+namespace {
+
+thread_local std::string g_err = "";
+
+void set_err(const char* fmt, ...) __attribute__((format(printf, 1, 2)));
+void set_err(const char* fmt, ...) {
+    char buf[512];
+    va_list ap; va_start(ap, fmt); vsnprintf(buf, sizeof buf, fmt, ap); va_end(ap);
+    g_err = buf;
+}
+
+#define SW_CUDA(call)                                                                              \
+    do {                                                                                           \
+        cudaError_t e_ = (call);                                                                   \
+        if (e_ != cudaSuccess) {                                                                   \
+            set_err("CUDA error %s at %s:%d: %s", cudaGetErrorName(e_), __FILE__, __LINE__,        \
+                    cudaGetErrorString(e_));                                                       \
+            return SW_ECUDA;                                                                       \
+        }                                                                                          \
+    } while (0)
+
+constexpr size_t ALIGN = 256;
+constexpr int64_t DEFAULT_SERIES_CAP = 4096;
+constexpr int MAX_TIMED_SWEEPS = 4096;
+constexpr int EV_PER_SWEEP = 5;
+
+inline size_t align_up(size_t v) { return (v + ALIGN - 1) / ALIGN * ALIGN; }
+
+// tile shapes of the fast path
+enum TileKind { TILE_NONE = 0, TILE_64x64 = 1, TILE_256x32 = 2 };
+using Cfg64 = TileCfg<64, 64>;
+using Cfg256 = TileCfg<256, 32>;
+
+struct Layout {        // byte offsets into the workspace
+    size_t spins, bondE, bondS, D, label, gsize, olist, ocount, lat, ctl, rec_now, series, total;
+};
+
+size_t olist_entries(int L) {          // per lattice, maximum over the tile shapes usable for this L
+    size_t n = 0;
+    const size_t N = (size_t)L * L;
+    if (L % 64 == 0) n = std::max(n, N / Cfg64::SITES * Cfg64::CAP);
+    if (L % 256 == 0) n = std::max(n, N / Cfg256::SITES * Cfg256::CAP);
+    return n;
+}
+size_t tiles_max(int L) { return L % 64 == 0 ? (size_t)L * L / Cfg64::SITES : 0; }
+
+Layout make_layout(int L, int nb) {
+    const size_t N = (size_t)L * L, words = (N + 31) / 32;
+    Layout o; size_t p = 0;
+    o.spins = p;   p = align_up(p + (size_t)nb * N);
+    o.bondE = p;   p = align_up(p + (size_t)nb * words * 4);
+    o.bondS = p;   p = align_up(p + (size_t)nb * words * 4);
+    o.D = p;       p = align_up(p + (size_t)nb * ((words + 3) / 4 * 4) * 4);
+    o.label = p;   p = align_up(p + (size_t)nb * N * 4);
+    o.gsize = p;   p = align_up(p + (size_t)nb * N * 4);
+    o.olist = p;   p = align_up(p + (size_t)nb * olist_entries(L) * sizeof(int2));
+    o.ocount = p;  p = align_up(p + (size_t)nb * tiles_max(L) * 4);
+    o.lat = p;     p = align_up(p + (size_t)nb * sizeof(Lat));
+    o.ctl = p;     p = align_up(p + sizeof(Ctl));
+    o.rec_now = p; p = align_up(p + (size_t)nb * sizeof(Rec));
+    o.series = p;  p = align_up(p + (size_t)DEFAULT_SERIES_CAP * nb * sizeof(Rec));
+    o.total = p;
+    return o;
+}
+
+bool valid_dims(int32_t L, int32_t nb) {
+    return L >= 2 && L <= SW_MAX_L && nb >= 1 && nb <= 65535 && (uint64_t)L * L * (uint64_t)nb <= (1ull << 40);
+}
+
+uint32_t host_threshold(double T) {
+    // thr = min(floor(p 2^32), 2^32 - 1), p = 1 - exp(-2/T) via expm1
+    const double p = -std::expm1(-2.0 / T);
+    const double v = std::floor(p * 4294967296.0);
+    if (v >= 4294967295.0) return 0xFFFFFFFFu;
+    if (v <= 0.0) return 0u;
+    return (uint32_t)v;
+}
+
+} // namespace
+
+struct sw_handle {
+    int L = 0, nb = 0, N = 0, words = 0;
+    bool owns_ws = false;
+    char* ws = nullptr; size_t ws_bytes = 0;
+    int8_t* spins = nullptr; uint32_t *bondE = nullptr, *bondS = nullptr, *D = nullptr;
+    int *label = nullptr, *gsize = nullptr, *ocount = nullptr; int2* olist = nullptr;
+    Lat* lat = nullptr; Ctl* ctl = nullptr; Rec* rec_now = nullptr;
+    Rec* series = nullptr; Rec* series_owned = nullptr; int64_t series_cap = DEFAULT_SERIES_CAP;
+    std::vector<Lat> hlat;
+    uint64_t t = 0;
+    cudaStream_t stream = nullptr;
+    bool have_sweep = false;       // labels / bonds / cluster observables of a sweep exist
+    bool rec_valid = false;        // the last series slot holds E, M of the current spins
+    int64_t last_n = 0;
+    int path = 0; TileKind tile = TILE_NONE;
+    bool timing = false; std::vector<cudaEvent_t> ev; int64_t timed_sweeps = 0;
+    int64_t launches = 0;
+};
+
+namespace {
+
+TileKind pick_tile(int L, int path) {
+    if (path == 1) return TILE_NONE;
+    if (path == 2) return L % 64 == 0 ? TILE_64x64 : TILE_NONE;
+    if (path == 3) return L % 256 == 0 ? TILE_256x32 : TILE_NONE;
+    if (L % 256 == 0) return TILE_256x32;
+    if (L % 64 == 0) return TILE_64x64;
+    return TILE_NONE;
+}
+
+inline dim3 grid1(size_t n, int threads, int nb) { return dim3((unsigned)((n + threads - 1) / threads), (unsigned)nb); }
+
+template <int TW, int TH>
+size_t tile_smem_bytes() {
+    using C = TileCfg<TW, TH>;
+    return (size_t)C::SITES * 8 + (size_t)C::RW * 8 + C::WPR * 4 + TH + 16;
+}
+
+template <int TW, int TH>
+int launch_label_tiled(sw_handle* h) {
+    using C = TileCfg<TW, TH>;
+    const int tiles = h->N / C::SITES;
+    static bool attr_done = false;
+    const size_t smem = tile_smem_bytes<TW, TH>();
+    if (!attr_done) {
+        SW_CUDA(cudaFuncSetAttribute(k_tile_label<TW, TH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr_done = true;
+    }
+    k_tile_label<TW, TH><<<dim3(tiles, h->nb), C::THREADS, smem, h->stream>>>(
+        h->label, h->bondE, h->bondS, h->olist, h->ocount, h->series, h->ctl, h->L, h->N, h->words, h->nb);
+    const size_t nedge = (size_t)h->L * (h->L / TW + h->L / TH);
+    k_merge_tiled<TW, TH><<<grid1(nedge, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
+        h->label, h->bondE, h->bondS, h->L, h->N, h->words);
+    k_compress_tiled<<<grid1((size_t)h->N / 4, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
+        h->label, h->series, h->ctl, h->N, h->nb);
+    k_sizes_open<C::CAP><<<grid1((size_t)tiles * 32, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
+        h->label, h->olist, h->ocount, h->gsize, h->series, h->ctl, tiles, h->N, h->nb);
+    k_sizes_reset<C::CAP><<<grid1((size_t)tiles * 32, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
+        h->olist, h->ocount, h->gsize, tiles, h->N);
+    h->launches += 5;
+    return SW_OK;
+}
+
+int launch_label_generic(sw_handle* h) {
+    k_label_init<<<grid1(h->N, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(h->label, h->N);
+    k_union_generic<<<grid1(h->N, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(
+        h->label, h->bondE, h->bondS, h->L, h->N, h->words);
+    k_compress_generic<<<grid1(h->N, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(
+        h->label, h->gsize, h->series, h->ctl, h->N, h->nb);
+    k_maxsize_generic<<<grid1(h->N, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(
+        h->label, h->gsize, h->series, h->ctl, h->N, h->nb);
+    h->launches += 4;
+    return SW_OK;
+}
+
+int launch_label(sw_handle* h) {
+    switch (h->tile) {
+        case TILE_64x64:  return launch_label_tiled<64, 64>(h);
+        case TILE_256x32: return launch_label_tiled<256, 32>(h);
+        default:          return launch_label_generic(h);
+    }
+}
+
+int record(sw_handle* h, int64_t k, int which) {
+    if (!h->timing || k >= MAX_TIMED_SWEEPS) return SW_OK;
+    SW_CUDA(cudaEventRecord(h->ev[(size_t)k * EV_PER_SWEEP + which], h->stream));
+    return SW_OK;
+}
+
+// one full sweep on h->stream; the sweep index and series slot are read on the device from h->ctl
+int launch_sweep(sw_handle* h, int64_t k) {
+    int rc;
+    if ((rc = record(h, k, 0))) return rc;
+    // a1 bonds
+    if (h->tile != TILE_NONE)
+        k_bond_rows<<<grid1(h->words, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
+            h->spins, h->bondE, h->bondS, h->lat, h->ctl, h->L, h->N, h->words);
+    else
+        k_bond_generic<<<grid1(h->words, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(
+            h->spins, h->bondE, h->bondS, h->lat, h->ctl, h->L, h->N, h->words);
+    h->launches += 1;
+    if ((rc = record(h, k, 1))) return rc;
+    // a2-a4 labels (+ cluster count, largest cluster)
+    if ((rc = launch_label(h))) return rc;
+    if ((rc = record(h, k, 2))) return rc;
+    // a5-a6 assignment
+    k_flipbits<<<grid1(((size_t)h->words + 3) / 4, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(
+        h->D, h->lat, h->ctl, h->words);
+    if (h->tile != TILE_NONE)
+        k_flip_rows<<<grid1((size_t)h->N / 16, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
+            h->spins, h->label, h->D, h->series, h->ctl, h->N, h->words, h->nb);
+    else
+        k_flip_generic<<<grid1(h->N, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(
+            h->spins, h->label, h->D, h->N, h->words);
+    h->launches += 2;
+    if ((rc = record(h, k, 3))) return rc;
+    // a7 observables of the new configuration
+    if (h->tile != TILE_NONE)
+        k_energy_rows<<<grid1(h->words, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
+            h->spins, h->series, h->ctl, h->L, h->N, h->words, h->nb);
+    else
+        k_observe_generic<<<grid1(h->N, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(
+            h->spins, h->series, h->ctl, 1, h->L, h->N, h->nb);
+    k_advance<<<1, 64, 0, h->stream>>>(h->ctl, h->series, h->nb);
+    h->launches += 2;
+    if ((rc = record(h, k, 4))) return rc;
+    return SW_OK;
+}
+
+int init_handle(sw_handle* h, const double* T, const uint64_t* seed) {
+    const Layout o = make_layout(h->L, h->nb);
+    char* w = h->ws;
+    h->spins = (int8_t*)(w + o.spins);
+    h->bondE = (uint32_t*)(w + o.bondE); h->bondS = (uint32_t*)(w + o.bondS); h->D = (uint32_t*)(w + o.D);
+    h->label = (int*)(w + o.label); h->gsize = (int*)(w + o.gsize);
+    h->olist = (int2*)(w + o.olist); h->ocount = (int*)(w + o.ocount);
+    h->lat = (Lat*)(w + o.lat); h->ctl = (Ctl*)(w + o.ctl); h->rec_now = (Rec*)(w + o.rec_now);
+    h->series = (Rec*)(w + o.series);
+    h->hlat.resize(h->nb);
+    for (int b = 0; b < h->nb; ++b) {
+        h->hlat[b].key0 = (uint32_t)(seed[b] & 0xFFFFFFFFu);
+        h->hlat[b].key1 = (uint32_t)(seed[b] >> 32);
+        h->hlat[b].thr = host_threshold(T[b]);
+        h->hlat[b].pad = 0;
+    }
+    SW_CUDA(cudaMemcpyAsync(h->lat, h->hlat.data(), sizeof(Lat) * h->nb, cudaMemcpyHostToDevice, h->stream));
+    SW_CUDA(cudaMemsetAsync(h->gsize, 0, (size_t)h->nb * h->N * 4, h->stream));
+    SW_CUDA(cudaMemsetAsync(h->series, 0, (size_t)h->series_cap * h->nb * sizeof(Rec), h->stream));
+    k_set_ctl<<<1, 1, 0, h->stream>>>(h->ctl, 0ull, 0u, (uint32_t)h->series_cap);
+    k_init_random<<<grid1(h->words, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(h->spins, h->lat, h->N, h->words);
+    SW_CUDA(cudaGetLastError());
+    SW_CUDA(cudaStreamSynchronize(h->stream));       // hlat is read by the async copy
+    h->tile = pick_tile(h->L, h->path);
+    return SW_OK;
+}
+
+sw_handle* create_common(void* ws, uint64_t ws_bytes, int32_t L, int32_t nb, const double* T, const uint64_t* seed) {
+    if (!valid_dims(L, nb) || !T || !seed) { set_err("sw_create: invalid argument (L=%d, nb=%d)", L, nb); return nullptr; }
+    for (int b = 0; b < nb; ++b)
+        if (!(T[b] > 0.0) || !std::isfinite(T[b])) { set_err("sw_create: T[%d] = %g is not a positive finite number", b, T[b]); return nullptr; }
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess || ndev == 0) {
+        set_err("sw_create: no usable CUDA device (%s); this library has no CPU path", cudaGetErrorString(e));
+        (void)cudaGetLastError();
+        return nullptr;
+    }
+    sw_handle* h = new (std::nothrow) sw_handle();
+    if (!h) { set_err("sw_create: out of host memory"); return nullptr; }
+    h->L = L; h->nb = nb; h->N = L * L; h->words = (h->N + 31) / 32;
+    const size_t need = make_layout(L, nb).total;
+    if (ws) {
+        if (ws_bytes < need || ((uintptr_t)ws % ALIGN) != 0) {
+            set_err("sw_create_in: workspace of %llu bytes (need %llu, %zu-byte aligned)",
+                    (unsigned long long)ws_bytes, (unsigned long long)need, ALIGN);
+            delete h; return nullptr;
+        }
+        h->ws = (char*)ws; h->ws_bytes = ws_bytes; h->owns_ws = false;
+    } else {
+        void* p = nullptr;
+        e = cudaMalloc(&p, need);
+        if (e != cudaSuccess) { set_err("sw_create: cudaMalloc(%zu) failed: %s", need, cudaGetErrorString(e)); (void)cudaGetLastError(); delete h; return nullptr; }
+        h->ws = (char*)p; h->ws_bytes = need; h->owns_ws = true;
+    }
+    if (init_handle(h, T, seed) != SW_OK) { if (h->owns_ws) cudaFree(h->ws); delete h; return nullptr; }
+    return h;
+}
+
+void fill_obs(const sw_handle* h, const Rec& r, uint64_t sweep, sw_obs* o) {
+    o->energy = r.E; o->magnetisation = r.M; o->n_clusters = r.ncl; o->largest_cluster = r.maxcl;
+    o->sweep = sweep;
+    o->e_per_site = (double)r.E / (double)h->N;
+    o->abs_m_per_site = (double)(r.M < 0 ? -r.M : r.M) / (double)h->N;
+}
+
+} // namespace
+
+// =================================================================================================
+extern "C" {
+
+const char* sw_last_error(void) { return g_err.c_str(); }
+const char* sw_version(void) { return "sw-b200 0.1 (sm_100a)"; }
+
+uint64_t sw_workspace_bytes(int32_t L, int32_t nb) {
+    if (!valid_dims(L, nb)) return 0;
+    return make_layout(L, nb).total;
+}
+
+sw_handle* sw_create(int32_t L, double T, uint64_t seed) { return create_common(nullptr, 0, L, 1, &T, &seed); }
+sw_handle* sw_create_batch(int32_t L, int32_t nb, const double* T, const uint64_t* seed) {
+    return create_common(nullptr, 0, L, nb, T, seed);
+}
+sw_handle* sw_create_in(void* workspace, uint64_t workspace_bytes, int32_t L, int32_t nb,
+                        const double* T, const uint64_t* seed) {
+    if (!workspace) { set_err("sw_create_in: null workspace"); return nullptr; }
+    return create_common(workspace, workspace_bytes, L, nb, T, seed);
+}
+
+void sw_destroy(sw_handle* h) {
+    if (!h) return;
+    cudaStreamSynchronize(h->stream);
+    for (cudaEvent_t e : h->ev) cudaEventDestroy(e);
+    if (h->series_owned) cudaFree(h->series_owned);
+    if (h->owns_ws) cudaFree(h->ws);
+    (void)cudaGetLastError();
+    delete h;
+}
+
+int sw_sweep(sw_handle* h, int64_t n) {
+    if (!h || n < 0) { set_err("sw_sweep: invalid argument"); return SW_EINVAL; }
+    if (n == 0) return SW_OK;
+    h->launches = 0;
+    if (h->timing && h->ev.empty()) {
+        h->ev.resize((size_t)MAX_TIMED_SWEEPS * EV_PER_SWEEP);
+        for (auto& e : h->ev) SW_CUDA(cudaEventCreate(&e));
+    }
+    SW_CUDA(cudaMemsetAsync(h->series, 0, (size_t)h->nb * sizeof(Rec), h->stream));
+    k_set_ctl<<<1, 1, 0, h->stream>>>(h->ctl, (unsigned long long)h->t, 0u, (uint32_t)h->series_cap);
+    h->launches += 1;
+    for (int64_t k = 0; k < n; ++k) {
+        int rc = launch_sweep(h, k);
+        if (rc) return rc;
+    }
+    SW_CUDA(cudaGetLastError());
+    h->t += (uint64_t)n;
+    h->last_n = n;
+    h->timed_sweeps = h->timing ? std::min<int64_t>(n, MAX_TIMED_SWEEPS) : 0;
+    h->have_sweep = true; h->rec_valid = true;
+    return SW_OK;
+}
+
+const int32_t* sw_labels(sw_handle* h) {
+    if (!h) { set_err("sw_labels: null handle"); return nullptr; }
+    if (!h->have_sweep) { set_err("sw_labels: no sweep has run yet"); return nullptr; }
+    return h->label;            // every sweep leaves the labels flat
+}
+
+int sw_bonds(sw_handle* h, const uint32_t** bondE, const uint32_t** bondS) {
+    if (!h || !bondE || !bondS) { set_err("sw_bonds: null argument"); return SW_EINVAL; }
+    if (!h->have_sweep) { set_err("sw_bonds: no sweep has run yet"); return SW_ESTATE; }
+    *bondE = h->bondE; *bondS = h->bondS;
+    return SW_OK;
+}
+
+const int8_t* sw_spins(sw_handle* h) {
+    if (!h) { set_err("sw_spins: null handle"); return nullptr; }
+    return h->spins;
+}
+
+int sw_observables(sw_handle* h, sw_obs* out) {
+    if (!h || !out) { set_err("sw_observables: null argument"); return SW_EINVAL; }
+    std::vector<Rec> r(h->nb);
+    if (h->rec_valid) {
+        const int64_t slot = (h->last_n - 1) % h->series_cap;
+        SW_CUDA(cudaMemcpyAsync(r.data(), h->series + (size_t)slot * h->nb, sizeof(Rec) * h->nb,
+                                cudaMemcpyDeviceToHost, h->stream));
+    } else {
+        SW_CUDA(cudaMemsetAsync(h->rec_now, 0, sizeof(Rec) * h->nb, h->stream));
+        k_observe_generic<<<grid1(h->N, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(
+            h->spins, h->rec_now, h->ctl, 0, h->L, h->N, h->nb);
+        SW_CUDA(cudaGetLastError());
+        SW_CUDA(cudaMemcpyAsync(r.data(), h->rec_now, sizeof(Rec) * h->nb, cudaMemcpyDeviceToHost, h->stream));
+    }
+    SW_CUDA(cudaStreamSynchronize(h->stream));
+    for (int b = 0; b < h->nb; ++b) fill_obs(h, r[b], h->t, out + b);
+    return SW_OK;
+}
+
+int64_t sw_series(sw_handle* h, sw_obs* out, int64_t cap) {
+    if (!h || !out || cap < 0) { set_err("sw_series: invalid argument"); return SW_EINVAL; }
+    if (!h->rec_valid) return 0;
+    const int64_t kept = std::min(h->last_n, h->series_cap);
+    const int64_t give = std::min(kept, cap);
+    std::vector<Rec> r((size_t)h->series_cap * h->nb);
+    SW_CUDA(cudaMemcpyAsync(r.data(), h->series, r.size() * sizeof(Rec), cudaMemcpyDeviceToHost, h->stream));
+    SW_CUDA(cudaStreamSynchronize(h->stream));
+    const int64_t first = h->last_n - kept;          // index (within the call) of the oldest retained sweep
+    for (int64_t k = 0; k < give; ++k) {
+        const int64_t slot = (first + k) % h->series_cap;
+        for (int b = 0; b < h->nb; ++b)
+            fill_obs(h, r[(size_t)slot * h->nb + b], h->t - (uint64_t)h->last_n + (uint64_t)(first + k) + 1,
+                     out + (size_t)k * h->nb + b);
+    }
+    return kept;
+}
+
+int sw_set_series_capacity(sw_handle* h, int64_t sweeps) {
+    if (!h || sweeps < 1 || sweeps > (1ll << 26)) { set_err("sw_set_series_capacity: invalid argument"); return SW_EINVAL; }
+    SW_CUDA(cudaStreamSynchronize(h->stream));
+    Rec* p = nullptr;
+    cudaError_t e = cudaMalloc((void**)&p, (size_t)sweeps * h->nb * sizeof(Rec));
+    if (e != cudaSuccess) { (void)cudaGetLastError(); set_err("sw_set_series_capacity: cudaMalloc failed"); return SW_ENOMEM; }
+    if (h->series_owned) cudaFree(h->series_owned);
+    h->series_owned = p; h->series = p; h->series_cap = sweeps;
+    h->rec_valid = false;
+    return SW_OK;
+}
+
+int sw_set_spins(sw_handle* h, const int8_t* spins, int is_host) {
+    if (!h || !spins) { set_err("sw_set_spins: null argument"); return SW_EINVAL; }
+    SW_CUDA(cudaMemcpyAsync(h->spins, spins, (size_t)h->nb * h->N,
+                            is_host ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice, h->stream));
+    if (is_host) SW_CUDA(cudaStreamSynchronize(h->stream));
+    h->have_sweep = false; h->rec_valid = false;
+    return SW_OK;
+}
+
+int sw_set_cold(sw_handle* h) {
+    if (!h) { set_err("sw_set_cold: null handle"); return SW_EINVAL; }
+    const size_t n = (size_t)h->nb * h->N;
+    k_fill_i8<<<(unsigned)((n + GEN_THREADS - 1) / GEN_THREADS), GEN_THREADS, 0, h->stream>>>(h->spins, n, (int8_t)1);
+    SW_CUDA(cudaGetLastError());
+    h->have_sweep = false; h->rec_valid = false;
+    return SW_OK;
+}
+
+int sw_get_spins(sw_handle* h, int8_t* out_host) {
+    if (!h || !out_host) { set_err("sw_get_spins: null argument"); return SW_EINVAL; }
+    SW_CUDA(cudaMemcpyAsync(out_host, h->spins, (size_t)h->nb * h->N, cudaMemcpyDeviceToHost, h->stream));
+    SW_CUDA(cudaStreamSynchronize(h->stream));
+    return SW_OK;
+}
+
+int sw_get_labels(sw_handle* h, int32_t* out_host) {
+    if (!h || !out_host) { set_err("sw_get_labels: null argument"); return SW_EINVAL; }
+    const int32_t* l = sw_labels(h);
+    if (!l) return SW_ESTATE;
+    SW_CUDA(cudaMemcpyAsync(out_host, l, (size_t)h->nb * h->N * 4, cudaMemcpyDeviceToHost, h->stream));
+    SW_CUDA(cudaStreamSynchronize(h->stream));
+    return SW_OK;
+}
+
+int sw_set_sweep_index(sw_handle* h, uint64_t t) {
+    if (!h) { set_err("sw_set_sweep_index: null handle"); return SW_EINVAL; }
+    h->t = t;                   // written to the device at the start of the next sw_sweep
+    return SW_OK;
+}
+uint64_t sw_sweep_index(const sw_handle* h) { return h ? h->t : 0; }
+
+int sw_set_stream(sw_handle* h, void* cuda_stream) {
+    if (!h) { set_err("sw_set_stream: null handle"); return SW_EINVAL; }
+    SW_CUDA(cudaStreamSynchronize(h->stream));
+    h->stream = (cudaStream_t)cuda_stream;
+    return SW_OK;
+}
+
+int sw_set_stage_timing(sw_handle* h, int on) {
+    if (!h) { set_err("sw_set_stage_timing: null handle"); return SW_EINVAL; }
+    h->timing = on != 0;
+    if (!h->timing) h->timed_sweeps = 0;
+    return SW_OK;
+}
+
+int sw_stage_ms(sw_handle* h, float out[4]) {
+    if (!h || !out) { set_err("sw_stage_ms: null argument"); return SW_EINVAL; }
+    out[0] = out[1] = out[2] = out[3] = 0.f;
+    if (h->timed_sweeps == 0) { set_err("sw_stage_ms: the last sw_sweep ran without stage timing"); return SW_ESTATE; }
+    SW_CUDA(cudaStreamSynchronize(h->stream));
+    for (int64_t k = 0; k < h->timed_sweeps; ++k)
+        for (int s = 0; s < 4; ++s) {
+            float ms = 0.f;
+            SW_CUDA(cudaEventElapsedTime(&ms, h->ev[(size_t)k * EV_PER_SWEEP + s], h->ev[(size_t)k * EV_PER_SWEEP + s + 1]));
+            out[s] += ms;
+        }
+    return SW_OK;
+}
+
+int sw_set_path(sw_handle* h, int path) {
+    if (!h || path < 0 || path > 3) { set_err("sw_set_path: invalid argument"); return SW_EINVAL; }
+    h->path = path;
+    h->tile = pick_tile(h->L, path);
+    return SW_OK;
+}
+
+int64_t sw_last_launch_count(const sw_handle* h) { return h ? h->launches : 0; }
+uint32_t sw_threshold(const sw_handle* h, int32_t b) { return (h && b >= 0 && b < h->nb) ? h->hlat[b].thr : 0u; }
+int32_t sw_L(const sw_handle* h) { return h ? h->L : 0; }
+int32_t sw_batch(const sw_handle* h) { return h ? h->nb : 0; }
+
+int sw_test_philox(const uint32_t* ctr, const uint32_t* key, uint32_t* out, int64_t n) {
+    if (!ctr || !key || !out || n < 0) { set_err("sw_test_philox: invalid argument"); return SW_EINVAL; }
+    if (n == 0) return SW_OK;
+    uint32_t *dc = nullptr, *dk = nullptr, *dout = nullptr;
+    SW_CUDA(cudaMalloc((void**)&dc, (size_t)n * 16));
+    SW_CUDA(cudaMalloc((void**)&dk, (size_t)n * 8));
+    SW_CUDA(cudaMalloc((void**)&dout, (size_t)n * 16));
+    SW_CUDA(cudaMemcpy(dc, ctr, (size_t)n * 16, cudaMemcpyHostToDevice));
+    SW_CUDA(cudaMemcpy(dk, key, (size_t)n * 8, cudaMemcpyHostToDevice));
+    k_test_philox<<<(unsigned)((n + 255) / 256), 256>>>(dc, dk, dout, n);
+    SW_CUDA(cudaGetLastError());
+    SW_CUDA(cudaMemcpy(out, dout, (size_t)n * 16, cudaMemcpyDeviceToHost));
+    cudaFree(dc); cudaFree(dk); cudaFree(dout);
+    return SW_OK;
+}
+
+int sw_test_label(sw_handle* h, const uint32_t* bondE, const uint32_t* bondS, int32_t* labels_out) {
+    if (!h || !bondE || !bondS || !labels_out || h->nb != 1) { set_err("sw_test_label: invalid argument"); return SW_EINVAL; }
+    SW_CUDA(cudaMemcpyAsync(h->bondE, bondE, (size_t)h->words * 4, cudaMemcpyHostToDevice, h->stream));
+    SW_CUDA(cudaMemcpyAsync(h->bondS, bondS, (size_t)h->words * 4, cudaMemcpyHostToDevice, h->stream));
+    SW_CUDA(cudaMemsetAsync(h->series, 0, sizeof(Rec), h->stream));
+    k_set_ctl<<<1, 1, 0, h->stream>>>(h->ctl, (unsigned long long)h->t, 0u, (uint32_t)h->series_cap);
+    int rc = launch_label(h);
+    if (rc) return rc;
+    SW_CUDA(cudaGetLastError());
+    SW_CUDA(cudaMemcpyAsync(labels_out, h->label, (size_t)h->N * 4, cudaMemcpyDeviceToHost, h->stream));
+    SW_CUDA(cudaStreamSynchronize(h->stream));
+    h->have_sweep = false; h->rec_valid = false;
+    return SW_OK;
+}
+
+} // extern "C"

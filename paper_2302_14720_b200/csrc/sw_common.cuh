@@ -1,0 +1,145 @@
+// sw_common.cuh -- device-side types and helpers shared by the kernels of libsw_b200.so.
+// Product code (CUDA path).  Shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace sw {
+
+// Philox stream tags: counter = (block, t_lo, t_hi, TAG)
+constexpr uint32_t TAG_INIT = 0u, TAG_BOND = 1u, TAG_FLIP = 2u;
+
+// per-lattice parameters (device array of nb entries)
+struct Lat {
+    uint32_t key0, key1;   // Philox key = (seed & 0xffffffff, seed >> 32)
+    uint32_t thr;          // floor((1 - exp(-2/T)) * 2^32), clamped to 2^32 - 1
+    uint32_t pad;
+};
+
+// device-resident sweep control: lets one captured launch sequence serve every sweep
+struct Ctl {
+    unsigned long long t;  // sweep index the next sweep uses
+    uint32_t slot;         // series slot the running sweep accumulates into
+    uint32_t cap;          // number of series slots (ring)
+};
+
+// one per (series slot, lattice); accumulated with atomics during the sweep
+struct Rec {
+    long long E, M, ncl, maxcl;
+};
+
+// ------------------------------------------------------------------------------------------
+// Philox4x32-10.  mul.wide.u32 -> one IMAD.WIDE per multiply; the xor of three terms -> one LOP3.
+// ------------------------------------------------------------------------------------------
+constexpr uint32_t PHILOX_M0 = 0xD2511F53u, PHILOX_M1 = 0xCD9E8D57u;
+constexpr uint32_t PHILOX_W0 = 0x9E3779B9u, PHILOX_W1 = 0xBB67AE85u;
+
+struct PhiloxKey {          // the ten round keys, expanded once per thread
+    uint32_t k0[10], k1[10];
+    __device__ __forceinline__ PhiloxKey(uint32_t key0, uint32_t key1) {
+#pragma unroll
+        for (int r = 0; r < 10; ++r) { k0[r] = key0 + (uint32_t)r * PHILOX_W0; k1[r] = key1 + (uint32_t)r * PHILOX_W1; }
+    }
+};
+
+__device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                               const PhiloxKey& k) {
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const unsigned long long p0 = (unsigned long long)PHILOX_M0 * c0;
+        const unsigned long long p1 = (unsigned long long)PHILOX_M1 * c2;
+        const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k.k0[r];
+        const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k.k1[r];
+        c1 = (uint32_t)p1; c3 = (uint32_t)p0; c0 = n0; c2 = n2;
+    }
+    return make_uint4(c0, c1, c2, c3);
+}
+
+// ------------------------------------------------------------------------------------------
+// memory helpers
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ int ld_cg(const int* p) {            // L2-coherent load (labels under atomics)
+    int v; asm volatile("ld.global.cg.s32 %0, [%1];" : "=r"(v) : "l"(p)); return v;
+}
+__device__ __forceinline__ uint4 ld_stream_u4(const void* p) {   // read-once data: do not pollute L1
+    uint4 v; asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
+                          : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p)); return v;
+}
+__device__ __forceinline__ void st_stream_u4(void* p, uint4 v) {
+    asm volatile("st.global.L1::no_allocate.v4.u32 [%0], {%1,%2,%3,%4};"
+                 :: "l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
+
+// sign bits of four int8 spins (+1 = 0x01, -1 = 0xFF) gathered into a nibble: bit k = (spin k == -1)
+__device__ __forceinline__ uint32_t neg_nibble(uint32_t q) {
+    return (((q >> 7) & 0x01010101u) * 0x01020408u) >> 24;
+}
+// 32 spins held as two uint4 -> 32-bit mask, bit k = (spin k == -1)
+__device__ __forceinline__ uint32_t neg_mask32(uint4 a, uint4 b) {
+    return  neg_nibble(a.x)        | (neg_nibble(a.y) << 4)  | (neg_nibble(a.z) << 8)  | (neg_nibble(a.w) << 12)
+         | (neg_nibble(b.x) << 16) | (neg_nibble(b.y) << 20) | (neg_nibble(b.z) << 24) | (neg_nibble(b.w) << 28);
+}
+
+// block-wide sums / max into one atomic per block
+__device__ __forceinline__ long long warp_sum_ll(long long v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+__device__ __forceinline__ int warp_sum_i(int v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+__device__ __forceinline__ int warp_max_i(int v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = max(v, __shfl_xor_sync(0xffffffffu, v, o));
+    return v;
+}
+__device__ __forceinline__ void atomic_add_ll(long long* p, long long v) {
+    atomicAdd(reinterpret_cast<unsigned long long*>(p), (unsigned long long)v);
+}
+__device__ __forceinline__ void atomic_max_ll(long long* p, long long v) {   // values are >= 0
+    atomicMax(reinterpret_cast<unsigned long long*>(p), (unsigned long long)v);
+}
+
+// ------------------------------------------------------------------------------------------
+// lock-free union-find on a global int32 parent array; label[x] <= x, roots have label[r] == r.
+// Hooking is "larger root under smaller" with atomicMin, so the surviving root of a component is
+// its minimum site index whatever the race order (north_star stage 2).
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ int uf_find(const int* lab, int x) {
+    int p = ld_cg(lab + x);
+    while (p != x) { x = p; p = ld_cg(lab + x); }
+    return x;
+}
+// read-only find after all merging is done (ordinary cached loads)
+__device__ __forceinline__ int uf_find_ro(const int* __restrict__ lab, int x) {
+    int p = __ldg(lab + x);
+    while (p != x) { x = p; p = __ldg(lab + x); }
+    return x;
+}
+// find with one-shot compression of the starting node when the walk was longer than one hop
+// (only ever writes a smaller ancestor: safe under races)
+__device__ __forceinline__ int uf_find_compress(int* lab, int x) {
+    const int x0 = x;
+    int p = ld_cg(lab + x);
+    if (p == x) return x;
+    int q = ld_cg(lab + p);
+    if (q == p) return p;
+    x = q; p = ld_cg(lab + x);
+    while (p != x) { x = p; p = ld_cg(lab + x); }
+    atomicMin(lab + x0, x);
+    return x;
+}
+__device__ __forceinline__ void uf_union(int* lab, int a, int b) {
+    a = uf_find_compress(lab, a); b = uf_find_compress(lab, b);
+    while (a != b) {
+        if (a < b) { int s = a; a = b; b = s; }           // a is the larger
+        const int old = atomicMin(lab + a, b);
+        if (old == a) break;                               // a was a root and now hangs under b
+        a = old;                                           // a already had a parent: unite that with b
+    }
+}
+
+} // namespace sw

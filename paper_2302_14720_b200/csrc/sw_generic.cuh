@@ -1,0 +1,201 @@
+// sw_generic.cuh -- any-L kernels (L >= 2, any batch): the correct-first path and the fallback for
+// lattice sides that are not a multiple of the tile.  Global union-find, no tiles.
+// Batch lattice b = blockIdx.y everywhere; site / word index from blockIdx.x.
+#pragma once
+#include "sw_common.cuh"
+
+namespace sw {
+
+constexpr int GEN_THREADS = 256;
+
+// ---- start configuration: spins[i] = bit_INIT(i) ? +1 : -1 (Fig. 1) ----------
+// one thread per 32 sites (one word of the TAG_INIT bit field)
+__global__ void __launch_bounds__(GEN_THREADS)
+k_init_random(int8_t* __restrict__ spins, const Lat* __restrict__ lat, int N, int words) {
+    const int w = blockIdx.x * GEN_THREADS + threadIdx.x;
+    if (w >= words) return;
+    const Lat la = lat[blockIdx.y];
+    const PhiloxKey key(la.key0, la.key1);
+    const uint4 r = philox4x32_10((uint32_t)(w >> 2), 0u, 0u, TAG_INIT, key);
+    const uint32_t bits = (w & 3) == 0 ? r.x : (w & 3) == 1 ? r.y : (w & 3) == 2 ? r.z : r.w;
+    int8_t* s = spins + (size_t)blockIdx.y * N + (size_t)w * 32;
+    const int n = min(32, N - w * 32);
+    for (int k = 0; k < n; ++k) s[k] = ((bits >> k) & 1u) ? (int8_t)1 : (int8_t)-1;
+}
+
+__global__ void __launch_bounds__(GEN_THREADS)
+k_fill_i8(int8_t* __restrict__ p, size_t n, int8_t v) {
+    const size_t i = (size_t)blockIdx.x * GEN_THREADS + threadIdx.x;
+    if (i < n) p[i] = v;
+}
+
+// ---- a1 bond formation: one thread per bit-plane word = 32 sites = 16 Philox calls
+__global__ void __launch_bounds__(GEN_THREADS)
+k_bond_generic(const int8_t* __restrict__ spins, uint32_t* __restrict__ bondE, uint32_t* __restrict__ bondS,
+               const Lat* __restrict__ lat, const Ctl* __restrict__ ctl, int L, int N, int words) {
+    const int w = blockIdx.x * GEN_THREADS + threadIdx.x;
+    if (w >= words) return;
+    const Lat la = lat[blockIdx.y];
+    const PhiloxKey key(la.key0, la.key1);
+    const unsigned long long t = ctl->t;
+    const uint32_t tlo = (uint32_t)t, thi = (uint32_t)(t >> 32);
+    const int8_t* s = spins + (size_t)blockIdx.y * N;
+    uint32_t e = 0, so = 0;
+    const int i0 = w * 32;
+#pragma unroll 4
+    for (int c = 0; c < 16; ++c) {
+        const int i = i0 + 2 * c;
+        if (i >= N) break;
+        const uint4 r = philox4x32_10((uint32_t)(i >> 1), tlo, thi, TAG_BOND, key);
+#pragma unroll
+        for (int j = 0; j < 2; ++j) {
+            const int ii = i + j;
+            if (ii < N) {
+                const int y = ii / L, x = ii - y * L;
+                const int ie = y * L + (x + 1 == L ? 0 : x + 1);
+                const int is = (y + 1 == L ? 0 : y + 1) * L + x;
+                const int8_t v = s[ii];
+                const uint32_t we = j ? r.z : r.x, ws = j ? r.w : r.y;
+                if (v == s[ie] && we < la.thr) e  |= 1u << (2 * c + j);
+                if (v == s[is] && ws < la.thr) so |= 1u << (2 * c + j);
+            }
+        }
+    }
+    bondE[(size_t)blockIdx.y * words + w] = e;
+    bondS[(size_t)blockIdx.y * words + w] = so;
+}
+
+// ---- a2-a4 labelling, generic: label[i] = i; one thread per site unites along its two bonds ----
+__global__ void __launch_bounds__(GEN_THREADS)
+k_label_init(int* __restrict__ label, int N) {
+    const int i = blockIdx.x * GEN_THREADS + threadIdx.x;
+    if (i < N) label[(size_t)blockIdx.y * N + i] = i;
+}
+
+__global__ void __launch_bounds__(GEN_THREADS)
+k_union_generic(int* label, const uint32_t* __restrict__ bondE, const uint32_t* __restrict__ bondS,
+                int L, int N, int words) {
+    const int i = blockIdx.x * GEN_THREADS + threadIdx.x;
+    if (i >= N) return;
+    int* lab = label + (size_t)blockIdx.y * N;
+    const uint32_t e  = bondE[(size_t)blockIdx.y * words + (i >> 5)] >> (i & 31);
+    const uint32_t so = bondS[(size_t)blockIdx.y * words + (i >> 5)] >> (i & 31);
+    if (!((e | so) & 1u)) return;
+    const int y = i / L, x = i - y * L;
+    if (e & 1u)  uf_union(lab, i, y * L + (x + 1 == L ? 0 : x + 1));
+    if (so & 1u) uf_union(lab, i, (y + 1 == L ? 0 : y + 1) * L + x);
+}
+
+// label[i] = find(i); counts roots; accumulates cluster sizes into gsize[root] (generic path only)
+__global__ void __launch_bounds__(GEN_THREADS)
+k_compress_generic(int* label, int* __restrict__ gsize, Rec* __restrict__ rec, const Ctl* __restrict__ ctl,
+                   int N, int nb) {
+    const int i = blockIdx.x * GEN_THREADS + threadIdx.x;
+    int isroot = 0;
+    if (i < N) {
+        int* lab = label + (size_t)blockIdx.y * N;
+        const int r = uf_find(lab, i);
+        lab[i] = r;
+        isroot = (r == i);
+        atomicAdd(gsize + (size_t)blockIdx.y * N + r, 1);
+    }
+    isroot = warp_sum_i(isroot);
+    if ((threadIdx.x & 31) == 0 && isroot)
+        atomic_add_ll(&rec[(size_t)ctl->slot * nb + blockIdx.y].ncl, isroot);
+}
+
+// largest cluster from gsize; leaves gsize zero for the next sweep
+__global__ void __launch_bounds__(GEN_THREADS)
+k_maxsize_generic(const int* __restrict__ label, int* __restrict__ gsize, Rec* __restrict__ rec,
+                  const Ctl* __restrict__ ctl, int N, int nb) {
+    const int i = blockIdx.x * GEN_THREADS + threadIdx.x;
+    int m = 0;
+    if (i < N && label[(size_t)blockIdx.y * N + i] == i) {
+        m = gsize[(size_t)blockIdx.y * N + i];
+        gsize[(size_t)blockIdx.y * N + i] = 0;
+    }
+    m = warp_max_i(m);
+    if ((threadIdx.x & 31) == 0 && m)
+        atomic_max_ll(&rec[(size_t)ctl->slot * nb + blockIdx.y].maxcl, m);
+}
+
+// ---- a5 flip-bit plane: D word w = Philox(ctr = (w>>2, t, TAG_FLIP))[w&3];
+//      one thread per call = 4 words = 128 candidate root decisions ------------------------------
+__global__ void __launch_bounds__(GEN_THREADS)
+k_flipbits(uint32_t* __restrict__ D, const Lat* __restrict__ lat, const Ctl* __restrict__ ctl, int words) {
+    const int c = blockIdx.x * GEN_THREADS + threadIdx.x;      // call index
+    if (c * 4 >= words) return;
+    const Lat la = lat[blockIdx.y];
+    const PhiloxKey key(la.key0, la.key1);
+    const unsigned long long t = ctl->t;
+    const uint4 r = philox4x32_10((uint32_t)c, (uint32_t)t, (uint32_t)(t >> 32), TAG_FLIP, key);
+    uint32_t* d = D + (size_t)blockIdx.y * words + (size_t)c * 4;
+    if (c * 4 + 3 < words && (words & 3) == 0) {
+        *reinterpret_cast<uint4*>(d) = r;
+    } else {
+        const uint32_t v[4] = { r.x, r.y, r.z, r.w };
+        for (int k = 0; k < 4 && c * 4 + k < words; ++k) d[k] = v[k];
+    }
+}
+
+// ---- a6 assignment: spins[i] = D bit at label[i] ? +1 : -1 (labels flat) -----------
+__global__ void __launch_bounds__(GEN_THREADS)
+k_flip_generic(int8_t* __restrict__ spins, const int* __restrict__ label, const uint32_t* __restrict__ D,
+               int N, int words) {
+    const int i = blockIdx.x * GEN_THREADS + threadIdx.x;
+    if (i >= N) return;
+    const int r = label[(size_t)blockIdx.y * N + i];
+    const uint32_t d = D[(size_t)blockIdx.y * words + (r >> 5)];
+    spins[(size_t)blockIdx.y * N + i] = ((d >> (r & 31)) & 1u) ? (int8_t)1 : (int8_t)-1;
+}
+
+// ---- a7 observables: E = -sum_i s_i (s_E + s_S), M = sum_i s_i ----------------------
+// rec_base points at the nb records to accumulate into (a series slot, or the "now" scratch record)
+__global__ void __launch_bounds__(GEN_THREADS)
+k_observe_generic(const int8_t* __restrict__ spins, Rec* __restrict__ rec, const Ctl* __restrict__ ctl,
+                  int use_slot, int L, int N, int nb) {
+    const int i = blockIdx.x * GEN_THREADS + threadIdx.x;
+    int e = 0, m = 0;
+    if (i < N) {
+        const int8_t* s = spins + (size_t)blockIdx.y * N;
+        const int y = i / L, x = i - y * L;
+        const int v = s[i];
+        e = -v * ((int)s[y * L + (x + 1 == L ? 0 : x + 1)] + (int)s[(y + 1 == L ? 0 : y + 1) * L + x]);
+        m = v;
+    }
+    e = warp_sum_i(e); m = warp_sum_i(m);
+    __shared__ int se[GEN_THREADS / 32], sm[GEN_THREADS / 32];
+    if ((threadIdx.x & 31) == 0) { se[threadIdx.x >> 5] = e; sm[threadIdx.x >> 5] = m; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int te = 0, tm = 0;
+        for (int k = 0; k < GEN_THREADS / 32; ++k) { te += se[k]; tm += sm[k]; }
+        Rec* r = rec + (use_slot ? (size_t)ctl->slot * nb : 0) + blockIdx.y;
+        if (te) atomic_add_ll(&r->E, te);
+        if (tm) atomic_add_ll(&r->M, tm);
+    }
+}
+
+// ---- sweep control -------------------------------------------------------------------------------
+__global__ void k_set_ctl(Ctl* ctl, unsigned long long t, uint32_t slot, uint32_t cap) {
+    ctl->t = t; ctl->slot = slot; ctl->cap = cap;
+}
+// end of a sweep: t += 1, move to the next series slot and zero it
+__global__ void k_advance(Ctl* ctl, Rec* rec, int nb) {
+    const uint32_t next = (ctl->slot + 1 == ctl->cap) ? 0u : ctl->slot + 1;
+    for (int b = threadIdx.x; b < nb; b += blockDim.x) rec[(size_t)next * nb + b] = Rec{0, 0, 0, 0};
+    __syncthreads();
+    if (threadIdx.x == 0) { ctl->t += 1; ctl->slot = next; }
+}
+
+// ---- test hook: Philox on the device ---------------------------------------------------------------
+__global__ void k_test_philox(const uint32_t* __restrict__ ctr, const uint32_t* __restrict__ key,
+                              uint32_t* __restrict__ out, long long n) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const PhiloxKey k(key[2 * i], key[2 * i + 1]);
+    const uint4 r = philox4x32_10(ctr[4 * i], ctr[4 * i + 1], ctr[4 * i + 2], ctr[4 * i + 3], k);
+    out[4 * i] = r.x; out[4 * i + 1] = r.y; out[4 * i + 2] = r.z; out[4 * i + 3] = r.w;
+}
+
+} // namespace sw

@@ -1,0 +1,373 @@
+// sw_tiled.cuh -- the fast path for lattice sides that are a multiple of the tile width.
+//
+// Stage map:
+//   a1 k_bond_rows      Philox bond draws, one thread per bit-plane word (32 sites, 16 Philox calls)
+//   a2 k_tile_label     shared-memory union-find of one TW x TH tile: rows are pre-united by run
+//                       length from the East-bond word (bit tricks, no atomics), vertical unions only
+//                       where a South bond starts a new overlap of two runs; writes label[i] = global
+//                       index of the tile-local root; tile-local cluster sizes; the list of "open"
+//                       clusters (those with a bond across the tile edge)
+//   a3 k_merge_tiled    one thread per tile-edge bond: atomicMin hooking on the global parent array
+//   a4 k_compress_tiled label[i] = root(i), 128-bit loads/stores; counts roots
+//      k_sizes_open     sizes of clusters that span tiles (closed clusters were maximised in a2)
+//   a5 k_flipbits       (sw_generic.cuh) decision bit-plane
+//   a6 k_flip_rows      spins = gather(D, label); magnetisation
+//   a7 k_energy_rows    energy of the new configuration from sign masks + popc
+#pragma once
+#include "sw_common.cuh"
+
+namespace sw {
+
+constexpr int ROW_THREADS = 256;
+constexpr uint32_t OPEN_FLAG = 0x40000000u;
+
+// ---------------------------------------------------------------------------------------------
+// a1 bond formation, PAPER.md:37-39 (section 2.1).  Thread w owns sites 32w .. 32w+31 of one row.
+// Equal-spin masks come from the sign bits of the int8 spins; the draw masks from 16 Philox calls
+// (call c covers sites 2c, 2c+1: words x,y = East,South of the even site, z,w of the odd one).
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(ROW_THREADS)
+k_bond_rows(const int8_t* __restrict__ spins, uint32_t* __restrict__ bondE, uint32_t* __restrict__ bondS,
+            const Lat* __restrict__ lat, const Ctl* __restrict__ ctl, int L, int N, int words) {
+    const int w = blockIdx.x * ROW_THREADS + threadIdx.x;
+    if (w >= words) return;
+    const int wpr = L >> 5;
+    const int y = w / wpr, xw = w - y * wpr;
+    const int8_t* s = spins + (size_t)blockIdx.y * N;
+    const int8_t* row  = s + (size_t)y * L + xw * 32;
+    const int8_t* rowS = s + (size_t)(y + 1 == L ? 0 : y + 1) * L + xw * 32;
+    const uint4 a0 = *reinterpret_cast<const uint4*>(row),  a1 = *reinterpret_cast<const uint4*>(row + 16);
+    const uint4 b0 = *reinterpret_cast<const uint4*>(rowS), b1 = *reinterpret_cast<const uint4*>(rowS + 16);
+    const int8_t nx = s[(size_t)y * L + (xw + 1 == wpr ? 0 : (xw + 1) * 32)];
+    const uint32_t own = neg_mask32(a0, a1), south = neg_mask32(b0, b1);
+    const uint32_t eastm = (own >> 1) | (nx < 0 ? 0x80000000u : 0u);
+    const uint32_t eqE = ~(own ^ eastm), eqS = ~(own ^ south);
+
+    const Lat la = lat[blockIdx.y];
+    const PhiloxKey key(la.key0, la.key1);
+    const unsigned long long t = ctl->t;
+    const uint32_t tlo = (uint32_t)t, thi = (uint32_t)(t >> 32);
+    uint32_t dE = 0, dS = 0;
+#pragma unroll
+    for (int c = 0; c < 16; ++c) {
+        const uint4 r = philox4x32_10((uint32_t)w * 16u + c, tlo, thi, TAG_BOND, key);
+        dE |= (r.x < la.thr ? 1u : 0u) << (2 * c) | (r.z < la.thr ? 1u : 0u) << (2 * c + 1);
+        dS |= (r.y < la.thr ? 1u : 0u) << (2 * c) | (r.w < la.thr ? 1u : 0u) << (2 * c + 1);
+    }
+    bondE[(size_t)blockIdx.y * words + w] = eqE & dE;
+    bondS[(size_t)blockIdx.y * words + w] = eqS & dS;
+}
+
+// ---------------------------------------------------------------------------------------------
+// a2 tile-local labelling, PAPER.md:49-51 (section 2.3) with the algorithm north_star names:
+// shared-memory union-find, min-index roots.
+// ---------------------------------------------------------------------------------------------
+template <int TW, int TH>
+struct TileCfg {
+    static constexpr int SITES = TW * TH;
+    static constexpr int WPR = TW / 32;              // bond words per tile row
+    static constexpr int RW = TH * WPR;              // row-words per tile
+    static constexpr int THREADS = 1024;
+    static constexpr int RW_PER_WARP = RW / 32;      // each warp owns RW/32 row-words, lane = x in the word
+    static constexpr int CAP = 2 * (TW + TH);        // upper bound on open clusters per tile
+    static_assert(TW % 32 == 0 && RW % 32 == 0, "tile shape");
+};
+
+__device__ __forceinline__ int s_find(volatile int* lab, int x) {
+    int p = lab[x];
+    while (p != x) { x = p; p = lab[x]; }
+    return x;
+}
+__device__ __forceinline__ void s_union(int* lab, int a, int b) {
+    a = s_find(lab, a); b = s_find(lab, b);
+    while (a != b) {
+        if (a < b) { int s = a; a = b; b = s; }
+        const int old = atomicMin(lab + a, b);
+        if (old == a) break;
+        a = old;
+    }
+}
+
+template <int TW, int TH>
+__global__ void __launch_bounds__(TileCfg<TW, TH>::THREADS)
+k_tile_label(int* __restrict__ label, const uint32_t* __restrict__ bondE, const uint32_t* __restrict__ bondS,
+             int2* __restrict__ olist, int* __restrict__ ocount, Rec* __restrict__ rec,
+             const Ctl* __restrict__ ctl, int L, int N, int words, int nb) {
+    using C = TileCfg<TW, TH>;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    int* lab = reinterpret_cast<int*>(smem_raw);                  // [SITES] parent, tile-local index
+    int* cnt = lab + C::SITES;                                    // [SITES] size at roots (+ OPEN_FLAG)
+    uint32_t* eW = reinterpret_cast<uint32_t*>(cnt + C::SITES);   // [RW] East-bond words of the tile
+    uint32_t* sW = eW + C::RW;                                    // [RW] South-bond words
+    uint32_t* nIn = sW + C::RW;                                   // [WPR] South bonds entering from the North tile
+    int* s_misc = reinterpret_cast<int*>(nIn + C::WPR);           // [2] open-list cursor, closed maximum
+    uint8_t* wIn = reinterpret_cast<uint8_t*>(s_misc + 2);        // [TH] East bonds entering from the West tile
+    int& s_nopen = s_misc[0];
+    int& s_max = s_misc[1];
+
+    const int tilesX = L / TW;
+    const int ty = blockIdx.x / tilesX, tx = blockIdx.x - ty * tilesX;
+    const int y0 = ty * TH, x0 = tx * TW;
+    const int wprL = L >> 5;
+    const uint32_t* bE = bondE + (size_t)blockIdx.y * words;
+    const uint32_t* bS = bondS + (size_t)blockIdx.y * words;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+
+    // phase 0: the tile's bond words, plus the bonds that enter it from the West and North tiles
+    for (int idx = tid; idx < C::RW; idx += C::THREADS) {
+        const int row = idx / C::WPR, wx = idx - row * C::WPR;
+        const size_t gw = (size_t)(y0 + row) * wprL + (x0 >> 5) + wx;
+        eW[idx] = bE[gw]; sW[idx] = bS[gw];
+    }
+    if (tid < TH) {
+        const int wl = (x0 >> 5) == 0 ? wprL - 1 : (x0 >> 5) - 1;
+        wIn[tid] = (uint8_t)(bE[(size_t)(y0 + tid) * wprL + wl] >> 31);
+    }
+    if (tid < C::WPR) {
+        const int yn = y0 == 0 ? L - 1 : y0 - 1;
+        nIn[tid] = bS[(size_t)yn * wprL + (x0 >> 5) + tid];
+    }
+    if (tid == 0) { s_nopen = 0; s_max = 0; }
+    __syncthreads();
+
+    // phase 1: every site starts at the head of its horizontal run inside its 32-site word
+    int head_off[C::RW_PER_WARP];
+#pragma unroll
+    for (int k = 0; k < C::RW_PER_WARP; ++k) {
+        const int rw = warp + 32 * k;
+        const uint32_t e = eW[rw];
+        const int ones = lane ? __clz(~(e << (32 - lane))) : 0;      // bonded sites directly to my left
+        head_off[k] = ones;
+        const int row = rw / C::WPR, wx = rw - row * C::WPR;
+        const int l = row * TW + wx * 32 + lane;
+        lab[l] = l - ones;
+        cnt[l] = 0;
+    }
+    __syncthreads();
+
+    // phase 2: unions -- runs that continue across a word boundary, and South bonds.  A South bond
+    // is skipped when its left neighbour already joins the same two runs.
+#pragma unroll
+    for (int k = 0; k < C::RW_PER_WARP; ++k) {
+        const int rw = warp + 32 * k;
+        const int row = rw / C::WPR, wx = rw - row * C::WPR;
+        const int l = row * TW + wx * 32 + lane;
+        if (lane == 0 && wx > 0 && (eW[rw - 1] >> 31)) s_union(lab, l - 1, l);
+        if (row < TH - 1) {
+            const uint32_t s = sW[rw];
+            const uint32_t need = s & ~((s & eW[rw] & eW[rw + C::WPR]) << 1);
+            if ((need >> lane) & 1u) s_union(lab, l, l + TW);
+        }
+    }
+    __syncthreads();
+
+    // phase 3: roots, sizes (one shared atomic per run head), global labels
+    int root[C::RW_PER_WARP];
+    int* glab = label + (size_t)blockIdx.y * N;
+#pragma unroll
+    for (int k = 0; k < C::RW_PER_WARP; ++k) {
+        const int rw = warp + 32 * k;
+        const int row = rw / C::WPR, wx = rw - row * C::WPR;
+        const int l = row * TW + wx * 32 + lane;
+        const int r = s_find(lab, l);
+        root[k] = r;
+        if (head_off[k] == 0) {
+            const uint32_t tbits = ~(eW[rw] >> lane);                 // first 0 above me ends the run
+            const int len = min(tbits ? __ffs(tbits) : 33, 32 - lane);
+            atomicAdd(&cnt[r], len);
+        }
+        const int rr = r / TW, rx = r - rr * TW;
+        glab[(size_t)(y0 + row) * L + x0 + wx * 32 + lane] = (y0 + rr) * L + x0 + rx;
+    }
+    __syncthreads();
+
+    // phase 4: a cluster is "open" when one of its sites has a bond across the tile edge
+#pragma unroll
+    for (int k = 0; k < C::RW_PER_WARP; ++k) {
+        const int rw = warp + 32 * k;
+        const int row = rw / C::WPR, wx = rw - row * C::WPR;
+        bool open = false;
+        if (wx == C::WPR - 1 && lane == 31 && (eW[rw] >> 31)) open = true;
+        if (wx == 0 && lane == 0 && wIn[row]) open = true;
+        if (row == TH - 1 && ((sW[rw] >> lane) & 1u)) open = true;
+        if (row == 0 && ((nIn[wx] >> lane) & 1u)) open = true;
+        if (open) atomicOr(reinterpret_cast<unsigned int*>(&cnt[root[k]]), OPEN_FLAG);
+    }
+    __syncthreads();
+
+    // phase 5: closed clusters are complete -> maximise their size; open ones go to the tile's list
+    int mymax = 0;
+    int2* mylist = olist + ((size_t)blockIdx.y * gridDim.x + blockIdx.x) * C::CAP;
+#pragma unroll
+    for (int k = 0; k < C::RW_PER_WARP; ++k) {
+        const int rw = warp + 32 * k;
+        const int row = rw / C::WPR, wx = rw - row * C::WPR;
+        const int l = row * TW + wx * 32 + lane;
+        if (root[k] == l) {
+            const uint32_t c = (uint32_t)cnt[l];
+            if (c & OPEN_FLAG) {
+                const int pos = atomicAdd(&s_nopen, 1);
+                mylist[pos] = make_int2((y0 + row) * L + x0 + wx * 32 + lane, (int)(c & ~OPEN_FLAG));
+            } else {
+                mymax = max(mymax, (int)c);
+            }
+        }
+    }
+    mymax = warp_max_i(mymax);
+    if (lane == 0 && mymax) atomicMax(&s_max, mymax);
+    __syncthreads();
+    if (tid == 0) {
+        ocount[(size_t)blockIdx.y * gridDim.x + blockIdx.x] = s_nopen;
+        if (s_max) atomic_max_ll(&rec[(size_t)ctl->slot * nb + blockIdx.y].maxcl, s_max);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// a3 global boundary merge: one thread per site on a tile's East column or South row.
+// ---------------------------------------------------------------------------------------------
+template <int TW, int TH>
+__global__ void __launch_bounds__(ROW_THREADS)
+k_merge_tiled(int* label, const uint32_t* __restrict__ bondE, const uint32_t* __restrict__ bondS,
+              int L, int N, int words) {
+    const int tilesX = L / TW, tilesY = L / TH;
+    const int nV = L * tilesX;                       // East-edge sites
+    const int idx = blockIdx.x * ROW_THREADS + threadIdx.x;
+    if (idx >= nV + tilesY * L) return;
+    int* lab = label + (size_t)blockIdx.y * N;
+    const int wprL = L >> 5;
+    if (idx < nV) {
+        const int y = idx / tilesX, c = idx - y * tilesX;
+        const int x = c * TW + TW - 1;
+        if (bondE[(size_t)blockIdx.y * words + (size_t)y * wprL + (x >> 5)] >> 31)
+            uf_union(lab, y * L + x, y * L + (x + 1 == L ? 0 : x + 1));
+    } else {
+        const int j = idx - nV;
+        const int r = j / L, x = j - r * L;
+        const int y = r * TH + TH - 1;
+        if ((bondS[(size_t)blockIdx.y * words + (size_t)y * wprL + (x >> 5)] >> (x & 31)) & 1u)
+            uf_union(lab, y * L + x, (y + 1 == L ? 0 : y + 1) * L + x);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// a4 compress: label[i] = root(i); four sites per thread, 128-bit accesses; counts roots.
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(ROW_THREADS)
+k_compress_tiled(int* label, Rec* __restrict__ rec, const Ctl* __restrict__ ctl, int N, int nb) {
+    const int q = blockIdx.x * ROW_THREADS + threadIdx.x;       // quad index
+    int nroot = 0;
+    if (q * 4 < N) {
+        int* lab = label + (size_t)blockIdx.y * N;
+        int4 v = *reinterpret_cast<const int4*>(lab + q * 4);
+        int* pv = reinterpret_cast<int*>(&v);
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            int r = pv[k];
+            if (r == q * 4 + k) { ++nroot; continue; }
+            int p = lab[r];
+            while (p != r) { r = p; p = lab[r]; }
+            pv[k] = r;
+        }
+        *reinterpret_cast<int4*>(lab + q * 4) = v;
+    }
+    nroot = warp_sum_i(nroot);
+    if ((threadIdx.x & 31) == 0 && nroot)
+        atomic_add_ll(&rec[(size_t)ctl->slot * nb + blockIdx.y].ncl, nroot);
+}
+
+// sizes of the clusters that span tiles: every open tile-local piece adds its size to its root's
+// accumulator; the running total returned by the atomic peaks at the cluster's full size.
+// One warp per tile.  Labels are flat here.
+template <int CAP>
+__global__ void __launch_bounds__(ROW_THREADS)
+k_sizes_open(const int* __restrict__ label, int2* __restrict__ olist, const int* __restrict__ ocount,
+             int* __restrict__ gsize, Rec* __restrict__ rec, const Ctl* __restrict__ ctl,
+             int tiles, int N, int nb) {
+    const int tile = blockIdx.x * (ROW_THREADS / 32) + (threadIdx.x >> 5);
+    const int lane = threadIdx.x & 31;
+    int m = 0;
+    if (tile < tiles) {
+        const size_t t = (size_t)blockIdx.y * tiles + tile;
+        const int n = ocount[t];
+        for (int e = lane; e < n; e += 32) {
+            const int2 it = olist[t * CAP + e];
+            const int R = label[(size_t)blockIdx.y * N + it.x];
+            const int tot = atomicAdd(gsize + (size_t)blockIdx.y * N + R, it.y) + it.y;
+            m = max(m, tot);
+            olist[t * CAP + e].x = R;
+        }
+    }
+    m = warp_max_i(m);
+    if (lane == 0 && m) atomic_max_ll(&rec[(size_t)ctl->slot * nb + blockIdx.y].maxcl, m);
+}
+
+template <int CAP>
+__global__ void __launch_bounds__(ROW_THREADS)
+k_sizes_reset(const int2* __restrict__ olist, const int* __restrict__ ocount, int* __restrict__ gsize,
+              int tiles, int N) {
+    const int tile = blockIdx.x * (ROW_THREADS / 32) + (threadIdx.x >> 5);
+    const int lane = threadIdx.x & 31;
+    if (tile >= tiles) return;
+    const size_t t = (size_t)blockIdx.y * tiles + tile;
+    const int n = ocount[t];
+    for (int e = lane; e < n; e += 32) gsize[(size_t)blockIdx.y * N + olist[t * CAP + e].x] = 0;
+}
+
+// ---------------------------------------------------------------------------------------------
+// a6 assignment, PAPER.md:57 (section 2.4): 16 sites per thread; labels are flat.
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(ROW_THREADS)
+k_flip_rows(int8_t* __restrict__ spins, const int* __restrict__ label, const uint32_t* __restrict__ D,
+            Rec* __restrict__ rec, const Ctl* __restrict__ ctl, int N, int words, int nb) {
+    const int g = blockIdx.x * ROW_THREADS + threadIdx.x;       // group of 16 sites
+    int m = 0;
+    if (g * 16 < N) {
+        const int* lab = label + (size_t)blockIdx.y * N + (size_t)g * 16;
+        const uint32_t* d = D + (size_t)blockIdx.y * words;
+        uint32_t out[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const uint4 v = ld_stream_u4(lab + q * 4);
+            const uint32_t r[4] = { v.x, v.y, v.z, v.w };
+            uint32_t o = 0;
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const uint32_t up = (__ldg(d + (r[k] >> 5)) >> (r[k] & 31)) & 1u;
+                o |= (up ? 0x01u : 0xFFu) << (8 * k);
+                m += up ? 1 : -1;
+            }
+            out[q] = o;
+        }
+        st_stream_u4(spins + (size_t)blockIdx.y * N + (size_t)g * 16, make_uint4(out[0], out[1], out[2], out[3]));
+    }
+    m = warp_sum_i(m);
+    if ((threadIdx.x & 31) == 0 && m) atomic_add_ll(&rec[(size_t)ctl->slot * nb + blockIdx.y].M, m);
+}
+
+// ---------------------------------------------------------------------------------------------
+// a7 energy, PAPER.md:63 (section 2.5): E = -sum over East and South edges of s_i s_j
+//    = (#edges) - 2 (#equal pairs); 32 sites per thread from sign masks.
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(ROW_THREADS)
+k_energy_rows(const int8_t* __restrict__ spins, Rec* __restrict__ rec, const Ctl* __restrict__ ctl,
+              int L, int N, int words, int nb) {
+    const int w = blockIdx.x * ROW_THREADS + threadIdx.x;
+    int e = 0;
+    if (w < words) {
+        const int wpr = L >> 5;
+        const int y = w / wpr, xw = w - y * wpr;
+        const int8_t* s = spins + (size_t)blockIdx.y * N;
+        const int8_t* row  = s + (size_t)y * L + xw * 32;
+        const int8_t* rowS = s + (size_t)(y + 1 == L ? 0 : y + 1) * L + xw * 32;
+        const uint4 a0 = *reinterpret_cast<const uint4*>(row),  a1 = *reinterpret_cast<const uint4*>(row + 16);
+        const uint4 b0 = *reinterpret_cast<const uint4*>(rowS), b1 = *reinterpret_cast<const uint4*>(rowS + 16);
+        const int8_t nx = s[(size_t)y * L + (xw + 1 == wpr ? 0 : (xw + 1) * 32)];
+        const uint32_t own = neg_mask32(a0, a1), south = neg_mask32(b0, b1);
+        const uint32_t eastm = (own >> 1) | (nx < 0 ? 0x80000000u : 0u);
+        e = 64 - 2 * (__popc(~(own ^ eastm)) + __popc(~(own ^ south)));
+    }
+    e = warp_sum_i(e);
+    if ((threadIdx.x & 31) == 0 && e) atomic_add_ll(&rec[(size_t)ctl->slot * nb + blockIdx.y].E, e);
+}
+
+} // namespace sw

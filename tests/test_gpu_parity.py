@@ -1,0 +1,333 @@
+"""GPU <-> oracle parity (-m gpu): the CUDA path through the C ABI against the serial oracle, element by
+element on the same seeded inputs.  Bar (north_star): bit-exact spins, bond planes, labels and integer
+observables after every sweep; double observables within 1e-12 relative.
+"""
+import math
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+import oracle
+import invariants as inv
+from paper_2302_14720_b200 import workloads as wl
+
+T_C = wl.T_C
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2302_14720_b200 import binding
+    binding.lib()
+    return binding
+
+
+def _obs_tuple(o):
+    return (o.energy, o.magnetisation, o.n_clusters, o.largest_cluster)
+
+
+def _check_double_obs(o, N):
+    e = o.energy / N
+    m = abs(o.magnetisation) / N
+    assert abs(o.e_per_site - e) <= 1e-12 * max(1.0, abs(e))
+    assert abs(o.abs_m_per_site - m) <= 1e-12 * max(1.0, abs(m))
+
+
+def _compare_sweeps(B, L, T, seed, n, path=0, start=None, t0=0, every=1):
+    """n sweeps on the GPU, one at a time, each compared in full with the oracle."""
+    sw = B.SwendsenWang(L, T, seed, path=path)
+    N = L * L
+    if start is None:
+        s = oracle.init_random(L, seed)
+        assert np.array_equal(sw.spins_host()[0], s), "random start differs"
+    else:
+        s = np.asarray(start, dtype=np.int8)
+        sw.set_spins(s)
+    if t0:
+        sw.set_sweep_index(t0)
+    assert sw.threshold() == oracle.threshold(T)
+    for k in range(n):
+        t = t0 + k
+        s1, bE, bS, lab, obs = oracle.sweep(L, T, seed, t, s)
+        sw.sweep(1)
+        if k % every == 0 or k == n - 1:
+            gE, gS = sw.bonds_host()
+            assert np.array_equal(gE[0], wl.pack_bits(bE)), f"bondE differs at sweep {t}"
+            assert np.array_equal(gS[0], wl.pack_bits(bS)), f"bondS differs at sweep {t}"
+            assert np.array_equal(sw.labels_host()[0], lab), f"labels differ at sweep {t}"
+            assert np.array_equal(sw.spins_host()[0], s1), f"spins differ at sweep {t}"
+            o = sw.observables()[0]
+            assert _obs_tuple(o) == obs, f"observables differ at sweep {t}: {_obs_tuple(o)} vs {obs}"
+            assert o.sweep == t + 1
+            _check_double_obs(o, N)
+        s = s1
+    sw.close()
+
+
+# ------------------------------------------------------------------------------------------------
+def test_philox_on_device_matches_oracle_and_known_answers(B):
+    rng = np.random.default_rng(1)
+    ctr = rng.integers(0, 2 ** 32, size=(4096, 4), dtype=np.uint64).astype(np.uint32)
+    key = rng.integers(0, 2 ** 32, size=(4096, 2), dtype=np.uint64).astype(np.uint32)
+    ctr[0] = 0; key[0] = 0
+    ctr[1] = 0xFFFFFFFF; key[1] = 0xFFFFFFFF
+    ctr[2] = [0x243f6a88, 0x85a308d3, 0x13198a2e, 0x03707344]; key[2] = [0xa4093822, 0x299f31d0]
+    out = B.sw_test_philox(ctr, key)
+    assert out[0].tolist() == [0x6627e8d5, 0xe169c58d, 0xbc57ac4c, 0x9b00dbd8]
+    assert out[1].tolist() == [0x408f276d, 0x41c83b0e, 0xa20bc7c6, 0x6d5451fd]
+    assert out[2].tolist() == [0xd16cfe09, 0x94fdcceb, 0x5001e420, 0x24126ea1]
+    for i in range(0, 4096, 37):
+        assert out[i].tolist() == oracle.philox4x32_10(ctr[i], key[i]).tolist()
+
+
+def test_thresholds_match_oracle(B):
+    for T in (0.05, 1.5, 2.0, 2.269, 2.26919, T_C, 2.5, 3.0, 3.5, 10.0, 1e6, 1e12):
+        sw = B.SwendsenWang(8, T, 1)
+        assert sw.threshold() == oracle.threshold(T)
+        sw.close()
+
+
+@pytest.mark.parametrize("L", [2, 3, 4, 5, 8, 13, 31, 33, 64, 100])
+def test_generic_path_every_sweep(B, L):
+    for T, seed in ((1.5, 7), (T_C, 8), (3.5, 9)):
+        _compare_sweeps(B, L, T, seed + L, 8, path=1)
+
+
+@pytest.mark.parametrize("L,path", [(64, 0), (128, 0), (192, 0), (256, 0), (256, 2), (320, 0), (512, 0), (512, 2), (768, 3)])
+def test_tiled_path_every_sweep(B, L, path):
+    for T, seed in ((2.0, 1), (T_C, 2), (3.0, 3)):
+        _compare_sweeps(B, L, T, seed + L, 6, path=path)
+
+
+def test_config1_L64_many_sweeps(B):
+    # BASELINE configs[0]: L = 64, T = 2.26919, seed 2024 -- every sweep for the first 200, in full
+    _compare_sweeps(B, 64, wl.T_C_PRINTED, 2024, 200)
+
+
+def test_survey_golden_vector_on_gpu(B):
+    sw = B.SwendsenWang(4, 2.269, 12345)
+    assert "".join("+" if v > 0 else "-" for v in sw.spins_host()[0]) == "+------+-+++++--"
+    sw.sweep(1)
+    assert sw.labels_host()[0].tolist() == [0, 1, 2, 2, 4, 4, 4, 7, 4, 0, 7, 7, 0, 0, 2, 2]
+    assert _obs_tuple(sw.observables()[0]) == (-16, -10, 5, 4)
+    sw.sweep(2)
+    assert _obs_tuple(sw.observables()[0]) == (-16, -10, 4, 11)
+    assert sw.series()[:, 0, :].tolist() == [[-20, -12, 5, 10], [-16, -10, 4, 11]]
+    sw.close()
+
+
+@pytest.mark.parametrize("L,path", [(64, 0), (256, 0), (256, 2), (100, 1)])
+def test_special_starts(B, L, path):
+    for name, s0 in (("cold", wl.spins_cold(L)), ("down", wl.spins_all_down(L)),
+                     ("checker", wl.spins_checkerboard(L)), ("hstripes", wl.spins_stripes(L, 1)),
+                     ("vstripes", wl.spins_stripes(L, 1, vertical=True)), ("blocks", wl.spins_blocks(L, 24)),
+                     ("wide", wl.spins_stripes(L, 5))):
+        for T in (0.05, T_C, 1e12):      # all bonds / critical / no bonds
+            _compare_sweeps(B, L, T, 5, 2, path=path, start=s0)
+
+
+def _label_patterns(L):
+    yield "none", wl.bonds_none(L)
+    yield "all", wl.bonds_all(L)
+    yield "row_wrap", wl.bonds_row_wrap(L, L - 1)
+    yield "col_wrap", wl.bonds_col_wrap(L, L - 1)
+    yield "row0", wl.bonds_row_wrap(L, 0)
+    yield "comb", wl.bonds_comb(L)
+    yield "spiral", wl.bonds_spiral(L)
+    for k, d in enumerate((0.2, 0.45, 0.5, 0.55, 0.8)):
+        yield f"random{d}", wl.bonds_random(L, 7 * L + k, d)
+
+
+@pytest.mark.parametrize("L,path", [(64, 0), (128, 0), (256, 0), (256, 2), (320, 0), (100, 1), (512, 0)])
+def test_labelling_of_injected_bond_graphs(B, L, path):
+    """Labelling alone on adversarial bond graphs (long thin spiral, comb, wrap-around rows)."""
+    sw = B.SwendsenWang(L, 2.0, 1, path=path)
+    for name, (bE, bS) in _label_patterns(L):
+        got = B.sw_test_label(sw.h, wl.pack_bits(bE), wl.pack_bits(bS))
+        ref = oracle.labels(L, bE, bS)
+        assert np.array_equal(got, ref), f"{name}: {np.count_nonzero(got != ref)} labels differ"
+    sw.close()
+
+
+def test_race_order_independence(B):
+    """Same state, same sweep index, repeated: identical bits every time (min-index labels)."""
+    L, T, seed = 512, T_C, 3
+    sw = B.SwendsenWang(L, T, seed)
+    sw.sweep(5)
+    s5 = sw.spins_host().copy()
+    ref = None
+    for rep in range(5):
+        sw.set_spins(s5)
+        sw.set_sweep_index(5)
+        sw.sweep(1)
+        cur = (sw.labels_host().copy(), sw.spins_host().copy(), _obs_tuple(sw.observables()[0]))
+        if ref is None:
+            ref = cur
+        assert np.array_equal(cur[0], ref[0]) and np.array_equal(cur[1], ref[1]) and cur[2] == ref[2]
+    sw.close()
+
+
+def test_multi_sweep_call_equals_single_sweeps_and_series(B):
+    L, T, seed, n = 128, T_C, 11, 40
+    _, ser = oracle.run(L, T, seed, n)
+    sw = B.SwendsenWang(L, T, seed)
+    sw.sweep(n)
+    got = sw.series()
+    assert got.shape == (n, 1, 4) and np.array_equal(got[:, 0, :], ser)
+    assert _obs_tuple(sw.observables()[0]) == tuple(ser[-1])
+    sfin, _ = oracle.run(L, T, seed, n, series=False)
+    assert np.array_equal(sw.spins_host()[0], sfin)
+    sw.close()
+
+
+def test_series_ring_keeps_the_last_sweeps(B):
+    L, T, seed, n, cap = 64, 2.5, 4, 50, 16
+    _, ser = oracle.run(L, T, seed, n)
+    sw = B.SwendsenWang(L, T, seed)
+    B.sw_set_series_capacity(sw.h, cap)
+    sw.sweep(n)
+    got = sw.series()
+    assert got.shape == (cap, 1, 4) and np.array_equal(got[:, 0, :], ser[-cap:])
+    sw.close()
+
+
+def test_batch_of_independent_lattices(B):
+    """BASELINE configs[4] in small: several temperatures and seeds in one launch per stage."""
+    L, Ts, seeds, n = 256, [1.5, T_C, 3.5, 2.0], [1000, 1012, 1031, 5], 12
+    sw = B.SwendsenWang(L, Ts, seeds)
+    refs = [oracle.init_random(L, s) for s in seeds]
+    got0 = sw.spins_host()
+    for b in range(len(Ts)):
+        assert np.array_equal(got0[b], refs[b])
+        assert sw.threshold(b) == oracle.threshold(Ts[b])
+    for t in range(n):
+        sw.sweep(1)
+        gs, gl = sw.spins_host(), sw.labels_host()
+        gE, gS = sw.bonds_host()
+        obs = sw.observables()
+        for b in range(len(Ts)):
+            s1, bE, bS, lab, o = oracle.sweep(L, Ts[b], seeds[b], t, refs[b])
+            assert np.array_equal(gE[b], wl.pack_bits(bE)) and np.array_equal(gS[b], wl.pack_bits(bS))
+            assert np.array_equal(gl[b], lab) and np.array_equal(gs[b], s1)
+            assert _obs_tuple(obs[b]) == o
+            refs[b] = s1
+    sw.close()
+
+
+def test_batch_generic_path_odd_side(B):
+    L, Ts, seeds = 27, [2.0, T_C, 3.0], [1, 2, 3]
+    sw = B.SwendsenWang(L, Ts, seeds)
+    refs = [oracle.init_random(L, s) for s in seeds]
+    for t in range(6):
+        sw.sweep(1)
+        gs, gl = sw.spins_host(), sw.labels_host()
+        obs = sw.observables()
+        for b in range(3):
+            s1, bE, bS, lab, o = oracle.sweep(L, Ts[b], seeds[b], t, refs[b])
+            assert np.array_equal(gl[b], lab) and np.array_equal(gs[b], s1) and _obs_tuple(obs[b]) == o
+            refs[b] = s1
+    sw.close()
+
+
+def test_resume_from_checkpoint(B):
+    L, T, seed = 192, T_C, 21
+    a = B.SwendsenWang(L, T, seed)
+    a.sweep(7)
+    s7 = a.spins_host().copy()
+    a.sweep(5)
+    b = B.SwendsenWang(L, T, seed)
+    b.set_spins(s7)
+    b.set_sweep_index(7)
+    b.sweep(5)
+    assert np.array_equal(a.spins_host(), b.spins_host()) and a.sweep_index == b.sweep_index == 12
+    assert _obs_tuple(a.observables()[0]) == _obs_tuple(b.observables()[0])
+    # 64-bit sweep index reaches the counter's third word
+    t_big = (1 << 32) + 3
+    b.set_spins(s7); b.set_sweep_index(t_big); b.sweep(1)
+    s1, *_ , o = oracle.sweep(L, T, seed, t_big, s7[0])
+    assert np.array_equal(b.spins_host()[0], s1) and _obs_tuple(b.observables()[0]) == o
+    a.close(); b.close()
+
+
+def test_observables_before_any_sweep_and_after_set_spins(B):
+    L = 96
+    sw = B.SwendsenWang(L, 2.0, 5, path=1)
+    s = oracle.init_random(L, 5)
+    o = sw.observables()[0]
+    E, M, _, _ = oracle.observables(L, s)
+    assert (o.energy, o.magnetisation, o.n_clusters, o.largest_cluster, o.sweep) == (E, M, 0, 0, 0)
+    sw.set_cold()
+    o = sw.observables()[0]
+    assert (o.energy, o.magnetisation) == (-2 * L * L, L * L) and o.e_per_site == -2.0 and o.abs_m_per_site == 1.0
+    with pytest.raises(B.SwError):
+        sw.labels()
+    with pytest.raises(B.SwError):
+        sw.bonds()
+    sw.close()
+
+
+def test_argument_errors(B):
+    for bad in ((1, 2.0), (0, 2.0), (32769, 2.0), (8, 0.0), (8, -1.0), (8, float("nan")), (8, float("inf"))):
+        with pytest.raises(B.SwError):
+            B.sw_create(bad[0], bad[1], 1)
+    assert B.sw_workspace_bytes(1, 1) == 0 and B.sw_workspace_bytes(8, 0) == 0
+    h = B.sw_create(8, 2.0, 1)
+    with pytest.raises(B.SwError):
+        B.sw_sweep(h, -1)
+    B.sw_sweep(h, 0)
+    B.sw_destroy(h)
+    B.sw_destroy(None)
+
+
+# ---- one-step parity at the sizes the bench times ----------------------------------
+def _one_step(B, sw, L, T, seed):
+    t = sw.sweep_index
+    s = sw.spins_host()[0].copy()
+    sw.sweep(1)
+    s1, bE, bS, lab, obs = oracle.sweep(L, T, seed, t, s)
+    gE, gS = sw.bonds_host()
+    assert np.array_equal(gE[0], wl.pack_bits(bE)) and np.array_equal(gS[0], wl.pack_bits(bS))
+    assert np.array_equal(sw.labels_host()[0], lab)
+    assert np.array_equal(sw.spins_host()[0], s1)
+    o = sw.observables()[0]
+    assert _obs_tuple(o) == obs
+    _check_double_obs(o, L * L)
+
+
+@pytest.mark.parametrize("L,T,seed,start", [(1024, 2.0, 1, "random"), (1024, wl.T_C_PRINTED, 2, "random"),
+                                            (1024, 3.0, 3, "random"), (2048, T_C, 1012, "random"),
+                                            (4096, T_C, 4, "cold"), (4096, T_C, 5, "random")])
+def test_one_step_parity_configs_2_3_5(B, L, T, seed, start):
+    sw = B.SwendsenWang(L, T, seed)
+    if start == "cold":
+        sw.set_cold()
+    _one_step(B, sw, L, T, seed)          # t = 0
+    _one_step(B, sw, L, T, seed)          # t = 1
+    sw.sweep(30)
+    _one_step(B, sw, L, T, seed)          # t = 32, after the clusters have grown
+    sw.close()
+
+
+def test_one_step_parity_headline_L16384(B):
+    """BASELINE configs[3]: L = 16384, T_c, seed 6 -- in the launch configuration bench.py times."""
+    L, T, seed = 16384, T_C, 6
+    sw = B.SwendsenWang(L, T, seed)
+    _one_step(B, sw, L, T, seed)          # t = 0
+    sw.sweep(6)
+    _one_step(B, sw, L, T, seed)          # t = 7
+    sw.close()
+
+
+def test_invariants_hold_at_size_without_the_oracle(B):
+    """Properties that hold at any size, checked with numpy/scipy only (L = 2048 after 50 sweeps)."""
+    L, T, seed = 2048, T_C, 77
+    sw = B.SwendsenWang(L, T, seed)
+    sw.sweep(50)
+    before = sw.spins_host()[0].copy()
+    sw.sweep(1)
+    gE, gS = sw.bonds_host()
+    bE, bS = wl.unpack_bits(gE[0], L * L), wl.unpack_bits(gS[0], L * L)
+    o = sw.observables()[0]
+    inv.check_sweep(L, before, bE, bS, sw.labels_host()[0], sw.spins_host()[0], _obs_tuple(o))
+    sw.close()
