@@ -1,0 +1,328 @@
+#!/usr/bin/env python
+"""bench.py -- the headline measurement of BASELINE.json: site-updates/s of a full Swendsen-Wang sweep
+on the 2D periodic Ising lattice L = 16384 at T_c (configs[3]), and the achieved fraction of the HBM
+roofline, on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--L 16384] [--impl ours|reference]
+
+A "step" is ONE full sweep (bonds -> labels -> assignment -> observables) of the whole lattice.
+Prints ONE JSON line (rank 0).  N > 1 (torchrun): every rank owns an independent lattice with its own
+seed (the path shards as replicas: SURVEY.md 8(e)); no data-path collective; "scaling": "weak".
+
+--impl reference times the serial CPU oracle (oracle/), as it stands, on the host cores.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "site_updates_per_s_full_sw_sweep"
+UNIT = "site-updates/s"
+
+# Algorithmic bytes per site and per kernel launch (SURVEY.md 8(d) byte model).
+# label stage = tile_label + merge + compress = 0.25 + 4 + 8 + 8(1/TW + 1/TH); the sweep model is the
+# survey's 18.75 B/site (bond 1.25 + label 12.25 + flip 5.25; observables count 0: they can be fused).
+def kernel_bytes_per_site(tw: int, th: int):
+    return {
+        "bond": 1.25,                      # int8 spin read + 2 bond bits written
+        "tile_label": 4.25,                # 2 bond bits read + int32 label written
+        "merge": 8.0 * (1.0 / tw + 1.0 / th),
+        "compress": 8.0,                   # label read + label written
+        "sizes_open": 0.0, "sizes_reset": 0.0,
+        "flipbits": 0.125,                 # decision bit-plane written
+        "flip": 5.125,                     # label read + spin written + decision bit gathered
+        "energy": 1.0,                     # spin read
+        "advance": 0.0,
+    }
+SWEEP_MODEL_BYTES_PER_SITE = 18.75
+STAGE_MODEL = {"bond": 1.25, "label": 12.25, "flip": 5.25, "observe": 1.0}
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            j = json.load(open(p))
+            return float(j["hbm_gbs"]), "measured (MEASURED_PEAKS.json, device copy)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def ncu_traffic(kernel: str):
+    """Per-launch DRAM bytes of `kernel` from the committed ncu --set full summary, or None."""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(p):
+        try:
+            return json.load(open(p)).get(kernel)
+        except Exception:
+            return None
+    return None
+
+
+class ClockSampler:
+    QUERY = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+             "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+             "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(gpu_index), f"--query-gpu={self.QUERY}",
+                                       "--format=csv,noheader,nounits", "-lms", "100"],
+                                      stdout=self.f, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush(); self.f.seek(0)
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.f.read().splitlines():
+            c = [t.strip() for t in line.split(",")]
+            if len(c) < 9:
+                continue
+            try:
+                sm.append(float(c[1])); mx.append(float(c[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, c[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        self.f.close()
+        try:
+            os.unlink(self.f.name)
+        except OSError:
+            pass
+        if sm:
+            out.update(sm_mhz=statistics.median(sm), sm_max_mhz=max(mx), reasons=sorted(reasons), samples=len(sm))
+        return out
+
+
+def cpu_oracle_baseline(L_sample: int, T: float, seed: int, sweeps: int):
+    """The serial oracle, as it stands, on one host core: site-updates/s on a bounded sample."""
+    import oracle
+    oracle.lib()
+    s = oracle.init_random(L_sample, seed)
+    t0 = time.perf_counter()
+    oracle.run(L_sample, T, seed, sweeps, spins=s, series=False)
+    dt = time.perf_counter() - t0
+    return L_sample * L_sample * sweeps / dt, dt
+
+
+def run_reference(args):
+    """--impl reference: the oracle timed on the host cores (rank 0 only)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    import oracle
+    from paper_2302_14720_b200 import workloads as wl
+    oracle.lib()
+    Ls = args.ref_L
+    T, seed = wl.T_C, 6
+    s = oracle.init_random(Ls, seed)
+    t = 0
+    for _ in range(args.warmup):
+        s, _ = oracle.run(Ls, T, seed, 1, spins=s, t0=t, series=False); t += 1
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        s, _ = oracle.run(Ls, T, seed, 1, spins=s, t0=t, series=False); t += 1
+    dt = time.perf_counter() - t0
+    val = Ls * Ls * args.steps / dt
+    sample = (f"each step = one full sweep of an L={Ls} lattice at T_c (a {Ls}x{Ls} sample of the "
+              f"L={args.L} workload), serial C oracle, gcc -O2, 1 thread")
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int8/int32",
+        "data": "synthetic",
+        "config": {"workload": f"2D Ising SW sweep, L={args.L}, T=T_c, random start (BASELINE configs[3])",
+                   "reference_sample_L": Ls},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }))
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--L", type=int, default=16384)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--ref-L", type=int, default=2048, help="sample lattice side for --impl reference")
+    ap.add_argument("--cpu-sample-L", type=int, default=8192, help="sample side for the cpu_baseline leg")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--path", type=int, default=0, help="0 auto, 1 generic, 2 tiles 64x64, 3 tiles 256x32")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3)
+
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import numpy as np
+    import torch
+    from paper_2302_14720_b200 import binding as B, workloads as wl
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback); use --impl reference for the oracle")
+    B.lib()
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        torch.cuda.set_device(local)
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+    dev = torch.device(f"cuda:{local}")
+    torch.cuda.set_device(dev)
+
+    L, T, K, W = args.L, wl.T_C, args.steps, args.warmup
+    N = L * L
+    seed = 6 + rank                                   # configs[3] uses seed 6; replicas take 6 + rank
+    sw = B.SwendsenWang(L, T, seed, device=str(dev), path=args.path)
+    tw, th = (256, 32) if (L % 256 == 0 and args.path in (0, 3)) else (64, 64)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    # ---- device-resident measurement: W warm-up sweeps, then exactly K sweeps in one sw_sweep call
+    sw.sweep(W)
+    torch.cuda.synchronize(dev)
+    sw.set_stage_timing(True)                         # per-kernel CUDA events inside the timed region
+    stream = torch.cuda.current_stream(dev)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    clocks = ClockSampler(local)
+    time.sleep(0.3)
+    barrier()
+    e0.record(stream)
+    sw.sweep(K)
+    e1.record(stream)
+    barrier()
+    ms = e0.elapsed_time(e1)
+    time.sleep(0.2)
+    clk = clocks.stop()
+    launches = sw.launch_count()
+    kms = sw.kernel_ms()
+    stage = sw.stage_ms()
+    timed = min(K, 1024)
+    sw.set_stage_timing(False)
+    obs = sw.observables()[0]
+
+    if dist is not None:
+        tms = torch.tensor([ms], device=dev, dtype=torch.float64)
+        dist.all_reduce(tms, op=dist.ReduceOp.MAX)
+        ms = float(tms.item())
+    value = world * N * K / (ms * 1e-3)
+
+    # ---- end to end through the C ABI with HOST buffers: H2D spins, one sweep, D2H spins + observables
+    e2e = None
+    if not args.no_e2e:
+        host = torch.empty(N, dtype=torch.int8).pin_memory()
+        B.sw_get_spins(sw.h, host.data_ptr())
+        Ke = min(K, 20)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(Ke):
+            B.sw_set_spins(sw.h, host.data_ptr(), True)        # host -> device, N bytes
+            B.sw_sweep(sw.h, 1)
+            B.sw_get_spins(sw.h, host.data_ptr())              # device -> host, N bytes (synchronises)
+            o = B.sw_observables(sw.h)[0]                      # + the step's observables
+        barrier()
+        dt = time.perf_counter() - t0
+        if dist is not None:
+            tdt = torch.tensor([dt], device=dev, dtype=torch.float64)
+            dist.all_reduce(tdt, op=dist.ReduceOp.MAX)
+            dt = float(tdt.item())
+        e2e = {"value": world * N * Ke / dt, "unit": UNIT, "h2d_bytes_per_step": N,
+               "d2h_bytes_per_step": N + 56, "steps": Ke, "ms_per_step": 1e3 * dt / Ke}
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return 0
+
+    # ---- roofline of the dominant kernel, per-stage split
+    peak, peak_src = measured_peaks()
+    kb = kernel_bytes_per_site(tw, th)
+    dom = max(kms, key=lambda k: kms[k])
+    dom_ms = kms[dom] / timed
+    achieved = kb.get(dom, 0.0) * N / (dom_ms * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": achieved / peak, "traffic": ncu_traffic(dom), "peak_source": peak_src,
+                "bytes_per_site": kb.get(dom), "ms_per_launch": dom_ms,
+                "share_of_step": kms[dom] / max(1e-9, sum(kms.values()))}
+    stages = {}
+    for s, v in stage.items():
+        sms = v / timed
+        stages[s] = {"ms": sms, "site_updates_per_s": N / (sms * 1e-3) if sms > 0 else None,
+                     "model_bytes_per_site": STAGE_MODEL[s],
+                     "hbm_frac": (STAGE_MODEL[s] * N / (sms * 1e-3) / 1e9 / peak) if sms > 0 else None}
+    kernels = {k: {"ms": v / timed, "GBps_model": (kb.get(k, 0.0) * N / (v / timed * 1e-3) / 1e9) if v > 0 else None}
+               for k, v in kms.items()}
+    sweep_gbs = SWEEP_MODEL_BYTES_PER_SITE * N / (ms / K * 1e-3) / 1e9
+
+    cpu = None
+    if not args.no_cpu_baseline:
+        Ls = min(args.cpu_sample_L, L)
+        v, dt = cpu_oracle_baseline(Ls, T, 6, 1)
+        cpu = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle",
+               "sample": f"1 full sweep (t=0, random start) of an L={Ls} lattice at T_c, {dt:.1f} s of CPU work, "
+                         f"serial C oracle (gcc -O2), 1 of {os.cpu_count()} host cores"}
+
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+        "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "int8 spins / int32 labels / uint32 Philox", "data": "synthetic",
+        "config": {"workload": f"2D Ising Swendsen-Wang, L={L} periodic, J=1, T=T_c=2/ln(1+sqrt2), random start "
+                               f"seed {6}+rank, one sweep per step (BASELINE configs[3])",
+                   "sites_per_gpu": N, "tile": f"{tw}x{th}", "parallelism": f"replicas x{world}",
+                   "l2_policy": "inputs larger than L2 (1.3 GB of spins+labels per sweep vs 126 MB L2)",
+                   "state_after": {"sweep": int(obs.sweep), "e_per_site": obs.e_per_site,
+                                   "abs_m_per_site": obs.abs_m_per_site, "n_clusters": int(obs.n_clusters),
+                                   "largest_cluster": int(obs.largest_cluster)}},
+        "clocks": clk,
+        "e2e": e2e,
+        "gpu_launches": int(launches),
+        "roofline": roofline,
+        "sweep_model": {"bytes_per_site": SWEEP_MODEL_BYTES_PER_SITE, "achieved_GBps": sweep_gbs,
+                        "frac_of_peak": sweep_gbs / peak, "frac_of_8TBps_nominal": sweep_gbs / 8000.0},
+        "stages": stages, "kernels": kernels,
+        "cpu_baseline": cpu,
+        "paper_context": "paper: 17x (SW) / 90x (Wolff) over serial, Haswell E5-2695 vs Tesla P100; "
+                         "SW GPU rate 1.25e8 site-updates/s at L=4096 (PAPER.md:127,142)",
+    }
+    print(json.dumps(out))
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

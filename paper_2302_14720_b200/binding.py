@@ -60,6 +60,8 @@ PROTOTYPES = {
     "sw_set_series_capacity": (C.c_int, [_VP, _I64]),
     "sw_set_stage_timing": (C.c_int, [_VP, C.c_int]),
     "sw_stage_ms": (C.c_int, [_VP, C.POINTER(C.c_float)]),
+    "sw_kernel_ms": (C.c_int, [_VP, C.POINTER(C.c_float), _I32]),
+    "sw_kernel_name": (C.c_char_p, [_I32]),
     "sw_set_path": (C.c_int, [_VP, C.c_int]),
     "sw_last_launch_count": (_I64, [_VP]),
     "sw_threshold": (_U32, [_VP, _I32]),
@@ -205,6 +207,11 @@ def sw_stage_ms(h):
     _check(lib().sw_stage_ms(_ptr(h), out))
     return dict(zip(("bond", "label", "flip", "observe"), (float(v) for v in out)))
 
+def sw_kernel_ms(h):
+    out = (C.c_float * 32)()
+    n = _check(lib().sw_kernel_ms(_ptr(h), out, 32))
+    return {lib().sw_kernel_name(i).decode(): float(out[i]) for i in range(n)}
+
 def sw_set_path(h, path: int) -> None:
     _check(lib().sw_set_path(_ptr(h), path))
 
@@ -324,6 +331,9 @@ class SwendsenWang:
 
     def stage_ms(self):
         return sw_stage_ms(self.h)
+
+    def kernel_ms(self):
+        return sw_kernel_ms(self.h)
 
     def threshold(self, b: int = 0) -> int:
         return sw_threshold(self.h, b)

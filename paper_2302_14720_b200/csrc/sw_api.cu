@@ -40,8 +40,13 @@ void set_err(const char* fmt, ...) {
 
 constexpr size_t ALIGN = 256;
 constexpr int64_t DEFAULT_SERIES_CAP = 4096;
-constexpr int MAX_TIMED_SWEEPS = 4096;
-constexpr int EV_PER_SWEEP = 5;
+constexpr int MAX_TIMED_SWEEPS = 1024;
+// kernel slots for per-kernel event timing (sw_kernel_ms); one event before each launch + one at the end
+enum Kid { K_BOND = 0, K_TILE, K_MERGE, K_COMPRESS, K_SIZES, K_SIZES_RESET, K_FLIPBITS, K_FLIP, K_ENERGY, K_ADVANCE, K_COUNT };
+const char* const KERNEL_NAMES[K_COUNT] = { "bond", "tile_label", "merge", "compress", "sizes_open", "sizes_reset",
+                                            "flipbits", "flip", "energy", "advance" };
+const int KERNEL_STAGE[K_COUNT] = { 0, 1, 1, 1, 1, 1, 2, 2, 3, 3 };     // bond, label, flip, observe
+constexpr int EV_PER_SWEEP = K_COUNT + 1;
 
 inline size_t align_up(size_t v) { return (v + ALIGN - 1) / ALIGN * ALIGN; }
 
@@ -77,7 +82,7 @@ Layout make_layout(int L, int nb) {
     o.lat = p;     p = align_up(p + (size_t)nb * sizeof(Lat));
     o.ctl = p;     p = align_up(p + sizeof(Ctl));
     o.rec_now = p; p = align_up(p + (size_t)nb * sizeof(Rec));
-    o.series = p;  p = align_up(p + (size_t)DEFAULT_SERIES_CAP * nb * sizeof(Rec));
+    o.series = p;  p = align_up(p + (size_t)(DEFAULT_SERIES_CAP + 1) * nb * sizeof(Rec));
     o.total = p;
     return o;
 }
@@ -104,7 +109,9 @@ struct sw_handle {
     int8_t* spins = nullptr; uint32_t *bondE = nullptr, *bondS = nullptr, *D = nullptr;
     int *label = nullptr, *gsize = nullptr, *ocount = nullptr; int2* olist = nullptr;
     Lat* lat = nullptr; Ctl* ctl = nullptr; Rec* rec_now = nullptr;
-    Rec* series = nullptr; Rec* series_owned = nullptr; int64_t series_cap = DEFAULT_SERIES_CAP;
+    Rec* series = nullptr; Rec* series_owned = nullptr;
+    int64_t series_cap = DEFAULT_SERIES_CAP;       // sweeps retained; the ring has series_cap + 1 slots
+    int64_t ring() const { return series_cap + 1; }  // (the slot after the last sweep is already zeroed)
     std::vector<Lat> hlat;
     uint64_t t = 0;
     cudaStream_t stream = nullptr;
@@ -113,6 +120,8 @@ struct sw_handle {
     int64_t last_n = 0;
     int path = 0; TileKind tile = TILE_NONE;
     bool timing = false; std::vector<cudaEvent_t> ev; int64_t timed_sweeps = 0;
+    int ev_cursor = 0; std::vector<int> ev_seq;   // kernel ids in launch order within one sweep
+    int64_t cur_sweep = 0;
     int64_t launches = 0;
 };
 
@@ -128,6 +137,15 @@ TileKind pick_tile(int L, int path) {
 }
 
 inline dim3 grid1(size_t n, int threads, int nb) { return dim3((unsigned)((n + threads - 1) / threads), (unsigned)nb); }
+
+// timing mode: an event before kernel `kid` of sweep h->cur_sweep (kid == K_COUNT closes the sweep)
+int mark(sw_handle* h, int kid) {
+    if (!h->timing || h->cur_sweep >= MAX_TIMED_SWEEPS) return SW_OK;
+    if (h->cur_sweep == 0) h->ev_seq.push_back(kid);
+    SW_CUDA(cudaEventRecord(h->ev[(size_t)h->cur_sweep * EV_PER_SWEEP + h->ev_cursor++], h->stream));
+    return SW_OK;
+}
+#define SW_MARK(h, kid) do { int rc_ = mark((h), (kid)); if (rc_) return rc_; } while (0)
 
 template <int TW, int TH>
 size_t tile_smem_bytes() {
@@ -145,15 +163,20 @@ int launch_label_tiled(sw_handle* h) {
         SW_CUDA(cudaFuncSetAttribute(k_tile_label<TW, TH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         attr_done = true;
     }
+    SW_MARK(h, K_TILE);
     k_tile_label<TW, TH><<<dim3(tiles, h->nb), C::THREADS, smem, h->stream>>>(
         h->label, h->bondE, h->bondS, h->olist, h->ocount, h->series, h->ctl, h->L, h->N, h->words, h->nb);
     const size_t nedge = (size_t)h->L * (h->L / TW + h->L / TH);
+    SW_MARK(h, K_MERGE);
     k_merge_tiled<TW, TH><<<grid1(nedge, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
         h->label, h->bondE, h->bondS, h->L, h->N, h->words);
+    SW_MARK(h, K_COMPRESS);
     k_compress_tiled<<<grid1((size_t)h->N / 4, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
         h->label, h->series, h->ctl, h->N, h->nb);
+    SW_MARK(h, K_SIZES);
     k_sizes_open<C::CAP><<<grid1((size_t)tiles * 32, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
         h->label, h->olist, h->ocount, h->gsize, h->series, h->ctl, tiles, h->N, h->nb);
+    SW_MARK(h, K_SIZES_RESET);
     k_sizes_reset<C::CAP><<<grid1((size_t)tiles * 32, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
         h->olist, h->ocount, h->gsize, tiles, h->N);
     h->launches += 5;
@@ -161,11 +184,15 @@ int launch_label_tiled(sw_handle* h) {
 }
 
 int launch_label_generic(sw_handle* h) {
+    SW_MARK(h, K_TILE);
     k_label_init<<<grid1(h->N, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(h->label, h->N);
+    SW_MARK(h, K_MERGE);
     k_union_generic<<<grid1(h->N, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(
         h->label, h->bondE, h->bondS, h->L, h->N, h->words);
+    SW_MARK(h, K_COMPRESS);
     k_compress_generic<<<grid1(h->N, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(
         h->label, h->gsize, h->series, h->ctl, h->N, h->nb);
+    SW_MARK(h, K_SIZES);
     k_maxsize_generic<<<grid1(h->N, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(
         h->label, h->gsize, h->series, h->ctl, h->N, h->nb);
     h->launches += 4;
@@ -180,17 +207,12 @@ int launch_label(sw_handle* h) {
     }
 }
 
-int record(sw_handle* h, int64_t k, int which) {
-    if (!h->timing || k >= MAX_TIMED_SWEEPS) return SW_OK;
-    SW_CUDA(cudaEventRecord(h->ev[(size_t)k * EV_PER_SWEEP + which], h->stream));
-    return SW_OK;
-}
-
 // one full sweep on h->stream; the sweep index and series slot are read on the device from h->ctl
 int launch_sweep(sw_handle* h, int64_t k) {
     int rc;
-    if ((rc = record(h, k, 0))) return rc;
+    h->cur_sweep = k; h->ev_cursor = 0;
     // a1 bonds
+    SW_MARK(h, K_BOND);
     if (h->tile != TILE_NONE)
         k_bond_rows<<<grid1(h->words, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
             h->spins, h->bondE, h->bondS, h->lat, h->ctl, h->L, h->N, h->words);
@@ -198,13 +220,13 @@ int launch_sweep(sw_handle* h, int64_t k) {
         k_bond_generic<<<grid1(h->words, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(
             h->spins, h->bondE, h->bondS, h->lat, h->ctl, h->L, h->N, h->words);
     h->launches += 1;
-    if ((rc = record(h, k, 1))) return rc;
     // a2-a4 labels (+ cluster count, largest cluster)
     if ((rc = launch_label(h))) return rc;
-    if ((rc = record(h, k, 2))) return rc;
     // a5-a6 assignment
+    SW_MARK(h, K_FLIPBITS);
     k_flipbits<<<grid1(((size_t)h->words + 3) / 4, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(
         h->D, h->lat, h->ctl, h->words);
+    SW_MARK(h, K_FLIP);
     if (h->tile != TILE_NONE)
         k_flip_rows<<<grid1((size_t)h->N / 16, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
             h->spins, h->label, h->D, h->series, h->ctl, h->N, h->words, h->nb);
@@ -212,17 +234,18 @@ int launch_sweep(sw_handle* h, int64_t k) {
         k_flip_generic<<<grid1(h->N, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(
             h->spins, h->label, h->D, h->N, h->words);
     h->launches += 2;
-    if ((rc = record(h, k, 3))) return rc;
     // a7 observables of the new configuration
+    SW_MARK(h, K_ENERGY);
     if (h->tile != TILE_NONE)
         k_energy_rows<<<grid1(h->words, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
             h->spins, h->series, h->ctl, h->L, h->N, h->words, h->nb);
     else
         k_observe_generic<<<grid1(h->N, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(
             h->spins, h->series, h->ctl, 1, h->L, h->N, h->nb);
+    SW_MARK(h, K_ADVANCE);
     k_advance<<<1, 64, 0, h->stream>>>(h->ctl, h->series, h->nb);
     h->launches += 2;
-    if ((rc = record(h, k, 4))) return rc;
+    SW_MARK(h, K_COUNT);
     return SW_OK;
 }
 
@@ -244,8 +267,8 @@ int init_handle(sw_handle* h, const double* T, const uint64_t* seed) {
     }
     SW_CUDA(cudaMemcpyAsync(h->lat, h->hlat.data(), sizeof(Lat) * h->nb, cudaMemcpyHostToDevice, h->stream));
     SW_CUDA(cudaMemsetAsync(h->gsize, 0, (size_t)h->nb * h->N * 4, h->stream));
-    SW_CUDA(cudaMemsetAsync(h->series, 0, (size_t)h->series_cap * h->nb * sizeof(Rec), h->stream));
-    k_set_ctl<<<1, 1, 0, h->stream>>>(h->ctl, 0ull, 0u, (uint32_t)h->series_cap);
+    SW_CUDA(cudaMemsetAsync(h->series, 0, (size_t)h->ring() * h->nb * sizeof(Rec), h->stream));
+    k_set_ctl<<<1, 1, 0, h->stream>>>(h->ctl, 0ull, 0u, (uint32_t)h->ring());
     k_init_random<<<grid1(h->words, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(h->spins, h->lat, h->N, h->words);
     SW_CUDA(cudaGetLastError());
     SW_CUDA(cudaStreamSynchronize(h->stream));       // hlat is read by the async copy
@@ -329,12 +352,16 @@ int sw_sweep(sw_handle* h, int64_t n) {
     if (!h || n < 0) { set_err("sw_sweep: invalid argument"); return SW_EINVAL; }
     if (n == 0) return SW_OK;
     h->launches = 0;
-    if (h->timing && h->ev.empty()) {
-        h->ev.resize((size_t)MAX_TIMED_SWEEPS * EV_PER_SWEEP);
-        for (auto& e : h->ev) SW_CUDA(cudaEventCreate(&e));
+    if (h->timing) {
+        const size_t need = (size_t)std::min<int64_t>(n, MAX_TIMED_SWEEPS) * EV_PER_SWEEP;
+        while (h->ev.size() < need) {
+            cudaEvent_t e; SW_CUDA(cudaEventCreate(&e));
+            h->ev.push_back(e);
+        }
+        h->ev_seq.clear();
     }
     SW_CUDA(cudaMemsetAsync(h->series, 0, (size_t)h->nb * sizeof(Rec), h->stream));
-    k_set_ctl<<<1, 1, 0, h->stream>>>(h->ctl, (unsigned long long)h->t, 0u, (uint32_t)h->series_cap);
+    k_set_ctl<<<1, 1, 0, h->stream>>>(h->ctl, (unsigned long long)h->t, 0u, (uint32_t)h->ring());
     h->launches += 1;
     for (int64_t k = 0; k < n; ++k) {
         int rc = launch_sweep(h, k);
@@ -370,7 +397,7 @@ int sw_observables(sw_handle* h, sw_obs* out) {
     if (!h || !out) { set_err("sw_observables: null argument"); return SW_EINVAL; }
     std::vector<Rec> r(h->nb);
     if (h->rec_valid) {
-        const int64_t slot = (h->last_n - 1) % h->series_cap;
+        const int64_t slot = (h->last_n - 1) % h->ring();
         SW_CUDA(cudaMemcpyAsync(r.data(), h->series + (size_t)slot * h->nb, sizeof(Rec) * h->nb,
                                 cudaMemcpyDeviceToHost, h->stream));
     } else {
@@ -390,12 +417,12 @@ int64_t sw_series(sw_handle* h, sw_obs* out, int64_t cap) {
     if (!h->rec_valid) return 0;
     const int64_t kept = std::min(h->last_n, h->series_cap);
     const int64_t give = std::min(kept, cap);
-    std::vector<Rec> r((size_t)h->series_cap * h->nb);
+    std::vector<Rec> r((size_t)h->ring() * h->nb);
     SW_CUDA(cudaMemcpyAsync(r.data(), h->series, r.size() * sizeof(Rec), cudaMemcpyDeviceToHost, h->stream));
     SW_CUDA(cudaStreamSynchronize(h->stream));
     const int64_t first = h->last_n - kept;          // index (within the call) of the oldest retained sweep
     for (int64_t k = 0; k < give; ++k) {
-        const int64_t slot = (first + k) % h->series_cap;
+        const int64_t slot = (first + k) % h->ring();
         for (int b = 0; b < h->nb; ++b)
             fill_obs(h, r[(size_t)slot * h->nb + b], h->t - (uint64_t)h->last_n + (uint64_t)(first + k) + 1,
                      out + (size_t)k * h->nb + b);
@@ -407,7 +434,7 @@ int sw_set_series_capacity(sw_handle* h, int64_t sweeps) {
     if (!h || sweeps < 1 || sweeps > (1ll << 26)) { set_err("sw_set_series_capacity: invalid argument"); return SW_EINVAL; }
     SW_CUDA(cudaStreamSynchronize(h->stream));
     Rec* p = nullptr;
-    cudaError_t e = cudaMalloc((void**)&p, (size_t)sweeps * h->nb * sizeof(Rec));
+    cudaError_t e = cudaMalloc((void**)&p, (size_t)(sweeps + 1) * h->nb * sizeof(Rec));
     if (e != cudaSuccess) { (void)cudaGetLastError(); set_err("sw_set_series_capacity: cudaMalloc failed"); return SW_ENOMEM; }
     if (h->series_owned) cudaFree(h->series_owned);
     h->series_owned = p; h->series = p; h->series_cap = sweeps;
@@ -470,17 +497,30 @@ int sw_set_stage_timing(sw_handle* h, int on) {
     return SW_OK;
 }
 
+int sw_kernel_ms(sw_handle* h, float* out, int32_t cap) {
+    if (!h || !out || cap < 0) { set_err("sw_kernel_ms: invalid argument"); return SW_EINVAL; }
+    for (int i = 0; i < cap; ++i) out[i] = 0.f;
+    if (h->timed_sweeps == 0) { set_err("sw_kernel_ms: the last sw_sweep ran without stage timing"); return SW_ESTATE; }
+    SW_CUDA(cudaStreamSynchronize(h->stream));
+    const int ns = (int)h->ev_seq.size();            // launches per sweep + the closing mark
+    for (int64_t k = 0; k < h->timed_sweeps; ++k)
+        for (int j = 0; j + 1 < ns; ++j) {
+            float ms = 0.f;
+            SW_CUDA(cudaEventElapsedTime(&ms, h->ev[(size_t)k * EV_PER_SWEEP + j], h->ev[(size_t)k * EV_PER_SWEEP + j + 1]));
+            if (h->ev_seq[j] < cap) out[h->ev_seq[j]] += ms;
+        }
+    return K_COUNT;
+}
+
+const char* sw_kernel_name(int32_t i) { return (i >= 0 && i < K_COUNT) ? KERNEL_NAMES[i] : ""; }
+
 int sw_stage_ms(sw_handle* h, float out[4]) {
     if (!h || !out) { set_err("sw_stage_ms: null argument"); return SW_EINVAL; }
     out[0] = out[1] = out[2] = out[3] = 0.f;
-    if (h->timed_sweeps == 0) { set_err("sw_stage_ms: the last sw_sweep ran without stage timing"); return SW_ESTATE; }
-    SW_CUDA(cudaStreamSynchronize(h->stream));
-    for (int64_t k = 0; k < h->timed_sweeps; ++k)
-        for (int s = 0; s < 4; ++s) {
-            float ms = 0.f;
-            SW_CUDA(cudaEventElapsedTime(&ms, h->ev[(size_t)k * EV_PER_SWEEP + s], h->ev[(size_t)k * EV_PER_SWEEP + s + 1]));
-            out[s] += ms;
-        }
+    float k[K_COUNT];
+    const int rc = sw_kernel_ms(h, k, K_COUNT);
+    if (rc < 0) return rc;
+    for (int i = 0; i < K_COUNT; ++i) out[KERNEL_STAGE[i]] += k[i];
     return SW_OK;
 }
 
@@ -517,7 +557,7 @@ int sw_test_label(sw_handle* h, const uint32_t* bondE, const uint32_t* bondS, in
     SW_CUDA(cudaMemcpyAsync(h->bondE, bondE, (size_t)h->words * 4, cudaMemcpyHostToDevice, h->stream));
     SW_CUDA(cudaMemcpyAsync(h->bondS, bondS, (size_t)h->words * 4, cudaMemcpyHostToDevice, h->stream));
     SW_CUDA(cudaMemsetAsync(h->series, 0, sizeof(Rec), h->stream));
-    k_set_ctl<<<1, 1, 0, h->stream>>>(h->ctl, (unsigned long long)h->t, 0u, (uint32_t)h->series_cap);
+    k_set_ctl<<<1, 1, 0, h->stream>>>(h->ctl, (unsigned long long)h->t, 0u, (uint32_t)h->ring());
     int rc = launch_label(h);
     if (rc) return rc;
     SW_CUDA(cudaGetLastError());
