@@ -38,7 +38,7 @@ def kernel_bytes_per_site(tw: int, th: int):
         "tile_label": 4.25,                # 2 bond bits read + int32 label written
         "merge": 8.0 * (1.0 / tw + 1.0 / th),
         "compress": 8.0,                   # label read + label written
-        "sizes_open": 0.0, "sizes_reset": 0.0,
+        "roots_open": 0.0, "sizes_reset": 0.0,
         "flipbits": 0.125,                 # decision bit-plane written
         "flip": 5.125,                     # label read + spin written + decision bit gathered
         "energy": 1.0,                     # spin read

@@ -43,7 +43,7 @@ constexpr int64_t DEFAULT_SERIES_CAP = 4096;
 constexpr int MAX_TIMED_SWEEPS = 1024;
 // kernel slots for per-kernel event timing (sw_kernel_ms); one event before each launch + one at the end
 enum Kid { K_BOND = 0, K_TILE, K_MERGE, K_COMPRESS, K_SIZES, K_SIZES_RESET, K_FLIPBITS, K_FLIP, K_ENERGY, K_ADVANCE, K_COUNT };
-const char* const KERNEL_NAMES[K_COUNT] = { "bond", "tile_label", "merge", "compress", "sizes_open", "sizes_reset",
+const char* const KERNEL_NAMES[K_COUNT] = { "bond", "tile_label", "merge", "compress", "roots_open", "sizes_reset",
                                             "flipbits", "flip", "energy", "advance" };
 const int KERNEL_STAGE[K_COUNT] = { 0, 1, 1, 1, 1, 1, 2, 2, 3, 3 };     // bond, label, flip, observe
 constexpr int EV_PER_SWEEP = K_COUNT + 1;
@@ -170,12 +170,12 @@ int launch_label_tiled(sw_handle* h) {
     SW_MARK(h, K_MERGE);
     k_merge_tiled<TW, TH><<<grid1(nedge, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
         h->label, h->bondE, h->bondS, h->L, h->N, h->words);
+    SW_MARK(h, K_SIZES);
+    k_roots_open<C::CAP><<<grid1((size_t)tiles * 32, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
+        h->label, h->olist, h->ocount, h->gsize, h->series, h->ctl, tiles, h->N, h->nb);
     SW_MARK(h, K_COMPRESS);
     k_compress_tiled<<<grid1((size_t)h->N / 4, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
         h->label, h->series, h->ctl, h->N, h->nb);
-    SW_MARK(h, K_SIZES);
-    k_sizes_open<C::CAP><<<grid1((size_t)tiles * 32, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
-        h->label, h->olist, h->ocount, h->gsize, h->series, h->ctl, tiles, h->N, h->nb);
     SW_MARK(h, K_SIZES_RESET);
     k_sizes_reset<C::CAP><<<grid1((size_t)tiles * 32, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
         h->olist, h->ocount, h->gsize, tiles, h->N);

@@ -8,8 +8,9 @@
 //                       index of the tile-local root; tile-local cluster sizes; the list of "open"
 //                       clusters (those with a bond across the tile edge)
 //   a3 k_merge_tiled    one thread per tile-edge bond: atomicMin hooking on the global parent array
-//   a4 k_compress_tiled label[i] = root(i), 128-bit loads/stores; counts roots
-//      k_sizes_open     sizes of clusters that span tiles (closed clusters were maximised in a2)
+//      k_roots_open     points every hooked tile root at its global root; sizes of clusters that span
+//                       tiles (closed clusters were maximised in a2)
+//   a4 k_compress_tiled label[i] = label[label[i]] (two hops), 128-bit loads/stores; counts roots
 //   a5 k_flipbits       (sw_generic.cuh) decision bit-plane
 //   a6 k_flip_rows      spins = gather(D, label); magnetisation
 //   a7 k_energy_rows    energy of the new configuration from sign masks + popc
@@ -73,18 +74,27 @@ struct TileCfg {
     static_assert(TW % 32 == 0 && RW % 32 == 0, "tile shape");
 };
 
-__device__ __forceinline__ int s_find(volatile int* lab, int x) {
+// Shared-memory union-find.  Roots are hooked "larger under smaller" with a CAS that only succeeds
+// on a node that is still a root, so a parent is always a smaller index, trees never split, and
+// non-root parents change only through path halving (to an ancestor) -- safe under any interleaving.
+__device__ __forceinline__ int s_find(int* lab_, int x) {
+    volatile int* lab = lab_;
     int p = lab[x];
-    while (p != x) { x = p; p = lab[x]; }
+    while (p != x) {
+        const int g = lab[p];
+        if (g == p) return p;
+        lab[x] = g;                      // path halving
+        x = g; p = lab[x];
+    }
     return x;
 }
 __device__ __forceinline__ void s_union(int* lab, int a, int b) {
     a = s_find(lab, a); b = s_find(lab, b);
     while (a != b) {
-        if (a < b) { int s = a; a = b; b = s; }
-        const int old = atomicMin(lab + a, b);
-        if (old == a) break;
-        a = old;
+        if (a < b) { int s = a; a = b; b = s; }           // a is the larger root
+        const int old = atomicCAS(lab + a, a, b);
+        if (old == a) break;                               // hooked
+        a = s_find(lab, old);                              // a had been hooked meanwhile: climb on
     }
 }
 
@@ -131,13 +141,11 @@ k_tile_label(int* __restrict__ label, const uint32_t* __restrict__ bondE, const 
     __syncthreads();
 
     // phase 1: every site starts at the head of its horizontal run inside its 32-site word
-    int head_off[C::RW_PER_WARP];
 #pragma unroll
     for (int k = 0; k < C::RW_PER_WARP; ++k) {
         const int rw = warp + 32 * k;
         const uint32_t e = eW[rw];
         const int ones = lane ? __clz(~(e << (32 - lane))) : 0;      // bonded sites directly to my left
-        head_off[k] = ones;
         const int row = rw / C::WPR, wx = rw - row * C::WPR;
         const int l = row * TW + wx * 32 + lane;
         lab[l] = l - ones;
@@ -154,15 +162,14 @@ k_tile_label(int* __restrict__ label, const uint32_t* __restrict__ bondE, const 
         const int l = row * TW + wx * 32 + lane;
         if (lane == 0 && wx > 0 && (eW[rw - 1] >> 31)) s_union(lab, l - 1, l);
         if (row < TH - 1) {
-            const uint32_t s = sW[rw];
-            const uint32_t need = s & ~((s & eW[rw] & eW[rw + C::WPR]) << 1);
+            const uint32_t sb = sW[rw];
+            const uint32_t need = sb & ~((sb & eW[rw] & eW[rw + C::WPR]) << 1);
             if ((need >> lane) & 1u) s_union(lab, l, l + TW);
         }
     }
     __syncthreads();
 
-    // phase 3: roots, sizes (one shared atomic per run head), global labels
-    int root[C::RW_PER_WARP];
+    // phase 3: flatten (lab[l] = root), sizes (one shared atomic per run head), global labels
     int* glab = label + (size_t)blockIdx.y * N;
 #pragma unroll
     for (int k = 0; k < C::RW_PER_WARP; ++k) {
@@ -170,9 +177,11 @@ k_tile_label(int* __restrict__ label, const uint32_t* __restrict__ bondE, const 
         const int row = rw / C::WPR, wx = rw - row * C::WPR;
         const int l = row * TW + wx * 32 + lane;
         const int r = s_find(lab, l);
-        root[k] = r;
-        if (head_off[k] == 0) {
-            const uint32_t tbits = ~(eW[rw] >> lane);                 // first 0 above me ends the run
+        lab[l] = r;
+        const uint32_t e = eW[rw];
+        const bool head = lane == 0 || !((e >> (lane - 1)) & 1u);
+        if (head) {
+            const uint32_t tbits = ~(e >> lane);                      // first 0 above me ends the run
             const int len = min(tbits ? __ffs(tbits) : 33, 32 - lane);
             atomicAdd(&cnt[r], len);
         }
@@ -191,7 +200,7 @@ k_tile_label(int* __restrict__ label, const uint32_t* __restrict__ bondE, const 
         if (wx == 0 && lane == 0 && wIn[row]) open = true;
         if (row == TH - 1 && ((sW[rw] >> lane) & 1u)) open = true;
         if (row == 0 && ((nIn[wx] >> lane) & 1u)) open = true;
-        if (open) atomicOr(reinterpret_cast<unsigned int*>(&cnt[root[k]]), OPEN_FLAG);
+        if (open) atomicOr(reinterpret_cast<unsigned int*>(&cnt[lab[row * TW + wx * 32 + lane]]), OPEN_FLAG);
     }
     __syncthreads();
 
@@ -203,7 +212,7 @@ k_tile_label(int* __restrict__ label, const uint32_t* __restrict__ bondE, const 
         const int rw = warp + 32 * k;
         const int row = rw / C::WPR, wx = rw - row * C::WPR;
         const int l = row * TW + wx * 32 + lane;
-        if (root[k] == l) {
+        if (lab[l] == l) {
             const uint32_t c = (uint32_t)cnt[l];
             if (c & OPEN_FLAG) {
                 const int pos = atomicAdd(&s_nopen, 1);
@@ -251,6 +260,8 @@ k_merge_tiled(int* label, const uint32_t* __restrict__ bondE, const uint32_t* __
 
 // ---------------------------------------------------------------------------------------------
 // a4 compress: label[i] = root(i); four sites per thread, 128-bit accesses; counts roots.
+// k_roots_open has already pointed every hooked tile root at its global root, so every site is at
+// most two hops from it: site -> tile root -> global root.  No loops, no divergence.
 // ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(ROW_THREADS)
 k_compress_tiled(int* label, Rec* __restrict__ rec, const Ctl* __restrict__ ctl, int N, int nb) {
@@ -259,28 +270,23 @@ k_compress_tiled(int* label, Rec* __restrict__ rec, const Ctl* __restrict__ ctl,
     if (q * 4 < N) {
         int* lab = label + (size_t)blockIdx.y * N;
         int4 v = *reinterpret_cast<const int4*>(lab + q * 4);
-        int* pv = reinterpret_cast<int*>(&v);
-#pragma unroll
-        for (int k = 0; k < 4; ++k) {
-            int r = pv[k];
-            if (r == q * 4 + k) { ++nroot; continue; }
-            int p = lab[r];
-            while (p != r) { r = p; p = lab[r]; }
-            pv[k] = r;
-        }
-        *reinterpret_cast<int4*>(lab + q * 4) = v;
+        const int t0 = lab[v.x], t1 = lab[v.y], t2 = lab[v.z], t3 = lab[v.w];   // tile root's parent
+        nroot = (v.x == q * 4) + (v.y == q * 4 + 1) + (v.z == q * 4 + 2) + (v.w == q * 4 + 3);
+        if (t0 != v.x || t1 != v.y || t2 != v.z || t3 != v.w)
+            *reinterpret_cast<int4*>(lab + q * 4) = make_int4(t0, t1, t2, t3);
     }
     nroot = warp_sum_i(nroot);
     if ((threadIdx.x & 31) == 0 && nroot)
         atomic_add_ll(&rec[(size_t)ctl->slot * nb + blockIdx.y].ncl, nroot);
 }
 
-// sizes of the clusters that span tiles: every open tile-local piece adds its size to its root's
-// accumulator; the running total returned by the atomic peaks at the cluster's full size.
-// One warp per tile.  Labels are flat here.
+// After the merge: every open tile-local root is pointed straight at its global root (find + write
+// back), and the sizes of the clusters that span tiles are accumulated: each open piece adds its size
+// to its root's accumulator; the running total returned by the atomic peaks at the full size.
+// One warp per tile.
 template <int CAP>
 __global__ void __launch_bounds__(ROW_THREADS)
-k_sizes_open(const int* __restrict__ label, int2* __restrict__ olist, const int* __restrict__ ocount,
+k_roots_open(int* label, int2* __restrict__ olist, const int* __restrict__ ocount,
              int* __restrict__ gsize, Rec* __restrict__ rec, const Ctl* __restrict__ ctl,
              int tiles, int N, int nb) {
     const int tile = blockIdx.x * (ROW_THREADS / 32) + (threadIdx.x >> 5);
@@ -288,10 +294,16 @@ k_sizes_open(const int* __restrict__ label, int2* __restrict__ olist, const int*
     int m = 0;
     if (tile < tiles) {
         const size_t t = (size_t)blockIdx.y * tiles + tile;
+        int* lab = label + (size_t)blockIdx.y * N;
         const int n = ocount[t];
         for (int e = lane; e < n; e += 32) {
             const int2 it = olist[t * CAP + e];
-            const int R = label[(size_t)blockIdx.y * N + it.x];
+            const int p = ld_cg(lab + it.x);
+            int R = p;
+            if (p != it.x) {                                // hooked: walk to the root, point at it
+                R = uf_find(lab, p);
+                if (R != p) lab[it.x] = R;                  // only ever an ancestor: safe while others walk
+            }
             const int tot = atomicAdd(gsize + (size_t)blockIdx.y * N + R, it.y) + it.y;
             m = max(m, tot);
             olist[t * CAP + e].x = R;
