@@ -43,6 +43,8 @@ def kernel_bytes_per_site(tw: int, th: int):
         "flip": 5.125,                     # label read + spin written + decision bit gathered
         "energy": 1.0,                     # spin read
         "advance": 0.0,
+        "bond_label": 5.25,                # a1 + a2 fused: spin read + 2 bond bits written + int32 label written
+        "flip_tile": 5.125,                # a4 + a6 + a7 fused: label read + spin written + decision bit gathered
     }
 SWEEP_MODEL_BYTES_PER_SITE = 18.75
 STAGE_MODEL = {"bond": 1.25, "label": 12.25, "flip": 5.25, "observe": 1.0}
@@ -174,7 +176,7 @@ def main():
     ap.add_argument("--cpu-sample-L", type=int, default=8192, help="sample side for the cpu_baseline leg")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--path", type=int, default=0, help="0 auto, 1 generic, 2 tiles 64x64, 3 tiles 256x32")
+    ap.add_argument("--path", type=int, default=0, help="0 auto (fused scan-line), 1 generic, 2/3 first-generation tiles 64x64 / 256x32, 4/5 scan 64/128 wide, 6 unfused")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
 
@@ -205,7 +207,10 @@ def main():
     N = L * L
     seed = 6 + rank                                   # configs[3] uses seed 6; replicas take 6 + rank
     sw = B.SwendsenWang(L, T, seed, device=str(dev), path=args.path)
-    tw, th = (256, 32) if (L % 256 == 0 and args.path in (0, 3)) else (64, 64)
+    if args.path in (0, 4, 5, 6):
+        tw, th = (64 if args.path == 4 else 128 if args.path == 5 else 256 if L % 256 == 0 else 128 if L % 128 == 0 else 64), 32
+    else:
+        tw, th = (256, 32) if (L % 256 == 0 and args.path == 3) else (64, 64)
 
     def barrier():
         if dist is not None:

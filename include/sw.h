@@ -95,7 +95,8 @@ void       sw_destroy(sw_handle* h);                       /* NULL is a no-op */
 int        sw_sweep(sw_handle* h, int64_t n);
 
 /* DEVICE pointer to nb*N int32: flat minimum-index labels of the last sweep, each lattice indexed
- * within itself.  Flattens lazily if the last sweep left a parent forest.  NULL + SW_ESTATE text
+ * within itself.  Flattens lazily (one extra kernel on the handle's stream) if the last sweep left the
+ * two-level forest site -> tile root -> cluster root; sw_set_eager_labels(h, 1) stores them every sweep instead.  NULL + SW_ESTATE text
  * before the first sweep.  PAPER.md:51. */
 const int32_t* sw_labels(sw_handle* h);
 
@@ -110,6 +111,7 @@ const int8_t* sw_spins(sw_handle* h);                      /* DEVICE ptr, nb*N i
  * (i>>5), i the site index; lattice b starts at word b*words_per_lattice, words_per_lattice =
  * ceil(N/32).  SW_ESTATE before the first sweep.  PAPER.md:39, Fig. 2. */
 int        sw_bonds(sw_handle* h, const uint32_t** bondE, const uint32_t** bondS);
+int        sw_set_eager_labels(sw_handle* h, int on);       /* default 0 */
 
 /* Replace the spins (cold start, injected states).  `spins`: nb*N int8 of +1/-1, on the device
  * (is_host = 0) or on the host (is_host = 1).  Values are not validated. */
@@ -137,12 +139,19 @@ int        sw_set_stage_timing(sw_handle* h, int on);
 int        sw_stage_ms(sw_handle* h, float out[4]);
 /* The same measurement per kernel: out[i] = ms of kernel slot i summed over the timed sweeps (at most the
  * first 1024 sweeps of the call), i < cap; returns the number of kernel slots (or a negative code).
- * sw_kernel_name(i) names slot i ("bond", "tile_label", "merge", "roots_open", "compress", ...; "" past the end). */
+ * sw_kernel_name(i) names slot i ("bond", "tile_label", "merge", "roots_open", "compress", "bond_label" (a1 + a2 fused),
+ * "flip_tile" (a4 + a6 + a7 fused), ...; "" past the end). */
 int        sw_kernel_ms(sw_handle* h, float* out, int32_t cap);
 const char* sw_kernel_name(int32_t i);
 
-/* Select the kernel path: 0 = automatic (tiled path when L is a multiple of 64, generic otherwise),
- * 1 = force the generic any-L path (global union-find, no tiles).  Results are identical. */
+/* Select the kernel path.  Results are identical on every path.
+ *   0  automatic: the fused scan-line path when L is a multiple of 64 (tiles of 256, 128 or 64 x 32 sites,
+ *      the widest that divides L), the generic path otherwise
+ *   1  generic any-L path (global union-find, no tiles)
+ *   2, 3  the first-generation tiled kernels (64 x 64 / 256 x 32 tiles, thread-per-site union-find), kept for A/B timing
+ *   4, 5  scan-line path forced to 64- / 128-wide tiles
+ *   6  as 0 but UNFUSED: stand-alone bond kernel, then labelling from the bond planes (per-stage timing of
+ *      bond / label / flip, BASELINE config 3) */
 int        sw_set_path(sw_handle* h, int path);
 
 /* Number of kernel launches issued by the last sw_sweep call (for bench.py's gpu_launches). */

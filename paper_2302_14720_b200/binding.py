@@ -63,6 +63,7 @@ PROTOTYPES = {
     "sw_kernel_ms": (C.c_int, [_VP, C.POINTER(C.c_float), _I32]),
     "sw_kernel_name": (C.c_char_p, [_I32]),
     "sw_set_path": (C.c_int, [_VP, C.c_int]),
+    "sw_set_eager_labels": (C.c_int, [_VP, C.c_int]),
     "sw_last_launch_count": (_I64, [_VP]),
     "sw_threshold": (_U32, [_VP, _I32]),
     "sw_L": (_I32, [_VP]),
@@ -214,6 +215,9 @@ def sw_kernel_ms(h):
 
 def sw_set_path(h, path: int) -> None:
     _check(lib().sw_set_path(_ptr(h), path))
+
+def sw_set_eager_labels(h, on: bool) -> None:
+    _check(lib().sw_set_eager_labels(_ptr(h), 1 if on else 0))
 
 def sw_last_launch_count(h) -> int:
     return int(lib().sw_last_launch_count(_ptr(h)))

@@ -4,6 +4,7 @@
 #include "sw_common.cuh"
 #include "sw_generic.cuh"
 #include "sw_tiled.cuh"
+#include "sw_scan.cuh"
 
 #include <algorithm>
 #include <cmath>
@@ -42,16 +43,20 @@ constexpr size_t ALIGN = 256;
 constexpr int64_t DEFAULT_SERIES_CAP = 4096;
 constexpr int MAX_TIMED_SWEEPS = 1024;
 // kernel slots for per-kernel event timing (sw_kernel_ms); one event before each launch + one at the end
-enum Kid { K_BOND = 0, K_TILE, K_MERGE, K_COMPRESS, K_SIZES, K_SIZES_RESET, K_FLIPBITS, K_FLIP, K_ENERGY, K_ADVANCE, K_COUNT };
+enum Kid { K_BOND = 0, K_TILE, K_MERGE, K_COMPRESS, K_SIZES, K_SIZES_RESET, K_FLIPBITS, K_FLIP, K_ENERGY, K_ADVANCE,
+           K_BONDLABEL, K_FLIPTILE, K_COUNT };
 const char* const KERNEL_NAMES[K_COUNT] = { "bond", "tile_label", "merge", "compress", "roots_open", "sizes_reset",
-                                            "flipbits", "flip", "energy", "advance" };
-const int KERNEL_STAGE[K_COUNT] = { 0, 1, 1, 1, 1, 1, 2, 2, 3, 3 };     // bond, label, flip, observe
+                                            "flipbits", "flip", "energy", "advance", "bond_label", "flip_tile" };
+// stage of each kernel: bond, label, flip, observe.  The fused kernels are booked under the stage that
+// dominates them: bond_label (a1 + a2) under "label", flip_tile (a4 + a6 + a7) under "flip".
+const int KERNEL_STAGE[K_COUNT] = { 0, 1, 1, 1, 1, 1, 2, 2, 3, 3, 1, 2 };
 constexpr int EV_PER_SWEEP = K_COUNT + 1;
 
 inline size_t align_up(size_t v) { return (v + ALIGN - 1) / ALIGN * ALIGN; }
 
 // tile shapes of the fast path
-enum TileKind { TILE_NONE = 0, TILE_64x64 = 1, TILE_256x32 = 2 };
+enum TileKind { TILE_NONE = 0, TILE_64x64 = 1, TILE_256x32 = 2, SCAN_2 = 3, SCAN_4 = 4, SCAN_8 = 5 };
+inline int scan_nw(TileKind k) { return k == SCAN_2 ? 2 : k == SCAN_4 ? 4 : k == SCAN_8 ? 8 : 0; }
 using Cfg64 = TileCfg<64, 64>;
 using Cfg256 = TileCfg<256, 32>;
 
@@ -64,9 +69,18 @@ size_t olist_entries(int L) {          // per lattice, maximum over the tile sha
     const size_t N = (size_t)L * L;
     if (L % 64 == 0) n = std::max(n, N / Cfg64::SITES * Cfg64::CAP);
     if (L % 256 == 0) n = std::max(n, N / Cfg256::SITES * Cfg256::CAP);
+    for (int nw : {2, 4, 8})                                   // scan tiles: 32 nw x 32 sites
+        if (L % (32 * nw) == 0) n = std::max(n, N / (32 * nw * SCAN_TH) * (size_t)(2 * (32 * nw + SCAN_TH)));
     return n;
 }
-size_t tiles_max(int L) { return L % 64 == 0 ? (size_t)L * L / Cfg64::SITES : 0; }
+size_t tiles_max(int L) { return L % 64 == 0 ? (size_t)L * L / (64 * SCAN_TH) : 0; }
+
+DivL make_div(int d) {          // q = (v * m) >> p is exact for 0 <= v < 2^30 (error term < 1/d)
+    int k = 0; while ((1 << k) < d) ++k;
+    DivL D; D.p = 30 + k; D.d = d;
+    D.m = (uint32_t)(((1ull << D.p) + (uint64_t)d - 1) / (uint64_t)d);
+    return D;
+}
 
 Layout make_layout(int L, int nb) {
     const size_t N = (size_t)L * L, words = (N + 31) / 32;
@@ -116,6 +130,8 @@ struct sw_handle {
     uint64_t t = 0;
     cudaStream_t stream = nullptr;
     bool have_sweep = false;       // labels / bonds / cluster observables of a sweep exist
+    bool labels_flat = false;      // label[] holds roots (else: site -> tile root -> global root)
+    bool eager_labels = false;     // the flip kernel also stores the flat labels every sweep
     bool rec_valid = false;        // the last series slot holds E, M of the current spins
     int64_t last_n = 0;
     int path = 0; TileKind tile = TILE_NONE;
@@ -131,8 +147,11 @@ TileKind pick_tile(int L, int path) {
     if (path == 1) return TILE_NONE;
     if (path == 2) return L % 64 == 0 ? TILE_64x64 : TILE_NONE;
     if (path == 3) return L % 256 == 0 ? TILE_256x32 : TILE_NONE;
-    if (L % 256 == 0) return TILE_256x32;
-    if (L % 64 == 0) return TILE_64x64;
+    if (path == 4) return L % 64 == 0 ? SCAN_2 : TILE_NONE;
+    if (path == 5) return L % 128 == 0 ? SCAN_4 : TILE_NONE;
+    if (L % 256 == 0) return SCAN_8;
+    if (L % 128 == 0) return SCAN_4;
+    if (L % 64 == 0) return SCAN_2;
     return TILE_NONE;
 }
 
@@ -175,11 +194,53 @@ int launch_label_tiled(sw_handle* h) {
         h->label, h->olist, h->ocount, h->gsize, h->series, h->ctl, tiles, h->N, h->nb);
     SW_MARK(h, K_COMPRESS);
     k_compress_tiled<<<grid1((size_t)h->N / 4, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
-        h->label, h->series, h->ctl, h->N, h->nb);
+        h->label, h->series, h->ctl, h->N, h->nb, 1);
     SW_MARK(h, K_SIZES_RESET);
     k_sizes_reset<C::CAP><<<grid1((size_t)tiles * 32, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
         h->olist, h->ocount, h->gsize, tiles, h->N);
     h->launches += 5;
+    return SW_OK;
+}
+
+// fast path: fused bond + scan-line tile labelling, global merge, open roots (a1-a3)
+template <int NW>
+int launch_bond_label_scan(sw_handle* h, bool fused) {
+    constexpr int TW = 32 * NW, CAP = 2 * (TW + SCAN_TH);
+    const int tiles = h->N / (TW * SCAN_TH);
+    if (fused) {
+        SW_MARK(h, K_BONDLABEL);
+        k_bond_label<NW, true><<<dim3(tiles, h->nb), 32 * NW, 0, h->stream>>>(
+            h->spins, h->bondE, h->bondS, h->label, h->olist, h->ocount, h->series, h->lat, h->ctl,
+            h->L, h->N, h->words, h->nb);
+    } else {
+        SW_MARK(h, K_TILE);
+        k_bond_label<NW, false><<<dim3(tiles, h->nb), 32 * NW, 0, h->stream>>>(
+            h->spins, h->bondE, h->bondS, h->label, h->olist, h->ocount, h->series, h->lat, h->ctl,
+            h->L, h->N, h->words, h->nb);
+    }
+    const size_t nedge = (size_t)h->L * (h->L / TW + h->L / SCAN_TH);
+    SW_MARK(h, K_MERGE);
+    k_merge_tiled<TW, SCAN_TH><<<grid1(nedge, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
+        h->label, h->bondE, h->bondS, h->L, h->N, h->words);
+    SW_MARK(h, K_SIZES);
+    k_roots_open<CAP><<<grid1((size_t)tiles * 32, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
+        h->label, h->olist, h->ocount, h->gsize, h->series, h->ctl, tiles, h->N, h->nb);
+    h->launches += 3;
+    return SW_OK;
+}
+// a4-a7 fused, then the size accumulators of the open clusters are cleared for the next sweep
+template <int NW>
+int launch_flip_scan(sw_handle* h) {
+    constexpr int TW = 32 * NW, CAP = 2 * (TW + SCAN_TH);
+    const int tiles = h->N / (TW * SCAN_TH);
+    SW_MARK(h, K_FLIPTILE);
+    k_flip_tile<NW><<<dim3(tiles, h->nb), 32 * NW, 0, h->stream>>>(
+        h->spins, h->label, h->D, h->series, h->ctl, make_div(h->L), h->L, h->N, h->words, h->nb,
+        h->eager_labels ? 1 : 0);
+    SW_MARK(h, K_SIZES_RESET);
+    k_sizes_reset<CAP><<<grid1((size_t)tiles * 32, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
+        h->olist, h->ocount, h->gsize, tiles, h->N);
+    h->launches += 2;
     return SW_OK;
 }
 
@@ -199,8 +260,28 @@ int launch_label_generic(sw_handle* h) {
     return SW_OK;
 }
 
+// labelling alone from the bond planes, leaving flat labels (the unfused order; sw_test_label)
+template <int NW>
+int launch_label_scan(sw_handle* h) {
+    constexpr int TW = 32 * NW, CAP = 2 * (TW + SCAN_TH);
+    const int tiles = h->N / (TW * SCAN_TH);
+    int rc = launch_bond_label_scan<NW>(h, false);
+    if (rc) return rc;
+    SW_MARK(h, K_COMPRESS);
+    k_compress_tiled<<<grid1((size_t)h->N / 4, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
+        h->label, h->series, h->ctl, h->N, h->nb, 1);
+    SW_MARK(h, K_SIZES_RESET);
+    k_sizes_reset<CAP><<<grid1((size_t)tiles * 32, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
+        h->olist, h->ocount, h->gsize, tiles, h->N);
+    h->launches += 2;
+    return SW_OK;
+}
+
 int launch_label(sw_handle* h) {
     switch (h->tile) {
+        case SCAN_2:      return launch_label_scan<2>(h);
+        case SCAN_4:      return launch_label_scan<4>(h);
+        case SCAN_8:      return launch_label_scan<8>(h);
         case TILE_64x64:  return launch_label_tiled<64, 64>(h);
         case TILE_256x32: return launch_label_tiled<256, 32>(h);
         default:          return launch_label_generic(h);
@@ -211,6 +292,31 @@ int launch_label(sw_handle* h) {
 int launch_sweep(sw_handle* h, int64_t k) {
     int rc;
     h->cur_sweep = k; h->ev_cursor = 0;
+    if (const int nw = scan_nw(h->tile)) {
+        const bool fused = h->path != 6;
+        if (!fused) {                                   // stand-alone a1 for the per-stage split
+            SW_MARK(h, K_BOND);
+            k_bond_rows<<<grid1(h->words, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
+                h->spins, h->bondE, h->bondS, h->lat, h->ctl, h->L, h->N, h->words);
+            h->launches += 1;
+        }
+        rc = nw == 8 ? launch_bond_label_scan<8>(h, fused) : nw == 4 ? launch_bond_label_scan<4>(h, fused)
+                                                                     : launch_bond_label_scan<2>(h, fused);
+        if (rc) return rc;
+        SW_MARK(h, K_FLIPBITS);
+        k_flipbits<<<grid1(((size_t)h->words + 3) / 4, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(
+            h->D, h->lat, h->ctl, h->words);
+        h->launches += 1;
+        rc = nw == 8 ? launch_flip_scan<8>(h) : nw == 4 ? launch_flip_scan<4>(h) : launch_flip_scan<2>(h);
+        if (rc) return rc;
+        SW_MARK(h, K_ADVANCE);
+        k_advance<<<1, 64, 0, h->stream>>>(h->ctl, h->series, h->nb);
+        h->launches += 1;
+        SW_MARK(h, K_COUNT);
+        h->labels_flat = h->eager_labels;
+        return SW_OK;
+    }
+    h->labels_flat = true;
     // a1 bonds
     SW_MARK(h, K_BOND);
     if (h->tile != TILE_NONE)
@@ -378,7 +484,13 @@ int sw_sweep(sw_handle* h, int64_t n) {
 const int32_t* sw_labels(sw_handle* h) {
     if (!h) { set_err("sw_labels: null handle"); return nullptr; }
     if (!h->have_sweep) { set_err("sw_labels: no sweep has run yet"); return nullptr; }
-    return h->label;            // every sweep leaves the labels flat
+    if (!h->labels_flat) {      // the fast path leaves site -> tile root -> global root: flatten on demand (a4)
+        k_compress_tiled<<<grid1((size_t)h->N / 4, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
+            h->label, h->series, h->ctl, h->N, h->nb, 0);
+        if (cudaGetLastError() != cudaSuccess) { set_err("sw_labels: flatten launch failed"); return nullptr; }
+        h->labels_flat = true;
+    }
+    return h->label;
 }
 
 int sw_bonds(sw_handle* h, const uint32_t** bondE, const uint32_t** bondS) {
@@ -525,9 +637,15 @@ int sw_stage_ms(sw_handle* h, float out[4]) {
 }
 
 int sw_set_path(sw_handle* h, int path) {
-    if (!h || path < 0 || path > 3) { set_err("sw_set_path: invalid argument"); return SW_EINVAL; }
+    if (!h || path < 0 || path > 6) { set_err("sw_set_path: invalid argument"); return SW_EINVAL; }
     h->path = path;
     h->tile = pick_tile(h->L, path);
+    return SW_OK;
+}
+
+int sw_set_eager_labels(sw_handle* h, int on) {
+    if (!h) { set_err("sw_set_eager_labels: null handle"); return SW_EINVAL; }
+    h->eager_labels = on != 0;
     return SW_OK;
 }
 

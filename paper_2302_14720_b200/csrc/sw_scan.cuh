@@ -1,0 +1,357 @@
+// sw_scan.cuh -- the fast path: fused bond formation + tile-local labelling by a warp scan-line,
+// and the fused assignment / energy kernel.  Lattice side a multiple of 64.
+//
+// Stage map; one CTA per tile of TW x 32 sites, TW = 32 * NW, one warp per 32-column strip:
+//   a1+a2 k_bond_label<NW>
+//       phase 1  (FMA-pipe bound)  one thread per 32-site word: sign masks of the int8 spins, 16 Philox4x32-10
+//                calls, bond words to shared memory and to the canonical global bit-planes; the bonds that
+//                enter the tile from its North and West neighbours are recomputed (TW/2 + 32 extra calls)
+//       phase 2  (MIO-pipe bound)  scan-line labelling, lane = column, rows in sequence, uniform control flow:
+//                runs of East bonds from bit tricks on the row's bond word; a run takes the label of the
+//                first of its sites that has a South bond from the row above (one shuffle), or opens a new
+//                label (its head's index); other sites of the run whose upper neighbour carries a different
+//                root unite the two roots (atomicMin hooking, larger under smaller)
+//       phase 3  strip seams: one lane per row unites across each East bond that crosses a strip edge
+//       phase 4  flatten (root of every site), global label = global index of the tile-local root, cluster
+//                sizes counted into the spare bits of the root's parent word, open flags
+//       phase 5  closed clusters -> running maximum; open clusters -> the tile's list (root, size)
+//   a3    k_merge_tiled / k_roots_open (sw_tiled.cuh): global boundary merge on the int32 parent array
+//   a4-a7 k_flip_tile<NW>: root of every site in two hops through a shared-memory copy of the tile's labels,
+//         spins = gather(D, root), magnetisation, cluster count, and the energy of the NEW configuration
+//         (the new spins of the East / South halo are resolved through their own roots)
+#pragma once
+#include "sw_common.cuh"
+
+namespace sw {
+
+constexpr int SCAN_TH = 32;                     // tile height = rows a warp walks
+constexpr uint32_t IDX_MASK = 0x1FFFu;          // tile-local site index: 13 bits (TW * 32 <= 8192)
+constexpr int CNT_SHIFT = 13;                   // cluster size (<= 8192: 14 bits) lives in bits 13..26 of a root's word
+constexpr uint32_t CNT_MASK = 0x3FFFu;
+constexpr uint32_t OPEN_BIT = 0x40000000u;      // bit 30: the cluster has a bond across the tile edge
+
+// find on the shared parent array; roots may carry size / open bits above IDX_MASK
+__device__ __forceinline__ int sc_find(const int* par, int x) {
+    int p = par[x] & (int)IDX_MASK;
+    while (p != x) { x = p; p = par[x] & (int)IDX_MASK; }
+    return x;
+}
+// unite the trees of a and b (any nodes); hooking "larger under smaller" with atomicMin so the root of a
+// component is its minimum index whatever the interleaving.  Only used before any size / flag bit is set.
+__device__ __forceinline__ void sc_union(int* par, int a, int b) {
+    while (a != b) {
+        if (a < b) { const int s = a; a = b; b = s; }      // a is the larger
+        const int old = atomicMin(par + a, b);
+        if (old == a) break;                                // a was a root: hooked under b
+        a = old;                                            // a had parent `old`: unite that with b
+    }
+}
+
+// exact v / d for 0 <= v < 2^30 with a host-made magic (m, p): q = (v * m) >> p
+struct DivL { uint32_t m; int p; int d; };
+__device__ __forceinline__ int div_l(int v, const DivL& D) {
+    return (int)(((unsigned long long)(uint32_t)v * D.m) >> D.p);
+}
+
+// FUSE = true: phase 1 draws the bonds (a1 fused into a2).  FUSE = false: phase 1 reads the bond planes
+// that k_bond_rows (or a test) wrote -- per-stage timing (BASELINE config 3) and labelling-only tests.
+template <int NW, bool FUSE>
+__global__ void __launch_bounds__(32 * NW)
+k_bond_label(const int8_t* __restrict__ spins, uint32_t* bondE, uint32_t* bondS,
+             int* __restrict__ label, int2* __restrict__ olist, int* __restrict__ ocount,
+             Rec* __restrict__ rec, const Lat* __restrict__ lat, const Ctl* __restrict__ ctl,
+             int L, int N, int words, int nb) {
+    constexpr int TW = 32 * NW, TH = SCAN_TH, SITES = TW * TH, THREADS = 32 * NW;
+    constexpr int CAP = 2 * (TW + TH);
+    __shared__ int par[SITES];                 // parent, tile-local index (+ size / open bits at roots)
+    __shared__ uint2 es[TH * NW];              // [row][strip] = (East word, South word)
+    __shared__ uint32_t nIn[NW];               // South bonds entering from the tile above, per strip
+    __shared__ uint32_t wIn;                   // East bonds entering from the tile to the West, bit = row
+    __shared__ int s_nopen, s_max;
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int tilesX = L / TW;
+    const int ty = blockIdx.x / tilesX, tx = blockIdx.x - ty * tilesX;
+    const int y0 = ty * TH, x0 = tx * TW;
+    const int wprL = L >> 5;
+    const int8_t* s = spins + (size_t)blockIdx.y * N;
+    const Lat la = lat[blockIdx.y];
+    const unsigned long long t = ctl->t;
+    const uint32_t tlo = (uint32_t)t, thi = (uint32_t)(t >> 32);
+
+    if (tid < NW) nIn[tid] = 0;
+    if (tid == 0) { wIn = 0; s_nopen = 0; s_max = 0; }
+    __syncthreads();
+
+    // ---- phase 1: bonds of the tile, PAPER.md:37-39 (section 2.1) --------------------------------------
+    if (!FUSE) {
+        const uint32_t* bE = bondE + (size_t)blockIdx.y * words;
+        const uint32_t* bS = bondS + (size_t)blockIdx.y * words;
+        const int row = tid / NW, wx = tid - row * NW;
+        const size_t gw = (size_t)(y0 + row) * wprL + (x0 >> 5) + wx;
+        es[tid] = make_uint2(bE[gw], bS[gw]);
+        if (tid < NW) nIn[tid] = bS[(size_t)(y0 == 0 ? L - 1 : y0 - 1) * wprL + (x0 >> 5) + tid];
+        if (warp == NW - 1) {                                         // (not the warp that wrote nIn: no race with tid < NW)
+            const int wl = (x0 >> 5) == 0 ? wprL - 1 : (x0 >> 5) - 1;
+            const uint32_t b = __ballot_sync(0xffffffffu, bE[(size_t)(y0 + lane) * wprL + wl] >> 31);
+            if (lane == 0) wIn = b;
+        }
+    } else {
+        const PhiloxKey key(la.key0, la.key1);
+        {
+            const int row = tid / NW, wx = tid - row * NW;          // this thread's 32-site word
+            const int y = y0 + row;
+            const int xw = (x0 >> 5) + wx;
+            const int w = y * wprL + xw;                              // word index within the lattice
+            const int8_t* r0 = s + (size_t)y * L + xw * 32;
+            const int8_t* r1 = s + (size_t)(y + 1 == L ? 0 : y + 1) * L + xw * 32;
+            const uint4 a0 = *reinterpret_cast<const uint4*>(r0), a1 = *reinterpret_cast<const uint4*>(r0 + 16);
+            const uint4 b0 = *reinterpret_cast<const uint4*>(r1), b1 = *reinterpret_cast<const uint4*>(r1 + 16);
+            const int8_t nx = s[(size_t)y * L + (xw + 1 == wprL ? 0 : (xw + 1) * 32)];
+            const uint32_t own = neg_mask32(a0, a1), south = neg_mask32(b0, b1);
+            const uint32_t eastm = (own >> 1) | (nx < 0 ? 0x80000000u : 0u);
+            const uint32_t eqE = ~(own ^ eastm), eqS = ~(own ^ south);
+            uint32_t dE = 0, dS = 0;
+#pragma unroll
+            for (int c = 0; c < 16; ++c) {
+                const uint4 r = philox4x32_10((uint32_t)w * 16u + c, tlo, thi, TAG_BOND, key);
+                dE |= (r.x < la.thr ? 1u : 0u) << (2 * c) | (r.z < la.thr ? 1u : 0u) << (2 * c + 1);
+                dS |= (r.y < la.thr ? 1u : 0u) << (2 * c) | (r.w < la.thr ? 1u : 0u) << (2 * c + 1);
+            }
+            const uint32_t e = eqE & dE, so = eqS & dS;
+            es[tid] = make_uint2(e, so);
+            bondE[(size_t)blockIdx.y * words + w] = e;
+            bondS[(size_t)blockIdx.y * words + w] = so;
+        }
+        // bonds entering the tile: South bonds of the row above (TW / 2 calls), East bonds of the column to
+        // the West (32 calls).  They are owned by the neighbouring tiles; recomputed here from the same draws.
+        for (int j = tid; j < TW / 2 + TH; j += THREADS) {
+            if (j < TW / 2) {
+                const int yn = y0 == 0 ? L - 1 : y0 - 1;
+                const int x = x0 + 2 * j;
+                const int i = yn * L + x;                                  // even site; call covers i, i + 1
+                const uint4 r = philox4x32_10((uint32_t)(i >> 1), tlo, thi, TAG_BOND, key);
+                const int8_t u0 = s[i], u1 = s[i + 1];
+                const int8_t d0 = s[(size_t)y0 * L + x], d1 = s[(size_t)y0 * L + x + 1];
+                const uint32_t bits = ((u0 == d0 && r.y < la.thr) ? 1u : 0u) | ((u1 == d1 && r.w < la.thr) ? 2u : 0u);
+                if (bits) atomicOr(&nIn[(2 * j) >> 5], bits << ((2 * j) & 31));
+            } else {
+                const int row = j - TW / 2;
+                const int xwst = x0 == 0 ? L - 1 : x0 - 1;                 // odd column
+                const int i = (y0 + row) * L + xwst;
+                const uint4 r = philox4x32_10((uint32_t)(i >> 1), tlo, thi, TAG_BOND, key);
+                if (s[i] == s[(size_t)(y0 + row) * L + x0] && r.z < la.thr) atomicOr(&wIn, 1u << row);
+            }
+        }
+    }
+    __syncthreads();
+
+    // ---- phase 2: scan-line labelling of this warp's strip, PAPER.md:49-51 (section 2.3) --------------
+    const uint32_t lt = (1u << lane) - 1u;
+    {
+        int prev = 0;
+        uint32_t s_up = 0;
+#pragma unroll 4
+        for (int y = 0; y < TH; ++y) {
+            const uint2 w = es[y * NW + warp];
+            const uint32_t e = w.x & 0x7FFFFFFFu;                   // bonds inside the strip
+            const uint32_t nz = ~e;                                  // bit k: no bond between columns k, k + 1
+            const int h = 32 - __clz(nz & lt);                       // head column of my run
+            const int tl = __ffs(nz & ~lt) - 1;                      // tail column of my run (nz bit 31 is set)
+            const uint32_t runmask = (2u << tl) - (1u << h);
+            const uint32_t upm = s_up & runmask;                     // sites of my run bonded to the row above
+            const bool myUp = (s_up >> lane) & 1u;
+            int a = prev;
+            if (myUp) {                                              // root of the site above
+                int p = par[a];
+                while (p != a) { a = p; p = par[a]; }
+            }
+            const int got = __shfl_sync(0xffffffffu, a, (__ffs(upm) - 1) & 31);
+            const int c = upm ? got : y * TW + warp * 32 + h;     // a new label: the head's own index (its own root)
+            par[y * TW + warp * 32 + lane] = c;
+            if (myUp && a != c) sc_union(par, a, c);
+            __syncwarp();                                            // row y's parents are written before row y + 1 walks them
+            prev = c;
+            s_up = w.y;
+        }
+    }
+    __syncthreads();
+
+    // ---- phase 3: strip seams ---------------------------------------------------------------------------
+    if (NW > 1 && warp < NW - 1) {
+        if (es[lane * NW + warp].x >> 31) {
+            const int i = lane * TW + warp * 32 + 31;
+            sc_union(par, sc_find(par, i), sc_find(par, i + 1));
+        }
+    }
+    __syncthreads();
+
+    // ---- phase 4: flatten, global labels, sizes, open flags ---------------------------------------------
+    int* glab = label + (size_t)blockIdx.y * N;
+    uint32_t rootrows = 0;                                           // bit y: my site in row y is a tile-local root
+    {
+        const uint32_t north = nIn[warp];
+        const uint32_t west = wIn;
+#pragma unroll 4
+        for (int y = 0; y < TH; ++y) {
+            const uint2 w = es[y * NW + warp];
+            const int i = y * TW + warp * 32 + lane;
+            const int r = sc_find(par, i);
+            const int rr = r / TW, rc = r - rr * TW;
+            glab[(size_t)(y0 + y) * L + x0 + warp * 32 + lane] = (y0 + rr) * L + x0 + rc;
+            if (r == i) rootrows |= 1u << y;
+            // one size update per run (its head adds the run length)
+            const uint32_t nz = ~(w.x & 0x7FFFFFFFu);
+            const bool head = lane == 0 || ((nz >> (lane - 1)) & 1u);
+            uint32_t add = 0;
+            if (head) add = (uint32_t)(__ffs(nz & ~lt) - lane) << CNT_SHIFT;
+            bool open = false;
+            if (y == TH - 1 && ((w.y >> lane) & 1u)) open = true;
+            if (y == 0 && ((north >> lane) & 1u)) open = true;
+            if (warp == NW - 1 && lane == 31 && (w.x >> 31)) open = true;
+            if (warp == 0 && lane == 0 && ((west >> y) & 1u)) open = true;
+            if (open) atomicOr(reinterpret_cast<unsigned int*>(par + r), OPEN_BIT);
+            if (add) atomicAdd(reinterpret_cast<unsigned int*>(par + r), add);
+        }
+    }
+    __syncthreads();
+
+    // ---- phase 5: closed clusters are complete -> maximum; open ones -> the tile's list -----------------
+    {
+        int mymax = 0;
+        int2* mylist = olist + ((size_t)blockIdx.y * gridDim.x + blockIdx.x) * CAP;
+        while (rootrows) {
+            const int y = __ffs(rootrows) - 1;
+            rootrows &= rootrows - 1;
+            const uint32_t v = (uint32_t)par[y * TW + warp * 32 + lane];
+            const int cnt = (int)((v >> CNT_SHIFT) & CNT_MASK);
+            if (v & OPEN_BIT) {
+                const int pos = atomicAdd(&s_nopen, 1);
+                mylist[pos] = make_int2((y0 + y) * L + x0 + warp * 32 + lane, cnt);
+            } else {
+                mymax = max(mymax, cnt);
+            }
+        }
+        mymax = warp_max_i(mymax);
+        if (lane == 0 && mymax) atomicMax(&s_max, mymax);
+    }
+    __syncthreads();
+    if (tid == 0) {
+        ocount[(size_t)blockIdx.y * gridDim.x + blockIdx.x] = s_nopen;
+        if (s_max) atomic_max_ll(&rec[(size_t)ctl->slot * nb + blockIdx.y].maxcl, s_max);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// a4-a7 fused: root of every site (two hops: site -> tile root -> global root, the second through a
+// shared-memory copy of the tile's labels), assignment PAPER.md:57 (section 2.4), and the observables
+// of the new configuration PAPER.md:63 (section 2.5).  One CTA per tile, 32 sites per thread.
+// write_labels != 0 also stores the flat labels (a4); otherwise sw_labels() flattens on demand.
+// ---------------------------------------------------------------------------------------------------
+template <int NW>
+__global__ void __launch_bounds__(32 * NW)
+k_flip_tile(int8_t* __restrict__ spins, int* label, const uint32_t* __restrict__ D,
+            Rec* __restrict__ rec, const Ctl* __restrict__ ctl, DivL dv,
+            int L, int N, int words, int nb, int write_labels) {
+    constexpr int TW = 32 * NW, TH = SCAN_TH, SITES = TW * TH, THREADS = 32 * NW;
+    constexpr int QSTEPS = SITES / 4 / THREADS;      // = 8
+    __shared__ __align__(16) int lab[SITES];
+    __shared__ uint32_t neg[TH * NW];                // sign words of the new spins: bit = (spin == -1)
+    __shared__ uint32_t southRow[NW];                // new spins of the row below the tile
+    __shared__ uint32_t eastCol;                     // new spins of the column East of the tile, bit = row
+    __shared__ int s_red[3];                         // E, M, ncl of the tile
+
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int tilesX = L / TW;
+    const int ty = blockIdx.x / tilesX, tx = blockIdx.x - ty * tilesX;
+    const int y0 = ty * TH, x0 = tx * TW;
+    int* glab = label + (size_t)blockIdx.y * N;
+    const uint32_t* d = D + (size_t)blockIdx.y * words;
+
+    neg[tid] = 0;
+    if (tid < NW) southRow[tid] = 0;
+    if (tid == 0) { eastCol = 0; s_red[0] = 0; s_red[1] = 0; s_red[2] = 0; }
+
+    // stage the tile's labels (coalesced 128-bit loads)
+    int4 v[QSTEPS];
+#pragma unroll
+    for (int k = 0; k < QSTEPS; ++k) {
+        const int q = k * THREADS + tid;
+        const int row = (4 * q) / TW, col = (4 * q) - row * TW;
+        v[k] = *reinterpret_cast<const int4*>(glab + (size_t)(y0 + row) * L + x0 + col);
+        *reinterpret_cast<int4*>(lab + 4 * q) = v[k];
+    }
+    __syncthreads();
+
+    // halo: the new spin of a site outside the tile is the decision bit of its own root (three loads)
+    for (int j = tid; j < TH + TW; j += THREADS) {
+        int site;
+        if (j < TH) site = (y0 + j) * L + (x0 + TW == L ? 0 : x0 + TW);
+        else        site = (y0 + TH == L ? 0 : y0 + TH) * L + x0 + (j - TH);
+        const int g = glab[site];
+        const int R = glab[g];
+        const uint32_t up = (__ldg(d + (R >> 5)) >> (R & 31)) & 1u;
+        if (!up) {
+            if (j < TH) atomicOr(&eastCol, 1u << j);
+            else        atomicOr(&southRow[(j - TH) >> 5], 1u << ((j - TH) & 31));
+        }
+    }
+
+    const int tilebase = y0 * L + x0;
+    int m = 0, nroot = 0;
+#pragma unroll
+    for (int k = 0; k < QSTEPS; ++k) {
+        const int q = k * THREADS + tid;
+        const int row = (4 * q) / TW, col = (4 * q) - row * TW;
+        const int g[4] = { v[k].x, v[k].y, v[k].z, v[k].w };
+        int R[4];
+        uint32_t nib = 0, out = 0;
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            // g is this site's tile root (inside the tile: its word holds the cluster root), or -- when the
+            // site is itself a hooked tile root -- already the cluster root, possibly outside the tile
+            const uint32_t delta = (uint32_t)(g[u] - tilebase);
+            R[u] = g[u];
+            if (delta < (uint32_t)(TH * L)) {
+                const int ry = div_l((int)delta, dv);
+                const int rc = (int)delta - ry * L;
+                if (rc < TW) R[u] = lab[ry * TW + rc];
+            }
+        }
+        const int self = (y0 + row) * L + x0 + col;
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const uint32_t up = (__ldg(d + (R[u] >> 5)) >> (R[u] & 31)) & 1u;
+            out |= (up ? 0x01u : 0xFFu) << (8 * u);
+            nib |= (up ^ 1u) << u;
+            nroot += (R[u] == self + u);
+        }
+        m += 4 - 2 * __popc(nib);
+        *reinterpret_cast<uint32_t*>(spins + (size_t)blockIdx.y * N + self) = out;
+        if (write_labels) *reinterpret_cast<int4*>(glab + self) = make_int4(R[0], R[1], R[2], R[3]);
+        if (nib) atomicOr(&neg[row * NW + (col >> 5)], nib << (col & 31));
+    }
+    __syncthreads();
+
+    // energy of the new configuration: E = (#edges) - 2 (#equal pairs), one 32-site word per thread
+    int e;
+    {
+        const int row = tid / NW, wx = tid - row * NW;
+        const uint32_t own = neg[tid];
+        const uint32_t eb = wx + 1 < NW ? (neg[tid + 1] & 1u) : ((eastCol >> row) & 1u);
+        const uint32_t south = row + 1 < TH ? neg[tid + NW] : southRow[wx];
+        const uint32_t eastm = (own >> 1) | (eb << 31);
+        e = 64 - 2 * (__popc(~(own ^ eastm)) + __popc(~(own ^ south)));
+    }
+    e = warp_sum_i(e); m = warp_sum_i(m); nroot = warp_sum_i(nroot);
+    if (lane == 0) { atomicAdd(&s_red[0], e); atomicAdd(&s_red[1], m); atomicAdd(&s_red[2], nroot); }
+    __syncthreads();
+    if (tid == 0) {
+        Rec* r = rec + (size_t)ctl->slot * nb + blockIdx.y;
+        if (s_red[0]) atomic_add_ll(&r->E, s_red[0]);
+        if (s_red[1]) atomic_add_ll(&r->M, s_red[1]);
+        if (s_red[2]) atomic_add_ll(&r->ncl, s_red[2]);
+    }
+}
+
+} // namespace sw

@@ -232,7 +232,9 @@ k_tile_label(int* __restrict__ label, const uint32_t* __restrict__ bondE, const 
 }
 
 // ---------------------------------------------------------------------------------------------
-// a3 global boundary merge: one thread per site on a tile's East column or South row.
+// a3 global boundary merge: one thread per site on a tile's East column or South row.  The union starts
+// from the two sites' tile roots (label[site] after a2), so label[] of a non-root site is never written
+// here and stays "my tile root": the later passes rely on site -> tile root -> global root (two hops).
 // ---------------------------------------------------------------------------------------------
 template <int TW, int TH>
 __global__ void __launch_bounds__(ROW_THREADS)
@@ -248,13 +250,13 @@ k_merge_tiled(int* label, const uint32_t* __restrict__ bondE, const uint32_t* __
         const int y = idx / tilesX, c = idx - y * tilesX;
         const int x = c * TW + TW - 1;
         if (bondE[(size_t)blockIdx.y * words + (size_t)y * wprL + (x >> 5)] >> 31)
-            uf_union(lab, y * L + x, y * L + (x + 1 == L ? 0 : x + 1));
+            uf_union(lab, ld_cg(lab + y * L + x), ld_cg(lab + y * L + (x + 1 == L ? 0 : x + 1)));
     } else {
         const int j = idx - nV;
         const int r = j / L, x = j - r * L;
         const int y = r * TH + TH - 1;
         if ((bondS[(size_t)blockIdx.y * words + (size_t)y * wprL + (x >> 5)] >> (x & 31)) & 1u)
-            uf_union(lab, y * L + x, (y + 1 == L ? 0 : y + 1) * L + x);
+            uf_union(lab, ld_cg(lab + y * L + x), ld_cg(lab + (y + 1 == L ? 0 : y + 1) * L + x));
     }
 }
 
@@ -264,7 +266,7 @@ k_merge_tiled(int* label, const uint32_t* __restrict__ bondE, const uint32_t* __
 // most two hops from it: site -> tile root -> global root.  No loops, no divergence.
 // ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(ROW_THREADS)
-k_compress_tiled(int* label, Rec* __restrict__ rec, const Ctl* __restrict__ ctl, int N, int nb) {
+k_compress_tiled(int* label, Rec* __restrict__ rec, const Ctl* __restrict__ ctl, int N, int nb, int count) {
     const int q = blockIdx.x * ROW_THREADS + threadIdx.x;       // quad index
     int nroot = 0;
     if (q * 4 < N) {
@@ -275,6 +277,7 @@ k_compress_tiled(int* label, Rec* __restrict__ rec, const Ctl* __restrict__ ctl,
         if (t0 != v.x || t1 != v.y || t2 != v.z || t3 != v.w)
             *reinterpret_cast<int4*>(lab + q * 4) = make_int4(t0, t1, t2, t3);
     }
+    if (!count) return;
     nroot = warp_sum_i(nroot);
     if ((threadIdx.x & 31) == 0 && nroot)
         atomic_add_ll(&rec[(size_t)ctl->slot * nb + blockIdx.y].ncl, nroot);
