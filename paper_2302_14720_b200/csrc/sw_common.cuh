@@ -28,6 +28,13 @@ struct Rec {
     long long E, M, ncl, maxcl;
 };
 
+// Spins live bit-packed on the device: bit (i & 31) of word (i >> 5) is 1 for spin +1, 0 for spin -1
+// (the same bit-plane layout as the bond planes and the decision plane D, so "new spins = gather(D, root)"
+// is a gather of bits).  The int8 +-1 array of the C ABI is materialised from it on demand.
+__device__ __forceinline__ uint32_t get_bit(const uint32_t* __restrict__ plane, int i) {
+    return (plane[i >> 5] >> (i & 31)) & 1u;
+}
+
 // ------------------------------------------------------------------------------------------
 // Philox4x32-10.  mul.wide.u32 -> one IMAD.WIDE per multiply; the xor of three terms -> one LOP3.
 // ------------------------------------------------------------------------------------------
@@ -55,11 +62,27 @@ __device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_
     return make_uint4(c0, c1, c2, c3);
 }
 
+// the 32 East and 32 South draw bits of bit-plane word w (sites 32w .. 32w+31): call c covers sites
+// 2c, 2c+1; words x,y = East,South of the even site, z,w of the odd one.
+__device__ __forceinline__ void bond_draws(uint32_t w, uint32_t tlo, uint32_t thi, uint32_t thr,
+                                           const PhiloxKey& key, uint32_t& dE, uint32_t& dS) {
+    dE = 0; dS = 0;
+#pragma unroll
+    for (int c = 0; c < 16; ++c) {
+        const uint4 r = philox4x32_10(w * 16u + c, tlo, thi, TAG_BOND, key);
+        dE |= (r.x < thr ? 1u : 0u) << (2 * c) | (r.z < thr ? 1u : 0u) << (2 * c + 1);
+        dS |= (r.y < thr ? 1u : 0u) << (2 * c) | (r.w < thr ? 1u : 0u) << (2 * c + 1);
+    }
+}
+
 // ------------------------------------------------------------------------------------------
 // memory helpers
 // ------------------------------------------------------------------------------------------
 __device__ __forceinline__ int ld_cg(const int* p) {            // L2-coherent load (labels under atomics)
     int v; asm volatile("ld.global.cg.s32 %0, [%1];" : "=r"(v) : "l"(p)); return v;
+}
+__device__ __forceinline__ unsigned long long ld_cg64(const unsigned long long* p) {
+    unsigned long long v; asm volatile("ld.global.cg.u64 %0, [%1];" : "=l"(v) : "l"(p)); return v;
 }
 __device__ __forceinline__ uint4 ld_stream_u4(const void* p) {   // read-once data: do not pollute L1
     uint4 v; asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
@@ -79,6 +102,11 @@ __device__ __forceinline__ uint32_t neg_mask32(uint4 a, uint4 b) {
     return  neg_nibble(a.x)        | (neg_nibble(a.y) << 4)  | (neg_nibble(a.z) << 8)  | (neg_nibble(a.w) << 12)
          | (neg_nibble(b.x) << 16) | (neg_nibble(b.y) << 20) | (neg_nibble(b.z) << 24) | (neg_nibble(b.w) << 28);
 }
+// four spin bits (bit = 1: +1) -> four int8 bytes (+1 = 0x01, -1 = 0xFF)
+__device__ __forceinline__ uint32_t spin_bytes4(uint32_t nib) {
+    const uint32_t up = (nib * 0x00204081u) & 0x01010101u;       // bit k -> byte k (0x01 where up)
+    return up | ((up ^ 0x01010101u) * 0xFFu);                    // 0xFF where down
+}
 
 // block-wide sums / max into one atomic per block
 __device__ __forceinline__ long long warp_sum_ll(long long v) {
@@ -86,16 +114,8 @@ __device__ __forceinline__ long long warp_sum_ll(long long v) {
     for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
     return v;
 }
-__device__ __forceinline__ int warp_sum_i(int v) {
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-    return v;
-}
-__device__ __forceinline__ int warp_max_i(int v) {
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v = max(v, __shfl_xor_sync(0xffffffffu, v, o));
-    return v;
-}
+__device__ __forceinline__ int warp_sum_i(int v) { return __reduce_add_sync(0xffffffffu, v); }
+__device__ __forceinline__ int warp_max_i(int v) { return __reduce_max_sync(0xffffffffu, v); }
 __device__ __forceinline__ void atomic_add_ll(long long* p, long long v) {
     atomicAdd(reinterpret_cast<unsigned long long*>(p), (unsigned long long)v);
 }
@@ -104,19 +124,13 @@ __device__ __forceinline__ void atomic_max_ll(long long* p, long long v) {   // 
 }
 
 // ------------------------------------------------------------------------------------------
-// lock-free union-find on a global int32 parent array; label[x] <= x, roots have label[r] == r.
-// Hooking is "larger root under smaller" with atomicMin, so the surviving root of a component is
-// its minimum site index whatever the race order (north_star stage 2).
+// lock-free union-find on a global int32 parent array (generic path); label[x] <= x, roots have
+// label[r] == r.  Hooking is "larger root under smaller" with atomicMin, so the surviving root of a
+// component is its minimum site index whatever the race order (north_star stage 2).
 // ------------------------------------------------------------------------------------------
 __device__ __forceinline__ int uf_find(const int* lab, int x) {
     int p = ld_cg(lab + x);
     while (p != x) { x = p; p = ld_cg(lab + x); }
-    return x;
-}
-// read-only find after all merging is done (ordinary cached loads)
-__device__ __forceinline__ int uf_find_ro(const int* __restrict__ lab, int x) {
-    int p = __ldg(lab + x);
-    while (p != x) { x = p; p = __ldg(lab + x); }
     return x;
 }
 // find with one-shot compression of the starting node when the walk was longer than one hop
