@@ -5,6 +5,7 @@
 #include "sw_generic.cuh"
 #include "sw_tiled.cuh"
 #include "sw_scan.cuh"
+#include "sw_word.cuh"
 
 #include <algorithm>
 #include <cmath>
@@ -55,8 +56,9 @@ constexpr int EV_PER_SWEEP = K_COUNT + 1;
 inline size_t align_up(size_t v) { return (v + ALIGN - 1) / ALIGN * ALIGN; }
 
 // tile shapes of the fast path
-enum TileKind { TILE_NONE = 0, TILE_64x64 = 1, TILE_256x32 = 2, SCAN_2 = 3, SCAN_4 = 4, SCAN_8 = 5 };
-inline int scan_nw(TileKind k) { return k == SCAN_2 ? 2 : k == SCAN_4 ? 4 : k == SCAN_8 ? 8 : 0; }
+enum TileKind { TILE_NONE = 0, TILE_64x64 = 1, TILE_256x32 = 2, SCAN_2 = 3, SCAN_4 = 4, SCAN_8 = 5, WORD_8 = 6 };
+// width in 32-site words of the 32-row tiles the scan-line / word kernels and k_flip_tile share
+inline int scan_nw(TileKind k) { return k == SCAN_2 ? 2 : k == SCAN_4 ? 4 : (k == SCAN_8 || k == WORD_8) ? 8 : 0; }
 using Cfg64 = TileCfg<64, 64>;
 using Cfg256 = TileCfg<256, 32>;
 
@@ -149,6 +151,7 @@ TileKind pick_tile(int L, int path) {
     if (path == 3) return L % 256 == 0 ? TILE_256x32 : TILE_NONE;
     if (path == 4) return L % 64 == 0 ? SCAN_2 : TILE_NONE;
     if (path == 5) return L % 128 == 0 ? SCAN_4 : TILE_NONE;
+    if (path == 7) return L % 256 == 0 ? WORD_8 : TILE_NONE;
     if (L % 256 == 0) return SCAN_8;
     if (L % 128 == 0) return SCAN_4;
     if (L % 64 == 0) return SCAN_2;
@@ -207,7 +210,17 @@ template <int NW>
 int launch_bond_label_scan(sw_handle* h, bool fused) {
     constexpr int TW = 32 * NW, CAP = 2 * (TW + SCAN_TH);
     const int tiles = h->N / (TW * SCAN_TH);
-    if (fused) {
+    if (NW == 8 && h->tile == WORD_8) {       // thread-per-word labelling (sw_word.cuh)
+        SW_MARK(h, fused ? K_BONDLABEL : K_TILE);
+        if (fused)
+            k_word_label<8, SCAN_TH, true><<<dim3(tiles, h->nb), 8 * SCAN_TH, 0, h->stream>>>(
+                h->spins, h->bondE, h->bondS, h->label, h->olist, h->ocount, h->series, h->lat, h->ctl,
+                h->L, h->N, h->words, h->nb);
+        else
+            k_word_label<8, SCAN_TH, false><<<dim3(tiles, h->nb), 8 * SCAN_TH, 0, h->stream>>>(
+                h->spins, h->bondE, h->bondS, h->label, h->olist, h->ocount, h->series, h->lat, h->ctl,
+                h->L, h->N, h->words, h->nb);
+    } else if (fused) {
         SW_MARK(h, K_BONDLABEL);
         k_bond_label<NW, true><<<dim3(tiles, h->nb), 32 * NW, 0, h->stream>>>(
             h->spins, h->bondE, h->bondS, h->label, h->olist, h->ocount, h->series, h->lat, h->ctl,
@@ -281,7 +294,8 @@ int launch_label(sw_handle* h) {
     switch (h->tile) {
         case SCAN_2:      return launch_label_scan<2>(h);
         case SCAN_4:      return launch_label_scan<4>(h);
-        case SCAN_8:      return launch_label_scan<8>(h);
+        case SCAN_8:
+        case WORD_8:      return launch_label_scan<8>(h);
         case TILE_64x64:  return launch_label_tiled<64, 64>(h);
         case TILE_256x32: return launch_label_tiled<256, 32>(h);
         default:          return launch_label_generic(h);
@@ -637,7 +651,7 @@ int sw_stage_ms(sw_handle* h, float out[4]) {
 }
 
 int sw_set_path(sw_handle* h, int path) {
-    if (!h || path < 0 || path > 6) { set_err("sw_set_path: invalid argument"); return SW_EINVAL; }
+    if (!h || path < 0 || path > 7) { set_err("sw_set_path: invalid argument"); return SW_EINVAL; }
     h->path = path;
     h->tile = pick_tile(h->L, path);
     return SW_OK;

@@ -63,7 +63,7 @@ k_bond_label(const int8_t* __restrict__ spins, uint32_t* bondE, uint32_t* bondS,
              int L, int N, int words, int nb) {
     constexpr int TW = 32 * NW, TH = SCAN_TH, SITES = TW * TH, THREADS = 32 * NW;
     constexpr int CAP = 2 * (TW + TH);
-    __shared__ int par[SITES];                 // parent, tile-local index (+ size / open bits at roots)
+    __shared__ __align__(16) int par[SITES];   // parent, tile-local index (+ size / open bits at roots)
     __shared__ uint2 es[TH * NW];              // [row][strip] = (East word, South word)
     __shared__ uint32_t nIn[NW];               // South bonds entering from the tile above, per strip
     __shared__ uint32_t wIn;                   // East bonds entering from the tile to the West, bit = row
@@ -186,33 +186,56 @@ k_bond_label(const int8_t* __restrict__ spins, uint32_t* bondE, uint32_t* bondS,
     }
     __syncthreads();
 
-    // ---- phase 4: flatten, global labels, sizes, open flags ---------------------------------------------
+    // ---- phase 4: open flags (border sites only), then root / global label / size of every site ----------
+    // From here on roots carry size and open bits above IDX_MASK; every read of par[] masks them.
+    for (int j = tid; j < 2 * (TW + TH); j += THREADS) {
+        int site; bool open;
+        if (j < TW)               { site = j;                              open = (nIn[j >> 5] >> (j & 31)) & 1u; }
+        else if (j < 2 * TW)      { const int c = j - TW; site = (TH - 1) * TW + c;
+                                    open = (es[(TH - 1) * NW + (c >> 5)].y >> (c & 31)) & 1u; }
+        else if (j < 2 * TW + TH) { const int r = j - 2 * TW; site = r * TW; open = (wIn >> r) & 1u; }
+        else                      { const int r = j - 2 * TW - TH; site = r * TW + TW - 1;
+                                    open = es[r * NW + NW - 1].x >> 31; }
+        if (open) atomicOr(reinterpret_cast<unsigned int*>(par + sc_find(par, site)), OPEN_BIT);
+    }
+    constexpr int QSTEPS = SITES / 4 / THREADS;                      // = 8
+    constexpr int LOG_TW = 5 + (NW == 8 ? 3 : NW == 4 ? 2 : NW == 2 ? 1 : 0);
+    static_assert((1 << LOG_TW) == TW, "tile width is a power of two");
     int* glab = label + (size_t)blockIdx.y * N;
-    uint32_t rootrows = 0;                                           // bit y: my site in row y is a tile-local root
-    {
-        const uint32_t north = nIn[warp];
-        const uint32_t west = wIn;
-#pragma unroll 4
-        for (int y = 0; y < TH; ++y) {
-            const uint2 w = es[y * NW + warp];
-            const int i = y * TW + warp * 32 + lane;
-            const int r = sc_find(par, i);
-            const int rr = r / TW, rc = r - rr * TW;
-            glab[(size_t)(y0 + y) * L + x0 + warp * 32 + lane] = (y0 + rr) * L + x0 + rc;
-            if (r == i) rootrows |= 1u << y;
-            // one size update per run (its head adds the run length)
-            const uint32_t nz = ~(w.x & 0x7FFFFFFFu);
-            const bool head = lane == 0 || ((nz >> (lane - 1)) & 1u);
-            uint32_t add = 0;
-            if (head) add = (uint32_t)(__ffs(nz & ~lt) - lane) << CNT_SHIFT;
-            bool open = false;
-            if (y == TH - 1 && ((w.y >> lane) & 1u)) open = true;
-            if (y == 0 && ((north >> lane) & 1u)) open = true;
-            if (warp == NW - 1 && lane == 31 && (w.x >> 31)) open = true;
-            if (warp == 0 && lane == 0 && ((west >> y) & 1u)) open = true;
-            if (open) atomicOr(reinterpret_cast<unsigned int*>(par + r), OPEN_BIT);
-            if (add) atomicAdd(reinterpret_cast<unsigned int*>(par + r), add);
+    const int tilebase = y0 * L + x0;
+    uint32_t rootmask = 0;                                           // bit 4k+u: site 4 (k THREADS + tid) + u is a tile-local root
+#pragma unroll
+    for (int k = 0; k < QSTEPS; ++k) {
+        const int q = k * THREADS + tid;
+        const int l = 4 * q;
+        const int4 v = *reinterpret_cast<const int4*>(par + l);
+        int r[4] = { v.x & (int)IDX_MASK, v.y & (int)IDX_MASK, v.z & (int)IDX_MASK, v.w & (int)IDX_MASK };
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            if (r[u] != l + u) {                                     // the scan left "root at the time": usually 0 or 1 hop
+                int p = par[r[u]] & (int)IDX_MASK;
+                while (p != r[u]) { r[u] = p; p = par[p] & (int)IDX_MASK; }
+            } else {
+                rootmask |= 1u << (4 * k + u);
+            }
         }
+        int4 g;
+        g.x = tilebase + (r[0] >> LOG_TW) * L + (r[0] & (TW - 1));
+        g.y = tilebase + (r[1] >> LOG_TW) * L + (r[1] & (TW - 1));
+        g.z = tilebase + (r[2] >> LOG_TW) * L + (r[2] & (TW - 1));
+        g.w = tilebase + (r[3] >> LOG_TW) * L + (r[3] & (TW - 1));
+        *reinterpret_cast<int4*>(glab + (size_t)(y0 + (l >> LOG_TW)) * L + x0 + (l & (TW - 1))) = g;
+        // sizes: one shared atomic per group of equal neighbours in the quad
+        uint32_t acc = 1u << CNT_SHIFT;
+#pragma unroll
+        for (int u = 1; u < 4; ++u) {
+            if (r[u] != r[u - 1]) {
+                atomicAdd(reinterpret_cast<unsigned int*>(par + r[u - 1]), acc);
+                acc = 0;
+            }
+            acc += 1u << CNT_SHIFT;
+        }
+        atomicAdd(reinterpret_cast<unsigned int*>(par + r[3]), acc);
     }
     __syncthreads();
 
@@ -220,14 +243,15 @@ k_bond_label(const int8_t* __restrict__ spins, uint32_t* bondE, uint32_t* bondS,
     {
         int mymax = 0;
         int2* mylist = olist + ((size_t)blockIdx.y * gridDim.x + blockIdx.x) * CAP;
-        while (rootrows) {
-            const int y = __ffs(rootrows) - 1;
-            rootrows &= rootrows - 1;
-            const uint32_t v = (uint32_t)par[y * TW + warp * 32 + lane];
+        while (rootmask) {
+            const int b = __ffs(rootmask) - 1;
+            rootmask &= rootmask - 1;
+            const int l = 4 * ((b >> 2) * THREADS + tid) + (b & 3);
+            const uint32_t v = (uint32_t)par[l];
             const int cnt = (int)((v >> CNT_SHIFT) & CNT_MASK);
             if (v & OPEN_BIT) {
                 const int pos = atomicAdd(&s_nopen, 1);
-                mylist[pos] = make_int2((y0 + y) * L + x0 + warp * 32 + lane, cnt);
+                mylist[pos] = make_int2(tilebase + (l >> LOG_TW) * L + (l & (TW - 1)), cnt);
             } else {
                 mymax = max(mymax, cnt);
             }
