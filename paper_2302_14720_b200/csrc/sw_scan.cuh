@@ -186,6 +186,36 @@ k_bond_label(const int8_t* __restrict__ spins, uint32_t* bondE, uint32_t* bondS,
     }
     __syncthreads();
 
+    // ---- phase 3b: flatten the label nodes ---------------------------------------------------------------
+    // The scan gave every site of a run the run's label = a root at that time; the only nodes that ever were
+    // roots are the heads of runs with no bond from the row above ("label nodes", ~0.15 per site at T_c).
+    // One thread per 32-site word finds them by bit tricks and points each at its root, so that afterwards
+    // root(site) = par[par[site]] for every site, without a loop.
+    uint32_t rootbits = 0;                                           // bit c: column c of my word is a tile-local root
+    const int mybase = (tid / NW) * TW + (tid % NW) * 32;
+    {
+        const uint32_t ew = es[tid].x & 0x7FFFFFFFu;
+        uint32_t up = tid >= NW ? es[tid - NW].y : 0u;               // South bonds of the row above
+        uint32_t m = ew;                                             // OR of the run's uplinks, gathered at its head
+        up |= (up >> 1) & m;  m &= m >> 1;
+        up |= (up >> 2) & m;  m &= m >> 2;
+        up |= (up >> 4) & m;  m &= m >> 4;
+        up |= (up >> 8) & m;  m &= m >> 8;
+        up |= (up >> 16) & m;
+        uint32_t o = ~(ew << 1) & ~up;                               // heads of runs without an uplink
+        while (o) {
+            const int c = __ffs(o) - 1;
+            o &= o - 1;
+            const int node = mybase + c;
+            const int p = par[node];
+            if (p == node) { rootbits |= 1u << c; continue; }
+            int r = p, q = par[r];
+            while (q != r) { r = q; q = par[r]; }
+            if (r != p) par[node] = r;
+        }
+    }
+    __syncthreads();
+
     // ---- phase 4: open flags (border sites only), then root / global label / size of every site ----------
     // From here on roots carry size and open bits above IDX_MASK; every read of par[] masks them.
     for (int j = tid; j < 2 * (TW + TH); j += THREADS) {
@@ -203,22 +233,14 @@ k_bond_label(const int8_t* __restrict__ spins, uint32_t* bondE, uint32_t* bondS,
     static_assert((1 << LOG_TW) == TW, "tile width is a power of two");
     int* glab = label + (size_t)blockIdx.y * N;
     const int tilebase = y0 * L + x0;
-    uint32_t rootmask = 0;                                           // bit 4k+u: site 4 (k THREADS + tid) + u is a tile-local root
 #pragma unroll
     for (int k = 0; k < QSTEPS; ++k) {
         const int q = k * THREADS + tid;
         const int l = 4 * q;
         const int4 v = *reinterpret_cast<const int4*>(par + l);
-        int r[4] = { v.x & (int)IDX_MASK, v.y & (int)IDX_MASK, v.z & (int)IDX_MASK, v.w & (int)IDX_MASK };
-#pragma unroll
-        for (int u = 0; u < 4; ++u) {
-            if (r[u] != l + u) {                                     // the scan left "root at the time": usually 0 or 1 hop
-                int p = par[r[u]] & (int)IDX_MASK;
-                while (p != r[u]) { r[u] = p; p = par[p] & (int)IDX_MASK; }
-            } else {
-                rootmask |= 1u << (4 * k + u);
-            }
-        }
+        // site -> its label node -> root (label nodes are flat; roots carry size / open bits)
+        int r[4] = { par[v.x & (int)IDX_MASK] & (int)IDX_MASK, par[v.y & (int)IDX_MASK] & (int)IDX_MASK,
+                     par[v.z & (int)IDX_MASK] & (int)IDX_MASK, par[v.w & (int)IDX_MASK] & (int)IDX_MASK };
         int4 g;
         g.x = tilebase + (r[0] >> LOG_TW) * L + (r[0] & (TW - 1));
         g.y = tilebase + (r[1] >> LOG_TW) * L + (r[1] & (TW - 1));
@@ -243,10 +265,9 @@ k_bond_label(const int8_t* __restrict__ spins, uint32_t* bondE, uint32_t* bondS,
     {
         int mymax = 0;
         int2* mylist = olist + ((size_t)blockIdx.y * gridDim.x + blockIdx.x) * CAP;
-        while (rootmask) {
-            const int b = __ffs(rootmask) - 1;
-            rootmask &= rootmask - 1;
-            const int l = 4 * ((b >> 2) * THREADS + tid) + (b & 3);
+        while (rootbits) {
+            const int l = mybase + __ffs(rootbits) - 1;
+            rootbits &= rootbits - 1;
             const uint32_t v = (uint32_t)par[l];
             const int cnt = (int)((v >> CNT_SHIFT) & CNT_MASK);
             if (v & OPEN_BIT) {
