@@ -5,7 +5,6 @@
 #include "sw_generic.cuh"
 #include "sw_tiled.cuh"
 #include "sw_scan.cuh"
-#include "sw_word.cuh"
 
 #include <algorithm>
 #include <cmath>
@@ -56,14 +55,14 @@ constexpr int EV_PER_SWEEP = K_COUNT + 1;
 inline size_t align_up(size_t v) { return (v + ALIGN - 1) / ALIGN * ALIGN; }
 
 // tile shapes of the fast path
-enum TileKind { TILE_NONE = 0, TILE_64x64 = 1, TILE_256x32 = 2, SCAN_2 = 3, SCAN_4 = 4, SCAN_8 = 5, WORD_8 = 6 };
-// width in 32-site words of the 32-row tiles the scan-line / word kernels and k_flip_tile share
-inline int scan_nw(TileKind k) { return k == SCAN_2 ? 2 : k == SCAN_4 ? 4 : (k == SCAN_8 || k == WORD_8) ? 8 : 0; }
+enum TileKind { TILE_NONE = 0, TILE_64x64 = 1, TILE_256x32 = 2, SCAN_2 = 3, SCAN_4 = 4, SCAN_8 = 5 };
+// width in 32-site words of the 32-row tiles the scan-line kernel and k_flip16 share
+inline int scan_nw(TileKind k) { return k == SCAN_2 ? 2 : k == SCAN_4 ? 4 : k == SCAN_8 ? 8 : 0; }
 using Cfg64 = TileCfg<64, 64>;
 using Cfg256 = TileCfg<256, 32>;
 
 struct Layout {        // byte offsets into the workspace
-    size_t spins, bondE, bondS, D, label, gsize, olist, ocount, lat, ctl, rec_now, series, total;
+    size_t spins, bondE, bondS, D, label, lab16, gsize, olist, ocount, lat, ctl, rec_now, series, total;
 };
 
 size_t olist_entries(int L) {          // per lattice, maximum over the tile shapes usable for this L
@@ -92,6 +91,7 @@ Layout make_layout(int L, int nb) {
     o.bondS = p;   p = align_up(p + (size_t)nb * words * 4);
     o.D = p;       p = align_up(p + (size_t)nb * ((words + 3) / 4 * 4) * 4);
     o.label = p;   p = align_up(p + (size_t)nb * N * 4);
+    o.lab16 = p;   p = align_up(p + (L % 64 == 0 ? (size_t)nb * N * 2 : 0));
     o.gsize = p;   p = align_up(p + (size_t)nb * N * 4);
     o.olist = p;   p = align_up(p + (size_t)nb * olist_entries(L) * sizeof(int2));
     o.ocount = p;  p = align_up(p + (size_t)nb * tiles_max(L) * 4);
@@ -124,6 +124,7 @@ struct sw_handle {
     char* ws = nullptr; size_t ws_bytes = 0;
     int8_t* spins = nullptr; uint32_t *bondE = nullptr, *bondS = nullptr, *D = nullptr;
     int *label = nullptr, *gsize = nullptr, *ocount = nullptr; int2* olist = nullptr;
+    uint16_t* lab16 = nullptr;       // tile-local root index of every site (scan path)
     Lat* lat = nullptr; Ctl* ctl = nullptr; Rec* rec_now = nullptr;
     Rec* series = nullptr; Rec* series_owned = nullptr;
     int64_t series_cap = DEFAULT_SERIES_CAP;       // sweeps retained; the ring has series_cap + 1 slots
@@ -151,7 +152,6 @@ TileKind pick_tile(int L, int path) {
     if (path == 3) return L % 256 == 0 ? TILE_256x32 : TILE_NONE;
     if (path == 4) return L % 64 == 0 ? SCAN_2 : TILE_NONE;
     if (path == 5) return L % 128 == 0 ? SCAN_4 : TILE_NONE;
-    if (path == 7) return L % 256 == 0 ? WORD_8 : TILE_NONE;
     if (L % 256 == 0) return SCAN_8;
     if (L % 128 == 0) return SCAN_4;
     if (L % 64 == 0) return SCAN_2;
@@ -194,7 +194,7 @@ int launch_label_tiled(sw_handle* h) {
         h->label, h->bondE, h->bondS, h->L, h->N, h->words);
     SW_MARK(h, K_SIZES);
     k_roots_open<C::CAP><<<grid1((size_t)tiles * 32, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
-        h->label, h->olist, h->ocount, h->gsize, h->series, h->ctl, tiles, h->N, h->nb);
+        h->label, h->olist, h->ocount, h->gsize, h->series, h->ctl, tiles, h->N, h->nb, 0);
     SW_MARK(h, K_COMPRESS);
     k_compress_tiled<<<grid1((size_t)h->N / 4, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
         h->label, h->series, h->ctl, h->N, h->nb, 1);
@@ -210,25 +210,15 @@ template <int NW>
 int launch_bond_label_scan(sw_handle* h, bool fused) {
     constexpr int TW = 32 * NW, CAP = 2 * (TW + SCAN_TH);
     const int tiles = h->N / (TW * SCAN_TH);
-    if (NW == 8 && h->tile == WORD_8) {       // thread-per-word labelling (sw_word.cuh)
-        SW_MARK(h, fused ? K_BONDLABEL : K_TILE);
-        if (fused)
-            k_word_label<8, SCAN_TH, true><<<dim3(tiles, h->nb), 8 * SCAN_TH, 0, h->stream>>>(
-                h->spins, h->bondE, h->bondS, h->label, h->olist, h->ocount, h->series, h->lat, h->ctl,
-                h->L, h->N, h->words, h->nb);
-        else
-            k_word_label<8, SCAN_TH, false><<<dim3(tiles, h->nb), 8 * SCAN_TH, 0, h->stream>>>(
-                h->spins, h->bondE, h->bondS, h->label, h->olist, h->ocount, h->series, h->lat, h->ctl,
-                h->L, h->N, h->words, h->nb);
-    } else if (fused) {
+    if (fused) {
         SW_MARK(h, K_BONDLABEL);
         k_bond_label<NW, true><<<dim3(tiles, h->nb), 32 * NW, 0, h->stream>>>(
-            h->spins, h->bondE, h->bondS, h->label, h->olist, h->ocount, h->series, h->lat, h->ctl,
+            h->spins, h->bondE, h->bondS, h->label, h->lab16, h->olist, h->ocount, h->series, h->lat, h->ctl,
             h->L, h->N, h->words, h->nb);
     } else {
         SW_MARK(h, K_TILE);
         k_bond_label<NW, false><<<dim3(tiles, h->nb), 32 * NW, 0, h->stream>>>(
-            h->spins, h->bondE, h->bondS, h->label, h->olist, h->ocount, h->series, h->lat, h->ctl,
+            h->spins, h->bondE, h->bondS, h->label, h->lab16, h->olist, h->ocount, h->series, h->lat, h->ctl,
             h->L, h->N, h->words, h->nb);
     }
     const size_t nedge = (size_t)h->L * (h->L / TW + h->L / SCAN_TH);
@@ -237,7 +227,7 @@ int launch_bond_label_scan(sw_handle* h, bool fused) {
         h->label, h->bondE, h->bondS, h->L, h->N, h->words);
     SW_MARK(h, K_SIZES);
     k_roots_open<CAP><<<grid1((size_t)tiles * 32, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
-        h->label, h->olist, h->ocount, h->gsize, h->series, h->ctl, tiles, h->N, h->nb);
+        h->label, h->olist, h->ocount, h->gsize, h->series, h->ctl, tiles, h->N, h->nb, 1);
     h->launches += 3;
     return SW_OK;
 }
@@ -247,9 +237,14 @@ int launch_flip_scan(sw_handle* h) {
     constexpr int TW = 32 * NW, CAP = 2 * (TW + SCAN_TH);
     const int tiles = h->N / (TW * SCAN_TH);
     SW_MARK(h, K_FLIPTILE);
-    k_flip_tile<NW><<<dim3(tiles, h->nb), 32 * NW, 0, h->stream>>>(
-        h->spins, h->label, h->D, h->series, h->ctl, make_div(h->L), h->L, h->N, h->words, h->nb,
-        h->eager_labels ? 1 : 0);
+    k_flip16<NW><<<dim3(tiles, h->nb), 32 * NW, 0, h->stream>>>(
+        h->spins, h->label, h->lab16, h->D, h->olist, h->ocount, h->series, h->ctl, make_div(h->L),
+        h->L, h->N, h->words, h->nb);
+    if (h->eager_labels) {                          // a4 every sweep instead of on demand
+        k_compress_tiled<<<grid1((size_t)h->N / 4, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
+            h->label, h->series, h->ctl, h->N, h->nb, 0);
+        h->launches += 1;
+    }
     SW_MARK(h, K_SIZES_RESET);
     k_sizes_reset<CAP><<<grid1((size_t)tiles * 32, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
         h->olist, h->ocount, h->gsize, tiles, h->N);
@@ -282,7 +277,7 @@ int launch_label_scan(sw_handle* h) {
     if (rc) return rc;
     SW_MARK(h, K_COMPRESS);
     k_compress_tiled<<<grid1((size_t)h->N / 4, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
-        h->label, h->series, h->ctl, h->N, h->nb, 1);
+        h->label, h->series, h->ctl, h->N, h->nb, 0);   // roots are counted by bond_label + roots_open
     SW_MARK(h, K_SIZES_RESET);
     k_sizes_reset<CAP><<<grid1((size_t)tiles * 32, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
         h->olist, h->ocount, h->gsize, tiles, h->N);
@@ -294,8 +289,7 @@ int launch_label(sw_handle* h) {
     switch (h->tile) {
         case SCAN_2:      return launch_label_scan<2>(h);
         case SCAN_4:      return launch_label_scan<4>(h);
-        case SCAN_8:
-        case WORD_8:      return launch_label_scan<8>(h);
+        case SCAN_8:      return launch_label_scan<8>(h);
         case TILE_64x64:  return launch_label_tiled<64, 64>(h);
         case TILE_256x32: return launch_label_tiled<256, 32>(h);
         default:          return launch_label_generic(h);
@@ -374,7 +368,7 @@ int init_handle(sw_handle* h, const double* T, const uint64_t* seed) {
     char* w = h->ws;
     h->spins = (int8_t*)(w + o.spins);
     h->bondE = (uint32_t*)(w + o.bondE); h->bondS = (uint32_t*)(w + o.bondS); h->D = (uint32_t*)(w + o.D);
-    h->label = (int*)(w + o.label); h->gsize = (int*)(w + o.gsize);
+    h->label = (int*)(w + o.label); h->gsize = (int*)(w + o.gsize); h->lab16 = (uint16_t*)(w + o.lab16);
     h->olist = (int2*)(w + o.olist); h->ocount = (int*)(w + o.ocount);
     h->lat = (Lat*)(w + o.lat); h->ctl = (Ctl*)(w + o.ctl); h->rec_now = (Rec*)(w + o.rec_now);
     h->series = (Rec*)(w + o.series);
@@ -651,7 +645,7 @@ int sw_stage_ms(sw_handle* h, float out[4]) {
 }
 
 int sw_set_path(sw_handle* h, int path) {
-    if (!h || path < 0 || path > 7) { set_err("sw_set_path: invalid argument"); return SW_EINVAL; }
+    if (!h || path < 0 || path > 6) { set_err("sw_set_path: invalid argument"); return SW_EINVAL; }
     h->path = path;
     h->tile = pick_tile(h->L, path);
     return SW_OK;

@@ -58,7 +58,7 @@ __device__ __forceinline__ int div_l(int v, const DivL& D) {
 template <int NW, bool FUSE>
 __global__ void __launch_bounds__(32 * NW)
 k_bond_label(const int8_t* __restrict__ spins, uint32_t* bondE, uint32_t* bondS,
-             int* __restrict__ label, int2* __restrict__ olist, int* __restrict__ ocount,
+             int* __restrict__ label, uint16_t* __restrict__ lab16, int2* __restrict__ olist, int* __restrict__ ocount,
              Rec* __restrict__ rec, const Lat* __restrict__ lat, const Ctl* __restrict__ ctl,
              int L, int N, int words, int nb) {
     constexpr int TW = 32 * NW, TH = SCAN_TH, SITES = TW * TH, THREADS = 32 * NW;
@@ -67,7 +67,7 @@ k_bond_label(const int8_t* __restrict__ spins, uint32_t* bondE, uint32_t* bondS,
     __shared__ uint2 es[TH * NW];              // [row][strip] = (East word, South word)
     __shared__ uint32_t nIn[NW];               // South bonds entering from the tile above, per strip
     __shared__ uint32_t wIn;                   // East bonds entering from the tile to the West, bit = row
-    __shared__ int s_nopen, s_max;
+    __shared__ int s_nopen, s_max, s_nclosed;
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int tilesX = L / TW;
@@ -80,7 +80,7 @@ k_bond_label(const int8_t* __restrict__ spins, uint32_t* bondE, uint32_t* bondS,
     const uint32_t tlo = (uint32_t)t, thi = (uint32_t)(t >> 32);
 
     if (tid < NW) nIn[tid] = 0;
-    if (tid == 0) { wIn = 0; s_nopen = 0; s_max = 0; }
+    if (tid == 0) { wIn = 0; s_nopen = 0; s_max = 0; s_nclosed = 0; }
     __syncthreads();
 
     // ---- phase 1: bonds of the tile, PAPER.md:37-39 (section 2.1) --------------------------------------
@@ -246,7 +246,11 @@ k_bond_label(const int8_t* __restrict__ spins, uint32_t* bondE, uint32_t* bondS,
         g.y = tilebase + (r[1] >> LOG_TW) * L + (r[1] & (TW - 1));
         g.z = tilebase + (r[2] >> LOG_TW) * L + (r[2] & (TW - 1));
         g.w = tilebase + (r[3] >> LOG_TW) * L + (r[3] & (TW - 1));
-        *reinterpret_cast<int4*>(glab + (size_t)(y0 + (l >> LOG_TW)) * L + x0 + (l & (TW - 1))) = g;
+        const size_t gsite = (size_t)(y0 + (l >> LOG_TW)) * L + x0 + (l & (TW - 1));
+        *reinterpret_cast<int4*>(glab + gsite) = g;
+        // the same roots as tile-local 16-bit indices: what the assignment kernel reads (2 B / site)
+        *reinterpret_cast<uint2*>(lab16 + (size_t)blockIdx.y * N + gsite) =
+            make_uint2((uint32_t)r[0] | ((uint32_t)r[1] << 16), (uint32_t)r[2] | ((uint32_t)r[3] << 16));
         // sizes: one shared atomic per group of equal neighbours in the quad
         uint32_t acc = 1u << CNT_SHIFT;
 #pragma unroll
@@ -263,7 +267,7 @@ k_bond_label(const int8_t* __restrict__ spins, uint32_t* bondE, uint32_t* bondS,
 
     // ---- phase 5: closed clusters are complete -> maximum; open ones -> the tile's list -----------------
     {
-        int mymax = 0;
+        int mymax = 0, nclosed = 0;
         int2* mylist = olist + ((size_t)blockIdx.y * gridDim.x + blockIdx.x) * CAP;
         while (rootbits) {
             const int l = mybase + __ffs(rootbits) - 1;
@@ -275,59 +279,90 @@ k_bond_label(const int8_t* __restrict__ spins, uint32_t* bondE, uint32_t* bondS,
                 mylist[pos] = make_int2(tilebase + (l >> LOG_TW) * L + (l & (TW - 1)), cnt);
             } else {
                 mymax = max(mymax, cnt);
+                ++nclosed;                                           // a closed tile root is a cluster root
             }
         }
         mymax = warp_max_i(mymax);
+        nclosed = warp_sum_i(nclosed);
         if (lane == 0 && mymax) atomicMax(&s_max, mymax);
+        if (lane == 0 && nclosed) atomicAdd(&s_nclosed, nclosed);
     }
     __syncthreads();
     if (tid == 0) {
         ocount[(size_t)blockIdx.y * gridDim.x + blockIdx.x] = s_nopen;
-        if (s_max) atomic_max_ll(&rec[(size_t)ctl->slot * nb + blockIdx.y].maxcl, s_max);
+        Rec* rc = rec + (size_t)ctl->slot * nb + blockIdx.y;
+        if (s_max) atomic_max_ll(&rc->maxcl, s_max);
+        if (s_nclosed) atomic_add_ll(&rc->ncl, s_nclosed);
     }
 }
 
 // ---------------------------------------------------------------------------------------------------
-// a4-a7 fused: root of every site (two hops: site -> tile root -> global root, the second through a
-// shared-memory copy of the tile's labels), assignment PAPER.md:57 (section 2.4), and the observables
-// of the new configuration PAPER.md:63 (section 2.5).  One CTA per tile, 32 sites per thread.
-// write_labels != 0 also stores the flat labels (a4); otherwise sw_labels() flattens on demand.
+// a4-a7 fused: assignment PAPER.md:57 (section 2.4) and the observables of the new configuration
+// PAPER.md:63 (section 2.5).  One CTA per tile (the tiles of k_bond_label), 32 sites per thread.
+//
+// The decision of a site is the decision bit of its cluster root.  The kernel first builds, in shared
+// memory, one decision bit per TILE ROOT, indexed by the root's tile-local index:
+//   closed tile root g (cluster inside the tile): the cluster root is g itself -> bit D[g]: the tile's own
+//                      words of the decision plane, copied in bulk;
+//   open tile root g:  its cluster root R was found by k_roots_open and sits next to g in the tile's list ->
+//                      bit D[R] overwrites the copied bit (a few hundred per tile).
+// Then every site reads its 16-bit tile-local root index (2 B / site, written by k_bond_label) and looks the
+// bit up in shared memory: no global gather, no index arithmetic per site.
 // ---------------------------------------------------------------------------------------------------
 template <int NW>
 __global__ void __launch_bounds__(32 * NW)
-k_flip_tile(int8_t* __restrict__ spins, int* label, const uint32_t* __restrict__ D,
-            Rec* __restrict__ rec, const Ctl* __restrict__ ctl, DivL dv,
-            int L, int N, int words, int nb, int write_labels) {
+k_flip16(int8_t* __restrict__ spins, const int* __restrict__ label, const uint16_t* __restrict__ lab16,
+         const uint32_t* __restrict__ D, const int2* __restrict__ olist, const int* __restrict__ ocount,
+         Rec* __restrict__ rec, const Ctl* __restrict__ ctl, DivL dv, int L, int N, int words, int nb) {
     constexpr int TW = 32 * NW, TH = SCAN_TH, SITES = TW * TH, THREADS = 32 * NW;
-    constexpr int QSTEPS = SITES / 4 / THREADS;      // = 8
-    __shared__ __align__(16) int lab[SITES];
+    constexpr int CAP = 2 * (TW + TH);
+    constexpr int OSTEPS = SITES / 8 / THREADS;      // = 4
+    constexpr int LOG_TW = 5 + (NW == 8 ? 3 : NW == 4 ? 2 : NW == 2 ? 1 : 0);
+    __shared__ uint32_t dec[TH * NW];                // decision bit of the tile root with local index l: bit l & 31 of word l >> 5
     __shared__ uint32_t neg[TH * NW];                // sign words of the new spins: bit = (spin == -1)
     __shared__ uint32_t southRow[NW];                // new spins of the row below the tile
     __shared__ uint32_t eastCol;                     // new spins of the column East of the tile, bit = row
-    __shared__ int s_red[3];                         // E, M, ncl of the tile
+    __shared__ int s_red[2];                         // E, M of the tile
 
     const int tid = threadIdx.x, lane = tid & 31;
     const int tilesX = L / TW;
     const int ty = blockIdx.x / tilesX, tx = blockIdx.x - ty * tilesX;
     const int y0 = ty * TH, x0 = tx * TW;
-    int* glab = label + (size_t)blockIdx.y * N;
+    const int tilebase = y0 * L + x0;
+    const int* glab = label + (size_t)blockIdx.y * N;
     const uint32_t* d = D + (size_t)blockIdx.y * words;
+    const size_t tile = (size_t)blockIdx.y * gridDim.x + blockIdx.x;
 
-    neg[tid] = 0;
-    if (tid < NW) southRow[tid] = 0;
-    if (tid == 0) { eastCol = 0; s_red[0] = 0; s_red[1] = 0; s_red[2] = 0; }
-
-    // stage the tile's labels (coalesced 128-bit loads)
-    int4 v[QSTEPS];
+    // my sites' tile-root indices: issue the loads first
+    uint4 v[OSTEPS];
 #pragma unroll
-    for (int k = 0; k < QSTEPS; ++k) {
-        const int q = k * THREADS + tid;
-        const int row = (4 * q) / TW, col = (4 * q) - row * TW;
-        v[k] = *reinterpret_cast<const int4*>(glab + (size_t)(y0 + row) * L + x0 + col);
-        *reinterpret_cast<int4*>(lab + 4 * q) = v[k];
+    for (int k = 0; k < OSTEPS; ++k) {
+        const int l = 8 * (k * THREADS + tid);
+        v[k] = ld_stream_u4(lab16 + (size_t)blockIdx.y * N + (size_t)(y0 + (l >> LOG_TW)) * L + x0 + (l & (TW - 1)));
     }
+    {
+        const int row = tid / NW, wx = tid - row * NW;
+        dec[tid] = d[(size_t)(y0 + row) * (L >> 5) + (x0 >> 5) + wx];
+        neg[tid] = 0;
+    }
+    if (tid < NW) southRow[tid] = 0;
+    if (tid == 0) { eastCol = 0; s_red[0] = 0; s_red[1] = 0; }
     __syncthreads();
 
+    // open tile roots take the decision of their cluster root
+    {
+        const int n = ocount[tile];
+        const int2* mylist = olist + tile * CAP;
+        for (int e = tid; e < n; e += THREADS) {
+            const int2 it = mylist[e];                                 // (tile root, cluster root)
+            const uint32_t up = (__ldg(d + (it.y >> 5)) >> (it.y & 31)) & 1u;
+            const int delta = it.x - tilebase;
+            const int ry = div_l(delta, dv);
+            const int l = ry * TW + (delta - ry * L);
+            if (up) atomicOr(&dec[l >> 5], 1u << (l & 31));
+            else    atomicAnd(&dec[l >> 5], ~(1u << (l & 31)));
+        }
+    }
     // halo: the new spin of a site outside the tile is the decision bit of its own root (three loads)
     for (int j = tid; j < TH + TW; j += THREADS) {
         int site;
@@ -341,40 +376,24 @@ k_flip_tile(int8_t* __restrict__ spins, int* label, const uint32_t* __restrict__
             else        atomicOr(&southRow[(j - TH) >> 5], 1u << ((j - TH) & 31));
         }
     }
+    __syncthreads();
 
-    const int tilebase = y0 * L + x0;
-    int m = 0, nroot = 0;
+    int m = 0;
 #pragma unroll
-    for (int k = 0; k < QSTEPS; ++k) {
-        const int q = k * THREADS + tid;
-        const int row = (4 * q) / TW, col = (4 * q) - row * TW;
-        const int g[4] = { v[k].x, v[k].y, v[k].z, v[k].w };
-        int R[4];
-        uint32_t nib = 0, out = 0;
+    for (int k = 0; k < OSTEPS; ++k) {
+        const int l = 8 * (k * THREADS + tid);
+        const uint32_t w4[4] = { v[k].x, v[k].y, v[k].z, v[k].w };
+        uint32_t b8 = 0;                                               // bit u: site l + u goes up
 #pragma unroll
-        for (int u = 0; u < 4; ++u) {
-            // g is this site's tile root (inside the tile: its word holds the cluster root), or -- when the
-            // site is itself a hooked tile root -- already the cluster root, possibly outside the tile
-            const uint32_t delta = (uint32_t)(g[u] - tilebase);
-            R[u] = g[u];
-            if (delta < (uint32_t)(TH * L)) {
-                const int ry = div_l((int)delta, dv);
-                const int rc = (int)delta - ry * L;
-                if (rc < TW) R[u] = lab[ry * TW + rc];
-            }
+        for (int u = 0; u < 8; ++u) {
+            const uint32_t r = (u & 1) ? (w4[u >> 1] >> 16) : (w4[u >> 1] & 0xFFFFu);
+            b8 |= (__funnelshift_r(dec[r >> 5], 0u, r) & 1u) << u;
         }
-        const int self = (y0 + row) * L + x0 + col;
-#pragma unroll
-        for (int u = 0; u < 4; ++u) {
-            const uint32_t up = (__ldg(d + (R[u] >> 5)) >> (R[u] & 31)) & 1u;
-            out |= (up ? 0x01u : 0xFFu) << (8 * u);
-            nib |= (up ^ 1u) << u;
-            nroot += (R[u] == self + u);
-        }
-        m += 4 - 2 * __popc(nib);
-        *reinterpret_cast<uint32_t*>(spins + (size_t)blockIdx.y * N + self) = out;
-        if (write_labels) *reinterpret_cast<int4*>(glab + self) = make_int4(R[0], R[1], R[2], R[3]);
-        if (nib) atomicOr(&neg[row * NW + (col >> 5)], nib << (col & 31));
+        m += 2 * __popc(b8) - 8;
+        *reinterpret_cast<uint2*>(spins + (size_t)blockIdx.y * N + (size_t)(y0 + (l >> LOG_TW)) * L + x0 + (l & (TW - 1))) =
+            make_uint2(spin_bytes4(b8 & 15u), spin_bytes4(b8 >> 4));
+        const uint32_t nb8 = b8 ^ 0xFFu;
+        if (nb8) atomicOr(&neg[l >> 5], nb8 << (l & 31));
     }
     __syncthreads();
 
@@ -388,14 +407,13 @@ k_flip_tile(int8_t* __restrict__ spins, int* label, const uint32_t* __restrict__
         const uint32_t eastm = (own >> 1) | (eb << 31);
         e = 64 - 2 * (__popc(~(own ^ eastm)) + __popc(~(own ^ south)));
     }
-    e = warp_sum_i(e); m = warp_sum_i(m); nroot = warp_sum_i(nroot);
-    if (lane == 0) { atomicAdd(&s_red[0], e); atomicAdd(&s_red[1], m); atomicAdd(&s_red[2], nroot); }
+    e = warp_sum_i(e); m = warp_sum_i(m);
+    if (lane == 0) { atomicAdd(&s_red[0], e); atomicAdd(&s_red[1], m); }
     __syncthreads();
     if (tid == 0) {
         Rec* r = rec + (size_t)ctl->slot * nb + blockIdx.y;
         if (s_red[0]) atomic_add_ll(&r->E, s_red[0]);
         if (s_red[1]) atomic_add_ll(&r->M, s_red[1]);
-        if (s_red[2]) atomic_add_ll(&r->ncl, s_red[2]);
     }
 }
 

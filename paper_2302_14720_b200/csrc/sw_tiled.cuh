@@ -286,15 +286,17 @@ k_compress_tiled(int* label, Rec* __restrict__ rec, const Ctl* __restrict__ ctl,
 // After the merge: every open tile-local root is pointed straight at its global root (find + write
 // back), and the sizes of the clusters that span tiles are accumulated: each open piece adds its size
 // to its root's accumulator; the running total returned by the atomic peaks at the full size.
-// One warp per tile.
+// The list entry (tile root, size) becomes (tile root, cluster root) for the assignment kernel.
+// count_roots != 0 (scan path): open tile roots that are cluster roots are counted here (closed ones
+// were counted by k_bond_label).  One warp per tile.
 template <int CAP>
 __global__ void __launch_bounds__(ROW_THREADS)
 k_roots_open(int* label, int2* __restrict__ olist, const int* __restrict__ ocount,
              int* __restrict__ gsize, Rec* __restrict__ rec, const Ctl* __restrict__ ctl,
-             int tiles, int N, int nb) {
+             int tiles, int N, int nb, int count_roots) {
     const int tile = blockIdx.x * (ROW_THREADS / 32) + (threadIdx.x >> 5);
     const int lane = threadIdx.x & 31;
-    int m = 0;
+    int m = 0, nroot = 0;
     if (tile < tiles) {
         const size_t t = (size_t)blockIdx.y * tiles + tile;
         int* lab = label + (size_t)blockIdx.y * N;
@@ -306,14 +308,20 @@ k_roots_open(int* label, int2* __restrict__ olist, const int* __restrict__ ocoun
             if (p != it.x) {                                // hooked: walk to the root, point at it
                 R = uf_find(lab, p);
                 if (R != p) lab[it.x] = R;                  // only ever an ancestor: safe while others walk
+            } else {
+                ++nroot;
             }
             const int tot = atomicAdd(gsize + (size_t)blockIdx.y * N + R, it.y) + it.y;
             m = max(m, tot);
-            olist[t * CAP + e].x = R;
+            olist[t * CAP + e].y = R;
         }
     }
     m = warp_max_i(m);
     if (lane == 0 && m) atomic_max_ll(&rec[(size_t)ctl->slot * nb + blockIdx.y].maxcl, m);
+    if (count_roots) {
+        nroot = warp_sum_i(nroot);
+        if (lane == 0 && nroot) atomic_add_ll(&rec[(size_t)ctl->slot * nb + blockIdx.y].ncl, nroot);
+    }
 }
 
 template <int CAP>
@@ -325,7 +333,7 @@ k_sizes_reset(const int2* __restrict__ olist, const int* __restrict__ ocount, in
     if (tile >= tiles) return;
     const size_t t = (size_t)blockIdx.y * tiles + tile;
     const int n = ocount[t];
-    for (int e = lane; e < n; e += 32) gsize[(size_t)blockIdx.y * N + olist[t * CAP + e].x] = 0;
+    for (int e = lane; e < n; e += 32) gsize[(size_t)blockIdx.y * N + olist[t * CAP + e].y] = 0;
 }
 
 // ---------------------------------------------------------------------------------------------
