@@ -139,6 +139,7 @@ struct sw_handle {
     int64_t last_n = 0;
     int path = 0; TileKind tile = TILE_NONE;
     bool timing = false; std::vector<cudaEvent_t> ev; int64_t timed_sweeps = 0;
+    cudaEvent_t ev_tail[2] = { nullptr, nullptr };   // around the trailing k_observe_rows of a call
     int ev_cursor = 0; std::vector<int> ev_seq;   // kernel ids in launch order within one sweep
     int64_t cur_sweep = 0;
     int64_t launches = 0;
@@ -207,19 +208,19 @@ int launch_label_tiled(sw_handle* h) {
 
 // fast path: fused bond + scan-line tile labelling, global merge, open roots (a1-a3)
 template <int NW>
-int launch_bond_label_scan(sw_handle* h, bool fused) {
+int launch_bond_label_scan(sw_handle* h, bool fused, bool obs_prev) {
     constexpr int TW = 32 * NW, CAP = 2 * (TW + SCAN_TH);
     const int tiles = h->N / (TW * SCAN_TH);
     if (fused) {
         SW_MARK(h, K_BONDLABEL);
         k_bond_label<NW, true><<<dim3(tiles, h->nb), 32 * NW, 0, h->stream>>>(
             h->spins, h->bondE, h->bondS, h->label, h->lab16, h->olist, h->ocount, h->series, h->lat, h->ctl,
-            h->L, h->N, h->words, h->nb);
+            h->L, h->N, h->words, h->nb, obs_prev ? 1 : 0);
     } else {
         SW_MARK(h, K_TILE);
         k_bond_label<NW, false><<<dim3(tiles, h->nb), 32 * NW, 0, h->stream>>>(
             h->spins, h->bondE, h->bondS, h->label, h->lab16, h->olist, h->ocount, h->series, h->lat, h->ctl,
-            h->L, h->N, h->words, h->nb);
+            h->L, h->N, h->words, h->nb, obs_prev ? 1 : 0);
     }
     const size_t nedge = (size_t)h->L * (h->L / TW + h->L / SCAN_TH);
     SW_MARK(h, K_MERGE);
@@ -238,8 +239,7 @@ int launch_flip_scan(sw_handle* h) {
     const int tiles = h->N / (TW * SCAN_TH);
     SW_MARK(h, K_FLIPTILE);
     k_flip16<NW><<<dim3(tiles, h->nb), 32 * NW, 0, h->stream>>>(
-        h->spins, h->label, h->lab16, h->D, h->olist, h->ocount, h->series, h->ctl, make_div(h->L),
-        h->L, h->N, h->words, h->nb);
+        h->spins, h->lab16, h->D, h->olist, h->ocount, make_div(h->L), h->L, h->N, h->words);
     if (h->eager_labels) {                          // a4 every sweep instead of on demand
         k_compress_tiled<<<grid1((size_t)h->N / 4, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
             h->label, h->series, h->ctl, h->N, h->nb, 0);
@@ -273,7 +273,7 @@ template <int NW>
 int launch_label_scan(sw_handle* h) {
     constexpr int TW = 32 * NW, CAP = 2 * (TW + SCAN_TH);
     const int tiles = h->N / (TW * SCAN_TH);
-    int rc = launch_bond_label_scan<NW>(h, false);
+    int rc = launch_bond_label_scan<NW>(h, false, false);
     if (rc) return rc;
     SW_MARK(h, K_COMPRESS);
     k_compress_tiled<<<grid1((size_t)h->N / 4, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
@@ -302,14 +302,15 @@ int launch_sweep(sw_handle* h, int64_t k) {
     h->cur_sweep = k; h->ev_cursor = 0;
     if (const int nw = scan_nw(h->tile)) {
         const bool fused = h->path != 6;
+        const bool obs_prev = k > 0;                    // E, M of sweep k - 1 come out of this sweep's bond test
         if (!fused) {                                   // stand-alone a1 for the per-stage split
             SW_MARK(h, K_BOND);
             k_bond_rows<<<grid1(h->words, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
-                h->spins, h->bondE, h->bondS, h->lat, h->ctl, h->L, h->N, h->words);
+                h->spins, h->bondE, h->bondS, h->lat, h->ctl, h->L, h->N, h->words, h->series, h->nb, obs_prev ? 1 : 0);
             h->launches += 1;
         }
-        rc = nw == 8 ? launch_bond_label_scan<8>(h, fused) : nw == 4 ? launch_bond_label_scan<4>(h, fused)
-                                                                     : launch_bond_label_scan<2>(h, fused);
+        rc = nw == 8 ? launch_bond_label_scan<8>(h, fused, obs_prev) : nw == 4 ? launch_bond_label_scan<4>(h, fused, obs_prev)
+                                                                               : launch_bond_label_scan<2>(h, fused, obs_prev);
         if (rc) return rc;
         SW_MARK(h, K_FLIPBITS);
         k_flipbits<<<grid1(((size_t)h->words + 3) / 4, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(
@@ -329,7 +330,7 @@ int launch_sweep(sw_handle* h, int64_t k) {
     SW_MARK(h, K_BOND);
     if (h->tile != TILE_NONE)
         k_bond_rows<<<grid1(h->words, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
-            h->spins, h->bondE, h->bondS, h->lat, h->ctl, h->L, h->N, h->words);
+            h->spins, h->bondE, h->bondS, h->lat, h->ctl, h->L, h->N, h->words, h->series, h->nb, 0);
     else
         k_bond_generic<<<grid1(h->words, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(
             h->spins, h->bondE, h->bondS, h->lat, h->ctl, h->L, h->N, h->words);
@@ -456,6 +457,7 @@ void sw_destroy(sw_handle* h) {
     if (!h) return;
     cudaStreamSynchronize(h->stream);
     for (cudaEvent_t e : h->ev) cudaEventDestroy(e);
+    for (cudaEvent_t e : h->ev_tail) if (e) cudaEventDestroy(e);
     if (h->series_owned) cudaFree(h->series_owned);
     if (h->owns_ws) cudaFree(h->ws);
     (void)cudaGetLastError();
@@ -467,6 +469,8 @@ int sw_sweep(sw_handle* h, int64_t n) {
     if (n == 0) return SW_OK;
     h->launches = 0;
     if (h->timing) {
+        for (int i = 0; i < 2; ++i)
+            if (!h->ev_tail[i]) SW_CUDA(cudaEventCreate(&h->ev_tail[i]));
         const size_t need = (size_t)std::min<int64_t>(n, MAX_TIMED_SWEEPS) * EV_PER_SWEEP;
         while (h->ev.size() < need) {
             cudaEvent_t e; SW_CUDA(cudaEventCreate(&e));
@@ -480,6 +484,13 @@ int sw_sweep(sw_handle* h, int64_t n) {
     for (int64_t k = 0; k < n; ++k) {
         int rc = launch_sweep(h, k);
         if (rc) return rc;
+    }
+    if (scan_nw(h->tile)) {                             // a7 of the configuration the call ends with
+        if (h->timing) SW_CUDA(cudaEventRecord(h->ev_tail[0], h->stream));
+        k_observe_rows<<<grid1(h->words, 256, h->nb), 256, 0, h->stream>>>(
+            h->spins, h->series, h->ctl, h->L, h->N, h->words, h->nb);
+        if (h->timing) SW_CUDA(cudaEventRecord(h->ev_tail[1], h->stream));
+        h->launches += 1;
     }
     SW_CUDA(cudaGetLastError());
     h->t += (uint64_t)n;
@@ -629,6 +640,11 @@ int sw_kernel_ms(sw_handle* h, float* out, int32_t cap) {
             SW_CUDA(cudaEventElapsedTime(&ms, h->ev[(size_t)k * EV_PER_SWEEP + j], h->ev[(size_t)k * EV_PER_SWEEP + j + 1]));
             if (h->ev_seq[j] < cap) out[h->ev_seq[j]] += ms;
         }
+    if (scan_nw(h->tile) && K_ENERGY < cap) {           // the trailing observables pass of the call
+        float ms = 0.f;
+        SW_CUDA(cudaEventElapsedTime(&ms, h->ev_tail[0], h->ev_tail[1]));
+        out[K_ENERGY] += ms;
+    }
     return K_COUNT;
 }
 

@@ -16,9 +16,9 @@
 //                sizes counted into the spare bits of the root's parent word, open flags
 //       phase 5  closed clusters -> running maximum; open clusters -> the tile's list (root, size)
 //   a3    k_merge_tiled / k_roots_open (sw_tiled.cuh): global boundary merge on the int32 parent array
-//   a4-a7 k_flip_tile<NW>: root of every site in two hops through a shared-memory copy of the tile's labels,
-//         spins = gather(D, root), magnetisation, cluster count, and the energy of the NEW configuration
-//         (the new spins of the East / South halo are resolved through their own roots)
+//   a4-a6 k_flip16<NW>: one decision bit per tile root in shared memory, spins = lookup by 16-bit tile-local root
+//   a7    E, M of a configuration: by-product of the next sweep's bond test (k_bond_label), k_observe_rows at
+//         the end of a call; cluster count and largest cluster: k_bond_label + k_roots_open
 #pragma once
 #include "sw_common.cuh"
 
@@ -60,14 +60,14 @@ __global__ void __launch_bounds__(32 * NW)
 k_bond_label(const int8_t* __restrict__ spins, uint32_t* bondE, uint32_t* bondS,
              int* __restrict__ label, uint16_t* __restrict__ lab16, int2* __restrict__ olist, int* __restrict__ ocount,
              Rec* __restrict__ rec, const Lat* __restrict__ lat, const Ctl* __restrict__ ctl,
-             int L, int N, int words, int nb) {
+             int L, int N, int words, int nb, int obs_prev) {
     constexpr int TW = 32 * NW, TH = SCAN_TH, SITES = TW * TH, THREADS = 32 * NW;
     constexpr int CAP = 2 * (TW + TH);
     __shared__ __align__(16) int par[SITES];   // parent, tile-local index (+ size / open bits at roots)
     __shared__ uint2 es[TH * NW];              // [row][strip] = (East word, South word)
     __shared__ uint32_t nIn[NW];               // South bonds entering from the tile above, per strip
     __shared__ uint32_t wIn;                   // East bonds entering from the tile to the West, bit = row
-    __shared__ int s_nopen, s_max, s_nclosed;
+    __shared__ int s_nopen, s_max, s_nclosed, s_obs[2];
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int tilesX = L / TW;
@@ -80,7 +80,7 @@ k_bond_label(const int8_t* __restrict__ spins, uint32_t* bondE, uint32_t* bondS,
     const uint32_t tlo = (uint32_t)t, thi = (uint32_t)(t >> 32);
 
     if (tid < NW) nIn[tid] = 0;
-    if (tid == 0) { wIn = 0; s_nopen = 0; s_max = 0; s_nclosed = 0; }
+    if (tid == 0) { wIn = 0; s_nopen = 0; s_max = 0; s_nclosed = 0; s_obs[0] = 0; s_obs[1] = 0; }
     __syncthreads();
 
     // ---- phase 1: bonds of the tile, PAPER.md:37-39 (section 2.1) --------------------------------------
@@ -111,6 +111,13 @@ k_bond_label(const int8_t* __restrict__ spins, uint32_t* bondE, uint32_t* bondS,
             const uint32_t own = neg_mask32(a0, a1), south = neg_mask32(b0, b1);
             const uint32_t eastm = (own >> 1) | (nx < 0 ? 0x80000000u : 0u);
             const uint32_t eqE = ~(own ^ eastm), eqS = ~(own ^ south);
+            if (obs_prev) {
+                // a7 for free: the equal-pair masks of the bond test are the energy of the
+                // configuration the previous sweep left: E = (#edges) - 2 (#equal pairs), M = N - 2 (#down)
+                const int eo = warp_sum_i(64 - 2 * (__popc(eqE) + __popc(eqS)));
+                const int mo = warp_sum_i(32 - 2 * __popc(own));
+                if (lane == 0) { atomicAdd(&s_obs[0], eo); atomicAdd(&s_obs[1], mo); }
+            }
             uint32_t dE = 0, dS = 0;
 #pragma unroll
             for (int c = 0; c < 16; ++c) {
@@ -293,12 +300,18 @@ k_bond_label(const int8_t* __restrict__ spins, uint32_t* bondE, uint32_t* bondS,
         Rec* rc = rec + (size_t)ctl->slot * nb + blockIdx.y;
         if (s_max) atomic_max_ll(&rc->maxcl, s_max);
         if (s_nclosed) atomic_add_ll(&rc->ncl, s_nclosed);
+        if (FUSE && obs_prev) {                                      // E, M of the previous sweep's configuration
+            Rec* rp = rec + (size_t)(ctl->slot == 0 ? ctl->cap - 1 : ctl->slot - 1) * nb + blockIdx.y;
+            if (s_obs[0]) atomic_add_ll(&rp->E, s_obs[0]);
+            if (s_obs[1]) atomic_add_ll(&rp->M, s_obs[1]);
+        }
     }
 }
 
 // ---------------------------------------------------------------------------------------------------
-// a4-a7 fused: assignment PAPER.md:57 (section 2.4) and the observables of the new configuration
-// PAPER.md:63 (section 2.5).  One CTA per tile (the tiles of k_bond_label), 32 sites per thread.
+// a4-a6 fused: assignment PAPER.md:57 (section 2.4).  One CTA per tile (the tiles of k_bond_label), 32 sites
+// per thread.  (a7: E and M of the new configuration fall out of the NEXT sweep's bond test, or of
+// k_observe_rows after the last sweep of a call.)
 //
 // The decision of a site is the decision bit of its cluster root.  The kernel first builds, in shared
 // memory, one decision bit per TILE ROOT, indexed by the root's tile-local index:
@@ -310,26 +323,20 @@ k_bond_label(const int8_t* __restrict__ spins, uint32_t* bondE, uint32_t* bondS,
 // bit up in shared memory: no global gather, no index arithmetic per site.
 // ---------------------------------------------------------------------------------------------------
 template <int NW>
-__global__ void __launch_bounds__(32 * NW)
-k_flip16(int8_t* __restrict__ spins, const int* __restrict__ label, const uint16_t* __restrict__ lab16,
-         const uint32_t* __restrict__ D, const int2* __restrict__ olist, const int* __restrict__ ocount,
-         Rec* __restrict__ rec, const Ctl* __restrict__ ctl, DivL dv, int L, int N, int words, int nb) {
+__global__ void __launch_bounds__(32 * NW, 1536 / (32 * NW))
+k_flip16(int8_t* __restrict__ spins, const uint16_t* __restrict__ lab16, const uint32_t* __restrict__ D,
+         const int2* __restrict__ olist, const int* __restrict__ ocount, DivL dv, int L, int N, int words) {
     constexpr int TW = 32 * NW, TH = SCAN_TH, SITES = TW * TH, THREADS = 32 * NW;
     constexpr int CAP = 2 * (TW + TH);
     constexpr int OSTEPS = SITES / 8 / THREADS;      // = 4
     constexpr int LOG_TW = 5 + (NW == 8 ? 3 : NW == 4 ? 2 : NW == 2 ? 1 : 0);
     __shared__ uint32_t dec[TH * NW];                // decision bit of the tile root with local index l: bit l & 31 of word l >> 5
-    __shared__ uint32_t neg[TH * NW];                // sign words of the new spins: bit = (spin == -1)
-    __shared__ uint32_t southRow[NW];                // new spins of the row below the tile
-    __shared__ uint32_t eastCol;                     // new spins of the column East of the tile, bit = row
-    __shared__ int s_red[2];                         // E, M of the tile
 
-    const int tid = threadIdx.x, lane = tid & 31;
+    const int tid = threadIdx.x;
     const int tilesX = L / TW;
     const int ty = blockIdx.x / tilesX, tx = blockIdx.x - ty * tilesX;
     const int y0 = ty * TH, x0 = tx * TW;
     const int tilebase = y0 * L + x0;
-    const int* glab = label + (size_t)blockIdx.y * N;
     const uint32_t* d = D + (size_t)blockIdx.y * words;
     const size_t tile = (size_t)blockIdx.y * gridDim.x + blockIdx.x;
 
@@ -340,18 +347,14 @@ k_flip16(int8_t* __restrict__ spins, const int* __restrict__ label, const uint16
         const int l = 8 * (k * THREADS + tid);
         v[k] = ld_stream_u4(lab16 + (size_t)blockIdx.y * N + (size_t)(y0 + (l >> LOG_TW)) * L + x0 + (l & (TW - 1)));
     }
+    const int n = ocount[tile];
     {
         const int row = tid / NW, wx = tid - row * NW;
         dec[tid] = d[(size_t)(y0 + row) * (L >> 5) + (x0 >> 5) + wx];
-        neg[tid] = 0;
     }
-    if (tid < NW) southRow[tid] = 0;
-    if (tid == 0) { eastCol = 0; s_red[0] = 0; s_red[1] = 0; }
     __syncthreads();
-
     // open tile roots take the decision of their cluster root
     {
-        const int n = ocount[tile];
         const int2* mylist = olist + tile * CAP;
         for (int e = tid; e < n; e += THREADS) {
             const int2 it = mylist[e];                                 // (tile root, cluster root)
@@ -363,22 +366,8 @@ k_flip16(int8_t* __restrict__ spins, const int* __restrict__ label, const uint16
             else    atomicAnd(&dec[l >> 5], ~(1u << (l & 31)));
         }
     }
-    // halo: the new spin of a site outside the tile is the decision bit of its own root (three loads)
-    for (int j = tid; j < TH + TW; j += THREADS) {
-        int site;
-        if (j < TH) site = (y0 + j) * L + (x0 + TW == L ? 0 : x0 + TW);
-        else        site = (y0 + TH == L ? 0 : y0 + TH) * L + x0 + (j - TH);
-        const int g = glab[site];
-        const int R = glab[g];
-        const uint32_t up = (__ldg(d + (R >> 5)) >> (R & 31)) & 1u;
-        if (!up) {
-            if (j < TH) atomicOr(&eastCol, 1u << j);
-            else        atomicOr(&southRow[(j - TH) >> 5], 1u << ((j - TH) & 31));
-        }
-    }
     __syncthreads();
 
-    int m = 0;
 #pragma unroll
     for (int k = 0; k < OSTEPS; ++k) {
         const int l = 8 * (k * THREADS + tid);
@@ -389,31 +378,42 @@ k_flip16(int8_t* __restrict__ spins, const int* __restrict__ label, const uint16
             const uint32_t r = (u & 1) ? (w4[u >> 1] >> 16) : (w4[u >> 1] & 0xFFFFu);
             b8 |= (__funnelshift_r(dec[r >> 5], 0u, r) & 1u) << u;
         }
-        m += 2 * __popc(b8) - 8;
         *reinterpret_cast<uint2*>(spins + (size_t)blockIdx.y * N + (size_t)(y0 + (l >> LOG_TW)) * L + x0 + (l & (TW - 1))) =
             make_uint2(spin_bytes4(b8 & 15u), spin_bytes4(b8 >> 4));
-        const uint32_t nb8 = b8 ^ 0xFFu;
-        if (nb8) atomicOr(&neg[l >> 5], nb8 << (l & 31));
     }
-    __syncthreads();
+}
 
-    // energy of the new configuration: E = (#edges) - 2 (#equal pairs), one 32-site word per thread
-    int e;
-    {
-        const int row = tid / NW, wx = tid - row * NW;
-        const uint32_t own = neg[tid];
-        const uint32_t eb = wx + 1 < NW ? (neg[tid + 1] & 1u) : ((eastCol >> row) & 1u);
-        const uint32_t south = row + 1 < TH ? neg[tid + NW] : southRow[wx];
-        const uint32_t eastm = (own >> 1) | (eb << 31);
+// a7 of the configuration a sw_sweep call ends with (the sweeps before it get theirs from the next sweep's
+// bond test): E and M from sign masks, 32 sites per thread, into the slot of the sweep that just finished.
+__global__ void __launch_bounds__(256)
+k_observe_rows(const int8_t* __restrict__ spins, Rec* __restrict__ rec, const Ctl* __restrict__ ctl,
+               int L, int N, int words, int nb) {
+    const int w = blockIdx.x * 256 + threadIdx.x;
+    int e = 0, m = 0;
+    if (w < words) {
+        const int wpr = L >> 5;
+        const int y = w / wpr, xw = w - y * wpr;
+        const int8_t* s = spins + (size_t)blockIdx.y * N;
+        const int8_t* row  = s + (size_t)y * L + xw * 32;
+        const int8_t* rowS = s + (size_t)(y + 1 == L ? 0 : y + 1) * L + xw * 32;
+        const uint4 a0 = *reinterpret_cast<const uint4*>(row),  a1 = *reinterpret_cast<const uint4*>(row + 16);
+        const uint4 b0 = *reinterpret_cast<const uint4*>(rowS), b1 = *reinterpret_cast<const uint4*>(rowS + 16);
+        const int8_t nx = s[(size_t)y * L + (xw + 1 == wpr ? 0 : (xw + 1) * 32)];
+        const uint32_t own = neg_mask32(a0, a1), south = neg_mask32(b0, b1);
+        const uint32_t eastm = (own >> 1) | (nx < 0 ? 0x80000000u : 0u);
         e = 64 - 2 * (__popc(~(own ^ eastm)) + __popc(~(own ^ south)));
+        m = 32 - 2 * __popc(own);
     }
     e = warp_sum_i(e); m = warp_sum_i(m);
-    if (lane == 0) { atomicAdd(&s_red[0], e); atomicAdd(&s_red[1], m); }
+    __shared__ int se[8], sm[8];
+    if ((threadIdx.x & 31) == 0) { se[threadIdx.x >> 5] = e; sm[threadIdx.x >> 5] = m; }
     __syncthreads();
-    if (tid == 0) {
-        Rec* r = rec + (size_t)ctl->slot * nb + blockIdx.y;
-        if (s_red[0]) atomic_add_ll(&r->E, s_red[0]);
-        if (s_red[1]) atomic_add_ll(&r->M, s_red[1]);
+    if (threadIdx.x == 0) {
+        int te = 0, tm = 0;
+        for (int k = 0; k < 8; ++k) { te += se[k]; tm += sm[k]; }
+        Rec* r = rec + (size_t)(ctl->slot == 0 ? ctl->cap - 1 : ctl->slot - 1) * nb + blockIdx.y;
+        if (te) atomic_add_ll(&r->E, te);
+        if (tm) atomic_add_ll(&r->M, tm);
     }
 }
 

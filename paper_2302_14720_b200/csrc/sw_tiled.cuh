@@ -29,9 +29,10 @@ constexpr uint32_t OPEN_FLAG = 0x40000000u;
 // ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(ROW_THREADS)
 k_bond_rows(const int8_t* __restrict__ spins, uint32_t* __restrict__ bondE, uint32_t* __restrict__ bondS,
-            const Lat* __restrict__ lat, const Ctl* __restrict__ ctl, int L, int N, int words) {
+            const Lat* __restrict__ lat, const Ctl* __restrict__ ctl, int L, int N, int words,
+            Rec* __restrict__ rec, int nb, int obs_prev) {
     const int w = blockIdx.x * ROW_THREADS + threadIdx.x;
-    if (w >= words) return;
+    if (w >= words) return;                          // (words is a multiple of 32 here: whole warps leave)
     const int wpr = L >> 5;
     const int y = w / wpr, xw = w - y * wpr;
     const int8_t* s = spins + (size_t)blockIdx.y * N;
@@ -43,6 +44,15 @@ k_bond_rows(const int8_t* __restrict__ spins, uint32_t* __restrict__ bondE, uint
     const uint32_t own = neg_mask32(a0, a1), south = neg_mask32(b0, b1);
     const uint32_t eastm = (own >> 1) | (nx < 0 ? 0x80000000u : 0u);
     const uint32_t eqE = ~(own ^ eastm), eqS = ~(own ^ south);
+    if (obs_prev) {     // scan path: E, M of the configuration the previous sweep left (see k_bond_label)
+        const int eo = warp_sum_i(64 - 2 * (__popc(eqE) + __popc(eqS)));
+        const int mo = warp_sum_i(32 - 2 * __popc(own));
+        if ((threadIdx.x & 31) == 0) {
+            Rec* rp = rec + (size_t)(ctl->slot == 0 ? ctl->cap - 1 : ctl->slot - 1) * nb + blockIdx.y;
+            if (eo) atomic_add_ll(&rp->E, eo);
+            if (mo) atomic_add_ll(&rp->M, mo);
+        }
+    }
 
     const Lat la = lat[blockIdx.y];
     const PhiloxKey key(la.key0, la.key1);
@@ -297,24 +307,46 @@ k_roots_open(int* label, int2* __restrict__ olist, const int* __restrict__ ocoun
     const int tile = blockIdx.x * (ROW_THREADS / 32) + (threadIdx.x >> 5);
     const int lane = threadIdx.x & 31;
     int m = 0, nroot = 0;
-    if (tile < tiles) {
+    if (tile < tiles) {                                     // (warp-uniform)
         const size_t t = (size_t)blockIdx.y * tiles + tile;
         int* lab = label + (size_t)blockIdx.y * N;
+        int* gs = gsize + (size_t)blockIdx.y * N;
         const int n = ocount[t];
-        for (int e = lane; e < n; e += 32) {
-            const int2 it = olist[t * CAP + e];
-            const int p = ld_cg(lab + it.x);
-            int R = p;
-            if (p != it.x) {                                // hooked: walk to the root, point at it
-                R = uf_find(lab, p);
-                if (R != p) lab[it.x] = R;                  // only ever an ancestor: safe while others walk
-            } else {
-                ++nroot;
+        // At T_c one cluster owns many pieces in every tile; a per-piece atomic on its accumulator would
+        // serialise in L2.  Pieces are summed per root inside the warp first (match + reduce), and the
+        // root with the largest sum of the first round ("hot") is carried in a register across rounds.
+        int hot = -1, hotacc = 0;
+        for (int e0 = 0; e0 < n; e0 += 32) {
+            const int e = e0 + lane;
+            const bool on = e < n;
+            int R = -1 - lane, sz = 0;                      // idle lanes: distinct keys, nothing to add
+            if (on) {
+                const int2 it = olist[t * CAP + e];
+                const int p = ld_cg(lab + it.x);
+                R = p; sz = it.y;
+                if (p != it.x) {                            // hooked: walk to the root, point at it
+                    R = uf_find(lab, p);
+                    if (R != p) lab[it.x] = R;              // only ever an ancestor: safe while others walk
+                } else {
+                    ++nroot;
+                }
+                olist[t * CAP + e].y = R;
             }
-            const int tot = atomicAdd(gsize + (size_t)blockIdx.y * N + R, it.y) + it.y;
-            m = max(m, tot);
-            olist[t * CAP + e].y = R;
+            const unsigned grp = __match_any_sync(0xffffffffu, R);
+            const int tot = __reduce_add_sync(grp, sz);
+            if (e0 == 0) {                                  // choose the hot root
+                const int best = __reduce_max_sync(0xffffffffu, tot);
+                const unsigned who = __ballot_sync(0xffffffffu, tot == best && on);
+                if (who) hot = __shfl_sync(0xffffffffu, R, __ffs(who) - 1);
+            }
+            const bool leader = on && lane == __ffs(grp) - 1;
+            if (leader) {
+                if (R == hot) hotacc += tot;                // (at most one leader per round has R == hot)
+                else m = max(m, atomicAdd(gs + R, tot) + tot);
+            }
         }
+        hotacc = warp_sum_i(hotacc);
+        if (lane == 0 && hotacc) m = max(m, atomicAdd(gs + hot, hotacc) + hotacc);
     }
     m = warp_max_i(m);
     if (lane == 0 && m) atomic_max_ll(&rec[(size_t)ctl->slot * nb + blockIdx.y].maxcl, m);
