@@ -176,7 +176,7 @@ def main():
     ap.add_argument("--cpu-sample-L", type=int, default=8192, help="sample side for the cpu_baseline leg")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--path", type=int, default=0, help="0 auto (fused scan-line), 1 generic, 2/3 first-generation tiles 64x64 / 256x32, 4/5 scan 64/128 wide, 6 unfused")
+    ap.add_argument("--path", type=int, default=0, help="0 auto (fused scan-line, 256x64 tiles), 1 generic, 2/3 first-generation tiles 64x64 / 256x32, 4/5 scan 64/128 wide, 6 unfused, 7 scan 256x32")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
 
@@ -207,8 +207,10 @@ def main():
     N = L * L
     seed = 6 + rank                                   # configs[3] uses seed 6; replicas take 6 + rank
     sw = B.SwendsenWang(L, T, seed, device=str(dev), path=args.path)
-    if args.path in (0, 4, 5, 6):
-        tw, th = (64 if args.path == 4 else 128 if args.path == 5 else 256 if L % 256 == 0 else 128 if L % 128 == 0 else 64), 32
+    if args.path in (0, 4, 5, 6, 7, 8, 9):
+        tw, th = (64 if args.path == 4 else 256 if (args.path in (7, 8) and L % 256 == 0) else 128 if L % 128 == 0 else 64), 32
+        if args.path == 8 or (tw == 128 and args.path != 5):
+            th = 64
     else:
         tw, th = (256, 32) if (L % 256 == 0 and args.path == 3) else (64, 64)
 

@@ -55,9 +55,10 @@ constexpr int EV_PER_SWEEP = K_COUNT + 1;
 inline size_t align_up(size_t v) { return (v + ALIGN - 1) / ALIGN * ALIGN; }
 
 // tile shapes of the fast path
-enum TileKind { TILE_NONE = 0, TILE_64x64 = 1, TILE_256x32 = 2, SCAN_2 = 3, SCAN_4 = 4, SCAN_8 = 5 };
+enum TileKind { TILE_NONE = 0, TILE_64x64 = 1, TILE_256x32 = 2, SCAN_2 = 3, SCAN_4 = 4, SCAN_8 = 5, SCAN_8x64 = 6, SCAN_4x64 = 7 };
 // width in 32-site words of the 32-row tiles the scan-line kernel and k_flip16 share
-inline int scan_nw(TileKind k) { return k == SCAN_2 ? 2 : k == SCAN_4 ? 4 : k == SCAN_8 ? 8 : 0; }
+inline int scan_nw(TileKind k) { return k == SCAN_2 ? 2 : (k == SCAN_4 || k == SCAN_4x64) ? 4 : (k == SCAN_8 || k == SCAN_8x64) ? 8 : 0; }
+inline int scan_th(TileKind k) { return (k == SCAN_8x64 || k == SCAN_4x64) ? 64 : 32; }
 using Cfg64 = TileCfg<64, 64>;
 using Cfg256 = TileCfg<256, 32>;
 
@@ -71,10 +72,10 @@ size_t olist_entries(int L) {          // per lattice, maximum over the tile sha
     if (L % 64 == 0) n = std::max(n, N / Cfg64::SITES * Cfg64::CAP);
     if (L % 256 == 0) n = std::max(n, N / Cfg256::SITES * Cfg256::CAP);
     for (int nw : {2, 4, 8})                                   // scan tiles: 32 nw x 32 sites
-        if (L % (32 * nw) == 0) n = std::max(n, N / (32 * nw * SCAN_TH) * (size_t)(2 * (32 * nw + SCAN_TH)));
+        if (L % (32 * nw) == 0) n = std::max(n, N / (32 * nw * 32) * (size_t)(2 * (32 * nw + 32)));   // (the 64-row tile needs less)
     return n;
 }
-size_t tiles_max(int L) { return L % 64 == 0 ? (size_t)L * L / (64 * SCAN_TH) : 0; }
+size_t tiles_max(int L) { return L % 64 == 0 ? (size_t)L * L / (64 * 32) : 0; }
 
 DivL make_div(int d) {          // q = (v * m) >> p is exact for 0 <= v < 2^30 (error term < 1/d)
     int k = 0; while ((1 << k) < d) ++k;
@@ -153,8 +154,10 @@ TileKind pick_tile(int L, int path) {
     if (path == 3) return L % 256 == 0 ? TILE_256x32 : TILE_NONE;
     if (path == 4) return L % 64 == 0 ? SCAN_2 : TILE_NONE;
     if (path == 5) return L % 128 == 0 ? SCAN_4 : TILE_NONE;
-    if (L % 256 == 0) return SCAN_8;
-    if (L % 128 == 0) return SCAN_4;
+    if (path == 7) return L % 256 == 0 ? SCAN_8 : TILE_NONE;
+    if (path == 8) return L % 256 == 0 ? SCAN_8x64 : TILE_NONE;
+    if (path == 9) return L % 128 == 0 ? SCAN_4x64 : TILE_NONE;
+    if (L % 128 == 0) return SCAN_4x64;
     if (L % 64 == 0) return SCAN_2;
     return TILE_NONE;
 }
@@ -207,24 +210,31 @@ int launch_label_tiled(sw_handle* h) {
 }
 
 // fast path: fused bond + scan-line tile labelling, global merge, open roots (a1-a3)
-template <int NW>
+template <int NW, int TH>
 int launch_bond_label_scan(sw_handle* h, bool fused, bool obs_prev) {
-    constexpr int TW = 32 * NW, CAP = 2 * (TW + SCAN_TH);
-    const int tiles = h->N / (TW * SCAN_TH);
+    constexpr int TW = 32 * NW, CAP = 2 * (TW + TH);
+    const int tiles = h->N / (TW * TH);
+    constexpr size_t smem = (size_t)TW * TH * sizeof(int);          // the parent array (dynamic: > 48 KB at TH = 64)
+    static bool attr_done = false;
+    if (!attr_done) {
+        SW_CUDA(cudaFuncSetAttribute(k_bond_label<NW, TH, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        SW_CUDA(cudaFuncSetAttribute(k_bond_label<NW, TH, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr_done = true;
+    }
     if (fused) {
         SW_MARK(h, K_BONDLABEL);
-        k_bond_label<NW, true><<<dim3(tiles, h->nb), 32 * NW, 0, h->stream>>>(
+        k_bond_label<NW, TH, true><<<dim3(tiles, h->nb), NW * TH, smem, h->stream>>>(
             h->spins, h->bondE, h->bondS, h->label, h->lab16, h->olist, h->ocount, h->series, h->lat, h->ctl,
             h->L, h->N, h->words, h->nb, obs_prev ? 1 : 0);
     } else {
         SW_MARK(h, K_TILE);
-        k_bond_label<NW, false><<<dim3(tiles, h->nb), 32 * NW, 0, h->stream>>>(
+        k_bond_label<NW, TH, false><<<dim3(tiles, h->nb), NW * TH, smem, h->stream>>>(
             h->spins, h->bondE, h->bondS, h->label, h->lab16, h->olist, h->ocount, h->series, h->lat, h->ctl,
             h->L, h->N, h->words, h->nb, obs_prev ? 1 : 0);
     }
-    const size_t nedge = (size_t)h->L * (h->L / TW + h->L / SCAN_TH);
+    const size_t nedge = (size_t)h->L * (h->L / TW + h->L / TH);
     SW_MARK(h, K_MERGE);
-    k_merge_tiled<TW, SCAN_TH><<<grid1(nedge, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
+    k_merge_tiled<TW, TH><<<grid1(nedge, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
         h->label, h->bondE, h->bondS, h->L, h->N, h->words);
     SW_MARK(h, K_SIZES);
     k_roots_open<CAP><<<grid1((size_t)tiles * 32, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
@@ -233,12 +243,12 @@ int launch_bond_label_scan(sw_handle* h, bool fused, bool obs_prev) {
     return SW_OK;
 }
 // a4-a7 fused, then the size accumulators of the open clusters are cleared for the next sweep
-template <int NW>
+template <int NW, int TH>
 int launch_flip_scan(sw_handle* h) {
-    constexpr int TW = 32 * NW, CAP = 2 * (TW + SCAN_TH);
-    const int tiles = h->N / (TW * SCAN_TH);
+    constexpr int TW = 32 * NW, CAP = 2 * (TW + TH);
+    const int tiles = h->N / (TW * TH);
     SW_MARK(h, K_FLIPTILE);
-    k_flip16<NW><<<dim3(tiles, h->nb), 32 * NW, 0, h->stream>>>(
+    k_flip16<NW, TH><<<dim3(tiles, h->nb), NW * TH, 0, h->stream>>>(
         h->spins, h->lab16, h->D, h->olist, h->ocount, make_div(h->L), h->L, h->N, h->words);
     if (h->eager_labels) {                          // a4 every sweep instead of on demand
         k_compress_tiled<<<grid1((size_t)h->N / 4, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
@@ -269,11 +279,11 @@ int launch_label_generic(sw_handle* h) {
 }
 
 // labelling alone from the bond planes, leaving flat labels (the unfused order; sw_test_label)
-template <int NW>
+template <int NW, int TH>
 int launch_label_scan(sw_handle* h) {
-    constexpr int TW = 32 * NW, CAP = 2 * (TW + SCAN_TH);
-    const int tiles = h->N / (TW * SCAN_TH);
-    int rc = launch_bond_label_scan<NW>(h, false, false);
+    constexpr int TW = 32 * NW, CAP = 2 * (TW + TH);
+    const int tiles = h->N / (TW * TH);
+    int rc = launch_bond_label_scan<NW, TH>(h, false, false);
     if (rc) return rc;
     SW_MARK(h, K_COMPRESS);
     k_compress_tiled<<<grid1((size_t)h->N / 4, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
@@ -287,9 +297,11 @@ int launch_label_scan(sw_handle* h) {
 
 int launch_label(sw_handle* h) {
     switch (h->tile) {
-        case SCAN_2:      return launch_label_scan<2>(h);
-        case SCAN_4:      return launch_label_scan<4>(h);
-        case SCAN_8:      return launch_label_scan<8>(h);
+        case SCAN_2:      return launch_label_scan<2, 32>(h);
+        case SCAN_4:      return launch_label_scan<4, 32>(h);
+        case SCAN_8:      return launch_label_scan<8, 32>(h);
+        case SCAN_8x64:   return launch_label_scan<8, 64>(h);
+        case SCAN_4x64:   return launch_label_scan<4, 64>(h);
         case TILE_64x64:  return launch_label_tiled<64, 64>(h);
         case TILE_256x32: return launch_label_tiled<256, 32>(h);
         default:          return launch_label_generic(h);
@@ -309,14 +321,17 @@ int launch_sweep(sw_handle* h, int64_t k) {
                 h->spins, h->bondE, h->bondS, h->lat, h->ctl, h->L, h->N, h->words, h->series, h->nb, obs_prev ? 1 : 0);
             h->launches += 1;
         }
-        rc = nw == 8 ? launch_bond_label_scan<8>(h, fused, obs_prev) : nw == 4 ? launch_bond_label_scan<4>(h, fused, obs_prev)
-                                                                               : launch_bond_label_scan<2>(h, fused, obs_prev);
+        rc = h->tile == SCAN_8x64 ? launch_bond_label_scan<8, 64>(h, fused, obs_prev)
+           : h->tile == SCAN_4x64 ? launch_bond_label_scan<4, 64>(h, fused, obs_prev)
+           : nw == 8 ? launch_bond_label_scan<8, 32>(h, fused, obs_prev)
+           : nw == 4 ? launch_bond_label_scan<4, 32>(h, fused, obs_prev) : launch_bond_label_scan<2, 32>(h, fused, obs_prev);
         if (rc) return rc;
         SW_MARK(h, K_FLIPBITS);
         k_flipbits<<<grid1(((size_t)h->words + 3) / 4, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(
             h->D, h->lat, h->ctl, h->words);
         h->launches += 1;
-        rc = nw == 8 ? launch_flip_scan<8>(h) : nw == 4 ? launch_flip_scan<4>(h) : launch_flip_scan<2>(h);
+        rc = h->tile == SCAN_8x64 ? launch_flip_scan<8, 64>(h) : h->tile == SCAN_4x64 ? launch_flip_scan<4, 64>(h) : nw == 8 ? launch_flip_scan<8, 32>(h)
+           : nw == 4 ? launch_flip_scan<4, 32>(h) : launch_flip_scan<2, 32>(h);
         if (rc) return rc;
         SW_MARK(h, K_ADVANCE);
         k_advance<<<1, 64, 0, h->stream>>>(h->ctl, h->series, h->nb);
@@ -661,7 +676,7 @@ int sw_stage_ms(sw_handle* h, float out[4]) {
 }
 
 int sw_set_path(sw_handle* h, int path) {
-    if (!h || path < 0 || path > 6) { set_err("sw_set_path: invalid argument"); return SW_EINVAL; }
+    if (!h || path < 0 || path > 9) { set_err("sw_set_path: invalid argument"); return SW_EINVAL; }
     h->path = path;
     h->tile = pick_tile(h->L, path);
     return SW_OK;

@@ -133,6 +133,27 @@ __device__ __forceinline__ int uf_find(const int* lab, int x) {
     while (p != x) { x = p; p = ld_cg(lab + x); }
     return x;
 }
+// the same walk through L1 (ld.global.ca).  A stale line can only show an older parent, which is still an
+// ancestor, so the walk ends at a node that was a root when its line was fetched; callers either run when no
+// root changes any more (k_roots_open) or let an atomic on the result arbitrate (uf_union_l1).  At T_c one
+// cluster owns ~1/3 of all sites: its root's line would otherwise be fetched from one L2 slice by every walker.
+__device__ __forceinline__ int ld_ca(const int* p) {
+    int v; asm volatile("ld.global.ca.s32 %0, [%1];" : "=r"(v) : "l"(p)); return v;
+}
+__device__ __forceinline__ int uf_find_l1(const int* lab, int x) {
+    int p = ld_ca(lab + x);
+    while (p != x) { x = p; p = ld_ca(lab + x); }
+    return x;
+}
+__device__ __forceinline__ void uf_union_l1(int* lab, int a, int b) {
+    a = uf_find_l1(lab, a); b = uf_find_l1(lab, b);
+    while (a != b) {
+        if (a < b) { int s = a; a = b; b = s; }           // a is the larger
+        const int old = atomicMin(lab + a, b);            // L2 decides whether a still is a root
+        if (old == a) break;
+        a = old;
+    }
+}
 // find with one-shot compression of the starting node when the walk was longer than one hop
 // (only ever writes a smaller ancestor: safe under races)
 __device__ __forceinline__ int uf_find_compress(int* lab, int x) {

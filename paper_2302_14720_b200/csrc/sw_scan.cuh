@@ -24,16 +24,16 @@
 
 namespace sw {
 
-constexpr int SCAN_TH = 32;                     // tile height = rows a warp walks
-constexpr uint32_t IDX_MASK = 0x1FFFu;          // tile-local site index: 13 bits (TW * 32 <= 8192)
-constexpr int CNT_SHIFT = 13;                   // cluster size (<= 8192: 14 bits) lives in bits 13..26 of a root's word
-constexpr uint32_t CNT_MASK = 0x3FFFu;
-constexpr uint32_t OPEN_BIT = 0x40000000u;      // bit 30: the cluster has a bond across the tile edge
+constexpr int BAND = 32;                        // rows a warp walks; a tile is TH / 32 bands of NW strips
+constexpr uint32_t OPEN_BIT = 0x40000000u;      // bit 30 of a root's word: the cluster has a bond across the tile edge
+// A root's word: bits 0 .. LS-1 tile-local index (LS = log2 of the sites per tile <= 14), bits LS .. 2 LS the
+// cluster size (<= 2^LS), bit 30 open.
+__host__ __device__ constexpr int ilog2_c(int v) { return v <= 1 ? 0 : 1 + ilog2_c(v >> 1); }
 
-// find on the shared parent array; roots may carry size / open bits above IDX_MASK
-__device__ __forceinline__ int sc_find(const int* par, int x) {
-    int p = par[x] & (int)IDX_MASK;
-    while (p != x) { x = p; p = par[x] & (int)IDX_MASK; }
+// find on the shared parent array; roots may carry size / open bits above the index mask
+__device__ __forceinline__ int sc_find(const int* par, int x, int mask) {
+    int p = par[x] & mask;
+    while (p != x) { x = p; p = par[x] & mask; }
     return x;
 }
 // unite the trees of a and b (any nodes); hooking "larger under smaller" with atomicMin so the root of a
@@ -55,18 +55,20 @@ __device__ __forceinline__ int div_l(int v, const DivL& D) {
 
 // FUSE = true: phase 1 draws the bonds (a1 fused into a2).  FUSE = false: phase 1 reads the bond planes
 // that k_bond_rows (or a test) wrote -- per-stage timing (BASELINE config 3) and labelling-only tests.
-template <int NW, bool FUSE>
-__global__ void __launch_bounds__(32 * NW)
+template <int NW, int TH, bool FUSE>
+__global__ void __launch_bounds__(NW * TH)
 k_bond_label(const int8_t* __restrict__ spins, uint32_t* bondE, uint32_t* bondS,
              int* __restrict__ label, uint16_t* __restrict__ lab16, int2* __restrict__ olist, int* __restrict__ ocount,
              Rec* __restrict__ rec, const Lat* __restrict__ lat, const Ctl* __restrict__ ctl,
              int L, int N, int words, int nb, int obs_prev) {
-    constexpr int TW = 32 * NW, TH = SCAN_TH, SITES = TW * TH, THREADS = 32 * NW;
+    constexpr int TW = 32 * NW, SITES = TW * TH, THREADS = NW * TH;   // one thread per 32-site word
     constexpr int CAP = 2 * (TW + TH);
-    __shared__ __align__(16) int par[SITES];   // parent, tile-local index (+ size / open bits at roots)
+    constexpr int LS = ilog2_c(SITES), IDX_MASK = SITES - 1, CNT_SHIFT = LS, CNT_MASK = 2 * SITES - 1;
+    static_assert(TH % BAND == 0 && TH <= 64 && (1 << LS) == SITES && LS <= 14, "tile shape");
+    extern __shared__ __align__(16) int par[];  // [SITES] parent, tile-local index (+ size / open bits at roots); dynamic: 64 KB at TH = 64
     __shared__ uint2 es[TH * NW];              // [row][strip] = (East word, South word)
     __shared__ uint32_t nIn[NW];               // South bonds entering from the tile above, per strip
-    __shared__ uint32_t wIn;                   // East bonds entering from the tile to the West, bit = row
+    __shared__ uint32_t wIn[2];                // East bonds entering from the tile to the West, bit = row
     __shared__ int s_nopen, s_max, s_nclosed, s_obs[2];
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -80,7 +82,7 @@ k_bond_label(const int8_t* __restrict__ spins, uint32_t* bondE, uint32_t* bondS,
     const uint32_t tlo = (uint32_t)t, thi = (uint32_t)(t >> 32);
 
     if (tid < NW) nIn[tid] = 0;
-    if (tid == 0) { wIn = 0; s_nopen = 0; s_max = 0; s_nclosed = 0; s_obs[0] = 0; s_obs[1] = 0; }
+    if (tid == 0) { wIn[0] = 0; wIn[1] = 0; s_nopen = 0; s_max = 0; s_nclosed = 0; s_obs[0] = 0; s_obs[1] = 0; }
     __syncthreads();
 
     // ---- phase 1: bonds of the tile, PAPER.md:37-39 (section 2.1) --------------------------------------
@@ -91,10 +93,9 @@ k_bond_label(const int8_t* __restrict__ spins, uint32_t* bondE, uint32_t* bondS,
         const size_t gw = (size_t)(y0 + row) * wprL + (x0 >> 5) + wx;
         es[tid] = make_uint2(bE[gw], bS[gw]);
         if (tid < NW) nIn[tid] = bS[(size_t)(y0 == 0 ? L - 1 : y0 - 1) * wprL + (x0 >> 5) + tid];
-        if (warp == NW - 1) {                                         // (not the warp that wrote nIn: no race with tid < NW)
+        if (tid < TH) {
             const int wl = (x0 >> 5) == 0 ? wprL - 1 : (x0 >> 5) - 1;
-            const uint32_t b = __ballot_sync(0xffffffffu, bE[(size_t)(y0 + lane) * wprL + wl] >> 31);
-            if (lane == 0) wIn = b;
+            if (bE[(size_t)(y0 + tid) * wprL + wl] >> 31) atomicOr(&wIn[tid >> 5], 1u << (tid & 31));
         }
     } else {
         const PhiloxKey key(la.key0, la.key1);
@@ -147,36 +148,42 @@ k_bond_label(const int8_t* __restrict__ spins, uint32_t* bondE, uint32_t* bondS,
                 const int xwst = x0 == 0 ? L - 1 : x0 - 1;                 // odd column
                 const int i = (y0 + row) * L + xwst;
                 const uint4 r = philox4x32_10((uint32_t)(i >> 1), tlo, thi, TAG_BOND, key);
-                if (s[i] == s[(size_t)(y0 + row) * L + x0] && r.z < la.thr) atomicOr(&wIn, 1u << row);
+                if (s[i] == s[(size_t)(y0 + row) * L + x0] && r.z < la.thr) atomicOr(&wIn[row >> 5], 1u << (row & 31));
             }
         }
     }
     __syncthreads();
 
-    // ---- phase 2: scan-line labelling of this warp's strip, PAPER.md:49-51 (section 2.3) --------------
-    const uint32_t lt = (1u << lane) - 1u;
+    // ---- phase 2: scan-line labelling of this warp's block (32 columns x 32 rows), PAPER.md:49-51 -------
     {
+        const uint32_t lanebit = 1u << lane, lt = lanebit - 1u;
+        const int strip = warp % NW, yb = (warp / NW) * BAND;
+        int* prow = par + yb * TW + strip * 32;                      // first site of the row in this strip
         int prev = 0;
-        uint32_t s_up = 0;
+        uint32_t s_up = 0;                                           // (a band's first row adopts nothing: seams come later)
 #pragma unroll 4
-        for (int y = 0; y < TH; ++y) {
-            const uint2 w = es[y * NW + warp];
-            const uint32_t e = w.x & 0x7FFFFFFFu;                   // bonds inside the strip
-            const uint32_t nz = ~e;                                  // bit k: no bond between columns k, k + 1
-            const int h = 32 - __clz(nz & lt);                       // head column of my run
-            const int tl = __ffs(nz & ~lt) - 1;                      // tail column of my run (nz bit 31 is set)
-            const uint32_t runmask = (2u << tl) - (1u << h);
+        for (int y = yb; y < yb + BAND; ++y, prow += TW) {
+            const uint2 w = es[y * NW + strip];
+            const uint32_t nz = ~w.x | 0x80000000u;                  // bit k: no bond between columns k, k + 1 of the strip
+            const uint32_t below = nz & lt, above = nz & ~lt;        // run boundaries left of me / at or right of me
+            const int h = 32 - __clz(below);                         // head column of my run
+            // my run: bits h .. tail, tail = lowest set bit of `above` (bit 31 is always set)
+            const uint32_t runmask = (above ^ (above - 1u)) & ~((1u << h) - 1u);
             const uint32_t upm = s_up & runmask;                     // sites of my run bonded to the row above
-            const bool myUp = (s_up >> lane) & 1u;
+            const bool myUp = s_up & lanebit;
             int a = prev;
             if (myUp) {                                              // root of the site above
                 int p = par[a];
                 while (p != a) { a = p; p = par[a]; }
             }
             const int got = __shfl_sync(0xffffffffu, a, (__ffs(upm) - 1) & 31);
-            const int c = upm ? got : y * TW + warp * 32 + h;     // a new label: the head's own index (its own root)
-            par[y * TW + warp * 32 + lane] = c;
-            if (myUp && a != c) sc_union(par, a, c);
+            const int c = upm ? got : (int)(prow - par) + h;         // a new label: the head's own index (its own root)
+            prow[lane] = c;
+            if (myUp && a != c) {                                    // two roots meet in my run: hook the larger under the smaller
+                const int hi = max(a, c), lo = min(a, c);
+                const int old = atomicMin(par + hi, lo);
+                if (old != hi) sc_union(par, old, lo);               // hi had been hooked meanwhile (rare)
+            }
             __syncwarp();                                            // row y's parents are written before row y + 1 walks them
             prev = c;
             s_up = w.y;
@@ -184,11 +191,21 @@ k_bond_label(const int8_t* __restrict__ spins, uint32_t* bondE, uint32_t* bondS,
     }
     __syncthreads();
 
-    // ---- phase 3: strip seams ---------------------------------------------------------------------------
-    if (NW > 1 && warp < NW - 1) {
-        if (es[lane * NW + warp].x >> 31) {
-            const int i = lane * TW + warp * 32 + 31;
-            sc_union(par, sc_find(par, i), sc_find(par, i + 1));
+    // ---- phase 3: seams between the warps' blocks: East bonds across strip edges, South bonds across bands
+    for (int j = tid; j < (NW - 1) * TH + (TH / BAND - 1) * TW; j += THREADS) {
+        if (j < (NW - 1) * TH) {
+            const int row = j / (NW - 1), st = j - row * (NW - 1);
+            if (es[row * NW + st].x >> 31) {
+                const int i = row * TW + st * 32 + 31;
+                sc_union(par, sc_find(par, i, IDX_MASK), sc_find(par, i + 1, IDX_MASK));
+            }
+        } else {
+            const int k = j - (NW - 1) * TH;
+            const int row = (k / TW + 1) * BAND - 1, c = k % TW;
+            if ((es[row * NW + (c >> 5)].y >> (c & 31)) & 1u) {
+                const int i = row * TW + c;
+                sc_union(par, sc_find(par, i, IDX_MASK), sc_find(par, i + TW, IDX_MASK));
+            }
         }
     }
     __syncthreads();
@@ -202,7 +219,7 @@ k_bond_label(const int8_t* __restrict__ spins, uint32_t* bondE, uint32_t* bondS,
     const int mybase = (tid / NW) * TW + (tid % NW) * 32;
     {
         const uint32_t ew = es[tid].x & 0x7FFFFFFFu;
-        uint32_t up = tid >= NW ? es[tid - NW].y : 0u;               // South bonds of the row above
+        uint32_t up = (tid / NW) % BAND ? es[tid - NW].y : 0u;       // South bonds of the row above, within the band
         uint32_t m = ew;                                             // OR of the run's uplinks, gathered at its head
         up |= (up >> 1) & m;  m &= m >> 1;
         up |= (up >> 2) & m;  m &= m >> 2;
@@ -230,10 +247,10 @@ k_bond_label(const int8_t* __restrict__ spins, uint32_t* bondE, uint32_t* bondS,
         if (j < TW)               { site = j;                              open = (nIn[j >> 5] >> (j & 31)) & 1u; }
         else if (j < 2 * TW)      { const int c = j - TW; site = (TH - 1) * TW + c;
                                     open = (es[(TH - 1) * NW + (c >> 5)].y >> (c & 31)) & 1u; }
-        else if (j < 2 * TW + TH) { const int r = j - 2 * TW; site = r * TW; open = (wIn >> r) & 1u; }
+        else if (j < 2 * TW + TH) { const int r = j - 2 * TW; site = r * TW; open = (wIn[r >> 5] >> (r & 31)) & 1u; }
         else                      { const int r = j - 2 * TW - TH; site = r * TW + TW - 1;
                                     open = es[r * NW + NW - 1].x >> 31; }
-        if (open) atomicOr(reinterpret_cast<unsigned int*>(par + sc_find(par, site)), OPEN_BIT);
+        if (open) atomicOr(reinterpret_cast<unsigned int*>(par + sc_find(par, site, IDX_MASK)), OPEN_BIT);
     }
     constexpr int QSTEPS = SITES / 4 / THREADS;                      // = 8
     constexpr int LOG_TW = 5 + (NW == 8 ? 3 : NW == 4 ? 2 : NW == 2 ? 1 : 0);
@@ -246,8 +263,8 @@ k_bond_label(const int8_t* __restrict__ spins, uint32_t* bondE, uint32_t* bondS,
         const int l = 4 * q;
         const int4 v = *reinterpret_cast<const int4*>(par + l);
         // site -> its label node -> root (label nodes are flat; roots carry size / open bits)
-        int r[4] = { par[v.x & (int)IDX_MASK] & (int)IDX_MASK, par[v.y & (int)IDX_MASK] & (int)IDX_MASK,
-                     par[v.z & (int)IDX_MASK] & (int)IDX_MASK, par[v.w & (int)IDX_MASK] & (int)IDX_MASK };
+        int r[4] = { par[v.x & IDX_MASK] & IDX_MASK, par[v.y & IDX_MASK] & IDX_MASK,
+                     par[v.z & IDX_MASK] & IDX_MASK, par[v.w & IDX_MASK] & IDX_MASK };
         int4 g;
         g.x = tilebase + (r[0] >> LOG_TW) * L + (r[0] & (TW - 1));
         g.y = tilebase + (r[1] >> LOG_TW) * L + (r[1] & (TW - 1));
@@ -322,14 +339,14 @@ k_bond_label(const int8_t* __restrict__ spins, uint32_t* bondE, uint32_t* bondS,
 // Then every site reads its 16-bit tile-local root index (2 B / site, written by k_bond_label) and looks the
 // bit up in shared memory: no global gather, no index arithmetic per site.
 // ---------------------------------------------------------------------------------------------------
-template <int NW>
-__global__ void __launch_bounds__(32 * NW, 1536 / (32 * NW))
+template <int NW, int TH>
+__global__ void __launch_bounds__(NW * TH, 1536 / (NW * TH))
 k_flip16(int8_t* __restrict__ spins, const uint16_t* __restrict__ lab16, const uint32_t* __restrict__ D,
          const int2* __restrict__ olist, const int* __restrict__ ocount, DivL dv, int L, int N, int words) {
-    constexpr int TW = 32 * NW, TH = SCAN_TH, SITES = TW * TH, THREADS = 32 * NW;
+    constexpr int TW = 32 * NW, SITES = TW * TH, THREADS = NW * TH;
     constexpr int CAP = 2 * (TW + TH);
     constexpr int OSTEPS = SITES / 8 / THREADS;      // = 4
-    constexpr int LOG_TW = 5 + (NW == 8 ? 3 : NW == 4 ? 2 : NW == 2 ? 1 : 0);
+    constexpr int LOG_TW = ilog2_c(TW);
     __shared__ uint32_t dec[TH * NW];                // decision bit of the tile root with local index l: bit l & 31 of word l >> 5
 
     const int tid = threadIdx.x;

@@ -260,13 +260,13 @@ k_merge_tiled(int* label, const uint32_t* __restrict__ bondE, const uint32_t* __
         const int y = idx / tilesX, c = idx - y * tilesX;
         const int x = c * TW + TW - 1;
         if (bondE[(size_t)blockIdx.y * words + (size_t)y * wprL + (x >> 5)] >> 31)
-            uf_union(lab, ld_cg(lab + y * L + x), ld_cg(lab + y * L + (x + 1 == L ? 0 : x + 1)));
+            uf_union_l1(lab, ld_cg(lab + y * L + x), ld_cg(lab + y * L + (x + 1 == L ? 0 : x + 1)));
     } else {
         const int j = idx - nV;
         const int r = j / L, x = j - r * L;
         const int y = r * TH + TH - 1;
         if ((bondS[(size_t)blockIdx.y * words + (size_t)y * wprL + (x >> 5)] >> (x & 31)) & 1u)
-            uf_union(lab, ld_cg(lab + y * L + x), ld_cg(lab + (y + 1 == L ? 0 : y + 1) * L + x));
+            uf_union_l1(lab, ld_cg(lab + y * L + x), ld_cg(lab + (y + 1 == L ? 0 : y + 1) * L + x));
     }
 }
 
@@ -325,7 +325,7 @@ k_roots_open(int* label, int2* __restrict__ olist, const int* __restrict__ ocoun
                 const int p = ld_cg(lab + it.x);
                 R = p; sz = it.y;
                 if (p != it.x) {                            // hooked: walk to the root, point at it
-                    R = uf_find(lab, p);
+                    R = uf_find_l1(lab, p);                 // (no root changes during this kernel)
                     if (R != p) lab[it.x] = R;              // only ever an ancestor: safe while others walk
                 } else {
                     ++nroot;

@@ -95,7 +95,7 @@ def test_generic_path_every_sweep(B, L):
 
 
 @pytest.mark.parametrize("L,path", [(64, 0), (128, 0), (192, 0), (256, 0), (256, 2), (320, 0), (512, 0), (512, 2), (768, 3),
-                                    (256, 4), (256, 5), (384, 0), (512, 6), (768, 0), (128, 6)])
+                                    (256, 4), (256, 5), (384, 0), (512, 6), (768, 0), (128, 6), (256, 7), (512, 7), (1024, 0), (256, 9), (384, 9), (512, 8)])
 def test_tiled_path_every_sweep(B, L, path):
     for T, seed in ((2.0, 1), (T_C, 2), (3.0, 3)):
         _compare_sweeps(B, L, T, seed + L, 6, path=path)
@@ -118,7 +118,7 @@ def test_survey_golden_vector_on_gpu(B):
     sw.close()
 
 
-@pytest.mark.parametrize("L,path", [(64, 0), (256, 0), (256, 2), (100, 1), (128, 0), (256, 6)])
+@pytest.mark.parametrize("L,path", [(64, 0), (256, 0), (256, 2), (100, 1), (128, 0), (256, 6), (256, 7)])
 def test_special_starts(B, L, path):
     for name, s0 in (("cold", wl.spins_cold(L)), ("down", wl.spins_all_down(L)),
                      ("checker", wl.spins_checkerboard(L)), ("hstripes", wl.spins_stripes(L, 1)),
@@ -140,7 +140,7 @@ def _label_patterns(L):
         yield f"random{d}", wl.bonds_random(L, 7 * L + k, d)
 
 
-@pytest.mark.parametrize("L,path", [(64, 0), (128, 0), (256, 0), (256, 2), (256, 4), (320, 0), (100, 1), (512, 0), (512, 3)])
+@pytest.mark.parametrize("L,path", [(64, 0), (128, 0), (256, 0), (256, 2), (256, 4), (320, 0), (100, 1), (512, 0), (512, 3), (512, 7)])
 def test_labelling_of_injected_bond_graphs(B, L, path):
     """Labelling alone on adversarial bond graphs (long thin spiral, comb, wrap-around rows)."""
     sw = B.SwendsenWang(L, 2.0, 1, path=path)
