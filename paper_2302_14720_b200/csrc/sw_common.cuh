@@ -75,6 +75,11 @@ __device__ __forceinline__ void bond_draws(uint32_t w, uint32_t tlo, uint32_t th
     }
 }
 
+// position of the highest set bit, 0xffffffff for 0 (one FLO)
+__device__ __forceinline__ int bfind_u32(uint32_t x) {
+    int r; asm("bfind.u32 %0, %1;" : "=r"(r) : "r"(x)); return r;
+}
+
 // ------------------------------------------------------------------------------------------
 // memory helpers
 // ------------------------------------------------------------------------------------------

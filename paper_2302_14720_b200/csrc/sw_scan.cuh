@@ -158,27 +158,26 @@ k_bond_label(const int8_t* __restrict__ spins, uint32_t* bondE, uint32_t* bondS,
     {
         const uint32_t lanebit = 1u << lane, lt = lanebit - 1u;
         const int strip = warp % NW, yb = (warp / NW) * BAND;
-        int* prow = par + yb * TW + strip * 32;                      // first site of the row in this strip
+        int rowbase = yb * TW + strip * 32;                          // first site of the row in this strip
         int prev = 0;
         uint32_t s_up = 0;                                           // (a band's first row adopts nothing: seams come later)
 #pragma unroll 4
-        for (int y = yb; y < yb + BAND; ++y, prow += TW) {
+        for (int y = yb; y < yb + BAND; ++y, rowbase += TW) {
             const uint2 w = es[y * NW + strip];
             const uint32_t nz = ~w.x | 0x80000000u;                  // bit k: no bond between columns k, k + 1 of the strip
             const uint32_t below = nz & lt, above = nz & ~lt;        // run boundaries left of me / at or right of me
-            const int h = 32 - __clz(below);                         // head column of my run
+            const int h = bfind_u32(below) + 1;                      // head column of my run
             // my run: bits h .. tail, tail = lowest set bit of `above` (bit 31 is always set)
             const uint32_t runmask = (above ^ (above - 1u)) & ~((1u << h) - 1u);
             const uint32_t upm = s_up & runmask;                     // sites of my run bonded to the row above
             const bool myUp = s_up & lanebit;
             int a = prev;
             if (myUp) {                                              // root of the site above
-                int p = par[a];
-                while (p != a) { a = p; p = par[a]; }
+                for (int p = par[a]; p != a; p = par[a]) a = p;
             }
-            const int got = __shfl_sync(0xffffffffu, a, (__ffs(upm) - 1) & 31);
-            const int c = upm ? got : (int)(prow - par) + h;         // a new label: the head's own index (its own root)
-            prow[lane] = c;
+            const int got = __shfl_sync(0xffffffffu, a, __ffs(upm) - 1);   // (source lane is taken mod 32)
+            const int c = upm ? got : rowbase + h;                   // a new label: the head's own index (its own root)
+            par[rowbase + lane] = c;
             if (myUp && a != c) {                                    // two roots meet in my run: hook the larger under the smaller
                 const int hi = max(a, c), lo = min(a, c);
                 const int old = atomicMin(par + hi, lo);
