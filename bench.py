@@ -44,7 +44,7 @@ def kernel_bytes_per_site(tw: int, th: int):
         "energy": 1.0,                     # spin read
         "advance": 0.0,
         "bond_label": 5.25,                # a1 + a2 fused: spin read + 2 bond bits written + int32 label written
-        "flip_tile": 5.125,                # a4 + a6 + a7 fused: label read + spin written + decision bit gathered
+        "flip16": 5.125,                   # a4 + a6 fused: label read + spin written + decision bit gathered (model; the kernel reads 2 B labels)
     }
 SWEEP_MODEL_BYTES_PER_SITE = 18.75
 STAGE_MODEL = {"bond": 1.25, "label": 12.25, "flip": 5.25, "observe": 1.0}

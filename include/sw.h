@@ -140,7 +140,7 @@ int        sw_stage_ms(sw_handle* h, float out[4]);
 /* The same measurement per kernel: out[i] = ms of kernel slot i summed over the timed sweeps (at most the
  * first 1024 sweeps of the call), i < cap; returns the number of kernel slots (or a negative code).
  * sw_kernel_name(i) names slot i ("bond", "tile_label", "merge", "roots_open", "compress", "bond_label" (a1 + a2 fused),
- * "flip_tile" (a4 + a6 + a7 fused), ...; "" past the end). */
+ * "flip16" (a4 + a6 fused), ...; "" past the end). */
 int        sw_kernel_ms(sw_handle* h, float* out, int32_t cap);
 const char* sw_kernel_name(int32_t i);
 

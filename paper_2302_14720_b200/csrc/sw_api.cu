@@ -46,9 +46,9 @@ constexpr int MAX_TIMED_SWEEPS = 1024;
 enum Kid { K_BOND = 0, K_TILE, K_MERGE, K_COMPRESS, K_SIZES, K_SIZES_RESET, K_FLIPBITS, K_FLIP, K_ENERGY, K_ADVANCE,
            K_BONDLABEL, K_FLIPTILE, K_COUNT };
 const char* const KERNEL_NAMES[K_COUNT] = { "bond", "tile_label", "merge", "compress", "roots_open", "sizes_reset",
-                                            "flipbits", "flip", "energy", "advance", "bond_label", "flip_tile" };
+                                            "flipbits", "flip", "energy", "advance", "bond_label", "flip16" };
 // stage of each kernel: bond, label, flip, observe.  The fused kernels are booked under the stage that
-// dominates them: bond_label (a1 + a2) under "label", flip_tile (a4 + a6 + a7) under "flip".
+// dominates them: bond_label (a1 + a2) under "label", flip16 (a4 + a6) under "flip".
 const int KERNEL_STAGE[K_COUNT] = { 0, 1, 1, 1, 1, 1, 2, 2, 3, 3, 1, 2 };
 constexpr int EV_PER_SWEEP = K_COUNT + 1;
 
@@ -58,12 +58,11 @@ inline size_t align_up(size_t v) { return (v + ALIGN - 1) / ALIGN * ALIGN; }
 enum TileKind { TILE_NONE = 0, TILE_64x64 = 1, TILE_256x32 = 2, SCAN_2 = 3, SCAN_4 = 4, SCAN_8 = 5, SCAN_8x64 = 6, SCAN_4x64 = 7 };
 // width in 32-site words of the 32-row tiles the scan-line kernel and k_flip16 share
 inline int scan_nw(TileKind k) { return k == SCAN_2 ? 2 : (k == SCAN_4 || k == SCAN_4x64) ? 4 : (k == SCAN_8 || k == SCAN_8x64) ? 8 : 0; }
-inline int scan_th(TileKind k) { return (k == SCAN_8x64 || k == SCAN_4x64) ? 64 : 32; }
 using Cfg64 = TileCfg<64, 64>;
 using Cfg256 = TileCfg<256, 32>;
 
 struct Layout {        // byte offsets into the workspace
-    size_t spins, bondE, bondS, D, label, lab16, gsize, olist, ocount, lat, ctl, rec_now, series, total;
+    size_t spins, bondE, bondS, D, label, lab16, gsize, olist, ocount, npar, nsize, nmin, bslot, lat, ctl, rec_now, series, total;
 };
 
 size_t olist_entries(int L) {          // per lattice, maximum over the tile shapes usable for this L
@@ -96,6 +95,10 @@ Layout make_layout(int L, int nb) {
     o.gsize = p;   p = align_up(p + (size_t)nb * N * 4);
     o.olist = p;   p = align_up(p + (size_t)nb * olist_entries(L) * sizeof(int2));
     o.ocount = p;  p = align_up(p + (size_t)nb * tiles_max(L) * 4);
+    o.npar = p;    p = align_up(p + (size_t)nb * olist_entries(L) * 4);      // node arrays of the scan path
+    o.nsize = p;   p = align_up(p + (size_t)nb * olist_entries(L) * 4);
+    o.nmin = p;    p = align_up(p + (size_t)nb * olist_entries(L) * 4);
+    o.bslot = p;   p = align_up(p + (size_t)nb * olist_entries(L) * 2);
     o.lat = p;     p = align_up(p + (size_t)nb * sizeof(Lat));
     o.ctl = p;     p = align_up(p + sizeof(Ctl));
     o.rec_now = p; p = align_up(p + (size_t)nb * sizeof(Rec));
@@ -126,6 +129,8 @@ struct sw_handle {
     int8_t* spins = nullptr; uint32_t *bondE = nullptr, *bondS = nullptr, *D = nullptr;
     int *label = nullptr, *gsize = nullptr, *ocount = nullptr; int2* olist = nullptr;
     uint16_t* lab16 = nullptr;       // tile-local root index of every site (scan path)
+    int *npar = nullptr, *nsize = nullptr, *nmin = nullptr;   // union-find over open tile roots: parent, size, min site
+    uint16_t* bslot = nullptr;       // per tile: slot of the root of each border site
     Lat* lat = nullptr; Ctl* ctl = nullptr; Rec* rec_now = nullptr;
     Rec* series = nullptr; Rec* series_owned = nullptr;
     int64_t series_cap = DEFAULT_SERIES_CAP;       // sweeps retained; the ring has series_cap + 1 slots
@@ -224,41 +229,62 @@ int launch_bond_label_scan(sw_handle* h, bool fused, bool obs_prev) {
     if (fused) {
         SW_MARK(h, K_BONDLABEL);
         k_bond_label<NW, TH, true><<<dim3(tiles, h->nb), NW * TH, smem, h->stream>>>(
-            h->spins, h->bondE, h->bondS, h->label, h->lab16, h->olist, h->ocount, h->series, h->lat, h->ctl,
+            h->spins, h->bondE, h->bondS, h->label, h->lab16, h->olist, h->ocount, h->npar, h->nsize, h->nmin, h->bslot,
+            h->series, h->lat, h->ctl,
             h->L, h->N, h->words, h->nb, obs_prev ? 1 : 0);
     } else {
         SW_MARK(h, K_TILE);
         k_bond_label<NW, TH, false><<<dim3(tiles, h->nb), NW * TH, smem, h->stream>>>(
-            h->spins, h->bondE, h->bondS, h->label, h->lab16, h->olist, h->ocount, h->series, h->lat, h->ctl,
+            h->spins, h->bondE, h->bondS, h->label, h->lab16, h->olist, h->ocount, h->npar, h->nsize, h->nmin, h->bslot,
+            h->series, h->lat, h->ctl,
             h->L, h->N, h->words, h->nb, obs_prev ? 1 : 0);
     }
     const size_t nedge = (size_t)h->L * (h->L / TW + h->L / TH);
     SW_MARK(h, K_MERGE);
-    k_merge_tiled<TW, TH><<<grid1(nedge, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
-        h->label, h->bondE, h->bondS, h->L, h->N, h->words);
+    k_merge_nodes<TW, TH><<<grid1(nedge, 256, h->nb), 256, 0, h->stream>>>(
+        h->npar, h->bslot, h->bondE, h->bondS, h->L, h->words);
     SW_MARK(h, K_SIZES);
-    k_roots_open<CAP><<<grid1((size_t)tiles * 32, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
-        h->label, h->olist, h->ocount, h->gsize, h->series, h->ctl, tiles, h->N, h->nb, 1);
+    k_roots_nodes<CAP><<<grid1((size_t)tiles * 32, 256, h->nb), 256, 0, h->stream>>>(
+        h->npar, h->nsize, h->nmin, h->olist, h->ocount, tiles);
     h->launches += 3;
     return SW_OK;
 }
-// a4-a7 fused, then the size accumulators of the open clusters are cleared for the next sweep
+// a4 for the scan path: open tile roots take their cluster's label, then two hops per site
+template <int NW, int TH>
+int launch_flatten_scan(sw_handle* h) {
+    constexpr int TW = 32 * NW, CAP = 2 * (TW + TH);
+    const int tiles = h->N / (TW * TH);
+    k_apply_roots<CAP><<<grid1((size_t)tiles * 32, 256, h->nb), 256, 0, h->stream>>>(
+        h->label, h->nmin, h->olist, h->ocount, tiles, h->N);
+    k_compress_tiled<<<grid1((size_t)h->N / 4, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
+        h->label, h->series, h->ctl, h->N, h->nb, 0);
+    h->launches += 2;
+    return SW_OK;
+}
+int flatten_scan(sw_handle* h) {
+    switch (h->tile) {
+        case SCAN_2:    return launch_flatten_scan<2, 32>(h);
+        case SCAN_4:    return launch_flatten_scan<4, 32>(h);
+        case SCAN_8:    return launch_flatten_scan<8, 32>(h);
+        case SCAN_8x64: return launch_flatten_scan<8, 64>(h);
+        case SCAN_4x64: return launch_flatten_scan<4, 64>(h);
+        default:        return SW_ESTATE;
+    }
+}
+// a4-a6 fused (+ count and largest of the clusters that span tiles)
 template <int NW, int TH>
 int launch_flip_scan(sw_handle* h) {
-    constexpr int TW = 32 * NW, CAP = 2 * (TW + TH);
+    constexpr int TW = 32 * NW;
     const int tiles = h->N / (TW * TH);
     SW_MARK(h, K_FLIPTILE);
     k_flip16<NW, TH><<<dim3(tiles, h->nb), NW * TH, 0, h->stream>>>(
-        h->spins, h->lab16, h->D, h->olist, h->ocount, make_div(h->L), h->L, h->N, h->words);
+        h->spins, h->lab16, h->D, h->olist, h->ocount, h->nsize, h->nmin, h->series, h->ctl, make_div(h->L),
+        h->L, h->N, h->words, h->nb);
+    h->launches += 1;
     if (h->eager_labels) {                          // a4 every sweep instead of on demand
-        k_compress_tiled<<<grid1((size_t)h->N / 4, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
-            h->label, h->series, h->ctl, h->N, h->nb, 0);
-        h->launches += 1;
+        SW_MARK(h, K_COMPRESS);
+        return launch_flatten_scan<NW, TH>(h);
     }
-    SW_MARK(h, K_SIZES_RESET);
-    k_sizes_reset<CAP><<<grid1((size_t)tiles * 32, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
-        h->olist, h->ocount, h->gsize, tiles, h->N);
-    h->launches += 2;
     return SW_OK;
 }
 
@@ -281,18 +307,10 @@ int launch_label_generic(sw_handle* h) {
 // labelling alone from the bond planes, leaving flat labels (the unfused order; sw_test_label)
 template <int NW, int TH>
 int launch_label_scan(sw_handle* h) {
-    constexpr int TW = 32 * NW, CAP = 2 * (TW + TH);
-    const int tiles = h->N / (TW * TH);
     int rc = launch_bond_label_scan<NW, TH>(h, false, false);
     if (rc) return rc;
     SW_MARK(h, K_COMPRESS);
-    k_compress_tiled<<<grid1((size_t)h->N / 4, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
-        h->label, h->series, h->ctl, h->N, h->nb, 0);   // roots are counted by bond_label + roots_open
-    SW_MARK(h, K_SIZES_RESET);
-    k_sizes_reset<CAP><<<grid1((size_t)tiles * 32, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
-        h->olist, h->ocount, h->gsize, tiles, h->N);
-    h->launches += 2;
-    return SW_OK;
+    return launch_flatten_scan<NW, TH>(h);
 }
 
 int launch_label(sw_handle* h) {
@@ -385,6 +403,7 @@ int init_handle(sw_handle* h, const double* T, const uint64_t* seed) {
     h->spins = (int8_t*)(w + o.spins);
     h->bondE = (uint32_t*)(w + o.bondE); h->bondS = (uint32_t*)(w + o.bondS); h->D = (uint32_t*)(w + o.D);
     h->label = (int*)(w + o.label); h->gsize = (int*)(w + o.gsize); h->lab16 = (uint16_t*)(w + o.lab16);
+    h->npar = (int*)(w + o.npar); h->nsize = (int*)(w + o.nsize); h->nmin = (int*)(w + o.nmin); h->bslot = (uint16_t*)(w + o.bslot);
     h->olist = (int2*)(w + o.olist); h->ocount = (int*)(w + o.ocount);
     h->lat = (Lat*)(w + o.lat); h->ctl = (Ctl*)(w + o.ctl); h->rec_now = (Rec*)(w + o.rec_now);
     h->series = (Rec*)(w + o.series);
@@ -518,10 +537,8 @@ int sw_sweep(sw_handle* h, int64_t n) {
 const int32_t* sw_labels(sw_handle* h) {
     if (!h) { set_err("sw_labels: null handle"); return nullptr; }
     if (!h->have_sweep) { set_err("sw_labels: no sweep has run yet"); return nullptr; }
-    if (!h->labels_flat) {      // the fast path leaves site -> tile root -> global root: flatten on demand (a4)
-        k_compress_tiled<<<grid1((size_t)h->N / 4, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
-            h->label, h->series, h->ctl, h->N, h->nb, 0);
-        if (cudaGetLastError() != cudaSuccess) { set_err("sw_labels: flatten launch failed"); return nullptr; }
+    if (!h->labels_flat) {      // the fast path leaves site -> tile root -> cluster root: flatten on demand (a4)
+        if (flatten_scan(h) != SW_OK || cudaGetLastError() != cudaSuccess) { set_err("sw_labels: flatten launch failed"); return nullptr; }
         h->labels_flat = true;
     }
     return h->label;

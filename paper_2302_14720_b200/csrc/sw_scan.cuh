@@ -59,6 +59,7 @@ template <int NW, int TH, bool FUSE>
 __global__ void __launch_bounds__(NW * TH)
 k_bond_label(const int8_t* __restrict__ spins, uint32_t* bondE, uint32_t* bondS,
              int* __restrict__ label, uint16_t* __restrict__ lab16, int2* __restrict__ olist, int* __restrict__ ocount,
+             int* __restrict__ npar, int* __restrict__ nsize, int* __restrict__ nmin, uint16_t* __restrict__ bslot,
              Rec* __restrict__ rec, const Lat* __restrict__ lat, const Ctl* __restrict__ ctl,
              int L, int N, int words, int nb, int obs_prev) {
     constexpr int TW = 32 * NW, SITES = TW * TH, THREADS = NW * TH;   // one thread per 32-site word
@@ -291,7 +292,11 @@ k_bond_label(const int8_t* __restrict__ spins, uint32_t* bondE, uint32_t* bondS,
     // ---- phase 5: closed clusters are complete -> maximum; open ones -> the tile's list -----------------
     {
         int mymax = 0, nclosed = 0;
-        int2* mylist = olist + ((size_t)blockIdx.y * gridDim.x + blockIdx.x) * CAP;
+        // an open tile root becomes node (tile, slot) of the global union-find: dense arrays of CAP entries per
+        // tile (L2-resident at L = 16384) instead of the N-entry label array (random DRAM sectors)
+        const int nodebase = blockIdx.x * CAP;                       // node ids are local to the lattice
+        const size_t lb = (size_t)blockIdx.y * gridDim.x * CAP;
+        int2* mylist = olist + lb + nodebase;
         while (rootbits) {
             const int l = mybase + __ffs(rootbits) - 1;
             rootbits &= rootbits - 1;
@@ -299,7 +304,12 @@ k_bond_label(const int8_t* __restrict__ spins, uint32_t* bondE, uint32_t* bondS,
             const int cnt = (int)((v >> CNT_SHIFT) & CNT_MASK);
             if (v & OPEN_BIT) {
                 const int pos = atomicAdd(&s_nopen, 1);
-                mylist[pos] = make_int2(tilebase + (l >> LOG_TW) * L + (l & (TW - 1)), cnt);
+                const int g = tilebase + (l >> LOG_TW) * L + (l & (TW - 1));
+                mylist[pos] = make_int2(g, cnt);
+                npar[lb + nodebase + pos] = nodebase + pos;          // its own root
+                nsize[lb + nodebase + pos] = cnt;                    // size of the cluster rooted here (so far: this piece)
+                nmin[lb + nodebase + pos] = g;                       // minimum site index of the cluster rooted here
+                par[l] = l | (pos << LS);                            // the root's word now carries its slot
             } else {
                 mymax = max(mymax, cnt);
                 ++nclosed;                                           // a closed tile root is a cluster root
@@ -322,6 +332,132 @@ k_bond_label(const int8_t* __restrict__ spins, uint32_t* bondE, uint32_t* bondS,
             if (s_obs[1]) atomic_add_ll(&rp->M, s_obs[1]);
         }
     }
+
+    // ---- phase 6: slot of the root of every border site with a bond across the tile edge ----------------
+    // (order: North row, South row, West column, East column; what k_merge_nodes reads instead of label[])
+    {
+        uint16_t* myb = bslot + ((size_t)blockIdx.y * gridDim.x + blockIdx.x) * CAP;
+        for (int j = tid; j < 2 * (TW + TH); j += THREADS) {
+            int site; bool open;
+            if (j < TW)               { site = j;                              open = (nIn[j >> 5] >> (j & 31)) & 1u; }
+            else if (j < 2 * TW)      { const int c = j - TW; site = (TH - 1) * TW + c;
+                                        open = (es[(TH - 1) * NW + (c >> 5)].y >> (c & 31)) & 1u; }
+            else if (j < 2 * TW + TH) { const int r = j - 2 * TW; site = r * TW; open = (wIn[r >> 5] >> (r & 31)) & 1u; }
+            else                      { const int r = j - 2 * TW - TH; site = r * TW + TW - 1;
+                                        open = es[r * NW + NW - 1].x >> 31; }
+            uint32_t slot = 0xFFFFu;
+            if (open) {
+                const int r = par[par[site] & IDX_MASK] & IDX_MASK;  // site -> label node -> root
+                slot = ((uint32_t)par[r] >> LS) & (uint32_t)CNT_MASK;
+            }
+            myb[j] = (uint16_t)slot;
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// a3 global boundary merge on the NODE arrays (north_star stage 2): one thread per site on a
+// tile's East column or South row; if its bond crosses the edge, the two tile roots (read as slots from the
+// border arrays of the two tiles) are united: find through L1, hook "larger id under smaller" with atomicMin.
+// Node id = tile * CAP + slot.  Any total order gives a valid forest; the canonical label (minimum SITE index,
+// PAPER.md:51) is accumulated per root in nmin[] by k_roots_nodes.
+// ---------------------------------------------------------------------------------------------------
+template <int TW, int TH>
+__global__ void __launch_bounds__(256)
+k_merge_nodes(int* npar, const uint16_t* __restrict__ bslot, const uint32_t* __restrict__ bondE,
+              const uint32_t* __restrict__ bondS, int L, int words) {
+    constexpr int CAP = 2 * (TW + TH);
+    const int tilesX = L / TW, tilesY = L / TH;
+    const int nV = L * tilesX;                       // East-edge sites
+    const int idx = blockIdx.x * 256 + threadIdx.x;
+    if (idx >= nV + tilesY * L) return;
+    const size_t lb = (size_t)blockIdx.y * tilesX * tilesY * CAP;
+    int* par = npar + lb;
+    const uint16_t* bs = bslot + lb;
+    const int wprL = L >> 5;
+    int ta, ka, tb, kb;
+    if (idx < nV) {
+        const int y = idx / tilesX, c = idx - y * tilesX;
+        const int x = c * TW + TW - 1;
+        if (!(bondE[(size_t)blockIdx.y * words + (size_t)y * wprL + (x >> 5)] >> 31)) return;
+        const int r = y / TH, rl = y - r * TH;
+        ta = r * tilesX + c;                          ka = 2 * TW + TH + rl;     // my East column
+        tb = r * tilesX + (c + 1 == tilesX ? 0 : c + 1); kb = 2 * TW + rl;       // the neighbour's West column
+    } else {
+        const int j = idx - nV;
+        const int r = j / L, x = j - r * L;
+        const int y = r * TH + TH - 1;
+        if (!((bondS[(size_t)blockIdx.y * words + (size_t)y * wprL + (x >> 5)] >> (x & 31)) & 1u)) return;
+        const int c = x / TW, cl = x - c * TW;
+        ta = r * tilesX + c;                               ka = TW + cl;         // my South row
+        tb = (r + 1 == tilesY ? 0 : r + 1) * tilesX + c;   kb = cl;              // the neighbour's North row
+    }
+    uf_union_l1(par, ta * CAP + (int)bs[(size_t)ta * CAP + ka], tb * CAP + (int)bs[(size_t)tb * CAP + kb]);
+}
+
+// After the merge: every open piece adds its size and its root's site index to the node it hangs under
+// (sum -> cluster size, min -> canonical label).  Pieces are combined per root inside the warp first, and the
+// root with the largest sum of the first round is carried in registers across rounds: at T_c one cluster owns
+// many pieces in every tile.  The list entry (site index of the tile root, size) becomes (site index, root node).
+// One warp per tile.
+template <int CAP>
+__global__ void __launch_bounds__(256)
+k_roots_nodes(const int* __restrict__ npar, int* __restrict__ nsize, int* __restrict__ nmin,
+              int2* __restrict__ olist, const int* __restrict__ ocount, int tiles) {
+    const int tile = blockIdx.x * 8 + (threadIdx.x >> 5);
+    const int lane = threadIdx.x & 31;
+    if (tile >= tiles) return;                              // (warp-uniform)
+    const size_t lb = (size_t)blockIdx.y * tiles * CAP;
+    const int* par = npar + lb;
+    int* sz = nsize + lb; int* mn = nmin + lb;
+    int2* list = olist + lb;
+    const int n = ocount[(size_t)blockIdx.y * tiles + tile];
+    int hot = -1, hotacc = 0, hotmin = 0x7fffffff;
+    for (int e0 = 0; e0 < n; e0 += 32) {
+        const int e = e0 + lane;
+        const bool on = e < n;
+        int root = -1 - lane, add = 0, g = 0x7fffffff;      // idle lanes: distinct keys, nothing to add
+        if (on) {
+            const int id = tile * CAP + e;
+            const int2 it = list[id];
+            root = uf_find_l1(par, id);                     // (no root changes during this kernel)
+            list[id].y = root;
+            g = it.x;
+            if (root != id) add = it.y;                     // a root's own piece is already in nsize / nmin
+        }
+        const unsigned grp = __match_any_sync(0xffffffffu, root);
+        const int tot = __reduce_add_sync(grp, add);
+        const int gm = __reduce_min_sync(grp, g);
+        if (e0 == 0) {                                      // choose the hot root
+            const int best = __reduce_max_sync(0xffffffffu, tot);
+            const unsigned who = __ballot_sync(0xffffffffu, tot == best && on);
+            if (who) hot = __shfl_sync(0xffffffffu, root, __ffs(who) - 1);
+        }
+        if (on && lane == __ffs(grp) - 1) {                 // one lane per root and round
+            if (root == hot) { hotacc += tot; hotmin = min(hotmin, gm); }
+            else if (tot) { atomicAdd(sz + root, tot); atomicMin(mn + root, gm); }
+        }
+    }
+    hotacc = warp_sum_i(hotacc);
+    hotmin = __reduce_min_sync(0xffffffffu, hotmin);
+    if (lane == 0 && hotacc) { atomicAdd(sz + hot, hotacc); atomicMin(mn + hot, hotmin); }
+}
+
+// a4 on demand (sw_labels): the label of an open tile root becomes its cluster's canonical label, so that
+// k_compress_tiled's two hops (site -> tile root -> cluster root) flatten the label array.
+template <int CAP>
+__global__ void __launch_bounds__(256)
+k_apply_roots(int* __restrict__ label, const int* __restrict__ nmin, const int2* __restrict__ olist,
+              const int* __restrict__ ocount, int tiles, int N) {
+    const int tile = blockIdx.x * 8 + (threadIdx.x >> 5);
+    const int lane = threadIdx.x & 31;
+    if (tile >= tiles) return;
+    const size_t lb = (size_t)blockIdx.y * tiles * CAP;
+    const int n = ocount[(size_t)blockIdx.y * tiles + tile];
+    for (int e = lane; e < n; e += 32) {
+        const int2 it = olist[lb + (size_t)tile * CAP + e];
+        label[(size_t)blockIdx.y * N + it.x] = nmin[lb + it.y];
+    }
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -341,7 +477,9 @@ k_bond_label(const int8_t* __restrict__ spins, uint32_t* bondE, uint32_t* bondS,
 template <int NW, int TH>
 __global__ void __launch_bounds__(NW * TH, 1536 / (NW * TH))
 k_flip16(int8_t* __restrict__ spins, const uint16_t* __restrict__ lab16, const uint32_t* __restrict__ D,
-         const int2* __restrict__ olist, const int* __restrict__ ocount, DivL dv, int L, int N, int words) {
+         const int2* __restrict__ olist, const int* __restrict__ ocount, const int* __restrict__ nsize,
+         const int* __restrict__ nmin, Rec* __restrict__ rec, const Ctl* __restrict__ ctl,
+         DivL dv, int L, int N, int words, int nb) {
     constexpr int TW = 32 * NW, SITES = TW * TH, THREADS = NW * TH;
     constexpr int CAP = 2 * (TW + TH);
     constexpr int OSTEPS = SITES / 8 / THREADS;      // = 4
@@ -369,17 +507,30 @@ k_flip16(int8_t* __restrict__ spins, const uint16_t* __restrict__ lab16, const u
         dec[tid] = d[(size_t)(y0 + row) * (L >> 5) + (x0 >> 5) + wx];
     }
     __syncthreads();
-    // open tile roots take the decision of their cluster root
+    // open tile roots take the decision of their cluster root = the minimum site index under their root node;
+    // the nodes that are roots are the clusters that span tiles: counted, and their sizes maximised, here
     {
-        const int2* mylist = olist + tile * CAP;
+        const size_t lb = (size_t)blockIdx.y * gridDim.x * CAP;
+        const int nodebase = blockIdx.x * CAP;
+        int nroot = 0, big = 0;
         for (int e = tid; e < n; e += THREADS) {
-            const int2 it = mylist[e];                                 // (tile root, cluster root)
-            const uint32_t up = (__ldg(d + (it.y >> 5)) >> (it.y & 31)) & 1u;
+            const int2 it = olist[lb + nodebase + e];                  // (site index of the tile root, root node)
+            const int R = nmin[lb + it.y];
+            if (it.y == nodebase + e) { ++nroot; big = max(big, nsize[lb + it.y]); }
+            const uint32_t up = (__ldg(d + (R >> 5)) >> (R & 31)) & 1u;
             const int delta = it.x - tilebase;
             const int ry = div_l(delta, dv);
             const int l = ry * TW + (delta - ry * L);
             if (up) atomicOr(&dec[l >> 5], 1u << (l & 31));
             else    atomicAnd(&dec[l >> 5], ~(1u << (l & 31)));
+        }
+        if (tid < ((n + 31) & ~31)) {                                  // (whole warps)
+            nroot = warp_sum_i(nroot); big = warp_max_i(big);
+            if ((tid & 31) == 0) {
+                Rec* r = rec + (size_t)ctl->slot * nb + blockIdx.y;
+                if (nroot) atomic_add_ll(&r->ncl, nroot);
+                if (big) atomic_max_ll(&r->maxcl, big);
+            }
         }
     }
     __syncthreads();
