@@ -242,7 +242,7 @@ int launch_bond_label_scan(sw_handle* h, bool fused, bool obs_prev) {
     const size_t nedge = (size_t)h->L * (h->L / TW + h->L / TH);
     SW_MARK(h, K_MERGE);
     k_merge_nodes<TW, TH><<<grid1(nedge, 256, h->nb), 256, 0, h->stream>>>(
-        h->npar, h->bslot, h->bondE, h->bondS, h->L, h->words);
+        h->npar, h->bslot, h->L / TW, h->L / TH);
     SW_MARK(h, K_SIZES);
     k_roots_nodes<CAP><<<grid1((size_t)tiles * 32, 256, h->nb), 256, 0, h->stream>>>(
         h->npar, h->nsize, h->nmin, h->olist, h->ocount, tiles);

@@ -357,42 +357,28 @@ k_bond_label(const int8_t* __restrict__ spins, uint32_t* bondE, uint32_t* bondS,
 
 // ---------------------------------------------------------------------------------------------------
 // a3 global boundary merge on the NODE arrays (north_star stage 2): one thread per site on a
-// tile's East column or South row; if its bond crosses the edge, the two tile roots (read as slots from the
-// border arrays of the two tiles) are united: find through L1, hook "larger id under smaller" with atomicMin.
+// tile's East column or South row; if its bond crosses the edge (its border entry holds a slot), the two tile
+// roots (slots from the border arrays of the two tiles) are united: find through L1, hook "larger id under smaller" with atomicMin.
 // Node id = tile * CAP + slot.  Any total order gives a valid forest; the canonical label (minimum SITE index,
 // PAPER.md:51) is accumulated per root in nmin[] by k_roots_nodes.
 // ---------------------------------------------------------------------------------------------------
 template <int TW, int TH>
 __global__ void __launch_bounds__(256)
-k_merge_nodes(int* npar, const uint16_t* __restrict__ bslot, const uint32_t* __restrict__ bondE,
-              const uint32_t* __restrict__ bondS, int L, int words) {
-    constexpr int CAP = 2 * (TW + TH);
-    const int tilesX = L / TW, tilesY = L / TH;
-    const int nV = L * tilesX;                       // East-edge sites
+k_merge_nodes(int* npar, const uint16_t* __restrict__ bslot, int tilesX, int tilesY) {
+    constexpr int CAP = 2 * (TW + TH), PER = TW + TH;       // per tile: TW South-row sites, TH East-column sites
     const int idx = blockIdx.x * 256 + threadIdx.x;
-    if (idx >= nV + tilesY * L) return;
-    const size_t lb = (size_t)blockIdx.y * tilesX * tilesY * CAP;
-    int* par = npar + lb;
+    const int tiles = tilesX * tilesY;
+    if (idx >= tiles * PER) return;
+    const size_t lb = (size_t)blockIdx.y * tiles * CAP;
     const uint16_t* bs = bslot + lb;
-    const int wprL = L >> 5;
-    int ta, ka, tb, kb;
-    if (idx < nV) {
-        const int y = idx / tilesX, c = idx - y * tilesX;
-        const int x = c * TW + TW - 1;
-        if (!(bondE[(size_t)blockIdx.y * words + (size_t)y * wprL + (x >> 5)] >> 31)) return;
-        const int r = y / TH, rl = y - r * TH;
-        ta = r * tilesX + c;                          ka = 2 * TW + TH + rl;     // my East column
-        tb = r * tilesX + (c + 1 == tilesX ? 0 : c + 1); kb = 2 * TW + rl;       // the neighbour's West column
-    } else {
-        const int j = idx - nV;
-        const int r = j / L, x = j - r * L;
-        const int y = r * TH + TH - 1;
-        if (!((bondS[(size_t)blockIdx.y * words + (size_t)y * wprL + (x >> 5)] >> (x & 31)) & 1u)) return;
-        const int c = x / TW, cl = x - c * TW;
-        ta = r * tilesX + c;                               ka = TW + cl;         // my South row
-        tb = (r + 1 == tilesY ? 0 : r + 1) * tilesX + c;   kb = cl;              // the neighbour's North row
-    }
-    uf_union_l1(par, ta * CAP + (int)bs[(size_t)ta * CAP + ka], tb * CAP + (int)bs[(size_t)tb * CAP + kb]);
+    const int ta = idx / PER, j = idx - ta * PER;
+    const int r = ta / tilesX, c = ta - r * tilesX;
+    int ka, tb, kb;
+    if (j < TW) { ka = TW + j;                tb = (r + 1 == tilesY ? 0 : r + 1) * tilesX + c; kb = j; }            // South row -> North row below
+    else        { ka = 2 * TW + TH + (j - TW); tb = r * tilesX + (c + 1 == tilesX ? 0 : c + 1); kb = 2 * TW + (j - TW); }  // East column -> West column
+    const int sa = bs[(size_t)ta * CAP + ka];
+    if (sa == 0xFFFF) return;                               // no bond across the edge here
+    uf_union_l1(npar + lb, ta * CAP + sa, tb * CAP + (int)bs[(size_t)tb * CAP + kb]);
 }
 
 // After the merge: every open piece adds its size and its root's site index to the node it hangs under
