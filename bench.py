@@ -185,7 +185,7 @@ def main():
 
     import numpy as np
     import torch
-    from paper_2302_14720_b200 import binding as B, workloads as wl
+    from paper_2302_14720_b200 import binding as B, workloads as wl, replicas as rp
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (no CPU fallback); use --impl reference for the oracle")
@@ -205,7 +205,7 @@ def main():
 
     L, T, K, W = args.L, wl.T_C, args.steps, args.warmup
     N = L * L
-    seed = 6 + rank                                   # configs[3] uses seed 6; replicas take 6 + rank
+    seed = rp.replica_seed(rank)                      # configs[3] uses seed 6; replicas take 6 + rank
     sw = B.SwendsenWang(L, T, seed, device=str(dev), path=args.path)
     if args.path in (0, 4, 5, 6, 7, 8, 9):
         tw, th = (64 if args.path == 4 else 256 if (args.path in (7, 8) and L % 256 == 0) else 128 if L % 128 == 0 else 64), 32
@@ -242,11 +242,8 @@ def main():
     sw.set_stage_timing(False)
     obs = sw.observables()[0]
 
-    if dist is not None:
-        tms = torch.tensor([ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(tms, op=dist.ReduceOp.MAX)
-        ms = float(tms.item())
-    value = world * N * K / (ms * 1e-3)
+    ms = rp.max_over_ranks(ms, dist, dev)
+    value = rp.whole_job_rate(N, K, world, ms)
 
     # ---- end to end through the C ABI with HOST buffers: H2D spins, one sweep, D2H spins + observables
     e2e = None
@@ -263,11 +260,8 @@ def main():
             o = B.sw_observables(sw.h)[0]                      # + the step's observables
         barrier()
         dt = time.perf_counter() - t0
-        if dist is not None:
-            tdt = torch.tensor([dt], device=dev, dtype=torch.float64)
-            dist.all_reduce(tdt, op=dist.ReduceOp.MAX)
-            dt = float(tdt.item())
-        e2e = {"value": world * N * Ke / dt, "unit": UNIT, "h2d_bytes_per_step": N,
+        dt = rp.max_over_ranks(dt, dist, dev)
+        e2e = {"value": rp.whole_job_rate(N, Ke, world, dt * 1e3), "unit": UNIT, "h2d_bytes_per_step": N,
                "d2h_bytes_per_step": N + 56, "steps": Ke, "ms_per_step": 1e3 * dt / Ke}
 
     if rank != 0:
@@ -281,8 +275,10 @@ def main():
     dom = max(kms, key=lambda k: kms[k])
     dom_ms = kms[dom] / timed
     achieved = kb.get(dom, 0.0) * N / (dom_ms * 1e-3) / 1e9
+    issue = (ncu_traffic("_issue_active_pct") or {}).get(dom)
     roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "traffic": ncu_traffic(dom), "peak_source": peak_src,
+                "issue_active_pct": issue,      # ncu smsp__issue_active of this kernel (profiles/): what really binds it
                 "bytes_per_site": kb.get(dom), "ms_per_launch": dom_ms,
                 "share_of_step": kms[dom] / max(1e-9, sum(kms.values()))}
     stages = {}
