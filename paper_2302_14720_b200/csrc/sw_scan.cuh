@@ -172,10 +172,10 @@ k_bond_label(const int8_t* __restrict__ spins, uint32_t* bondE, uint32_t* bondS,
             const uint32_t runmask = (above ^ (above - 1u)) & ~((1u << h) - 1u);
             const uint32_t upm = s_up & runmask;                     // sites of my run bonded to the row above
             const bool myUp = s_up & lanebit;
-            int a = prev;
-            if (myUp) {                                              // root of the site above
-                for (int p = par[a]; p != a; p = par[a]) a = p;
-            }
+            // label of the site above, one hop fresher: its parent (itself while it still is a root; the root it was
+            // hooked under in the previous row otherwise).  Nothing below needs an exact root: a stale node is
+            // still a label node of the right tree, and the hook falls back to sc_union, which takes any nodes.
+            const int a = par[prev];
             const int got = __shfl_sync(0xffffffffu, a, __ffs(upm) - 1);   // (source lane is taken mod 32)
             const int c = upm ? got : rowbase + h;                   // a new label: the head's own index (its own root)
             par[rowbase + lane] = c;
