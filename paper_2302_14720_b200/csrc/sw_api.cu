@@ -62,7 +62,7 @@ using Cfg64 = TileCfg<64, 64>;
 using Cfg256 = TileCfg<256, 32>;
 
 struct Layout {        // byte offsets into the workspace
-    size_t spins, bondE, bondS, D, label, lab16, gsize, olist, ocount, npar, nsize, nmin, bslot, lat, ctl, rec_now, series, total;
+    size_t spins, bondE, bondS, D, label, lab16, gsize, olist, ocount, nodes, bslot, lat, ctl, rec_now, series, total;
 };
 
 size_t olist_entries(int L) {          // per lattice, maximum over the tile shapes usable for this L
@@ -95,9 +95,7 @@ Layout make_layout(int L, int nb) {
     o.gsize = p;   p = align_up(p + (size_t)nb * N * 4);
     o.olist = p;   p = align_up(p + (size_t)nb * olist_entries(L) * sizeof(int2));
     o.ocount = p;  p = align_up(p + (size_t)nb * tiles_max(L) * 4);
-    o.npar = p;    p = align_up(p + (size_t)nb * olist_entries(L) * 4);      // node arrays of the scan path
-    o.nsize = p;   p = align_up(p + (size_t)nb * olist_entries(L) * 4);
-    o.nmin = p;    p = align_up(p + (size_t)nb * olist_entries(L) * 4);
+    o.nodes = p;   p = align_up(p + (size_t)nb * olist_entries(L) * 16);     // node array of the scan path
     o.bslot = p;   p = align_up(p + (size_t)nb * olist_entries(L) * 2);
     o.lat = p;     p = align_up(p + (size_t)nb * sizeof(Lat));
     o.ctl = p;     p = align_up(p + sizeof(Ctl));
@@ -129,7 +127,7 @@ struct sw_handle {
     int8_t* spins = nullptr; uint32_t *bondE = nullptr, *bondS = nullptr, *D = nullptr;
     int *label = nullptr, *gsize = nullptr, *ocount = nullptr; int2* olist = nullptr;
     uint16_t* lab16 = nullptr;       // tile-local root index of every site (scan path)
-    int *npar = nullptr, *nsize = nullptr, *nmin = nullptr;   // union-find over open tile roots: parent, size, min site
+    int4* nodes = nullptr;           // union-find over open tile roots: (parent, size, min site, site)
     uint16_t* bslot = nullptr;       // per tile: slot of the root of each border site
     Lat* lat = nullptr; Ctl* ctl = nullptr; Rec* rec_now = nullptr;
     Rec* series = nullptr; Rec* series_owned = nullptr;
@@ -229,23 +227,23 @@ int launch_bond_label_scan(sw_handle* h, bool fused, bool obs_prev) {
     if (fused) {
         SW_MARK(h, K_BONDLABEL);
         k_bond_label<NW, TH, true><<<dim3(tiles, h->nb), NW * TH, smem, h->stream>>>(
-            h->spins, h->bondE, h->bondS, h->label, h->lab16, h->olist, h->ocount, h->npar, h->nsize, h->nmin, h->bslot,
+            h->spins, h->bondE, h->bondS, h->label, h->lab16, h->nodes, h->ocount, h->bslot,
             h->series, h->lat, h->ctl,
             h->L, h->N, h->words, h->nb, obs_prev ? 1 : 0);
     } else {
         SW_MARK(h, K_TILE);
         k_bond_label<NW, TH, false><<<dim3(tiles, h->nb), NW * TH, smem, h->stream>>>(
-            h->spins, h->bondE, h->bondS, h->label, h->lab16, h->olist, h->ocount, h->npar, h->nsize, h->nmin, h->bslot,
+            h->spins, h->bondE, h->bondS, h->label, h->lab16, h->nodes, h->ocount, h->bslot,
             h->series, h->lat, h->ctl,
             h->L, h->N, h->words, h->nb, obs_prev ? 1 : 0);
     }
     const size_t nedge = (size_t)h->L * (h->L / TW + h->L / TH);
     SW_MARK(h, K_MERGE);
     k_merge_nodes<TW, TH><<<grid1(nedge, 256, h->nb), 256, 0, h->stream>>>(
-        h->npar, h->bslot, h->L / TW, h->L / TH);
+        h->nodes, h->bslot, h->L / TW, h->L / TH);
     SW_MARK(h, K_SIZES);
     k_roots_nodes<CAP><<<grid1((size_t)tiles * 32, 256, h->nb), 256, 0, h->stream>>>(
-        h->npar, h->nsize, h->nmin, h->olist, h->ocount, tiles);
+        h->nodes, h->ocount, tiles);
     h->launches += 3;
     return SW_OK;
 }
@@ -255,7 +253,7 @@ int launch_flatten_scan(sw_handle* h) {
     constexpr int TW = 32 * NW, CAP = 2 * (TW + TH);
     const int tiles = h->N / (TW * TH);
     k_apply_roots<CAP><<<grid1((size_t)tiles * 32, 256, h->nb), 256, 0, h->stream>>>(
-        h->label, h->nmin, h->olist, h->ocount, tiles, h->N);
+        h->label, h->nodes, h->ocount, tiles, h->N);
     k_compress_tiled<<<grid1((size_t)h->N / 4, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
         h->label, h->series, h->ctl, h->N, h->nb, 0);
     h->launches += 2;
@@ -278,7 +276,7 @@ int launch_flip_scan(sw_handle* h) {
     const int tiles = h->N / (TW * TH);
     SW_MARK(h, K_FLIPTILE);
     k_flip16<NW, TH><<<dim3(tiles, h->nb), NW * TH, 0, h->stream>>>(
-        h->spins, h->lab16, h->D, h->olist, h->ocount, h->nsize, h->nmin, h->series, h->ctl, make_div(h->L),
+        h->spins, h->lab16, h->D, h->nodes, h->ocount, h->series, h->ctl, make_div(h->L),
         h->L, h->N, h->words, h->nb);
     h->launches += 1;
     if (h->eager_labels) {                          // a4 every sweep instead of on demand
@@ -403,7 +401,7 @@ int init_handle(sw_handle* h, const double* T, const uint64_t* seed) {
     h->spins = (int8_t*)(w + o.spins);
     h->bondE = (uint32_t*)(w + o.bondE); h->bondS = (uint32_t*)(w + o.bondS); h->D = (uint32_t*)(w + o.D);
     h->label = (int*)(w + o.label); h->gsize = (int*)(w + o.gsize); h->lab16 = (uint16_t*)(w + o.lab16);
-    h->npar = (int*)(w + o.npar); h->nsize = (int*)(w + o.nsize); h->nmin = (int*)(w + o.nmin); h->bslot = (uint16_t*)(w + o.bslot);
+    h->nodes = (int4*)(w + o.nodes); h->bslot = (uint16_t*)(w + o.bslot);
     h->olist = (int2*)(w + o.olist); h->ocount = (int*)(w + o.ocount);
     h->lat = (Lat*)(w + o.lat); h->ctl = (Ctl*)(w + o.ctl); h->rec_now = (Rec*)(w + o.rec_now);
     h->series = (Rec*)(w + o.series);

@@ -58,8 +58,8 @@ __device__ __forceinline__ int div_l(int v, const DivL& D) {
 template <int NW, int TH, bool FUSE>
 __global__ void __launch_bounds__(NW * TH)
 k_bond_label(const int8_t* __restrict__ spins, uint32_t* bondE, uint32_t* bondS,
-             int* __restrict__ label, uint16_t* __restrict__ lab16, int2* __restrict__ olist, int* __restrict__ ocount,
-             int* __restrict__ npar, int* __restrict__ nsize, int* __restrict__ nmin, uint16_t* __restrict__ bslot,
+             int* __restrict__ label, uint16_t* __restrict__ lab16, int4* __restrict__ nodes, int* __restrict__ ocount,
+             uint16_t* __restrict__ bslot,
              Rec* __restrict__ rec, const Lat* __restrict__ lat, const Ctl* __restrict__ ctl,
              int L, int N, int words, int nb, int obs_prev) {
     constexpr int TW = 32 * NW, SITES = TW * TH, THREADS = NW * TH;   // one thread per 32-site word
@@ -296,7 +296,7 @@ k_bond_label(const int8_t* __restrict__ spins, uint32_t* bondE, uint32_t* bondS,
         // tile (L2-resident at L = 16384) instead of the N-entry label array (random DRAM sectors)
         const int nodebase = blockIdx.x * CAP;                       // node ids are local to the lattice
         const size_t lb = (size_t)blockIdx.y * gridDim.x * CAP;
-        int2* mylist = olist + lb + nodebase;
+        int4* mynodes = nodes + lb + nodebase;
         while (rootbits) {
             const int l = mybase + __ffs(rootbits) - 1;
             rootbits &= rootbits - 1;
@@ -305,10 +305,9 @@ k_bond_label(const int8_t* __restrict__ spins, uint32_t* bondE, uint32_t* bondS,
             if (v & OPEN_BIT) {
                 const int pos = atomicAdd(&s_nopen, 1);
                 const int g = tilebase + (l >> LOG_TW) * L + (l & (TW - 1));
-                mylist[pos] = make_int2(g, cnt);
-                npar[lb + nodebase + pos] = nodebase + pos;          // its own root
-                nsize[lb + nodebase + pos] = cnt;                    // size of the cluster rooted here (so far: this piece)
-                nmin[lb + nodebase + pos] = g;                       // minimum site index of the cluster rooted here
+                // node = (parent: its own root, size of the cluster rooted here: so far this piece,
+                //         minimum site index of the cluster rooted here, site index of this tile root)
+                mynodes[pos] = make_int4(nodebase + pos, cnt, g, g);
                 par[l] = l | (pos << LS);                            // the root's word now carries its slot
             } else {
                 mymax = max(mymax, cnt);
@@ -362,9 +361,26 @@ k_bond_label(const int8_t* __restrict__ spins, uint32_t* bondE, uint32_t* bondS,
 // Node id = tile * CAP + slot.  Any total order gives a valid forest; the canonical label (minimum SITE index,
 // PAPER.md:51) is accumulated per root in nmin[] by k_roots_nodes.
 // ---------------------------------------------------------------------------------------------------
+// union-find on the node array: the parent is field x of the node.  Walks go through L1 (a stale line shows an
+// older parent = still an ancestor); the atomicMin in L2 decides whether a node still is a root.
+__device__ __forceinline__ int nd_find(const int4* nodes, int x) {
+    int p = ld_ca(&nodes[x].x);
+    while (p != x) { x = p; p = ld_ca(&nodes[x].x); }
+    return x;
+}
+__device__ __forceinline__ void nd_union(int4* nodes, int a, int b) {
+    a = nd_find(nodes, a); b = nd_find(nodes, b);
+    while (a != b) {
+        if (a < b) { const int s = a; a = b; b = s; }      // a is the larger
+        const int old = atomicMin(&nodes[a].x, b);
+        if (old == a) break;
+        a = old;
+    }
+}
+
 template <int TW, int TH>
 __global__ void __launch_bounds__(256)
-k_merge_nodes(int* npar, const uint16_t* __restrict__ bslot, int tilesX, int tilesY) {
+k_merge_nodes(int4* nodes, const uint16_t* __restrict__ bslot, int tilesX, int tilesY) {
     constexpr int CAP = 2 * (TW + TH), PER = TW + TH;       // per tile: TW South-row sites, TH East-column sites
     const int idx = blockIdx.x * 256 + threadIdx.x;
     const int tiles = tilesX * tilesY;
@@ -378,25 +394,20 @@ k_merge_nodes(int* npar, const uint16_t* __restrict__ bslot, int tilesX, int til
     else        { ka = 2 * TW + TH + (j - TW); tb = r * tilesX + (c + 1 == tilesX ? 0 : c + 1); kb = 2 * TW + (j - TW); }  // East column -> West column
     const int sa = bs[(size_t)ta * CAP + ka];
     if (sa == 0xFFFF) return;                               // no bond across the edge here
-    uf_union_l1(npar + lb, ta * CAP + sa, tb * CAP + (int)bs[(size_t)tb * CAP + kb]);
+    nd_union(nodes + lb, ta * CAP + sa, tb * CAP + (int)bs[(size_t)tb * CAP + kb]);
 }
 
-// After the merge: every open piece adds its size and its root's site index to the node it hangs under
-// (sum -> cluster size, min -> canonical label).  Pieces are combined per root inside the warp first, and the
-// root with the largest sum of the first round is carried in registers across rounds: at T_c one cluster owns
-// many pieces in every tile.  The list entry (site index of the tile root, size) becomes (site index, root node).
-// One warp per tile.
+// After the merge: every open piece adds its size and its site index to the node it hangs under (sum -> cluster
+// size, min -> canonical label) and points straight at it.  Pieces are combined per root inside the warp first,
+// and the root with the largest sum of the first round is carried in registers across rounds: at T_c one cluster
+// owns many pieces in every tile.  One warp per tile.
 template <int CAP>
 __global__ void __launch_bounds__(256)
-k_roots_nodes(const int* __restrict__ npar, int* __restrict__ nsize, int* __restrict__ nmin,
-              int2* __restrict__ olist, const int* __restrict__ ocount, int tiles) {
+k_roots_nodes(int4* nodes, const int* __restrict__ ocount, int tiles) {
     const int tile = blockIdx.x * 8 + (threadIdx.x >> 5);
     const int lane = threadIdx.x & 31;
     if (tile >= tiles) return;                              // (warp-uniform)
-    const size_t lb = (size_t)blockIdx.y * tiles * CAP;
-    const int* par = npar + lb;
-    int* sz = nsize + lb; int* mn = nmin + lb;
-    int2* list = olist + lb;
+    int4* nd = nodes + (size_t)blockIdx.y * tiles * CAP;
     const int n = ocount[(size_t)blockIdx.y * tiles + tile];
     int hot = -1, hotacc = 0, hotmin = 0x7fffffff;
     for (int e0 = 0; e0 < n; e0 += 32) {
@@ -405,11 +416,14 @@ k_roots_nodes(const int* __restrict__ npar, int* __restrict__ nsize, int* __rest
         int root = -1 - lane, add = 0, g = 0x7fffffff;      // idle lanes: distinct keys, nothing to add
         if (on) {
             const int id = tile * CAP + e;
-            const int2 it = list[id];
-            root = uf_find_l1(par, id);                     // (no root changes during this kernel)
-            list[id].y = root;
-            g = it.x;
-            if (root != id) add = it.y;                     // a root's own piece is already in nsize / nmin
+            const int4 me = nd[id];
+            root = me.x;
+            if (root != id) {                               // hooked: (no root changes during this kernel)
+                root = nd_find(nd, root);
+                if (root != me.x) nd[id].x = root;          // only ever an ancestor: safe while others walk
+                add = me.y;                                 // a root's own piece is already in its size / min
+            }
+            g = me.w;
         }
         const unsigned grp = __match_any_sync(0xffffffffu, root);
         const int tot = __reduce_add_sync(grp, add);
@@ -421,28 +435,27 @@ k_roots_nodes(const int* __restrict__ npar, int* __restrict__ nsize, int* __rest
         }
         if (on && lane == __ffs(grp) - 1) {                 // one lane per root and round
             if (root == hot) { hotacc += tot; hotmin = min(hotmin, gm); }
-            else if (tot) { atomicAdd(sz + root, tot); atomicMin(mn + root, gm); }
+            else if (tot) { atomicAdd(&nd[root].y, tot); atomicMin(&nd[root].z, gm); }
         }
     }
     hotacc = warp_sum_i(hotacc);
     hotmin = __reduce_min_sync(0xffffffffu, hotmin);
-    if (lane == 0 && hotacc) { atomicAdd(sz + hot, hotacc); atomicMin(mn + hot, hotmin); }
+    if (lane == 0 && hotacc) { atomicAdd(&nd[hot].y, hotacc); atomicMin(&nd[hot].z, hotmin); }
 }
 
 // a4 on demand (sw_labels): the label of an open tile root becomes its cluster's canonical label, so that
 // k_compress_tiled's two hops (site -> tile root -> cluster root) flatten the label array.
 template <int CAP>
 __global__ void __launch_bounds__(256)
-k_apply_roots(int* __restrict__ label, const int* __restrict__ nmin, const int2* __restrict__ olist,
-              const int* __restrict__ ocount, int tiles, int N) {
+k_apply_roots(int* __restrict__ label, const int4* __restrict__ nodes, const int* __restrict__ ocount, int tiles, int N) {
     const int tile = blockIdx.x * 8 + (threadIdx.x >> 5);
     const int lane = threadIdx.x & 31;
     if (tile >= tiles) return;
-    const size_t lb = (size_t)blockIdx.y * tiles * CAP;
+    const int4* nd = nodes + (size_t)blockIdx.y * tiles * CAP;
     const int n = ocount[(size_t)blockIdx.y * tiles + tile];
     for (int e = lane; e < n; e += 32) {
-        const int2 it = olist[lb + (size_t)tile * CAP + e];
-        label[(size_t)blockIdx.y * N + it.x] = nmin[lb + it.y];
+        const int4 me = nd[tile * CAP + e];
+        label[(size_t)blockIdx.y * N + me.w] = nd[me.x].z;
     }
 }
 
@@ -463,8 +476,7 @@ k_apply_roots(int* __restrict__ label, const int* __restrict__ nmin, const int2*
 template <int NW, int TH>
 __global__ void __launch_bounds__(NW * TH, 1536 / (NW * TH))
 k_flip16(int8_t* __restrict__ spins, const uint16_t* __restrict__ lab16, const uint32_t* __restrict__ D,
-         const int2* __restrict__ olist, const int* __restrict__ ocount, const int* __restrict__ nsize,
-         const int* __restrict__ nmin, Rec* __restrict__ rec, const Ctl* __restrict__ ctl,
+         const int4* __restrict__ nodes, const int* __restrict__ ocount, Rec* __restrict__ rec, const Ctl* __restrict__ ctl,
          DivL dv, int L, int N, int words, int nb) {
     constexpr int TW = 32 * NW, SITES = TW * TH, THREADS = NW * TH;
     constexpr int CAP = 2 * (TW + TH);
@@ -500,11 +512,11 @@ k_flip16(int8_t* __restrict__ spins, const uint16_t* __restrict__ lab16, const u
         const int nodebase = blockIdx.x * CAP;
         int nroot = 0, big = 0;
         for (int e = tid; e < n; e += THREADS) {
-            const int2 it = olist[lb + nodebase + e];                  // (site index of the tile root, root node)
-            const int R = nmin[lb + it.y];
-            if (it.y == nodebase + e) { ++nroot; big = max(big, nsize[lb + it.y]); }
+            const int4 me = nodes[lb + nodebase + e];                  // (root node, size, min site, site of the tile root)
+            const int R = me.x == nodebase + e ? me.z : nodes[lb + me.x].z;
+            if (me.x == nodebase + e) { ++nroot; big = max(big, me.y); }
             const uint32_t up = (__ldg(d + (R >> 5)) >> (R & 31)) & 1u;
-            const int delta = it.x - tilebase;
+            const int delta = me.w - tilebase;
             const int ry = div_l(delta, dv);
             const int l = ry * TW + (delta - ry * L);
             if (up) atomicOr(&dec[l >> 5], 1u << (l & 31));
