@@ -132,6 +132,22 @@ int        sw_set_stream(sw_handle* h, void* cuda_stream); /* a cudaStream_t; NU
 int64_t    sw_series(sw_handle* h, sw_obs* out, int64_t cap);
 int        sw_set_series_capacity(sw_handle* h, int64_t sweeps);
 
+/* Moments of the per-sweep observables over every sweep since creation or the last sw_moments_reset
+ * (the paper validates on E, the specific heat and M against T: PAPER.md:113-123,
+ * section 4, Figs. 5-7).  Per configuration e = E/N, a = |M|/N; summed on the device one
+ * sweep at a time in double, in sweep order, unfused.  e_mean = <e>, e2_mean = <e^2>, absm_mean = <|m|>,
+ * m2_mean = <m^2>, m4_mean = <m^4>; specific_heat = N (<e^2> - <e>^2) / T^2; susceptibility =
+ * N (<m^2> - <|m|>^2) / T; binder = 1 - <m^4> / (3 <m^2>^2).  n = 0 (all fields 0) before any sweep.
+ * sw_moments synchronises and fills out[0..nb-1] (HOST); discard thermalisation with sw_moments_reset
+ * (asynchronous on the handle's stream).  Sweeps are counted whatever the start state was set to. */
+typedef struct {
+    int64_t n;
+    double  e_mean, e2_mean, absm_mean, m2_mean, m4_mean;
+    double  specific_heat, susceptibility, binder;
+} sw_mom;
+int        sw_moments(sw_handle* h, sw_mom* out);
+int        sw_moments_reset(sw_handle* h);
+
 /* Per-stage device time in ms, summed over the sweeps of the last sw_sweep call that ran with stage
  * timing on: out = {bond, label, flip, observe}.  Stage timing brackets each stage with CUDA events
  * (it serialises nothing but adds event records; off by default).  BASELINE config 3. */

@@ -28,6 +28,16 @@ class sw_obs(C.Structure):
         return (self.energy, self.magnetisation, self.n_clusters, self.largest_cluster)
 
 
+class sw_mom(C.Structure):
+    """Mirror of include/sw.h sw_mom (moments of the per-sweep observables)."""
+    _fields_ = [("n", C.c_int64), ("e_mean", C.c_double), ("e2_mean", C.c_double), ("absm_mean", C.c_double),
+                ("m2_mean", C.c_double), ("m4_mean", C.c_double), ("specific_heat", C.c_double),
+                ("susceptibility", C.c_double), ("binder", C.c_double)]
+
+    def as_dict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_}
+
+
 class SwError(RuntimeError):
     def __init__(self, code: int, text: str):
         super().__init__(f"sw error {code}: {text}")
@@ -58,6 +68,8 @@ PROTOTYPES = {
     "sw_set_stream": (C.c_int, [_VP, _VP]),
     "sw_series": (_I64, [_VP, C.POINTER(sw_obs), _I64]),
     "sw_set_series_capacity": (C.c_int, [_VP, _I64]),
+    "sw_moments": (C.c_int, [_VP, C.POINTER(sw_mom)]),
+    "sw_moments_reset": (C.c_int, [_VP]),
     "sw_set_stage_timing": (C.c_int, [_VP, C.c_int]),
     "sw_stage_ms": (C.c_int, [_VP, C.POINTER(C.c_float)]),
     "sw_kernel_ms": (C.c_int, [_VP, C.POINTER(C.c_float), _I32]),
@@ -175,6 +187,16 @@ def sw_series(h, cap: Optional[int] = None) -> np.ndarray:
     for k in range(n * nb):
         a[k // nb, k % nb] = buf[k].as_tuple()
     return a
+
+def sw_moments(h) -> List[dict]:
+    """Moments of the per-sweep observables since creation / the last reset, one dict per lattice."""
+    nb = lib().sw_batch(_ptr(h))
+    out = (sw_mom * nb)()
+    _check(lib().sw_moments(h, out))
+    return [m.as_dict() for m in out]
+
+def sw_moments_reset(h) -> None:
+    _check(lib().sw_moments_reset(_ptr(h)))
 
 def sw_set_series_capacity(h, sweeps: int) -> None:
     _check(lib().sw_set_series_capacity(_ptr(h), sweeps))
@@ -309,6 +331,12 @@ class SwendsenWang:
 
     def series(self, cap=None):
         return sw_series(self.h, cap)
+
+    def moments(self):
+        return sw_moments(self.h)
+
+    def moments_reset(self):
+        sw_moments_reset(self.h)
 
     # -- state
     def set_spins(self, spins):

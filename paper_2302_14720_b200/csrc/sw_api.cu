@@ -62,7 +62,7 @@ using Cfg64 = TileCfg<64, 64>;
 using Cfg256 = TileCfg<256, 32>;
 
 struct Layout {        // byte offsets into the workspace
-    size_t spins, bondE, bondS, D, label, lab16, gsize, olist, ocount, nodes, bslot, lat, ctl, rec_now, series, total;
+    size_t spins, bondE, bondS, D, label, lab16, gsize, olist, ocount, nodes, bslot, lat, ctl, rec_now, mom, series, total;
 };
 
 size_t olist_entries(int L) {          // per lattice, maximum over the tile shapes usable for this L
@@ -100,6 +100,7 @@ Layout make_layout(int L, int nb) {
     o.lat = p;     p = align_up(p + (size_t)nb * sizeof(Lat));
     o.ctl = p;     p = align_up(p + sizeof(Ctl));
     o.rec_now = p; p = align_up(p + (size_t)nb * sizeof(Rec));
+    o.mom = p;     p = align_up(p + (size_t)nb * sizeof(Mom));
     o.series = p;  p = align_up(p + (size_t)(DEFAULT_SERIES_CAP + 1) * nb * sizeof(Rec));
     o.total = p;
     return o;
@@ -129,7 +130,8 @@ struct sw_handle {
     uint16_t* lab16 = nullptr;       // tile-local root index of every site (scan path)
     int4* nodes = nullptr;           // union-find over open tile roots: (parent, size, min site, site)
     uint16_t* bslot = nullptr;       // per tile: slot of the root of each border site
-    Lat* lat = nullptr; Ctl* ctl = nullptr; Rec* rec_now = nullptr;
+    Lat* lat = nullptr; Ctl* ctl = nullptr; Rec* rec_now = nullptr; Mom* mom = nullptr;
+    std::vector<double> hT;          // temperatures (sw_moments: specific heat, susceptibility)
     Rec* series = nullptr; Rec* series_owned = nullptr;
     int64_t series_cap = DEFAULT_SERIES_CAP;       // sweeps retained; the ring has series_cap + 1 slots
     int64_t ring() const { return series_cap + 1; }  // (the slot after the last sweep is already zeroed)
@@ -350,7 +352,7 @@ int launch_sweep(sw_handle* h, int64_t k) {
            : nw == 4 ? launch_flip_scan<4, 32>(h) : launch_flip_scan<2, 32>(h);
         if (rc) return rc;
         SW_MARK(h, K_ADVANCE);
-        k_advance<<<1, 64, 0, h->stream>>>(h->ctl, h->series, h->nb);
+        k_advance<<<1, 64, 0, h->stream>>>(h->ctl, h->series, h->nb, h->mom, h->N, k > 0 ? 2 : 0);
         h->launches += 1;
         SW_MARK(h, K_COUNT);
         h->labels_flat = h->eager_labels;
@@ -389,7 +391,7 @@ int launch_sweep(sw_handle* h, int64_t k) {
         k_observe_generic<<<grid1(h->N, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(
             h->spins, h->series, h->ctl, 1, h->L, h->N, h->nb);
     SW_MARK(h, K_ADVANCE);
-    k_advance<<<1, 64, 0, h->stream>>>(h->ctl, h->series, h->nb);
+    k_advance<<<1, 64, 0, h->stream>>>(h->ctl, h->series, h->nb, h->mom, h->N, 1);
     h->launches += 2;
     SW_MARK(h, K_COUNT);
     return SW_OK;
@@ -403,7 +405,8 @@ int init_handle(sw_handle* h, const double* T, const uint64_t* seed) {
     h->label = (int*)(w + o.label); h->gsize = (int*)(w + o.gsize); h->lab16 = (uint16_t*)(w + o.lab16);
     h->nodes = (int4*)(w + o.nodes); h->bslot = (uint16_t*)(w + o.bslot);
     h->olist = (int2*)(w + o.olist); h->ocount = (int*)(w + o.ocount);
-    h->lat = (Lat*)(w + o.lat); h->ctl = (Ctl*)(w + o.ctl); h->rec_now = (Rec*)(w + o.rec_now);
+    h->lat = (Lat*)(w + o.lat); h->ctl = (Ctl*)(w + o.ctl); h->rec_now = (Rec*)(w + o.rec_now); h->mom = (Mom*)(w + o.mom);
+    h->hT.assign(T, T + h->nb);
     h->series = (Rec*)(w + o.series);
     h->hlat.resize(h->nb);
     for (int b = 0; b < h->nb; ++b) {
@@ -415,6 +418,7 @@ int init_handle(sw_handle* h, const double* T, const uint64_t* seed) {
     SW_CUDA(cudaMemcpyAsync(h->lat, h->hlat.data(), sizeof(Lat) * h->nb, cudaMemcpyHostToDevice, h->stream));
     SW_CUDA(cudaMemsetAsync(h->gsize, 0, (size_t)h->nb * h->N * 4, h->stream));
     SW_CUDA(cudaMemsetAsync(h->series, 0, (size_t)h->ring() * h->nb * sizeof(Rec), h->stream));
+    SW_CUDA(cudaMemsetAsync(h->mom, 0, (size_t)h->nb * sizeof(Mom), h->stream));
     k_set_ctl<<<1, 1, 0, h->stream>>>(h->ctl, 0ull, 0u, (uint32_t)h->ring());
     k_init_random<<<grid1(h->words, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(h->spins, h->lat, h->N, h->words);
     SW_CUDA(cudaGetLastError());
@@ -521,8 +525,9 @@ int sw_sweep(sw_handle* h, int64_t n) {
         if (h->timing) SW_CUDA(cudaEventRecord(h->ev_tail[0], h->stream));
         k_observe_rows<<<grid1(h->words, 256, h->nb), 256, 0, h->stream>>>(
             h->spins, h->series, h->ctl, h->L, h->N, h->words, h->nb);
+        k_moments_last<<<1, 64, 0, h->stream>>>(h->ctl, h->series, h->nb, h->mom, h->N);
         if (h->timing) SW_CUDA(cudaEventRecord(h->ev_tail[1], h->stream));
-        h->launches += 1;
+        h->launches += 2;
     }
     SW_CUDA(cudaGetLastError());
     h->t += (uint64_t)n;
@@ -589,6 +594,32 @@ int64_t sw_series(sw_handle* h, sw_obs* out, int64_t cap) {
                      out + (size_t)k * h->nb + b);
     }
     return kept;
+}
+
+int sw_moments(sw_handle* h, sw_mom* out) {
+    if (!h || !out) { set_err("sw_moments: null argument"); return SW_EINVAL; }
+    std::vector<Mom> m(h->nb);
+    SW_CUDA(cudaMemcpyAsync(m.data(), h->mom, sizeof(Mom) * h->nb, cudaMemcpyDeviceToHost, h->stream));
+    SW_CUDA(cudaStreamSynchronize(h->stream));
+    for (int b = 0; b < h->nb; ++b) {
+        sw_mom* o = out + b;
+        std::memset(o, 0, sizeof *o);
+        o->n = m[b].n;
+        if (m[b].n == 0) continue;
+        const double fn = (double)m[b].n, fN = (double)h->N, T = h->hT[b];
+        const double e = m[b].s_e / fn, e2 = m[b].s_e2 / fn, am = m[b].s_am / fn, m2 = m[b].s_m2 / fn, m4 = m[b].s_m4 / fn;
+        o->e_mean = e; o->e2_mean = e2; o->absm_mean = am; o->m2_mean = m2; o->m4_mean = m4;
+        o->specific_heat = fN * (e2 - e * e) / (T * T);
+        o->susceptibility = fN * (m2 - am * am) / T;
+        o->binder = m2 > 0.0 ? 1.0 - m4 / (3.0 * (m2 * m2)) : 0.0;
+    }
+    return SW_OK;
+}
+
+int sw_moments_reset(sw_handle* h) {
+    if (!h) { set_err("sw_moments_reset: null handle"); return SW_EINVAL; }
+    SW_CUDA(cudaMemsetAsync(h->mom, 0, (size_t)h->nb * sizeof(Mom), h->stream));
+    return SW_OK;
 }
 
 int sw_set_series_capacity(sw_handle* h, int64_t sweeps) {

@@ -28,9 +28,27 @@ struct Rec {
     long long E, M, ncl, maxcl;
 };
 
-// Spins live bit-packed on the device: bit (i & 31) of word (i >> 5) is 1 for spin +1, 0 for spin -1
-// (the same bit-plane layout as the bond planes and the decision plane D, so "new spins = gather(D, root)"
-// is a gather of bits).  The int8 +-1 array of the C ABI is materialised from it on demand.
+// running sums of the per-sweep observables of one lattice (sw_moments):
+// e = E / N, a = |M| / N per configuration, summed one sweep at a time in double, in sweep
+// order, with no fused operations -- the same arithmetic in the same order as the oracle's definition.
+struct Mom {
+    double s_e, s_e2, s_am, s_m2, s_m4;
+    long long n;
+};
+__device__ __forceinline__ void mom_add(Mom& m, long long E, long long M, int N) {
+    const double fN = (double)N;
+    const double e = __ddiv_rn((double)E, fN);
+    const double a = fabs(__ddiv_rn((double)M, fN));
+    const double a2 = __dmul_rn(a, a);
+    m.s_e = __dadd_rn(m.s_e, e);
+    m.s_e2 = __dadd_rn(m.s_e2, __dmul_rn(e, e));
+    m.s_am = __dadd_rn(m.s_am, a);
+    m.s_m2 = __dadd_rn(m.s_m2, a2);
+    m.s_m4 = __dadd_rn(m.s_m4, __dmul_rn(a2, a2));
+    m.n += 1;
+}
+
+// bit-plane layout shared by the bond planes and the decision plane D: bit (i & 31) of word (i >> 5)
 __device__ __forceinline__ uint32_t get_bit(const uint32_t* __restrict__ plane, int i) {
     return (plane[i >> 5] >> (i & 31)) & 1u;
 }

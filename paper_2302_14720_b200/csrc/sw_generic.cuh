@@ -180,12 +180,34 @@ k_observe_generic(const int8_t* __restrict__ spins, Rec* __restrict__ rec, const
 __global__ void k_set_ctl(Ctl* ctl, unsigned long long t, uint32_t slot, uint32_t cap) {
     ctl->t = t; ctl->slot = slot; ctl->cap = cap;
 }
-// end of a sweep: t += 1, move to the next series slot and zero it
-__global__ void k_advance(Ctl* ctl, Rec* rec, int nb) {
-    const uint32_t next = (ctl->slot + 1 == ctl->cap) ? 0u : ctl->slot + 1;
-    for (int b = threadIdx.x; b < nb; b += blockDim.x) rec[(size_t)next * nb + b] = Rec{0, 0, 0, 0};
+// end of a sweep: t += 1, move to the next series slot and zero it.  acc: which record feeds the running
+// moments -- 1: this sweep's (its E, M are complete), 2: the previous sweep's (scan path: E, M of a sweep
+// arrive with the next sweep's bond test), 0: none.  One thread per lattice: sweep order, fixed arithmetic.
+__global__ void k_advance(Ctl* ctl, Rec* rec, int nb, Mom* mom, int N, int acc) {
+    const uint32_t cur = ctl->slot;
+    const uint32_t next = (cur + 1 == ctl->cap) ? 0u : cur + 1;
+    const uint32_t from = acc == 2 ? (cur == 0 ? ctl->cap - 1 : cur - 1) : cur;
+    for (int b = threadIdx.x; b < nb; b += blockDim.x) {
+        if (acc) {
+            const Rec r = rec[(size_t)from * nb + b];
+            Mom m = mom[b];
+            mom_add(m, r.E, r.M, N);
+            mom[b] = m;
+        }
+        rec[(size_t)next * nb + b] = Rec{0, 0, 0, 0};
+    }
     __syncthreads();
     if (threadIdx.x == 0) { ctl->t += 1; ctl->slot = next; }
+}
+// scan path, end of a sw_sweep call (after k_observe_rows): the last sweep's record, now complete
+__global__ void k_moments_last(const Ctl* ctl, const Rec* rec, int nb, Mom* mom, int N) {
+    const uint32_t from = ctl->slot == 0 ? ctl->cap - 1 : ctl->slot - 1;
+    for (int b = threadIdx.x; b < nb; b += blockDim.x) {
+        const Rec r = rec[(size_t)from * nb + b];
+        Mom m = mom[b];
+        mom_add(m, r.E, r.M, N);
+        mom[b] = m;
+    }
 }
 
 // ---- test hook: Philox on the device ---------------------------------------------------------------

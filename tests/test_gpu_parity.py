@@ -332,3 +332,46 @@ def test_invariants_hold_at_size_without_the_oracle(B):
     o = sw.observables()[0]
     inv.check_sweep(L, before, bE, bS, sw.labels_host()[0], sw.spins_host()[0], _obs_tuple(o))
     sw.close()
+
+
+# ------------------------------------------------------------------------------------------------
+# moments accumulated on the device against oracle/moments.py on the oracle's series
+@pytest.mark.parametrize("L,path,T", [(64, 0, T_C), (256, 0, 2.0), (128, 0, 3.0), (20, 1, T_C), (256, 2, T_C), (256, 6, 2.5)])
+def test_moments_match_oracle(B, L, path, T):
+    from oracle import moments as om
+    seed, therm, n = 31 + L, 7, 40
+    N = L * L
+    sw = B.SwendsenWang(L, T, seed, path=path)
+    assert sw.moments()[0]["n"] == 0
+    sw.sweep(therm)
+    sw.moments_reset()                               # discard thermalisation
+    sw.sweep(25)                                     # several calls: the scan path closes each with its own pass
+    sw.sweep(1)
+    sw.sweep(n - 26)
+    got = sw.moments()[0]
+    _, ser = oracle.run(L, T, seed, therm + n)
+    ref = om.moments(ser[therm:, 0], ser[therm:, 1], N, T)
+    assert got["n"] == n
+    for k in ("e_mean", "e2_mean", "absm_mean", "m2_mean", "m4_mean"):
+        assert abs(got[k] - ref[k]) <= 1e-12 * max(1.0, abs(ref[k])), (k, got[k], ref[k])
+    # derived quantities subtract nearly equal means: same formula on the same doubles
+    for k in ("specific_heat", "susceptibility", "binder"):
+        assert abs(got[k] - ref[k]) <= 1e-12 * max(1.0, abs(ref[k])) * N, (k, got[k], ref[k])
+    sw.close()
+
+
+def test_moments_of_a_batch(B):
+    from oracle import moments as om
+    L, nb, n = 128, 3, 12
+    Ts = [2.0, T_C, 3.0]
+    seeds = [1000, 1001, 1002]
+    sw = B.SwendsenWang(L, Ts, seeds)
+    sw.sweep(n)
+    got = sw.moments()
+    for b in range(nb):
+        _, ser = oracle.run(L, Ts[b], seeds[b], n)
+        ref = om.moments(ser[:, 0], ser[:, 1], L * L, Ts[b])
+        assert got[b]["n"] == n
+        for k in ("e_mean", "absm_mean", "m2_mean"):
+            assert abs(got[b][k] - ref[k]) <= 1e-12 * max(1.0, abs(ref[k]))
+    sw.close()
