@@ -112,6 +112,11 @@ const int8_t* sw_spins(sw_handle* h);                      /* DEVICE ptr, nb*N i
  * ceil(N/32).  SW_ESTATE before the first sweep.  PAPER.md:39, Fig. 2. */
 int        sw_bonds(sw_handle* h, const uint32_t** bondE, const uint32_t** bondS);
 int        sw_set_eager_labels(sw_handle* h, int on);       /* default 0 */
+/* Default 1: on the fast path, sw_sweep(h, n >= 4) replays CUDA graphs of the steady sweep (the sweep index lives
+ * on the device, so every sweep but the first of a call launches the same kernels with the same arguments)
+ * on an internal stream ordered after / before the handle's stream by events.  0: plain launches.  Results are
+ * identical either way; graphs remove most of the launch overhead that dominates small lattices. */
+int        sw_set_graphs(sw_handle* h, int on);
 
 /* Replace the spins (cold start, injected states).  `spins`: nb*N int8 of +1/-1, on the device
  * (is_host = 0) or on the host (is_host = 1).  Values are not validated. */

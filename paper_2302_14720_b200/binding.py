@@ -76,6 +76,7 @@ PROTOTYPES = {
     "sw_kernel_name": (C.c_char_p, [_I32]),
     "sw_set_path": (C.c_int, [_VP, C.c_int]),
     "sw_set_eager_labels": (C.c_int, [_VP, C.c_int]),
+    "sw_set_graphs": (C.c_int, [_VP, C.c_int]),
     "sw_last_launch_count": (_I64, [_VP]),
     "sw_threshold": (_U32, [_VP, _I32]),
     "sw_L": (_I32, [_VP]),
@@ -197,6 +198,9 @@ def sw_moments(h) -> List[dict]:
 
 def sw_moments_reset(h) -> None:
     _check(lib().sw_moments_reset(_ptr(h)))
+
+def sw_set_graphs(h, on: bool) -> None:
+    _check(lib().sw_set_graphs(_ptr(h), 1 if on else 0))
 
 def sw_set_series_capacity(h, sweeps: int) -> None:
     _check(lib().sw_set_series_capacity(_ptr(h), sweeps))
@@ -331,6 +335,9 @@ class SwendsenWang:
 
     def series(self, cap=None):
         return sw_series(self.h, cap)
+
+    def set_graphs(self, on: bool):
+        sw_set_graphs(self.h, on)
 
     def moments(self):
         return sw_moments(self.h)

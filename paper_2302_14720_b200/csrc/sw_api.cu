@@ -146,6 +146,13 @@ struct sw_handle {
     int path = 0; TileKind tile = TILE_NONE;
     bool timing = false; std::vector<cudaEvent_t> ev; int64_t timed_sweeps = 0;
     cudaEvent_t ev_tail[2] = { nullptr, nullptr };   // around the trailing k_observe_rows of a call
+    // CUDA graphs of the steady sweep (every sweep of a call but the first launches the same kernels with the
+    // same arguments: the sweep index lives on the device).  Replayed on an internal stream ordered after /
+    // before the caller's stream by events, because the legacy default stream cannot be captured.
+    bool use_graphs = true, graph_failed = false;
+    cudaStream_t gstream = nullptr; cudaEvent_t gev[2] = { nullptr, nullptr };
+    cudaGraphExec_t gexec[2] = { nullptr, nullptr };  // GRAPH_UNROLL sweeps, 1 sweep
+    const void* gkey_series = nullptr; int gkey_path = -1, gkey_eager = -1; int64_t glaunches = 0;
     int ev_cursor = 0; std::vector<int> ev_seq;   // kernel ids in launch order within one sweep
     int64_t cur_sweep = 0;
     int64_t launches = 0;
@@ -494,16 +501,65 @@ void sw_destroy(sw_handle* h) {
     cudaStreamSynchronize(h->stream);
     for (cudaEvent_t e : h->ev) cudaEventDestroy(e);
     for (cudaEvent_t e : h->ev_tail) if (e) cudaEventDestroy(e);
+    for (cudaGraphExec_t g : h->gexec) if (g) cudaGraphExecDestroy(g);
+    for (cudaEvent_t e : h->gev) if (e) cudaEventDestroy(e);
+    if (h->gstream) cudaStreamDestroy(h->gstream);
     if (h->series_owned) cudaFree(h->series_owned);
     if (h->owns_ws) cudaFree(h->ws);
     (void)cudaGetLastError();
     delete h;
 }
 
+namespace {
+constexpr int GRAPH_UNROLL = 8;
+
+// (re)build the graphs of the steady sweep on h->gstream; on any failure the handle falls back to plain launches
+bool build_graphs(sw_handle* h) {
+    if (h->gexec[0] && h->gkey_series == h->series && h->gkey_path == h->path && h->gkey_eager == (int)h->eager_labels)
+        return true;
+    for (cudaGraphExec_t& g : h->gexec) if (g) { cudaGraphExecDestroy(g); g = nullptr; }
+    const int64_t keep = h->launches;
+    for (int v = 0; v < 2; ++v) {
+        const int reps = v == 0 ? GRAPH_UNROLL : 1;
+        cudaGraph_t graph = nullptr;
+        if (cudaStreamBeginCapture(h->gstream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) { (void)cudaGetLastError(); return false; }
+        h->launches = 0;
+        int rc = SW_OK;
+        for (int u = 0; u < reps && rc == SW_OK; ++u) rc = launch_sweep(h, 1);
+        const cudaError_t e = cudaStreamEndCapture(h->gstream, &graph);
+        if (rc != SW_OK || e != cudaSuccess || !graph) { (void)cudaGetLastError(); if (graph) cudaGraphDestroy(graph); h->launches = keep; return false; }
+        h->glaunches = h->launches / reps;
+        const cudaError_t ei = cudaGraphInstantiate(&h->gexec[v], graph, 0);
+        cudaGraphDestroy(graph);
+        if (ei != cudaSuccess) { (void)cudaGetLastError(); h->gexec[v] = nullptr; h->launches = keep; return false; }
+    }
+    h->launches = keep;
+    h->gkey_series = h->series; h->gkey_path = h->path; h->gkey_eager = (int)h->eager_labels;
+    return true;
+}
+} // namespace
+
 int sw_sweep(sw_handle* h, int64_t n) {
     if (!h || n < 0) { set_err("sw_sweep: invalid argument"); return SW_EINVAL; }
     if (n == 0) return SW_OK;
     h->launches = 0;
+    // graph replay: scan path, no per-kernel timing, enough sweeps to pay for the two stream hops
+    cudaStream_t const user = h->stream;
+    bool graphs = h->use_graphs && !h->graph_failed && !h->timing && scan_nw(h->tile) && n >= 4;
+    if (graphs) {
+        if (!h->gstream) {
+            if (cudaStreamCreateWithFlags(&h->gstream, cudaStreamNonBlocking) != cudaSuccess ||
+                cudaEventCreateWithFlags(&h->gev[0], cudaEventDisableTiming) != cudaSuccess ||
+                cudaEventCreateWithFlags(&h->gev[1], cudaEventDisableTiming) != cudaSuccess) {
+                (void)cudaGetLastError(); h->graph_failed = true; graphs = false;
+            }
+        }
+    }
+    if (graphs) {
+        SW_CUDA(cudaEventRecord(h->gev[0], user));
+        SW_CUDA(cudaStreamWaitEvent(h->gstream, h->gev[0], 0));
+        h->stream = h->gstream;                         // everything below runs on the internal stream
+    }
     if (h->timing) {
         for (int i = 0; i < 2; ++i)
             if (!h->ev_tail[i]) SW_CUDA(cudaEventCreate(&h->ev_tail[i]));
@@ -517,9 +573,25 @@ int sw_sweep(sw_handle* h, int64_t n) {
     SW_CUDA(cudaMemsetAsync(h->series, 0, (size_t)h->nb * sizeof(Rec), h->stream));
     k_set_ctl<<<1, 1, 0, h->stream>>>(h->ctl, (unsigned long long)h->t, 0u, (uint32_t)h->ring());
     h->launches += 1;
-    for (int64_t k = 0; k < n; ++k) {
+    {
+        int rc = launch_sweep(h, 0);                    // (also sets the kernels' attributes before any capture)
+        if (rc) { h->stream = user; return rc; }
+    }
+    int64_t k = 1;
+    if (graphs && !build_graphs(h)) { h->graph_failed = true; graphs = false; }
+    if (graphs) {
+        for (; k + GRAPH_UNROLL <= n; k += GRAPH_UNROLL) {
+            SW_CUDA(cudaGraphLaunch(h->gexec[0], h->stream));
+            h->launches += h->glaunches * GRAPH_UNROLL;
+        }
+        for (; k < n; ++k) {
+            SW_CUDA(cudaGraphLaunch(h->gexec[1], h->stream));
+            h->launches += h->glaunches;
+        }
+    }
+    for (; k < n; ++k) {
         int rc = launch_sweep(h, k);
-        if (rc) return rc;
+        if (rc) { h->stream = user; return rc; }
     }
     if (scan_nw(h->tile)) {                             // a7 of the configuration the call ends with
         if (h->timing) SW_CUDA(cudaEventRecord(h->ev_tail[0], h->stream));
@@ -528,6 +600,11 @@ int sw_sweep(sw_handle* h, int64_t n) {
         k_moments_last<<<1, 64, 0, h->stream>>>(h->ctl, h->series, h->nb, h->mom, h->N);
         if (h->timing) SW_CUDA(cudaEventRecord(h->ev_tail[1], h->stream));
         h->launches += 2;
+    }
+    if (h->stream != user) {                            // hand the result back to the caller's stream
+        SW_CUDA(cudaEventRecord(h->gev[1], h->stream));
+        h->stream = user;
+        SW_CUDA(cudaStreamWaitEvent(user, h->gev[1], 0));
     }
     SW_CUDA(cudaGetLastError());
     h->t += (uint64_t)n;
@@ -725,6 +802,12 @@ int sw_set_path(sw_handle* h, int path) {
     if (!h || path < 0 || path > 9) { set_err("sw_set_path: invalid argument"); return SW_EINVAL; }
     h->path = path;
     h->tile = pick_tile(h->L, path);
+    return SW_OK;
+}
+
+int sw_set_graphs(sw_handle* h, int on) {
+    if (!h) { set_err("sw_set_graphs: null handle"); return SW_EINVAL; }
+    h->use_graphs = on != 0;
     return SW_OK;
 }
 

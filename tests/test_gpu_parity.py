@@ -375,3 +375,24 @@ def test_moments_of_a_batch(B):
         for k in ("e_mean", "absm_mean", "m2_mean"):
             assert abs(got[b][k] - ref[k]) <= 1e-12 * max(1.0, abs(ref[k]))
     sw.close()
+
+
+# ------------------------------------------------------------------------------------------------
+# many sweeps in ONE call: the steady sweep is replayed from CUDA graphs (sw_set_graphs, default on)
+@pytest.mark.parametrize("L,path,n", [(128, 0, 37), (256, 0, 12), (256, 7, 21), (64, 0, 50), (512, 6, 9)])
+def test_many_sweeps_per_call_with_and_without_graphs(B, L, path, n):
+    T, seed = T_C, 77 + L
+    s_ref, ser_ref = oracle.run(L, T, seed, n)
+    for graphs in (True, False):
+        sw = B.SwendsenWang(L, T, seed, path=path)
+        sw.set_graphs(graphs)
+        sw.sweep(n)
+        assert np.array_equal(sw.series()[:, 0, :], ser_ref), f"series differ (graphs={graphs})"
+        assert np.array_equal(sw.spins_host()[0], s_ref)
+        assert _obs_tuple(sw.observables()[0]) == tuple(int(v) for v in ser_ref[-1])
+        # a second call continues the same Markov chain (graphs are reused)
+        sw.sweep(5)
+        s2, ser2 = oracle.run(L, T, seed, 5, spins=s_ref, t0=n)
+        assert np.array_equal(sw.series()[:, 0, :], ser2)
+        assert np.array_equal(sw.labels_host()[0], oracle.sweep(L, T, seed, n + 4, oracle.run(L, T, seed, 4, spins=s_ref, t0=n)[0])[3])
+        sw.close()
