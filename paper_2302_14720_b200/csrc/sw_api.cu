@@ -236,13 +236,13 @@ int launch_bond_label_scan(sw_handle* h, bool fused, bool obs_prev) {
     if (fused) {
         SW_MARK(h, K_BONDLABEL);
         k_bond_label<NW, TH, true><<<dim3(tiles, h->nb), NW * TH, smem, h->stream>>>(
-            h->spins, h->bondE, h->bondS, h->label, h->lab16, h->nodes, h->ocount, h->bslot,
+            h->spins, h->bondE, h->bondS, h->lab16, h->nodes, h->ocount, h->bslot,
             h->series, h->lat, h->ctl,
             h->L, h->N, h->words, h->nb, obs_prev ? 1 : 0);
     } else {
         SW_MARK(h, K_TILE);
         k_bond_label<NW, TH, false><<<dim3(tiles, h->nb), NW * TH, smem, h->stream>>>(
-            h->spins, h->bondE, h->bondS, h->label, h->lab16, h->nodes, h->ocount, h->bslot,
+            h->spins, h->bondE, h->bondS, h->lab16, h->nodes, h->ocount, h->bslot,
             h->series, h->lat, h->ctl,
             h->L, h->N, h->words, h->nb, obs_prev ? 1 : 0);
     }
@@ -259,13 +259,17 @@ int launch_bond_label_scan(sw_handle* h, bool fused, bool obs_prev) {
 // a4 for the scan path: open tile roots take their cluster's label, then two hops per site
 template <int NW, int TH>
 int launch_flatten_scan(sw_handle* h) {
-    constexpr int TW = 32 * NW, CAP = 2 * (TW + TH);
+    constexpr int TW = 32 * NW;
     const int tiles = h->N / (TW * TH);
-    k_apply_roots<CAP><<<grid1((size_t)tiles * 32, 256, h->nb), 256, 0, h->stream>>>(
-        h->label, h->nodes, h->ocount, tiles, h->N);
-    k_compress_tiled<<<grid1((size_t)h->N / 4, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
-        h->label, h->series, h->ctl, h->N, h->nb, 0);
-    h->launches += 2;
+    constexpr size_t smem = (size_t)TW * TH * sizeof(int);
+    static bool attr_done = false;
+    if (!attr_done) {
+        SW_CUDA(cudaFuncSetAttribute(k_labels16<NW, TH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr_done = true;
+    }
+    k_labels16<NW, TH><<<dim3(tiles, h->nb), NW * TH, smem, h->stream>>>(
+        h->label, h->lab16, h->nodes, h->ocount, make_div(h->L), h->L, h->N);
+    h->launches += 1;
     return SW_OK;
 }
 int flatten_scan(sw_handle* h) {

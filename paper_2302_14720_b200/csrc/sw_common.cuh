@@ -98,6 +98,12 @@ __device__ __forceinline__ int bfind_u32(uint32_t x) {
     int r; asm("bfind.u32 %0, %1;" : "=r"(r) : "r"(x)); return r;
 }
 
+// shared-memory add with no return value, predicated (no branch around it)
+__device__ __forceinline__ void red_shared_add_if(int* p, uint32_t v, bool c) {
+    asm volatile("{ .reg .pred q; setp.ne.u32 q, %2, 0; @q red.shared.add.u32 [%0], %1; }"
+                 :: "r"((uint32_t)__cvta_generic_to_shared(p)), "r"(v), "r"((uint32_t)c) : "memory");
+}
+
 // ------------------------------------------------------------------------------------------
 // memory helpers
 // ------------------------------------------------------------------------------------------

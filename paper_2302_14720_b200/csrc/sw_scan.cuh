@@ -58,7 +58,7 @@ __device__ __forceinline__ int div_l(int v, const DivL& D) {
 template <int NW, int TH, bool FUSE>
 __global__ void __launch_bounds__(NW * TH)
 k_bond_label(const int8_t* __restrict__ spins, uint32_t* bondE, uint32_t* bondS,
-             int* __restrict__ label, uint16_t* __restrict__ lab16, int4* __restrict__ nodes, int* __restrict__ ocount,
+             uint16_t* __restrict__ lab16, int4* __restrict__ nodes, int* __restrict__ ocount,
              uint16_t* __restrict__ bslot,
              Rec* __restrict__ rec, const Lat* __restrict__ lat, const Ctl* __restrict__ ctl,
              int L, int N, int words, int nb, int obs_prev) {
@@ -255,7 +255,6 @@ k_bond_label(const int8_t* __restrict__ spins, uint32_t* bondE, uint32_t* bondS,
     constexpr int QSTEPS = SITES / 4 / THREADS;                      // = 8
     constexpr int LOG_TW = 5 + (NW == 8 ? 3 : NW == 4 ? 2 : NW == 2 ? 1 : 0);
     static_assert((1 << LOG_TW) == TW, "tile width is a power of two");
-    int* glab = label + (size_t)blockIdx.y * N;
     const int tilebase = y0 * L + x0;
 #pragma unroll
     for (int k = 0; k < QSTEPS; ++k) {
@@ -265,27 +264,20 @@ k_bond_label(const int8_t* __restrict__ spins, uint32_t* bondE, uint32_t* bondS,
         // site -> its label node -> root (label nodes are flat; roots carry size / open bits)
         int r[4] = { par[v.x & IDX_MASK] & IDX_MASK, par[v.y & IDX_MASK] & IDX_MASK,
                      par[v.z & IDX_MASK] & IDX_MASK, par[v.w & IDX_MASK] & IDX_MASK };
-        int4 g;
-        g.x = tilebase + (r[0] >> LOG_TW) * L + (r[0] & (TW - 1));
-        g.y = tilebase + (r[1] >> LOG_TW) * L + (r[1] & (TW - 1));
-        g.z = tilebase + (r[2] >> LOG_TW) * L + (r[2] & (TW - 1));
-        g.w = tilebase + (r[3] >> LOG_TW) * L + (r[3] & (TW - 1));
+        // the tile-local 16-bit root of every site is all the sweep stores per site (2 B); the int32 labels
+        // of the C ABI are derived from it on demand (k_labels16)
         const size_t gsite = (size_t)(y0 + (l >> LOG_TW)) * L + x0 + (l & (TW - 1));
-        *reinterpret_cast<int4*>(glab + gsite) = g;
-        // the same roots as tile-local 16-bit indices: what the assignment kernel reads (2 B / site)
         *reinterpret_cast<uint2*>(lab16 + (size_t)blockIdx.y * N + gsite) =
             make_uint2((uint32_t)r[0] | ((uint32_t)r[1] << 16), (uint32_t)r[2] | ((uint32_t)r[3] << 16));
         // sizes: one shared atomic per group of equal neighbours in the quad
         uint32_t acc = 1u << CNT_SHIFT;
 #pragma unroll
         for (int u = 1; u < 4; ++u) {
-            if (r[u] != r[u - 1]) {
-                atomicAdd(reinterpret_cast<unsigned int*>(par + r[u - 1]), acc);
-                acc = 0;
-            }
-            acc += 1u << CNT_SHIFT;
+            const bool cut = r[u] != r[u - 1];
+            red_shared_add_if(par + r[u - 1], acc, cut);             // (predicated: no branch around the atomic)
+            acc = (cut ? 0u : acc) + (1u << CNT_SHIFT);
         }
-        atomicAdd(reinterpret_cast<unsigned int*>(par + r[3]), acc);
+        red_shared_add_if(par + r[3], acc, true);
     }
     __syncthreads();
 
@@ -443,19 +435,48 @@ k_roots_nodes(int4* nodes, const int* __restrict__ ocount, int tiles) {
     if (lane == 0 && hotacc) { atomicAdd(&nd[hot].y, hotacc); atomicMin(&nd[hot].z, hotmin); }
 }
 
-// a4 on demand (sw_labels): the label of an open tile root becomes its cluster's canonical label, so that
-// k_compress_tiled's two hops (site -> tile root -> cluster root) flatten the label array.
-template <int CAP>
-__global__ void __launch_bounds__(256)
-k_apply_roots(int* __restrict__ label, const int4* __restrict__ nodes, const int* __restrict__ ocount, int tiles, int N) {
-    const int tile = blockIdx.x * 8 + (threadIdx.x >> 5);
-    const int lane = threadIdx.x & 31;
-    if (tile >= tiles) return;
-    const int4* nd = nodes + (size_t)blockIdx.y * tiles * CAP;
-    const int n = ocount[(size_t)blockIdx.y * tiles + tile];
-    for (int e = lane; e < n; e += 32) {
-        const int4 me = nd[tile * CAP + e];
-        label[(size_t)blockIdx.y * N + me.w] = nd[me.x].z;
+// a4 on demand (sw_labels; every sweep with sw_set_eager_labels): flat int32 labels from the 16-bit tile-local
+// roots.  One CTA per tile: a table in shared memory holds, for every open tile root, its cluster's canonical
+// label (minimum site index under its root node); a closed tile root IS its cluster's label.  PAPER.md:51.
+template <int NW, int TH>
+__global__ void __launch_bounds__(NW * TH)
+k_labels16(int* __restrict__ label, const uint16_t* __restrict__ lab16, const int4* __restrict__ nodes,
+           const int* __restrict__ ocount, DivL dv, int L, int N) {
+    constexpr int TW = 32 * NW, SITES = TW * TH, THREADS = NW * TH, CAP = 2 * (TW + TH);
+    constexpr int LOG_TW = ilog2_c(TW);
+    extern __shared__ int tab[];                     // [SITES] canonical label of the open tile root with this local index, else -1
+    const int tid = threadIdx.x;
+    const int tilesX = L / TW;
+    const int ty = blockIdx.x / tilesX, tx = blockIdx.x - ty * tilesX;
+    const int y0 = ty * TH, x0 = tx * TW;
+    const int tilebase = y0 * L + x0;
+    for (int i = tid; i < SITES; i += THREADS) tab[i] = -1;
+    __syncthreads();
+    {
+        const size_t lb = (size_t)blockIdx.y * gridDim.x * CAP;
+        const int nodebase = blockIdx.x * CAP;
+        const int n = ocount[(size_t)blockIdx.y * gridDim.x + blockIdx.x];
+        for (int e = tid; e < n; e += THREADS) {
+            const int4 me = nodes[lb + nodebase + e];
+            const int R = me.x == nodebase + e ? me.z : nodes[lb + me.x].z;
+            const int delta = me.w - tilebase;
+            const int ry = div_l(delta, dv);
+            tab[ry * TW + (delta - ry * L)] = R;
+        }
+    }
+    __syncthreads();
+    for (int q = tid; q < SITES / 4; q += THREADS) {
+        const int l = 4 * q;
+        const size_t gsite = (size_t)(y0 + (l >> LOG_TW)) * L + x0 + (l & (TW - 1));
+        const uint2 w = *reinterpret_cast<const uint2*>(lab16 + (size_t)blockIdx.y * N + gsite);
+        const int r[4] = { (int)(w.x & 0xFFFFu), (int)(w.x >> 16), (int)(w.y & 0xFFFFu), (int)(w.y >> 16) };
+        int g[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int t = tab[r[u]];
+            g[u] = t >= 0 ? t : tilebase + (r[u] >> LOG_TW) * L + (r[u] & (TW - 1));
+        }
+        *reinterpret_cast<int4*>(label + (size_t)blockIdx.y * N + gsite) = make_int4(g[0], g[1], g[2], g[3]);
     }
 }
 
