@@ -99,9 +99,10 @@ __device__ __forceinline__ int bfind_u32(uint32_t x) {
 }
 
 // shared-memory add with no return value, predicated (no branch around it)
-__device__ __forceinline__ void red_shared_add_if(int* p, uint32_t v, bool c) {
+// (addr: address in the shared window, from __cvta_generic_to_shared)
+__device__ __forceinline__ void red_shared_add_if(uint32_t addr, uint32_t v, bool c) {
     asm volatile("{ .reg .pred q; setp.ne.u32 q, %2, 0; @q red.shared.add.u32 [%0], %1; }"
-                 :: "r"((uint32_t)__cvta_generic_to_shared(p)), "r"(v), "r"((uint32_t)c) : "memory");
+                 :: "r"(addr), "r"(v), "r"((uint32_t)c) : "memory");
 }
 
 // ------------------------------------------------------------------------------------------

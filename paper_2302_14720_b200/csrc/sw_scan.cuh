@@ -256,6 +256,7 @@ k_bond_label(const int8_t* __restrict__ spins, uint32_t* bondE, uint32_t* bondS,
     constexpr int LOG_TW = 5 + (NW == 8 ? 3 : NW == 4 ? 2 : NW == 2 ? 1 : 0);
     static_assert((1 << LOG_TW) == TW, "tile width is a power of two");
     const int tilebase = y0 * L + x0;
+    const uint32_t par_s = (uint32_t)__cvta_generic_to_shared(par);  // shared-window address of par[0]
 #pragma unroll
     for (int k = 0; k < QSTEPS; ++k) {
         const int q = k * THREADS + tid;
@@ -274,10 +275,10 @@ k_bond_label(const int8_t* __restrict__ spins, uint32_t* bondE, uint32_t* bondS,
 #pragma unroll
         for (int u = 1; u < 4; ++u) {
             const bool cut = r[u] != r[u - 1];
-            red_shared_add_if(par + r[u - 1], acc, cut);             // (predicated: no branch around the atomic)
+            red_shared_add_if(par_s + 4u * r[u - 1], acc, cut);      // (predicated: no branch around the atomic)
             acc = (cut ? 0u : acc) + (1u << CNT_SHIFT);
         }
-        red_shared_add_if(par + r[3], acc, true);
+        red_shared_add_if(par_s + 4u * r[3], acc, true);
     }
     __syncthreads();
 
