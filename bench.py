@@ -172,6 +172,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--L", type=int, default=16384)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-unfused", action="store_true", help="skip the short unfused (path 6) per-stage measurement")
     ap.add_argument("--ref-L", type=int, default=2048, help="sample lattice side for --impl reference")
     ap.add_argument("--cpu-sample-L", type=int, default=8192, help="sample side for the cpu_baseline leg")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -291,6 +292,26 @@ def main():
                for k, v in kms.items()}
     sweep_gbs = SWEEP_MODEL_BYTES_PER_SITE * N / (ms / K * 1e-3) / 1e9
 
+    # ---- the per-stage split with a stand-alone bond kernel (BASELINE config 3 asks for bond / label / flip):
+    # the same lattice on path 6 (k_bond_rows, then labelling from the bond planes), a few sweeps
+    unfused = None
+    if not args.no_unfused:
+        try:
+            sw6 = B.SwendsenWang(L, T, seed, device=str(dev), path=6)
+            sw6.sweep(W)
+            sw6.set_stage_timing(True)
+            K6 = min(K, 10)
+            sw6.sweep(K6)
+            st6 = sw6.stage_ms()
+            sw6.close()
+            unfused = {s_: {"ms": v / K6, "model_bytes_per_site": STAGE_MODEL[s_],
+                            "hbm_frac": (STAGE_MODEL[s_] * N / (v / K6 * 1e-3) / 1e9 / peak) if v > 0 else None}
+                       for s_, v in st6.items()}
+            unfused["note"] = ("stand-alone bond kernel: bound by the Philox4x32-10 integer work (>= 24 instructions per site), "
+                               "not by its 1.25 B/site")
+        except Exception as e:                       # never lose the headline line over the side measurement
+            unfused = {"error": str(e)}
+
     cpu = None
     if not args.no_cpu_baseline:
         Ls = min(args.cpu_sample_L, L)
@@ -316,7 +337,7 @@ def main():
         "roofline": roofline,
         "sweep_model": {"bytes_per_site": SWEEP_MODEL_BYTES_PER_SITE, "achieved_GBps": sweep_gbs,
                         "frac_of_peak": sweep_gbs / peak, "frac_of_8TBps_nominal": sweep_gbs / 8000.0},
-        "stages": stages, "kernels": kernels,
+        "stages": stages, "stages_unfused": unfused, "kernels": kernels,
         "cpu_baseline": cpu,
         "paper_context": "paper: 17x (SW) / 90x (Wolff) over serial, Haswell E5-2695 vs Tesla P100; "
                          "SW GPU rate 1.25e8 site-updates/s at L=4096 (PAPER.md:127,142)",
