@@ -1,24 +1,29 @@
-// sw_scan.cuh -- the fast path: fused bond formation + tile-local labelling by a warp scan-line,
-// and the fused assignment / energy kernel.  Lattice side a multiple of 64.
+// sw_scan.cuh -- the fast path (lattice side a multiple of 64; the default tile is 128 x 64).
 //
-// Stage map; one CTA per tile of TW x 32 sites, TW = 32 * NW, one warp per 32-column strip:
-//   a1+a2 k_bond_label<NW>
-//       phase 1  (FMA-pipe bound)  one thread per 32-site word: sign masks of the int8 spins, 16 Philox4x32-10
-//                calls, bond words to shared memory and to the canonical global bit-planes; the bonds that
-//                enter the tile from its North and West neighbours are recomputed (TW/2 + 32 extra calls)
-//       phase 2  (MIO-pipe bound)  scan-line labelling, lane = column, rows in sequence, uniform control flow:
+// Stage map; one CTA per tile of TW x TH sites, TW = 32 * NW, TH = 32 or 64; the tile is
+// NW x TH/32 blocks of 32 x 32 sites, one warp each; NW * TH threads = one thread per 32-site word.
+//   a1+a2 k_bond_label<NW, TH, FUSE>
+//       phase 1  thread per 32-site word: sign masks of the int8 spins, 16 Philox4x32-10 calls, bond words to
+//                shared memory and to the canonical global bit-planes; E, M of the previous sweep's
+//                configuration from the same equal-pair masks; the bonds that enter the tile from its North
+//                and West neighbours are recomputed (TW/2 + TH extra calls)
+//       phase 2  scan-line labelling, lane = column, the block's rows in sequence, uniform control flow:
 //                runs of East bonds from bit tricks on the row's bond word; a run takes the label of the
 //                first of its sites that has a South bond from the row above (one shuffle), or opens a new
-//                label (its head's index); other sites of the run whose upper neighbour carries a different
-//                root unite the two roots (atomicMin hooking, larger under smaller)
-//       phase 3  strip seams: one lane per row unites across each East bond that crosses a strip edge
-//       phase 4  flatten (root of every site), global label = global index of the tile-local root, cluster
-//                sizes counted into the spare bits of the root's parent word, open flags
-//       phase 5  closed clusters -> running maximum; open clusters -> the tile's list (root, size)
-//   a3    k_merge_tiled / k_roots_open (sw_tiled.cuh): global boundary merge on the int32 parent array
-//   a4-a6 k_flip16<NW>: one decision bit per tile root in shared memory, spins = lookup by 16-bit tile-local root
-//   a7    E, M of a configuration: by-product of the next sweep's bond test (k_bond_label), k_observe_rows at
-//         the end of a call; cluster count and largest cluster: k_bond_label + k_roots_open
+//                label (its head's index); other sites of the run whose upper label differs hook the larger
+//                under the smaller (atomicMin)
+//       phase 3  seams between blocks (East bonds across strips, South bonds across the band seam)
+//       phase 3b thread per word: the label nodes (heads of runs with no bond from above) point at their roots
+//       phase 4  open flags (border sites), then per site: root = par[par[site]], 16-bit tile-local root to
+//                global memory (2 B / site), cluster sizes into spare bits of the root's word
+//       phase 5  closed roots -> count, running maximum; open roots -> nodes (parent, size, min site, site)
+//       phase 6  per border site with a bond across the tile edge: the slot of its root
+//   a3    k_merge_nodes (union-find over the nodes of neighbouring tiles), k_roots_nodes (sizes and minimum
+//         site index of the clusters that span tiles)
+//   a4-a6 k_flip16<NW, TH>: one decision bit per tile root in shared memory, spins = lookup by 16-bit root;
+//         k_labels16<NW, TH>: flat int32 labels from the 16-bit roots, on demand (sw_labels)
+//   a7    E, M: by-product of the next sweep's bond test, k_observe_rows at the end of a call; cluster count
+//         and largest cluster: k_bond_label (closed) + k_flip16 (root nodes)
 #pragma once
 #include "sw_common.cuh"
 
