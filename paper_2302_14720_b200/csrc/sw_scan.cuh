@@ -232,15 +232,18 @@ k_bond_label(const int8_t* __restrict__ spins, uint32_t* bondE, uint32_t* bondS,
         up |= (up >> 8) & m;  m &= m >> 8;
         up |= (up >> 16) & m;
         uint32_t o = ~(ew << 1) & ~up;                               // heads of runs without an uplink
-        while (o) {
-            const int c = __ffs(o) - 1;
+        while (o) {                                                  // two label nodes per round: their loads overlap
+            const int c0 = __ffs(o) - 1;
             o &= o - 1;
-            const int node = mybase + c;
-            const int p = par[node];
-            if (p == node) { rootbits |= 1u << c; continue; }
-            int r = p, q = par[r];
-            while (q != r) { r = q; q = par[r]; }
-            if (r != p) par[node] = r;
+            const int c1 = o ? __ffs(o) - 1 : c0;
+            o &= o - 1;
+            const int n0 = mybase + c0, n1 = mybase + c1;
+            const int p0 = par[n0], p1 = par[n1];
+            int r0 = p0, r1 = p1;
+            int q0 = par[r0], q1 = par[r1];
+            while (q0 != r0 || q1 != r1) { r0 = q0; r1 = q1; q0 = par[r0]; q1 = par[r1]; }
+            if (p0 == n0) rootbits |= 1u << c0; else if (r0 != p0) par[n0] = r0;
+            if (p1 == n1) rootbits |= 1u << c1; else if (r1 != p1) par[n1] = r1;
         }
     }
     __syncthreads();
