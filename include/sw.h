@@ -172,8 +172,20 @@ const char* sw_kernel_name(int32_t i);
  *   2, 3  the first-generation tiled kernels (64 x 64 / 256 x 32 tiles, thread-per-site union-find), kept for A/B timing
  *   4, 5  scan-line path forced to 64- / 128-wide tiles
  *   6  as 0 but UNFUSED: stand-alone bond kernel, then labelling from the bond planes (per-stage timing of
- *      bond / label / flip, BASELINE config 3) */
+ *      bond / label / flip, BASELINE config 3)
+ *   7, 8, 9  scan-line path forced to 256 x 32, 256 x 64, 128 x 64 tiles
+ *   11 the paper's own labelling (section 2.3): the label-equivalence iteration scan -> collapse
+ *      -> relabel, repeated until a scan forms no reference, run to convergence by ONE cooperative kernel (in
+ *      place of the paper's dynamic-parallelism maintenance kernel); any L; kept for A/B timing
+ *      against the union-find paths.  Allocates nb*N*4 extra bytes with cudaMalloc on first use (freed by
+ *      sw_destroy). */
 int        sw_set_path(sw_handle* h, int path);
+
+/* Path 11 only: number of passes (scans, including the last one that formed no reference) the label-equivalence
+ * iteration of the last sweep / sw_test_label took -- a deterministic function of the bond graph (PAPER.md:53
+ * reports "5 or 6" for 512 x 512).  Synchronises.  SW_ESTATE on another path, before any labelling, or if the
+ * iteration did not converge within 1024 passes. */
+int        sw_label_passes(sw_handle* h, int32_t* passes);
 
 /* Number of kernel launches issued by the last sw_sweep call (for bench.py's gpu_launches). */
 int64_t    sw_last_launch_count(const sw_handle* h);

@@ -75,6 +75,7 @@ PROTOTYPES = {
     "sw_kernel_ms": (C.c_int, [_VP, C.POINTER(C.c_float), _I32]),
     "sw_kernel_name": (C.c_char_p, [_I32]),
     "sw_set_path": (C.c_int, [_VP, C.c_int]),
+    "sw_label_passes": (C.c_int, [_VP, C.POINTER(C.c_int32)]),
     "sw_set_eager_labels": (C.c_int, [_VP, C.c_int]),
     "sw_set_graphs": (C.c_int, [_VP, C.c_int]),
     "sw_last_launch_count": (_I64, [_VP]),
@@ -242,6 +243,11 @@ def sw_kernel_ms(h):
 def sw_set_path(h, path: int) -> None:
     _check(lib().sw_set_path(_ptr(h), path))
 
+def sw_label_passes(h) -> int:
+    out = C.c_int32(0)
+    _check(lib().sw_label_passes(_ptr(h), C.byref(out)))
+    return int(out.value)
+
 def sw_set_eager_labels(h, on: bool) -> None:
     _check(lib().sw_set_eager_labels(_ptr(h), 1 if on else 0))
 
@@ -376,6 +382,10 @@ class SwendsenWang:
 
     def threshold(self, b: int = 0) -> int:
         return sw_threshold(self.h, b)
+
+    def label_passes(self) -> int:
+        """Path 11: passes of the last label-equivalence iteration."""
+        return sw_label_passes(self.h)
 
     def launch_count(self) -> int:
         return sw_last_launch_count(self.h)

@@ -5,6 +5,7 @@
 #include "sw_generic.cuh"
 #include "sw_tiled.cuh"
 #include "sw_scan.cuh"
+#include "sw_equiv.cuh"
 
 #include <algorithm>
 #include <cmath>
@@ -130,6 +131,8 @@ struct sw_handle {
     uint16_t* lab16 = nullptr;       // tile-local root index of every site (scan path)
     int4* nodes = nullptr;           // union-find over open tile roots: (parent, size, min site, site)
     uint16_t* bslot = nullptr;       // per tile: slot of the root of each border site
+    int* eq_ref = nullptr; int* eq_flags = nullptr;   // path 11 (label equivalence): allocated on first use
+    bool eq_ran = false;
     Lat* lat = nullptr; Ctl* ctl = nullptr; Rec* rec_now = nullptr; Mom* mom = nullptr;
     std::vector<double> hT;          // temperatures (sw_moments: specific heat, susceptibility)
     Rec* series = nullptr; Rec* series_owned = nullptr;
@@ -169,6 +172,7 @@ TileKind pick_tile(int L, int path) {
     if (path == 7) return L % 256 == 0 ? SCAN_8 : TILE_NONE;
     if (path == 8) return L % 256 == 0 ? SCAN_8x64 : TILE_NONE;
     if (path == 9) return L % 128 == 0 ? SCAN_4x64 : TILE_NONE;
+    if (path == 11) return L % 64 == 0 ? TILE_64x64 : TILE_NONE;      // row kernels for bond / flip / energy; labels: sw_equiv.cuh
     if (L % 128 == 0) return SCAN_4x64;
     if (L % 64 == 0) return SCAN_2;
     return TILE_NONE;
@@ -315,6 +319,41 @@ int launch_label_generic(sw_handle* h) {
     return SW_OK;
 }
 
+// a2-a4 the paper's way: one cooperative kernel runs the label-equivalence passes to convergence
+int launch_label_equiv(sw_handle* h) {
+    static int max_blocks = 0;
+    if (!max_blocks) {
+        int dev = 0, sms = 0, per_sm = 0, coop = 0;
+        SW_CUDA(cudaGetDevice(&dev));
+        SW_CUDA(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev));
+        if (!coop) { set_err("path 11: the device does not support cooperative launches"); return SW_ECUDA; }
+        SW_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+        SW_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_label_equiv, EQ_THREADS, 0));
+        if (per_sm < 1) { set_err("path 11: k_label_equiv does not fit on an SM"); return SW_ECUDA; }
+        max_blocks = sms * per_sm;
+    }
+    if (!h->eq_ref) {
+        SW_CUDA(cudaMalloc(&h->eq_ref, (size_t)h->nb * h->N * sizeof(int)));
+        SW_CUDA(cudaMalloc(&h->eq_flags, (size_t)(EQ_MAX_PASSES + 1) * sizeof(int)));
+    }
+    SW_CUDA(cudaMemsetAsync(h->eq_flags, 0, (size_t)(EQ_MAX_PASSES + 1) * sizeof(int), h->stream));
+    const int blocks = std::max(1, std::min(max_blocks, (h->N + EQ_THREADS - 1) / EQ_THREADS));
+    DivL dv = make_div(h->L);
+    void* args[] = { &h->label, &h->eq_ref, &h->bondE, &h->bondS, &h->eq_flags, &dv, &h->L, &h->N, &h->words, &h->nb };
+    SW_MARK(h, K_TILE);
+    SW_CUDA(cudaLaunchCooperativeKernel((const void*)k_label_equiv, dim3(blocks), dim3(EQ_THREADS), args, 0, h->stream));
+    // cluster count and largest cluster from the flat labels (the generic path's kernels)
+    SW_MARK(h, K_COMPRESS);
+    k_compress_generic<<<grid1(h->N, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(
+        h->label, h->gsize, h->series, h->ctl, h->N, h->nb);
+    SW_MARK(h, K_SIZES);
+    k_maxsize_generic<<<grid1(h->N, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(
+        h->label, h->gsize, h->series, h->ctl, h->N, h->nb);
+    h->launches += 3;
+    h->eq_ran = true;
+    return SW_OK;
+}
+
 // labelling alone from the bond planes, leaving flat labels (the unfused order; sw_test_label)
 template <int NW, int TH>
 int launch_label_scan(sw_handle* h) {
@@ -325,6 +364,7 @@ int launch_label_scan(sw_handle* h) {
 }
 
 int launch_label(sw_handle* h) {
+    if (h->path == 11) return launch_label_equiv(h);
     switch (h->tile) {
         case SCAN_2:      return launch_label_scan<2, 32>(h);
         case SCAN_4:      return launch_label_scan<4, 32>(h);
@@ -509,6 +549,8 @@ void sw_destroy(sw_handle* h) {
     for (cudaEvent_t e : h->gev) if (e) cudaEventDestroy(e);
     if (h->gstream) cudaStreamDestroy(h->gstream);
     if (h->series_owned) cudaFree(h->series_owned);
+    if (h->eq_ref) cudaFree(h->eq_ref);
+    if (h->eq_flags) cudaFree(h->eq_flags);
     if (h->owns_ws) cudaFree(h->ws);
     (void)cudaGetLastError();
     delete h;
@@ -803,8 +845,9 @@ int sw_stage_ms(sw_handle* h, float out[4]) {
 }
 
 int sw_set_path(sw_handle* h, int path) {
-    if (!h || path < 0 || path > 9) { set_err("sw_set_path: invalid argument"); return SW_EINVAL; }
+    if (!h || path < 0 || path > 11 || path == 10) { set_err("sw_set_path: invalid argument"); return SW_EINVAL; }
     h->path = path;
+    h->eq_ran = false;
     h->tile = pick_tile(h->L, path);
     return SW_OK;
 }
@@ -839,6 +882,20 @@ int sw_test_philox(const uint32_t* ctr, const uint32_t* key, uint32_t* out, int6
     SW_CUDA(cudaGetLastError());
     SW_CUDA(cudaMemcpy(out, dout, (size_t)n * 16, cudaMemcpyDeviceToHost));
     cudaFree(dc); cudaFree(dk); cudaFree(dout);
+    return SW_OK;
+}
+
+int sw_label_passes(sw_handle* h, int32_t* passes) {
+    if (!h || !passes) { set_err("sw_label_passes: null argument"); return SW_EINVAL; }
+    if (h->path != 11 || !h->eq_ran) { set_err("sw_label_passes: no labelling has run on path 11 yet"); return SW_ESTATE; }
+    int tail[2] = { 0, 0 };
+    SW_CUDA(cudaMemcpyAsync(&tail[1], h->eq_flags + EQ_MAX_PASSES, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+    SW_CUDA(cudaStreamSynchronize(h->stream));
+    if (tail[1] < 1 || tail[1] > EQ_MAX_PASSES) { set_err("sw_label_passes: bad pass count %d", tail[1]); return SW_ESTATE; }
+    SW_CUDA(cudaMemcpyAsync(&tail[0], h->eq_flags + tail[1] - 1, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+    SW_CUDA(cudaStreamSynchronize(h->stream));
+    if (tail[0]) { set_err("sw_label_passes: no convergence within %d passes", EQ_MAX_PASSES); return SW_ESTATE; }
+    *passes = tail[1];
     return SW_OK;
 }
 

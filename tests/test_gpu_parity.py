@@ -396,3 +396,94 @@ def test_many_sweeps_per_call_with_and_without_graphs(B, L, path, n):
         assert np.array_equal(sw.series()[:, 0, :], ser2)
         assert np.array_equal(sw.labels_host()[0], oracle.sweep(L, T, seed, n + 4, oracle.run(L, T, seed, 4, spins=s_ref, t0=n)[0])[3])
         sw.close()
+
+
+# ------------------------------------------------------------------------------------------------
+# the paper's own labelling as path 11.  Labels are the same canonical
+# minimum-index labels (bit-exact with the definition), and the number of passes is a deterministic function of
+# the bond graph: it must equal the oracle's step-by-step statement of the iteration.
+from oracle import label_equivalence as le
+
+
+@pytest.mark.parametrize("L", [2, 3, 4, 13, 33, 64, 100, 128, 256])
+def test_label_equivalence_path_every_sweep(B, L):
+    for T, seed in ((2.0, 1), (T_C, 2), (3.0, 3)):
+        sw = B.SwendsenWang(L, T, seed + L, path=11)
+        s = oracle.init_random(L, seed + L)
+        for t in range(5):
+            s1, bE, bS, lab, obs = oracle.sweep(L, T, seed + L, t, s)
+            sw.sweep(1)
+            gE, gS = sw.bonds_host()
+            assert np.array_equal(gE[0], wl.pack_bits(bE)) and np.array_equal(gS[0], wl.pack_bits(bS))
+            assert np.array_equal(sw.labels_host()[0], lab), f"labels differ at sweep {t}"
+            assert np.array_equal(sw.spins_host()[0], s1), f"spins differ at sweep {t}"
+            assert _obs_tuple(sw.observables()[0]) == obs
+            assert sw.label_passes() == le.label_equivalence(L, bE, bS)[1], f"pass count differs at sweep {t}"
+            s = s1
+        sw.close()
+
+
+@pytest.mark.parametrize("L", [64, 100, 256, 512])
+def test_label_equivalence_on_injected_bond_graphs(B, L):
+    sw = B.SwendsenWang(L, 2.0, 1, path=11)
+    for name, (bE, bS) in _label_patterns(L):
+        got = B.sw_test_label(sw.h, wl.pack_bits(bE), wl.pack_bits(bS))
+        ref = oracle.labels(L, bE, bS)
+        assert np.array_equal(got, ref), f"{name}: {np.count_nonzero(got != ref)} labels differ"
+        assert sw.label_passes() == le.label_equivalence(L, bE, bS)[1], name
+    sw.close()
+
+
+def test_label_equivalence_pass_counts_worked_by_hand(B):
+    # the cases derived in tests/test_oracle_label_equivalence.py: no bonds 1, chain 2, U 3, hook 4
+    L = 8
+    sw = B.SwendsenWang(L, 2.0, 1, path=11)
+
+    def passes(bE, bS):
+        got = B.sw_test_label(sw.h, wl.pack_bits(bE), wl.pack_bits(bS))
+        assert np.array_equal(got, oracle.labels(L, bE, bS))
+        return sw.label_passes()
+
+    z = lambda: (np.zeros(L * L, dtype=np.uint8), np.zeros(L * L, dtype=np.uint8))
+    bE, bS = z()
+    assert passes(bE, bS) == 1
+    bE[0:4] = 1
+    assert passes(bE, bS) == 2
+    bE, bS = z()                                     # U: column 0 rows 0..5, row 5 columns 0..2, column 2 rows 0..5
+    for y in range(5):
+        bS[y * L] = 1; bS[y * L + 2] = 1
+    bE[5 * L] = 1; bE[5 * L + 1] = 1
+    assert passes(bE, bS) == 3
+    bE, bS = z()                                     # hook: ... column 2 rows 1..5, row 1 columns 2..4, column 4 rows 0..1
+    for y in range(5):
+        bS[y * L] = 1
+    bE[5 * L] = 1; bE[5 * L + 1] = 1
+    for y in range(1, 5):
+        bS[y * L + 2] = 1
+    bE[L + 2] = 1; bE[L + 3] = 1; bS[4] = 1
+    assert passes(bE, bS) == 4
+    sw.close()
+
+
+def test_label_equivalence_batch_and_errors(B):
+    L, Ts, seeds = 96, [1.5, T_C, 3.5], [11, 12, 13]
+    sw = B.SwendsenWang(L, Ts, seeds, path=11)
+    with pytest.raises(Exception):
+        sw.label_passes()                            # SW_ESTATE before any labelling
+    refs = [oracle.init_random(L, s) for s in seeds]
+    for t in range(4):
+        sw.sweep(1)
+        gs, gl, obs = sw.spins_host(), sw.labels_host(), sw.observables()
+        want = 0
+        for b in range(3):
+            s1, bE, bS, lab, o = oracle.sweep(L, Ts[b], seeds[b], t, refs[b])
+            assert np.array_equal(gl[b], lab) and np.array_equal(gs[b], s1) and _obs_tuple(obs[b]) == o
+            want = max(want, le.label_equivalence(L, bE, bS)[1])
+            refs[b] = s1
+        assert sw.label_passes() == want             # the lattices of a batch iterate together
+    sw.close()
+    sw = B.SwendsenWang(64, 2.0, 1)
+    sw.sweep(1)
+    with pytest.raises(Exception):
+        sw.label_passes()                            # not path 11
+    sw.close()
