@@ -312,6 +312,27 @@ def main():
         except Exception as e:                       # never lose the headline line over the side measurement
             unfused = {"error": str(e)}
 
+    # ---- A/B: the paper's own labelling (label equivalence) on the same lattice and sweeps
+    # (path 11: one cooperative kernel runs the passes to convergence)
+    equiv = None
+    if not args.no_unfused:
+        try:
+            sw11 = B.SwendsenWang(L, T, seed, device=str(dev), path=11)
+            sw11.sweep(W)
+            sw11.set_stage_timing(True)
+            K11 = min(K, 10)
+            sw11.sweep(K11)
+            st11, km11 = sw11.stage_ms(), sw11.kernel_ms()
+            passes = sw11.label_passes()
+            sw11.close()
+            equiv = {"label_ms": st11["label"] / K11, "k_label_equiv_ms": km11.get("tile_label", 0.0) / K11,
+                     "passes_last_sweep": passes, "sweeps": K11,
+                     "label_ms_union_find": stages["label"]["ms"],
+                     "note": "label stage of the paper's iteration (scan -> collapse -> relabel until no reference forms) "
+                             "vs the tile union-find path's bond_label + merge + roots (which also draws the bonds)"}
+        except Exception as e:
+            equiv = {"error": str(e)}
+
     cpu = None
     if not args.no_cpu_baseline:
         Ls = min(args.cpu_sample_L, L)
@@ -337,7 +358,7 @@ def main():
         "roofline": roofline,
         "sweep_model": {"bytes_per_site": SWEEP_MODEL_BYTES_PER_SITE, "achieved_GBps": sweep_gbs,
                         "frac_of_peak": sweep_gbs / peak, "frac_of_8TBps_nominal": sweep_gbs / 8000.0},
-        "stages": stages, "stages_unfused": unfused, "kernels": kernels,
+        "stages": stages, "stages_unfused": unfused, "label_equivalence": equiv, "kernels": kernels,
         "cpu_baseline": cpu,
         "paper_context": "paper: 17x (SW) / 90x (Wolff) over serial, Haswell E5-2695 vs Tesla P100; "
                          "SW GPU rate 1.25e8 site-updates/s at L=4096 (PAPER.md:127,142)",
