@@ -327,6 +327,7 @@ def main():
             sw11.close()
             equiv = {"label_ms": st11["label"] / K11, "k_label_equiv_ms": km11.get("tile_label", 0.0) / K11,
                      "passes_last_sweep": passes, "sweeps": K11,
+                     "kernels_ms": {k_: v_ / K11 for k_, v_ in km11.items() if v_ > 0},
                      "label_ms_union_find": stages["label"]["ms"],
                      "note": "label stage of the paper's iteration (scan -> collapse -> relabel until no reference forms) "
                              "vs the tile union-find path's bond_label + merge + roots (which also draws the bonds)"}

@@ -310,10 +310,11 @@ int launch_label_generic(sw_handle* h) {
     k_union_generic<<<grid1(h->N, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(
         h->label, h->bondE, h->bondS, h->L, h->N, h->words);
     SW_MARK(h, K_COMPRESS);
+    SW_CUDA(cudaMemsetAsync(h->gsize, 0, (size_t)h->nb * h->N * sizeof(int), h->stream));
     k_compress_generic<<<grid1(h->N, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(
         h->label, h->gsize, h->series, h->ctl, h->N, h->nb);
     SW_MARK(h, K_SIZES);
-    k_maxsize_generic<<<grid1(h->N, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(
+    k_maxsize_generic<<<grid1(h->N, MAXSIZE_SPAN, h->nb), GEN_THREADS, 0, h->stream>>>(
         h->label, h->gsize, h->series, h->ctl, h->N, h->nb);
     h->launches += 4;
     return SW_OK;
@@ -342,12 +343,13 @@ int launch_label_equiv(sw_handle* h) {
     void* args[] = { &h->label, &h->eq_ref, &h->bondE, &h->bondS, &h->eq_flags, &dv, &h->L, &h->N, &h->words, &h->nb };
     SW_MARK(h, K_TILE);
     SW_CUDA(cudaLaunchCooperativeKernel((const void*)k_label_equiv, dim3(blocks), dim3(EQ_THREADS), args, 0, h->stream));
-    // cluster count and largest cluster from the flat labels (the generic path's kernels)
+    // cluster count and largest cluster from the flat labels
     SW_MARK(h, K_COMPRESS);
-    k_compress_generic<<<grid1(h->N, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(
+    SW_CUDA(cudaMemsetAsync(h->gsize, 0, (size_t)h->nb * h->N * sizeof(int), h->stream));
+    k_count_flat<<<grid1(h->N, EQ_COUNT_SPAN, h->nb), EQ_THREADS, 0, h->stream>>>(
         h->label, h->gsize, h->series, h->ctl, h->N, h->nb);
     SW_MARK(h, K_SIZES);
-    k_maxsize_generic<<<grid1(h->N, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(
+    k_maxsize_generic<<<grid1(h->N, MAXSIZE_SPAN, h->nb), GEN_THREADS, 0, h->stream>>>(
         h->label, h->gsize, h->series, h->ctl, h->N, h->nb);
     h->launches += 3;
     h->eq_ran = true;
@@ -848,6 +850,8 @@ int sw_set_path(sw_handle* h, int path) {
     if (!h || path < 0 || path > 11 || path == 10) { set_err("sw_set_path: invalid argument"); return SW_EINVAL; }
     h->path = path;
     h->eq_ran = false;
+    // the tiled paths keep gsize zero between sweeps themselves; the generic / path-11 kernels leave sizes in it
+    SW_CUDA(cudaMemsetAsync(h->gsize, 0, (size_t)h->nb * h->N * sizeof(int), h->stream));
     h->tile = pick_tile(h->L, path);
     return SW_OK;
 }

@@ -27,7 +27,7 @@ k_label_equiv(int* label, int* ref, const uint32_t* __restrict__ bondE, const ui
               int* flags, DivL dv, int L, int N, int words, int nb) {
     cooperative_groups::grid_group grid = cooperative_groups::this_grid();
     const int stride = gridDim.x * EQ_THREADS;
-    const int i0 = blockIdx.x * EQ_THREADS + threadIdx.x;
+    const int i0 = blockIdx.x * EQ_THREADS + threadIdx.x, lane = threadIdx.x & 31;
 
     // "each site is labeled with a unique integer incrementing from zero"
     for (int b = 0; b < nb; ++b)
@@ -43,17 +43,28 @@ k_label_equiv(int* label, int* ref, const uint32_t* __restrict__ bondE, const ui
             int* rf = ref + (size_t)b * N;
             const uint32_t* E = bondE + (size_t)b * words;
             const uint32_t* S = bondS + (size_t)b * words;
-            for (int i = i0; i < N; i += stride) {
-                const int y = div_l(i, dv), x = i - y * L;
-                const int ie = x + 1 == L ? i - L + 1 : i + 1, is = y + 1 == L ? i - N + L : i + L;
-                const int iw = x ? i - 1 : i + L - 1,          in = y ? i - L : i + N - L;
-                const int l = lab[i];
-                int m = l;
-                if ((E[i >> 5] >> (i & 31)) & 1u)   m = min(m, lab[ie]);
-                if ((S[i >> 5] >> (i & 31)) & 1u)   m = min(m, lab[is]);
-                if ((E[iw >> 5] >> (iw & 31)) & 1u) m = min(m, lab[iw]);
-                if ((S[in >> 5] >> (in & 31)) & 1u) m = min(m, lab[in]);
-                if (m < l) { atomicMin(rf + l, m); formed = 1; }
+            for (int base = i0 - lane; base < N; base += stride) {   // whole warps stay together (aggregated atomics)
+                const int i = base + lane;
+                int l = 0, m = 0;
+                if (i < N) {
+                    const int y = div_l(i, dv), x = i - y * L;
+                    const int ie = x + 1 == L ? i - L + 1 : i + 1, is = y + 1 == L ? i - N + L : i + L;
+                    const int iw = x ? i - 1 : i + L - 1,          in = y ? i - L : i + N - L;
+                    l = lab[i];
+                    m = l;
+                    if ((E[i >> 5] >> (i & 31)) & 1u)   m = min(m, lab[ie]);
+                    if ((S[i >> 5] >> (i & 31)) & 1u)   m = min(m, lab[is]);
+                    if ((E[iw >> 5] >> (iw & 31)) & 1u) m = min(m, lab[iw]);
+                    if ((S[in >> 5] >> (in & 31)) & 1u) m = min(m, lab[in]);
+                }
+                const unsigned need = __ballot_sync(0xffffffffu, m < l);
+                if (m < l) {
+                    // lanes with the same label send one minimum (at T_c a third of all sites share one label)
+                    const unsigned grp = __match_any_sync(need, l);
+                    const int mn = __reduce_min_sync(grp, m);
+                    if (lane == __ffs(grp) - 1 && mn < ld_cg(rf + l)) atomicMin(rf + l, mn);
+                    formed = 1;
+                }
             }
         }
         formed = __syncthreads_or(formed);
@@ -89,6 +100,46 @@ k_label_equiv(int* label, int* ref, const uint32_t* __restrict__ bondE, const ui
         grid.sync();
     }
     if (blockIdx.x == 0 && threadIdx.x == 0) flags[EQ_MAX_PASSES] = pass;
+}
+
+// cluster count and sizes from FLAT labels (a7): no find, so no walk through the giant cluster's root.  A CTA
+// covers EQ_COUNT_SPAN sites; lanes of one cluster add their count once, into a small shared-memory table that
+// is flushed at the end (one global atomic per cluster and CTA: at T_c one cluster owns a third of all sites,
+// and its counter would otherwise take every warp's atomic).  k_maxsize_generic then takes the maximum and
+// clears gsize.
+constexpr int EQ_COUNT_SPAN = 16 * EQ_THREADS, EQ_SLOTS = 256;
+__global__ void __launch_bounds__(EQ_THREADS)
+k_count_flat(const int* __restrict__ label, int* __restrict__ gsize, Rec* __restrict__ rec, const Ctl* __restrict__ ctl,
+             int N, int nb) {
+    __shared__ int s_key[EQ_SLOTS], s_cnt[EQ_SLOTS];
+    for (int k = threadIdx.x; k < EQ_SLOTS; k += EQ_THREADS) { s_key[k] = -1; s_cnt[k] = 0; }
+    __syncthreads();
+    const int lane = threadIdx.x & 31;
+    int* gs = gsize + (size_t)blockIdx.y * N;
+    int nroot = 0;
+    const int first = blockIdx.x * EQ_COUNT_SPAN + threadIdx.x;
+#pragma unroll 4
+    for (int k = 0; k < EQ_COUNT_SPAN / EQ_THREADS; ++k) {
+        const int i = first + k * EQ_THREADS;
+        const unsigned act = __ballot_sync(0xffffffffu, i < N);
+        if (i < N) {
+            const int r = label[(size_t)blockIdx.y * N + i];
+            nroot += (r == i);
+            const unsigned grp = __match_any_sync(act, r);
+            if (lane == __ffs(grp) - 1) {
+                const int c = __popc(grp);
+                const int slot = (int)(((uint32_t)r * 2654435761u) >> 24) & (EQ_SLOTS - 1);
+                const int old = atomicCAS(&s_key[slot], -1, r);
+                if (old == -1 || old == r) atomicAdd(&s_cnt[slot], c);
+                else atomicAdd(gs + r, c);                          // slot taken by another cluster
+            }
+        }
+    }
+    __syncthreads();
+    for (int k = threadIdx.x; k < EQ_SLOTS; k += EQ_THREADS)
+        if (s_cnt[k]) atomicAdd(gs + s_key[k], s_cnt[k]);
+    nroot = warp_sum_i(nroot);
+    if (lane == 0 && nroot) atomic_add_ll(&rec[(size_t)ctl->slot * nb + blockIdx.y].ncl, nroot);
 }
 
 } // namespace sw

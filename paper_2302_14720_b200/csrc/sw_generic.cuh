@@ -92,31 +92,42 @@ k_compress_generic(int* label, int* __restrict__ gsize, Rec* __restrict__ rec, c
                    int N, int nb) {
     const int i = blockIdx.x * GEN_THREADS + threadIdx.x;
     int isroot = 0;
+    const unsigned act = __ballot_sync(0xffffffffu, i < N);
     if (i < N) {
         int* lab = label + (size_t)blockIdx.y * N;
         const int r = uf_find(lab, i);
         lab[i] = r;
         isroot = (r == i);
-        atomicAdd(gsize + (size_t)blockIdx.y * N + r, 1);
+        const unsigned grp = __match_any_sync(act, r);          // lanes of one cluster add their count once
+        if ((threadIdx.x & 31) == __ffs(grp) - 1) atomicAdd(gsize + (size_t)blockIdx.y * N + r, __popc(grp));
     }
     isroot = warp_sum_i(isroot);
     if ((threadIdx.x & 31) == 0 && isroot)
         atomic_add_ll(&rec[(size_t)ctl->slot * nb + blockIdx.y].ncl, isroot);
 }
 
-// largest cluster from gsize; leaves gsize zero for the next sweep
+// largest cluster from gsize (zeroed by a memset before the sizes are counted).  A CTA covers MAXSIZE_SPAN sites (several
+// independent loads per thread) and sends one maximum.
+constexpr int MAXSIZE_SPAN = 16 * GEN_THREADS;
 __global__ void __launch_bounds__(GEN_THREADS)
-k_maxsize_generic(const int* __restrict__ label, int* __restrict__ gsize, Rec* __restrict__ rec,
+k_maxsize_generic(const int* __restrict__ label, const int* __restrict__ gsize, Rec* __restrict__ rec,
                   const Ctl* __restrict__ ctl, int N, int nb) {
-    const int i = blockIdx.x * GEN_THREADS + threadIdx.x;
+    const int first = blockIdx.x * MAXSIZE_SPAN + threadIdx.x;
+    const int* lab = label + (size_t)blockIdx.y * N;
+    const int* gs = gsize + (size_t)blockIdx.y * N;
     int m = 0;
-    if (i < N && label[(size_t)blockIdx.y * N + i] == i) {
-        m = gsize[(size_t)blockIdx.y * N + i];
-        gsize[(size_t)blockIdx.y * N + i] = 0;
+#pragma unroll
+    for (int k = 0; k < MAXSIZE_SPAN / GEN_THREADS; ++k) {
+        const int i = first + k * GEN_THREADS;
+        if (i < N && lab[i] == i) m = max(m, gs[i]);
     }
+    __shared__ int s_m;
+    if (threadIdx.x == 0) s_m = 0;
+    __syncthreads();
     m = warp_max_i(m);
-    if ((threadIdx.x & 31) == 0 && m)
-        atomic_max_ll(&rec[(size_t)ctl->slot * nb + blockIdx.y].maxcl, m);
+    if ((threadIdx.x & 31) == 0 && m) atomicMax(&s_m, m);
+    __syncthreads();
+    if (threadIdx.x == 0 && s_m) atomic_max_ll(&rec[(size_t)ctl->slot * nb + blockIdx.y].maxcl, s_m);
 }
 
 // ---- a5 flip-bit plane: D word w = Philox(ctr = (w>>2, t, TAG_FLIP))[w&3];
