@@ -241,3 +241,117 @@ int orc_run(int32_t L, double T, uint64_t seed, uint64_t t0, int64_t n,
     free(bE); free(bS); free(lab);
     return rc;
 }
+
+/* ==========================================================================
+ * q-state Potts model, SURVEY.md 8(f) NEXT-3.  PAPER.md:33: "The approach can
+ * be generalized to other discrete spin systems" (and section 6).
+ * The paper gives no formulas for it; the readings are the textbook ones
+ * (Swendsen & Wang's algorithm was stated for the Potts model), DESIGN.md 7d:
+ *   - colours c_i in {0 .. q-1}, H = -J sum_<ij> delta(c_i, c_j), J = 1;
+ *   - bond between equal colours with p = 1 - exp(-J/T) (for q = 2 this is the
+ *     Ising rule at T_Ising = 2 T); same draws as orc_bonds (the rule there
+ *     is "equal values AND word < thr", so orc_bonds serves unchanged);
+ *   - clusters and labels as before (orc_labels);
+ *   - every cluster is assigned a colour uniform in {0 .. q-1}:
+ *       colour = floor(word * q / 2^32), word = 32-bit field `idx` of the
+ *       generator (call idx >> 2, word idx & 3), idx = the cluster's label;
+ *       start configuration: the same with TAG_INIT, t = 0, idx = site;
+ *   - observables: E = -#(equal East / South pairs), M = q max_c n_c - N
+ *     (n_c = sites of colour c; M / ((q-1) N) is the usual order parameter;
+ *     q = 2: M = |n_0 - n_1|), cluster count, largest cluster.
+ * Pins (tests/test_oracle_potts.py): exact enumeration of all 3^9 states of
+ * the 3x3 three-state lattice and of the 2^16 states of the 4x4 two-state one
+ * (= the Ising table at T_Ising = 2 T), the exact critical energy
+ * -(1 + 1/sqrt q) per site at T_c = 1/ln(1 + sqrt q), invariants.
+ * ========================================================================== */
+uint32_t orc_potts_threshold(double T)
+{
+    double p = -expm1(-1.0 / T);
+    double v = floor(p * 4294967296.0);
+    if (v >= 4294967295.0) return 0xFFFFFFFFu;
+    if (v <= 0.0) return 0u;
+    return (uint32_t)v;
+}
+
+int orc_potts_colour(uint64_t seed, uint64_t t, uint32_t tag, int64_t idx, int32_t q)
+{
+    uint32_t w[4];
+    orc_draw(seed, t, tag, (uint32_t)(idx >> 2), w);
+    return (int)(((uint64_t)w[idx & 3] * (uint64_t)(uint32_t)q) >> 32);
+}
+
+void orc_potts_init_random(int32_t L, int32_t q, uint64_t seed, int8_t *colours)
+{
+    int64_t N = (int64_t)L * L;
+    for (int64_t i = 0; i < N; ++i)
+        colours[i] = (int8_t)orc_potts_colour(seed, 0, ORC_TAG_INIT, i, q);
+}
+
+void orc_potts_assign(int32_t L, int32_t q, uint64_t seed, uint64_t t,
+                      const int32_t *label, int8_t *colours)
+{
+    int64_t N = (int64_t)L * L;
+    for (int64_t i = 0; i < N; ++i)
+        colours[i] = (int8_t)orc_potts_colour(seed, t, ORC_TAG_FLIP, (int64_t)label[i], q);
+}
+
+/* out = {E, M, ncl, maxcl}; counts (may be NULL) gets n_0 .. n_{q-1} */
+int orc_potts_observables(int32_t L, int32_t q, const int8_t *colours,
+                          const int32_t *label, int64_t out[4], int64_t *counts)
+{
+    int64_t N = (int64_t)L * L;
+    int64_t E = 0, ncl = 0, maxcl = 0, nmax = 0;
+    int64_t n[128];
+    if (q < 2 || q > 127) return -2;
+    for (int c = 0; c < q; ++c) n[c] = 0;
+    for (int64_t i = 0; i < N; ++i) {
+        if (colours[i] == colours[east_of(L, i)]) E -= 1;
+        if (colours[i] == colours[south_of(L, i)]) E -= 1;
+        n[colours[i]] += 1;
+    }
+    for (int c = 0; c < q; ++c) {
+        if (n[c] > nmax) nmax = n[c];
+        if (counts) counts[c] = n[c];
+    }
+    if (label) {
+        int64_t *size = (int64_t *)calloc((size_t)N, sizeof(int64_t));
+        if (!size) return -1;
+        for (int64_t i = 0; i < N; ++i) {
+            if (label[i] == (int32_t)i) ++ncl;
+            size[label[i]] += 1;
+        }
+        for (int64_t i = 0; i < N; ++i)
+            if (size[i] > maxcl) maxcl = size[i];
+        free(size);
+    }
+    out[0] = E; out[1] = (int64_t)q * nmax - N; out[2] = ncl; out[3] = maxcl;
+    return 0;
+}
+
+int orc_potts_sweep(int32_t L, int32_t q, uint32_t thr, uint64_t seed, uint64_t t,
+                    int8_t *colours, uint8_t *bondE, uint8_t *bondS, int32_t *label,
+                    int64_t obs[4])
+{
+    orc_bonds(L, thr, seed, t, colours, bondE, bondS);
+    if (orc_labels(L, bondE, bondS, label) != 0) return -1;
+    orc_potts_assign(L, q, seed, t, label, colours);
+    if (obs) return orc_potts_observables(L, q, colours, label, obs, NULL);
+    return 0;
+}
+
+int orc_potts_run(int32_t L, int32_t q, double T, uint64_t seed, uint64_t t0, int64_t n,
+                  int8_t *colours, int64_t *series)
+{
+    int64_t N = (int64_t)L * L;
+    uint32_t thr = orc_potts_threshold(T);
+    uint8_t *bE = (uint8_t *)malloc((size_t)N);
+    uint8_t *bS = (uint8_t *)malloc((size_t)N);
+    int32_t *lab = (int32_t *)malloc((size_t)N * sizeof(int32_t));
+    int rc = 0;
+    if (!bE || !bS || !lab) rc = -1;
+    for (int64_t k = 0; rc == 0 && k < n; ++k)
+        rc = orc_potts_sweep(L, q, thr, seed, t0 + (uint64_t)k, colours, bE, bS, lab,
+                             series ? series + 4 * k : NULL);
+    free(bE); free(bS); free(lab);
+    return rc;
+}
