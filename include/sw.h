@@ -88,6 +88,24 @@ sw_handle* sw_create_in(void* workspace, uint64_t workspace_bytes,
 
 void       sw_destroy(sw_handle* h);                       /* NULL is a no-op */
 
+/* ---- q-state Potts model on the same sweep ----
+ * PAPER.md:33 ("The approach can be generalized to other discrete spin systems").  The paper gives no
+ * formulas; the textbook readings are taken: colours 0 .. q-1 in the int8 plane sw_spins returns,
+ * H = -sum_<ij> delta(c_i, c_j) with J = 1, a bond between EQUAL colours with p = 1 - exp(-1/T) (drawn exactly as for
+ * the Ising model: same Philox words, same East / South ownership), the same labelling, and every cluster assigned the
+ * colour floor(word * q / 2^32), word = 32-bit field `label` of the TAG_FLIP stream of the sweep (Philox call
+ * label >> 2, word label & 3); random start: the same with TAG_INIT, t = 0, field = site index.
+ * q in 2 .. 127.  A Potts handle answers every call of this header; differences: sw_obs.energy = -#(equal East /
+ * South pairs), sw_obs.magnetisation = q * max_c n_c - N (n_c = sites of colour c), abs_m_per_site =
+ * magnetisation / N; sw_set_cold sets colour 0; sw_set_spins takes colours; paths 0 / 1 (generic kernels, any L) and
+ * 11 only.  sw_create_potts allocates its own workspace; sw_create_potts_in takes one of sw_workspace_bytes(L, nb)
+ * bytes like sw_create_in (plus nb*q*4 bytes the library allocates itself for the colour counts).
+ * NULL + error text on invalid arguments (q outside 2 .. 127, and as for sw_create). */
+sw_handle* sw_create_potts(int32_t L, int32_t q, double T, uint64_t seed);
+sw_handle* sw_create_potts_in(void* workspace, uint64_t workspace_bytes, int32_t L, int32_t q, int32_t nb,
+                              const double* T, const uint64_t* seed);
+int32_t    sw_q(const sw_handle* h);                       /* 0 for an Ising handle */
+
 /* ---- the hot path ---- */
 
 /* n >= 0 full sweeps (bonds -> labels -> assignment -> observables) on the handle's stream;

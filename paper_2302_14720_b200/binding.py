@@ -76,6 +76,9 @@ PROTOTYPES = {
     "sw_kernel_name": (C.c_char_p, [_I32]),
     "sw_set_path": (C.c_int, [_VP, C.c_int]),
     "sw_label_passes": (C.c_int, [_VP, C.POINTER(C.c_int32)]),
+    "sw_create_potts": (_VP, [C.c_int32, C.c_int32, C.c_double, C.c_uint64]),
+    "sw_create_potts_in": (_VP, [_VP, C.c_uint64, C.c_int32, C.c_int32, C.c_int32, C.POINTER(C.c_double), C.POINTER(C.c_uint64)]),
+    "sw_q": (C.c_int32, [_VP]),
     "sw_set_eager_labels": (C.c_int, [_VP, C.c_int]),
     "sw_set_graphs": (C.c_int, [_VP, C.c_int]),
     "sw_last_launch_count": (_I64, [_VP]),
@@ -132,6 +135,23 @@ def sw_create(L: int, T: float, seed: int):
     if not h:
         raise SwError(SW_EINVAL, sw_last_error())
     return h
+
+def sw_create_potts(L: int, q: int, T: float, seed: int):
+    h = lib().sw_create_potts(L, q, float(T), seed)
+    if not h:
+        raise SwError(SW_EINVAL, sw_last_error())
+    return h
+
+def sw_create_potts_in(ws_ptr: int, ws_bytes: int, L: int, q: int, T: Sequence[float], seed: Sequence[int]):
+    nb = len(T)
+    Ta = (C.c_double * nb)(*[float(t) for t in T]); Sa = (C.c_uint64 * nb)(*[int(s) for s in seed])
+    h = lib().sw_create_potts_in(ws_ptr, ws_bytes, L, q, nb, Ta, Sa)
+    if not h:
+        raise SwError(SW_EINVAL, sw_last_error())
+    return h
+
+def sw_q(h) -> int:
+    return int(lib().sw_q(_ptr(h)))
 
 def sw_create_batch(L: int, T: Sequence[float], seed: Sequence[int]):
     nb = len(T)
@@ -276,7 +296,7 @@ def sw_test_label(h, bondE_words: np.ndarray, bondS_words: np.ndarray) -> np.nda
 class SwendsenWang:
     """One handle (nb >= 1 lattices) whose device buffers live in a torch uint8 workspace tensor."""
 
-    def __init__(self, L: int, T, seed, device: str = "cuda:0", path: int = 0):
+    def __init__(self, L: int, T, seed, device: str = "cuda:0", path: int = 0, q: int = 0):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2302_14720_b200 needs a CUDA device; there is no CPU fallback")
@@ -294,7 +314,11 @@ class SwendsenWang:
             self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
             base = self.workspace.data_ptr()
             self._ws_off = (-base) % 256
-            self.h = sw_create_in(base + self._ws_off, nbytes, self.L, self.T, self.seed)
+            self.q = int(q)                            # 0: Ising; >= 2: q-state Potts (colours 0 .. q-1)
+            if self.q:
+                self.h = sw_create_potts_in(base + self._ws_off, nbytes, self.L, self.q, self.T, self.seed)
+            else:
+                self.h = sw_create_in(base + self._ws_off, nbytes, self.L, self.T, self.seed)
             sw_set_stream(self.h, torch.cuda.current_stream(self.device).cuda_stream)
         if path:
             sw_set_path(self.h, path)

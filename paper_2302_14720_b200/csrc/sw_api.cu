@@ -6,6 +6,7 @@
 #include "sw_tiled.cuh"
 #include "sw_scan.cuh"
 #include "sw_equiv.cuh"
+#include "sw_potts.cuh"
 
 #include <algorithm>
 #include <cmath>
@@ -120,6 +121,15 @@ uint32_t host_threshold(double T) {
     return (uint32_t)v;
 }
 
+uint32_t host_threshold_potts(double T) {
+    // Potts: p = 1 - exp(-1/T) (H = -sum delta; for q = 2 the Ising rule at T_Ising = 2 T)
+    const double p = -std::expm1(-1.0 / T);
+    const double v = std::floor(p * 4294967296.0);
+    if (v >= 4294967295.0) return 0xFFFFFFFFu;
+    if (v <= 0.0) return 0u;
+    return (uint32_t)v;
+}
+
 } // namespace
 
 struct sw_handle {
@@ -131,6 +141,8 @@ struct sw_handle {
     uint16_t* lab16 = nullptr;       // tile-local root index of every site (scan path)
     int4* nodes = nullptr;           // union-find over open tile roots: (parent, size, min site, site)
     uint16_t* bslot = nullptr;       // per tile: slot of the root of each border site
+    int q = 0;                       // 0: Ising (spins +-1); >= 2: q-state Potts (colours 0 .. q-1), sw_potts.cuh
+    int* potts_cnt = nullptr;        // [nb][q] sites per colour (Potts observables)
     int* eq_ref = nullptr; int* eq_flags = nullptr;   // path 11 (label equivalence): allocated on first use
     bool eq_ran = false;
     Lat* lat = nullptr; Ctl* ctl = nullptr; Rec* rec_now = nullptr; Mom* mom = nullptr;
@@ -379,8 +391,34 @@ int launch_label(sw_handle* h) {
     }
 }
 
+// Potts sweep (sw_potts.cuh): bonds between equal colours, labels (generic union-find, or path 11), a colour per
+// cluster, observables
+int launch_sweep_potts(sw_handle* h, int64_t k) {
+    int rc;
+    h->cur_sweep = k; h->ev_cursor = 0;
+    h->labels_flat = true;
+    SW_MARK(h, K_BOND);
+    k_bond_generic<<<grid1(h->words, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(
+        h->spins, h->bondE, h->bondS, h->lat, h->ctl, h->L, h->N, h->words);
+    h->launches += 1;
+    if ((rc = launch_label(h))) return rc;
+    SW_MARK(h, K_FLIP);
+    k_assign_potts<<<grid1(h->N, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(
+        h->spins, h->label, h->lat, h->ctl, h->q, h->N);
+    SW_MARK(h, K_ENERGY);
+    k_observe_potts<<<grid1(h->N, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(
+        h->spins, h->series, h->potts_cnt, h->ctl, 1, h->q, h->L, h->N, h->nb);
+    k_potts_finish<<<1, 64, 0, h->stream>>>(h->series, h->potts_cnt, h->ctl, 1, h->q, h->N, h->nb);
+    SW_MARK(h, K_ADVANCE);
+    k_advance<<<1, 64, 0, h->stream>>>(h->ctl, h->series, h->nb, h->mom, h->N, 1);
+    h->launches += 4;
+    SW_MARK(h, K_COUNT);
+    return SW_OK;
+}
+
 // one full sweep on h->stream; the sweep index and series slot are read on the device from h->ctl
 int launch_sweep(sw_handle* h, int64_t k) {
+    if (h->q) return launch_sweep_potts(h, k);
     int rc;
     h->cur_sweep = k; h->ev_cursor = 0;
     if (const int nw = scan_nw(h->tile)) {
@@ -465,7 +503,7 @@ int init_handle(sw_handle* h, const double* T, const uint64_t* seed) {
     for (int b = 0; b < h->nb; ++b) {
         h->hlat[b].key0 = (uint32_t)(seed[b] & 0xFFFFFFFFu);
         h->hlat[b].key1 = (uint32_t)(seed[b] >> 32);
-        h->hlat[b].thr = host_threshold(T[b]);
+        h->hlat[b].thr = h->q ? host_threshold_potts(T[b]) : host_threshold(T[b]);
         h->hlat[b].pad = 0;
     }
     SW_CUDA(cudaMemcpyAsync(h->lat, h->hlat.data(), sizeof(Lat) * h->nb, cudaMemcpyHostToDevice, h->stream));
@@ -473,14 +511,21 @@ int init_handle(sw_handle* h, const double* T, const uint64_t* seed) {
     SW_CUDA(cudaMemsetAsync(h->series, 0, (size_t)h->ring() * h->nb * sizeof(Rec), h->stream));
     SW_CUDA(cudaMemsetAsync(h->mom, 0, (size_t)h->nb * sizeof(Mom), h->stream));
     k_set_ctl<<<1, 1, 0, h->stream>>>(h->ctl, 0ull, 0u, (uint32_t)h->ring());
-    k_init_random<<<grid1(h->words, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(h->spins, h->lat, h->N, h->words);
+    if (h->q) {
+        SW_CUDA(cudaMalloc(&h->potts_cnt, (size_t)h->nb * h->q * sizeof(int)));
+        SW_CUDA(cudaMemsetAsync(h->potts_cnt, 0, (size_t)h->nb * h->q * sizeof(int), h->stream));
+        k_init_potts<<<grid1(((size_t)h->N + 3) / 4, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(h->spins, h->lat, h->q, h->N);
+    } else {
+        k_init_random<<<grid1(h->words, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(h->spins, h->lat, h->N, h->words);
+    }
     SW_CUDA(cudaGetLastError());
     SW_CUDA(cudaStreamSynchronize(h->stream));       // hlat is read by the async copy
-    h->tile = pick_tile(h->L, h->path);
+    h->tile = h->q ? TILE_NONE : pick_tile(h->L, h->path);
     return SW_OK;
 }
 
-sw_handle* create_common(void* ws, uint64_t ws_bytes, int32_t L, int32_t nb, const double* T, const uint64_t* seed) {
+sw_handle* create_common(void* ws, uint64_t ws_bytes, int32_t L, int32_t nb, const double* T, const uint64_t* seed, int q = 0) {
+    if (q != 0 && (q < 2 || q > POTTS_MAX_Q)) { set_err("sw_create_potts: q = %d is not in 2 .. %d", q, POTTS_MAX_Q); return nullptr; }
     if (!valid_dims(L, nb) || !T || !seed) { set_err("sw_create: invalid argument (L=%d, nb=%d)", L, nb); return nullptr; }
     for (int b = 0; b < nb; ++b)
         if (!(T[b] > 0.0) || !std::isfinite(T[b])) { set_err("sw_create: T[%d] = %g is not a positive finite number", b, T[b]); return nullptr; }
@@ -493,7 +538,7 @@ sw_handle* create_common(void* ws, uint64_t ws_bytes, int32_t L, int32_t nb, con
     }
     sw_handle* h = new (std::nothrow) sw_handle();
     if (!h) { set_err("sw_create: out of host memory"); return nullptr; }
-    h->L = L; h->nb = nb; h->N = L * L; h->words = (h->N + 31) / 32;
+    h->L = L; h->nb = nb; h->N = L * L; h->words = (h->N + 31) / 32; h->q = q;
     const size_t need = make_layout(L, nb).total;
     if (ws) {
         if (ws_bytes < need || ((uintptr_t)ws % ALIGN) != 0) {
@@ -508,7 +553,7 @@ sw_handle* create_common(void* ws, uint64_t ws_bytes, int32_t L, int32_t nb, con
         if (e != cudaSuccess) { set_err("sw_create: cudaMalloc(%zu) failed: %s", need, cudaGetErrorString(e)); (void)cudaGetLastError(); delete h; return nullptr; }
         h->ws = (char*)p; h->ws_bytes = need; h->owns_ws = true;
     }
-    if (init_handle(h, T, seed) != SW_OK) { if (h->owns_ws) cudaFree(h->ws); delete h; return nullptr; }
+    if (init_handle(h, T, seed) != SW_OK) { if (h->potts_cnt) cudaFree(h->potts_cnt); if (h->owns_ws) cudaFree(h->ws); delete h; return nullptr; }
     return h;
 }
 
@@ -536,6 +581,17 @@ sw_handle* sw_create(int32_t L, double T, uint64_t seed) { return create_common(
 sw_handle* sw_create_batch(int32_t L, int32_t nb, const double* T, const uint64_t* seed) {
     return create_common(nullptr, 0, L, nb, T, seed);
 }
+sw_handle* sw_create_potts(int32_t L, int32_t q, double T, uint64_t seed) {
+    if (q < 2) { set_err("sw_create_potts: q = %d is not in 2 .. %d", q, POTTS_MAX_Q); return nullptr; }
+    return create_common(nullptr, 0, L, 1, &T, &seed, q);
+}
+sw_handle* sw_create_potts_in(void* workspace, uint64_t workspace_bytes, int32_t L, int32_t q, int32_t nb,
+                              const double* T, const uint64_t* seed) {
+    if (!workspace) { set_err("sw_create_potts_in: null workspace"); return nullptr; }
+    if (q < 2) { set_err("sw_create_potts_in: q = %d is not in 2 .. %d", q, POTTS_MAX_Q); return nullptr; }
+    return create_common(workspace, workspace_bytes, L, nb, T, seed, q);
+}
+int32_t sw_q(const sw_handle* h) { return h ? h->q : 0; }
 sw_handle* sw_create_in(void* workspace, uint64_t workspace_bytes, int32_t L, int32_t nb,
                         const double* T, const uint64_t* seed) {
     if (!workspace) { set_err("sw_create_in: null workspace"); return nullptr; }
@@ -551,6 +607,7 @@ void sw_destroy(sw_handle* h) {
     for (cudaEvent_t e : h->gev) if (e) cudaEventDestroy(e);
     if (h->gstream) cudaStreamDestroy(h->gstream);
     if (h->series_owned) cudaFree(h->series_owned);
+    if (h->potts_cnt) cudaFree(h->potts_cnt);
     if (h->eq_ref) cudaFree(h->eq_ref);
     if (h->eq_flags) cudaFree(h->eq_flags);
     if (h->owns_ws) cudaFree(h->ws);
@@ -693,6 +750,11 @@ int sw_observables(sw_handle* h, sw_obs* out) {
                                 cudaMemcpyDeviceToHost, h->stream));
     } else {
         SW_CUDA(cudaMemsetAsync(h->rec_now, 0, sizeof(Rec) * h->nb, h->stream));
+        if (h->q) {
+            k_observe_potts<<<grid1(h->N, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(
+                h->spins, h->rec_now, h->potts_cnt, h->ctl, 0, h->q, h->L, h->N, h->nb);
+            k_potts_finish<<<1, 64, 0, h->stream>>>(h->rec_now, h->potts_cnt, h->ctl, 0, h->q, h->N, h->nb);
+        } else
         k_observe_generic<<<grid1(h->N, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(
             h->spins, h->rec_now, h->ctl, 0, h->L, h->N, h->nb);
         SW_CUDA(cudaGetLastError());
@@ -771,7 +833,7 @@ int sw_set_spins(sw_handle* h, const int8_t* spins, int is_host) {
 int sw_set_cold(sw_handle* h) {
     if (!h) { set_err("sw_set_cold: null handle"); return SW_EINVAL; }
     const size_t n = (size_t)h->nb * h->N;
-    k_fill_i8<<<(unsigned)((n + GEN_THREADS - 1) / GEN_THREADS), GEN_THREADS, 0, h->stream>>>(h->spins, n, (int8_t)1);
+    k_fill_i8<<<(unsigned)((n + GEN_THREADS - 1) / GEN_THREADS), GEN_THREADS, 0, h->stream>>>(h->spins, n, (int8_t)(h->q ? 0 : 1));
     SW_CUDA(cudaGetLastError());
     h->have_sweep = false; h->rec_valid = false;
     return SW_OK;
@@ -848,11 +910,12 @@ int sw_stage_ms(sw_handle* h, float out[4]) {
 
 int sw_set_path(sw_handle* h, int path) {
     if (!h || path < 0 || path > 11 || path == 10) { set_err("sw_set_path: invalid argument"); return SW_EINVAL; }
+    if (h->q && path != 0 && path != 1 && path != 11) { set_err("sw_set_path: a Potts handle runs on paths 0 / 1 (generic) and 11 only"); return SW_EINVAL; }
     h->path = path;
     h->eq_ran = false;
     // the tiled paths keep gsize zero between sweeps themselves; the generic / path-11 kernels leave sizes in it
     SW_CUDA(cudaMemsetAsync(h->gsize, 0, (size_t)h->nb * h->N * sizeof(int), h->stream));
-    h->tile = pick_tile(h->L, path);
+    h->tile = h->q ? TILE_NONE : pick_tile(h->L, path);
     return SW_OK;
 }
 

@@ -487,3 +487,87 @@ def test_label_equivalence_batch_and_errors(B):
     with pytest.raises(Exception):
         sw.label_passes()                            # not path 11
     sw.close()
+
+
+# ------------------------------------------------------------------------------------------------
+# q-state Potts model on the same sweep.  Bit-exact with oracle/potts.py:
+# colours, both bond planes, labels and the integer observables after every sweep.
+from oracle import potts as opotts
+
+
+def _compare_potts(B, L, q, T, seed, n, path=0, start=None, t0=0):
+    sw = B.SwendsenWang(L, T, seed, path=path, q=q)
+    assert B.sw_q(sw.h) == q
+    N = L * L
+    if start is None:
+        s = opotts.init_random(L, q, seed)
+        assert np.array_equal(sw.spins_host()[0], s), "random start differs"
+    else:
+        s = np.asarray(start, dtype=np.int8)
+        sw.set_spins(s)
+    if t0:
+        sw.set_sweep_index(t0)
+    assert sw.threshold() == opotts.threshold(T)
+    o0 = sw.observables()[0]                         # before any sweep: E, M of the start, no clusters
+    want0, _ = opotts.observables(L, q, s)
+    assert (o0.energy, o0.magnetisation, o0.n_clusters, o0.largest_cluster) == (want0[0], want0[1], 0, 0)
+    for k in range(n):
+        t = t0 + k
+        s1, bE, bS, lab, obs = opotts.sweep(L, q, T, seed, t, s)
+        sw.sweep(1)
+        gE, gS = sw.bonds_host()
+        assert np.array_equal(gE[0], wl.pack_bits(bE)), f"bondE differs at sweep {t}"
+        assert np.array_equal(gS[0], wl.pack_bits(bS)), f"bondS differs at sweep {t}"
+        assert np.array_equal(sw.labels_host()[0], lab), f"labels differ at sweep {t}"
+        assert np.array_equal(sw.spins_host()[0], s1), f"colours differ at sweep {t}"
+        o = sw.observables()[0]
+        assert _obs_tuple(o) == obs, f"observables differ at sweep {t}: {_obs_tuple(o)} vs {obs}"
+        assert o.sweep == t + 1
+        assert abs(o.e_per_site - obs[0] / N) <= 1e-12 and abs(o.abs_m_per_site - obs[1] / N) <= 1e-12
+        s = s1
+    sw.close()
+
+
+@pytest.mark.parametrize("L,q", [(2, 2), (3, 3), (5, 4), (13, 3), (32, 5), (33, 7), (64, 3), (100, 127), (128, 2), (256, 3)])
+def test_potts_every_sweep(B, L, q):
+    tc = 1.0 / math.log(1.0 + math.sqrt(q))
+    for T, seed in ((0.7 * tc, 1), (tc, 2), (1.6 * tc, 3)):
+        _compare_potts(B, L, q, T, seed + L, 6)
+
+
+@pytest.mark.parametrize("L,q,path", [(64, 3, 11), (100, 4, 11), (96, 3, 1)])
+def test_potts_on_other_paths(B, L, q, path):
+    _compare_potts(B, L, q, 1.0 / math.log(1.0 + math.sqrt(q)), 77, 5, path=path)
+
+
+def test_potts_special_starts_limits_and_sweep_index(B):
+    L, q = 48, 3
+    one = np.zeros(L * L, dtype=np.int8)
+    stripes = (np.arange(L * L, dtype=np.int64) // L % q).astype(np.int8)
+    for s0 in (one, stripes):
+        for T in (1e-3, 0.995, 1e12):                # all bonds between equal colours / critical / none
+            _compare_potts(B, L, q, T, 9, 2, start=s0)
+    _compare_potts(B, L, q, 0.995, 5, 3, t0=(1 << 40) + 3)
+
+
+def test_potts_many_sweeps_per_call_series_and_batch(B):
+    L, q, Ts, seeds, n = 64, 3, [0.8, 0.995, 1.4], [21, 22, 23], 15
+    sw = B.SwendsenWang(L, Ts, seeds, q=q)
+    sw.sweep(n)
+    ser = sw.series()                                # (n, nb, 4)
+    got = sw.spins_host()
+    for b in range(3):
+        s, want = opotts.run(L, q, Ts[b], seeds[b], n)
+        assert np.array_equal(got[b], s)
+        assert np.array_equal(ser[:, b, :], want)
+    sw.close()
+
+
+def test_potts_argument_errors(B):
+    for q in (1, -3, 128):
+        with pytest.raises(Exception):
+            B.sw_create_potts(16, q, 1.0, 1)
+    h = B.sw_create_potts(16, 3, 1.0, 1)
+    with pytest.raises(Exception):
+        B.sw_set_path(h, 2)                          # tiled Ising kernels read sign bits
+    B.sw_destroy(h)
