@@ -190,6 +190,9 @@ TileKind pick_tile(int L, int path) {
     return TILE_NONE;
 }
 
+// Potts handles: the scan-line path on 128 x 64 tiles when L allows it (path 0), else the generic kernels
+TileKind potts_tile(int L, int path) { return (path == 0 && L % 128 == 0) ? SCAN_4x64 : TILE_NONE; }
+
 inline dim3 grid1(size_t n, int threads, int nb) { return dim3((unsigned)((n + threads - 1) / threads), (unsigned)nb); }
 
 // timing mode: an event before kernel `kid` of sweep h->cur_sweep (kid == K_COUNT closes the sweep)
@@ -396,11 +399,28 @@ int launch_label(sw_handle* h) {
 int launch_sweep_potts(sw_handle* h, int64_t k) {
     int rc;
     h->cur_sweep = k; h->ev_cursor = 0;
-    h->labels_flat = true;
     SW_MARK(h, K_BOND);
     k_bond_generic<<<grid1(h->words, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(
         h->spins, h->bondE, h->bondS, h->lat, h->ctl, h->L, h->N, h->words);
     h->launches += 1;
+    if (h->tile == SCAN_4x64) {
+        // fast path: scan-line tile labelling from the bond planes + node merge, colour per tile root
+        if ((rc = launch_bond_label_scan<4, 64>(h, false, false))) return rc;
+        SW_MARK(h, K_FLIPTILE);
+        k_assign16_potts<4, 64><<<dim3(h->N / (128 * 64), h->nb), 256, 0, h->stream>>>(
+            h->spins, h->lab16, h->nodes, h->ocount, h->series, h->lat, h->ctl, make_div(h->L), h->q, h->L, h->N, h->nb);
+        SW_MARK(h, K_ENERGY);
+        k_observe_potts_rows<<<grid1((size_t)h->N / 16, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(
+            h->spins, h->series, h->potts_cnt, h->ctl, 1, h->q, h->L, h->N, h->nb);
+        k_potts_finish<<<1, 64, 0, h->stream>>>(h->series, h->potts_cnt, h->ctl, 1, h->q, h->N, h->nb);
+        SW_MARK(h, K_ADVANCE);
+        k_advance<<<1, 64, 0, h->stream>>>(h->ctl, h->series, h->nb, h->mom, h->N, 1);
+        h->launches += 4;
+        SW_MARK(h, K_COUNT);
+        h->labels_flat = false;                      // int32 labels on demand (k_labels16)
+        return SW_OK;
+    }
+    h->labels_flat = true;
     if ((rc = launch_label(h))) return rc;
     SW_MARK(h, K_FLIP);
     k_assign_potts<<<grid1(h->N, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(
@@ -520,7 +540,7 @@ int init_handle(sw_handle* h, const double* T, const uint64_t* seed) {
     }
     SW_CUDA(cudaGetLastError());
     SW_CUDA(cudaStreamSynchronize(h->stream));       // hlat is read by the async copy
-    h->tile = h->q ? TILE_NONE : pick_tile(h->L, h->path);
+    h->tile = h->q ? potts_tile(h->L, h->path) : pick_tile(h->L, h->path);
     return SW_OK;
 }
 
@@ -650,7 +670,7 @@ int sw_sweep(sw_handle* h, int64_t n) {
     h->launches = 0;
     // graph replay: scan path, no per-kernel timing, enough sweeps to pay for the two stream hops
     cudaStream_t const user = h->stream;
-    bool graphs = h->use_graphs && !h->graph_failed && !h->timing && scan_nw(h->tile) && n >= 4;
+    bool graphs = h->use_graphs && !h->graph_failed && !h->timing && scan_nw(h->tile) && n >= 4 && !h->q;
     if (graphs) {
         if (!h->gstream) {
             if (cudaStreamCreateWithFlags(&h->gstream, cudaStreamNonBlocking) != cudaSuccess ||
@@ -698,7 +718,7 @@ int sw_sweep(sw_handle* h, int64_t n) {
         int rc = launch_sweep(h, k);
         if (rc) { h->stream = user; return rc; }
     }
-    if (scan_nw(h->tile)) {                             // a7 of the configuration the call ends with
+    if (scan_nw(h->tile) && !h->q) {                    // a7 of the configuration the call ends with
         if (h->timing) SW_CUDA(cudaEventRecord(h->ev_tail[0], h->stream));
         k_observe_rows<<<grid1(h->words, 256, h->nb), 256, 0, h->stream>>>(
             h->spins, h->series, h->ctl, h->L, h->N, h->words, h->nb);
@@ -888,7 +908,7 @@ int sw_kernel_ms(sw_handle* h, float* out, int32_t cap) {
             SW_CUDA(cudaEventElapsedTime(&ms, h->ev[(size_t)k * EV_PER_SWEEP + j], h->ev[(size_t)k * EV_PER_SWEEP + j + 1]));
             if (h->ev_seq[j] < cap) out[h->ev_seq[j]] += ms;
         }
-    if (scan_nw(h->tile) && K_ENERGY < cap) {           // the trailing observables pass of the call
+    if (scan_nw(h->tile) && !h->q && K_ENERGY < cap) {  // the trailing observables pass of the call
         float ms = 0.f;
         SW_CUDA(cudaEventElapsedTime(&ms, h->ev_tail[0], h->ev_tail[1]));
         out[K_ENERGY] += ms;
@@ -915,7 +935,7 @@ int sw_set_path(sw_handle* h, int path) {
     h->eq_ran = false;
     // the tiled paths keep gsize zero between sweeps themselves; the generic / path-11 kernels leave sizes in it
     SW_CUDA(cudaMemsetAsync(h->gsize, 0, (size_t)h->nb * h->N * sizeof(int), h->stream));
-    h->tile = h->q ? TILE_NONE : pick_tile(h->L, path);
+    h->tile = h->q ? potts_tile(h->L, path) : pick_tile(h->L, path);
     return SW_OK;
 }
 

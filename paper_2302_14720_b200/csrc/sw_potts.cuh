@@ -9,6 +9,7 @@
 #pragma once
 #include "sw_common.cuh"
 #include "sw_generic.cuh"
+#include "sw_scan.cuh"
 
 namespace sw {
 
@@ -70,6 +71,144 @@ k_observe_potts(const int8_t* __restrict__ colours, Rec* __restrict__ rec, int* 
         e = -(int)(v == s[y * L + (x + 1 == L ? 0 : x + 1)]) - (int)(v == s[(y + 1 == L ? 0 : y + 1) * L + x]);
         const unsigned grp = __match_any_sync(act, v);
         if ((threadIdx.x & 31) == __ffs(grp) - 1) atomicAdd(&s_cnt[v & POTTS_MAX_Q], __popc(grp));
+    }
+    e = warp_sum_i(e);
+    if ((threadIdx.x & 31) == 0 && e) atomicAdd(&s_e, e);
+    __syncthreads();
+    for (int c = threadIdx.x; c < q; c += GEN_THREADS)
+        if (s_cnt[c]) atomicAdd(cnt + (size_t)blockIdx.y * q + c, s_cnt[c]);
+    if (threadIdx.x == 0 && s_e) {
+        Rec* r = rec + (use_slot ? (size_t)ctl->slot * nb : 0) + blockIdx.y;
+        atomic_add_ll(&r->E, s_e);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// Fast path (L a multiple of 128): the scan-line labelling of sw_scan.cuh runs on the Potts bond planes
+// (k_bond_label<4, 64, FUSE = false>, k_merge_nodes, k_roots_nodes), leaving the 16-bit tile-local root of every
+// site and the node array of the open tile roots.  k_assign16_potts is the Potts counterpart of k_flip16: one
+// colour per TILE ROOT in shared memory (a Philox call per root: closed roots draw for their own site index, open
+// ones for the minimum site index under their root node), then every site looks its colour up by its 16-bit root.
+// Also counts the clusters that span tiles and maximises their sizes, as k_flip16 does.
+// ---------------------------------------------------------------------------------------------------
+template <int NW, int TH>
+__global__ void __launch_bounds__(NW * TH)
+k_assign16_potts(int8_t* __restrict__ colours, const uint16_t* __restrict__ lab16, const int4* __restrict__ nodes,
+                 const int* __restrict__ ocount, Rec* __restrict__ rec, const Lat* __restrict__ lat,
+                 const Ctl* __restrict__ ctl, DivL dv, int q, int L, int N, int nb) {
+    constexpr int TW = 32 * NW, SITES = TW * TH, THREADS = NW * TH;
+    constexpr int CAP = 2 * (TW + TH);
+    constexpr int OSTEPS = SITES / 8 / THREADS;      // = 4
+    constexpr int LOG_TW = ilog2_c(TW);
+    __shared__ uint8_t col[SITES];                   // colour of the tile root with local index l
+
+    const int tid = threadIdx.x;
+    const int tilesX = L / TW;
+    const int ty = blockIdx.x / tilesX, tx = blockIdx.x - ty * tilesX;
+    const int y0 = ty * TH, x0 = tx * TW;
+    const int tilebase = y0 * L + x0;
+    const size_t tile = (size_t)blockIdx.y * gridDim.x + blockIdx.x;
+
+    uint4 v[OSTEPS];
+#pragma unroll
+    for (int k = 0; k < OSTEPS; ++k) {
+        const int l = 8 * (k * THREADS + tid);
+        v[k] = ld_stream_u4(lab16 + (size_t)blockIdx.y * N + (size_t)(y0 + (l >> LOG_TW)) * L + x0 + (l & (TW - 1)));
+    }
+    const int n = ocount[tile];
+    const Lat la = lat[blockIdx.y];
+    const PhiloxKey key(la.key0, la.key1);
+    const unsigned long long t = ctl->t;
+    const uint32_t tlo = (uint32_t)t, thi = (uint32_t)(t >> 32);
+
+    // which of my 32 sites are tile roots (their 16-bit root is their own local index)
+    uint32_t rootmask = 0;
+#pragma unroll
+    for (int k = 0; k < OSTEPS; ++k) {
+        const int l = 8 * (k * THREADS + tid);
+        const uint32_t w4[4] = { v[k].x, v[k].y, v[k].z, v[k].w };
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            const uint32_t r = (u & 1) ? (w4[u >> 1] >> 16) : (w4[u >> 1] & 0xFFFFu);
+            rootmask |= (r == (uint32_t)(l + u) ? 1u : 0u) << (8 * k + u);
+        }
+    }
+    while (rootmask) {                               // one Philox call per tile root
+        const int b = __ffs(rootmask) - 1;
+        rootmask &= rootmask - 1;
+        const int l = 8 * ((b >> 3) * THREADS + tid) + (b & 7);
+        const int g = tilebase + (l >> LOG_TW) * L + (l & (TW - 1));
+        col[l] = (uint8_t)__umulhi(potts_word((uint32_t)g, tlo, thi, TAG_FLIP, key), (uint32_t)q);
+    }
+    __syncthreads();
+    {   // open tile roots take the colour of their cluster root = the minimum site index under their root node
+        const size_t lb = (size_t)blockIdx.y * gridDim.x * CAP;
+        const int nodebase = blockIdx.x * CAP;
+        int nroot = 0, big = 0;
+        for (int e = tid; e < n; e += THREADS) {
+            const int4 me = nodes[lb + nodebase + e];                  // (root node, size, min site, site of the tile root)
+            const int R = me.x == nodebase + e ? me.z : nodes[lb + me.x].z;
+            if (me.x == nodebase + e) { ++nroot; big = max(big, me.y); }
+            const int delta = me.w - tilebase;
+            const int ry = div_l(delta, dv);
+            col[ry * TW + (delta - ry * L)] = (uint8_t)__umulhi(potts_word((uint32_t)R, tlo, thi, TAG_FLIP, key), (uint32_t)q);
+        }
+        if (tid < ((n + 31) & ~31)) {                                  // (whole warps)
+            nroot = warp_sum_i(nroot); big = warp_max_i(big);
+            if ((tid & 31) == 0) {
+                Rec* r = rec + (size_t)ctl->slot * nb + blockIdx.y;
+                if (nroot) atomic_add_ll(&r->ncl, nroot);
+                if (big) atomic_max_ll(&r->maxcl, big);
+            }
+        }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < OSTEPS; ++k) {
+        const int l = 8 * (k * THREADS + tid);
+        const uint32_t w4[4] = { v[k].x, v[k].y, v[k].z, v[k].w };
+        uint32_t out[2] = { 0u, 0u };
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            const uint32_t r = (u & 1) ? (w4[u >> 1] >> 16) : (w4[u >> 1] & 0xFFFFu);
+            out[u >> 2] |= (uint32_t)col[r] << (8 * (u & 3));
+        }
+        *reinterpret_cast<uint2*>(colours + (size_t)blockIdx.y * N + (size_t)(y0 + (l >> LOG_TW)) * L + x0 + (l & (TW - 1))) =
+            make_uint2(out[0], out[1]);
+    }
+}
+
+// observables on rows (L a multiple of 16): 16 sites per thread, byte-wise compares (__vcmpeq4) with the East-
+// shifted and the South words; colour counts through a shared-memory histogram (lanes of one colour add once)
+__global__ void __launch_bounds__(GEN_THREADS)
+k_observe_potts_rows(const int8_t* __restrict__ colours, Rec* __restrict__ rec, int* __restrict__ cnt,
+                     const Ctl* __restrict__ ctl, int use_slot, int q, int L, int N, int nb) {
+    __shared__ int s_cnt[POTTS_MAX_Q + 1];
+    __shared__ int s_e;
+    for (int c = threadIdx.x; c <= POTTS_MAX_Q; c += GEN_THREADS) s_cnt[c] = 0;
+    if (threadIdx.x == 0) s_e = 0;
+    __syncthreads();
+    const int g = blockIdx.x * GEN_THREADS + threadIdx.x;              // group of 16 sites (N / 16 is a multiple of 32)
+    int e = 0;
+    if (g * 16 < N) {
+        const int8_t* s = colours + (size_t)blockIdx.y * N;
+        const int i = g * 16;
+        const int y = i / L, x = i - y * L;
+        const uint4 a = *reinterpret_cast<const uint4*>(s + i);
+        const uint4 b = *reinterpret_cast<const uint4*>(s + (size_t)(y + 1 == L ? 0 : y + 1) * L + x);
+        const uint32_t nx = (uint8_t)s[(size_t)y * L + (x + 16 == L ? 0 : x + 16)];
+        const uint32_t w[4] = { a.x, a.y, a.z, a.w }, so[4] = { b.x, b.y, b.z, b.w };
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const uint32_t east = __funnelshift_r(w[k], k < 3 ? w[k < 3 ? k + 1 : 3] : nx, 8);
+            e -= (__popc(__vcmpeq4(w[k], east)) + __popc(__vcmpeq4(w[k], so[k]))) >> 3;
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const int c = (w[k] >> (8 * u)) & POTTS_MAX_Q;
+                const unsigned grp = __match_any_sync(0xffffffffu, c);
+                if ((threadIdx.x & 31) == __ffs(grp) - 1) atomicAdd(&s_cnt[c], __popc(grp));
+            }
+        }
     }
     e = warp_sum_i(e);
     if ((threadIdx.x & 31) == 0 && e) atomicAdd(&s_e, e);

@@ -528,20 +528,22 @@ def _compare_potts(B, L, q, T, seed, n, path=0, start=None, t0=0):
     sw.close()
 
 
-@pytest.mark.parametrize("L,q", [(2, 2), (3, 3), (5, 4), (13, 3), (32, 5), (33, 7), (64, 3), (100, 127), (128, 2), (256, 3)])
+@pytest.mark.parametrize("L,q", [(2, 2), (3, 3), (5, 4), (13, 3), (32, 5), (33, 7), (64, 3), (100, 127), (128, 2), (256, 3),
+                                 (384, 5), (512, 127)])      # L % 128 == 0: scan-line tiles + k_assign16_potts
 def test_potts_every_sweep(B, L, q):
     tc = 1.0 / math.log(1.0 + math.sqrt(q))
     for T, seed in ((0.7 * tc, 1), (tc, 2), (1.6 * tc, 3)):
         _compare_potts(B, L, q, T, seed + L, 6)
 
 
-@pytest.mark.parametrize("L,q,path", [(64, 3, 11), (100, 4, 11), (96, 3, 1)])
+@pytest.mark.parametrize("L,q,path", [(64, 3, 11), (100, 4, 11), (96, 3, 1), (128, 4, 1), (128, 3, 11)])
 def test_potts_on_other_paths(B, L, q, path):
     _compare_potts(B, L, q, 1.0 / math.log(1.0 + math.sqrt(q)), 77, 5, path=path)
 
 
-def test_potts_special_starts_limits_and_sweep_index(B):
-    L, q = 48, 3
+@pytest.mark.parametrize("L", [48, 128])
+def test_potts_special_starts_limits_and_sweep_index(B, L):
+    q = 3
     one = np.zeros(L * L, dtype=np.int8)
     stripes = (np.arange(L * L, dtype=np.int64) // L % q).astype(np.int8)
     for s0 in (one, stripes):
@@ -551,16 +553,18 @@ def test_potts_special_starts_limits_and_sweep_index(B):
 
 
 def test_potts_many_sweeps_per_call_series_and_batch(B):
-    L, q, Ts, seeds, n = 64, 3, [0.8, 0.995, 1.4], [21, 22, 23], 15
-    sw = B.SwendsenWang(L, Ts, seeds, q=q)
-    sw.sweep(n)
-    ser = sw.series()                                # (n, nb, 4)
-    got = sw.spins_host()
-    for b in range(3):
-        s, want = opotts.run(L, q, Ts[b], seeds[b], n)
-        assert np.array_equal(got[b], s)
-        assert np.array_equal(ser[:, b, :], want)
-    sw.close()
+    for L in (64, 128):                              # generic kernels / scan-line tiles
+        q, Ts, seeds, n = 3, [0.8, 0.995, 1.4], [21, 22, 23], 15
+        sw = B.SwendsenWang(L, Ts, seeds, q=q)
+        sw.sweep(n)
+        ser = sw.series()                            # (n, nb, 4)
+        got, lab = sw.spins_host(), sw.labels_host()
+        for b in range(3):
+            s, want = opotts.run(L, q, Ts[b], seeds[b], n - 1)
+            s1, bE, bS, lab_b, o = opotts.sweep(L, q, Ts[b], seeds[b], n - 1, s)
+            assert np.array_equal(got[b], s1) and np.array_equal(lab[b], lab_b)
+            assert np.array_equal(ser[:n - 1, b, :], want) and tuple(ser[n - 1, b, :]) == o
+        sw.close()
 
 
 def test_potts_argument_errors(B):
