@@ -400,8 +400,12 @@ int launch_sweep_potts(sw_handle* h, int64_t k) {
     int rc;
     h->cur_sweep = k; h->ev_cursor = 0;
     SW_MARK(h, K_BOND);
-    k_bond_generic<<<grid1(h->words, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(
-        h->spins, h->bondE, h->bondS, h->lat, h->ctl, h->L, h->N, h->words);
+    if (h->tile == SCAN_4x64)
+        k_bond_rows_potts<<<grid1(h->words, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(
+            h->spins, h->bondE, h->bondS, h->lat, h->ctl, h->L, h->N, h->words);
+    else
+        k_bond_generic<<<grid1(h->words, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(
+            h->spins, h->bondE, h->bondS, h->lat, h->ctl, h->L, h->N, h->words);
     h->launches += 1;
     if (h->tile == SCAN_4x64) {
         // fast path: scan-line tile labelling from the bond planes + node merge, colour per tile root
