@@ -15,10 +15,26 @@ namespace sw {
 
 constexpr int POTTS_MAX_Q = 127;          // colours live in int8
 
+// Philox4x32-10 with the round keys advanced on the fly (2 registers instead of the 20 of PhiloxKey): for the
+// kernels here, which draw once per cluster or per site next to other register-hungry work
+__device__ __forceinline__ uint4 philox4x32_10_rk(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                                  uint32_t k0, uint32_t k1) {
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const unsigned long long p0 = (unsigned long long)PHILOX_M0 * c0;
+        const unsigned long long p1 = (unsigned long long)PHILOX_M1 * c2;
+        const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0;
+        const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1;
+        c1 = (uint32_t)p1; c3 = (uint32_t)p0; c0 = n0; c2 = n2;
+        k0 += PHILOX_W0; k1 += PHILOX_W1;
+    }
+    return make_uint4(c0, c1, c2, c3);
+}
+
 // 32-bit field idx of the (t, tag) stream: word idx & 3 of call idx >> 2
 __device__ __forceinline__ uint32_t potts_word(uint32_t idx, uint32_t tlo, uint32_t thi, uint32_t tag,
-                                               const PhiloxKey& key) {
-    const uint4 r = philox4x32_10(idx >> 2, tlo, thi, tag, key);
+                                               uint32_t key0, uint32_t key1) {
+    const uint4 r = philox4x32_10_rk(idx >> 2, tlo, thi, tag, key0, key1);
     const uint32_t s = idx & 3u;
     return s == 0 ? r.x : s == 1 ? r.y : s == 2 ? r.z : r.w;
 }
@@ -45,10 +61,9 @@ k_assign_potts(int8_t* __restrict__ colours, const int* __restrict__ label, cons
     const int i = blockIdx.x * GEN_THREADS + threadIdx.x;
     if (i >= N) return;
     const Lat la = lat[blockIdx.y];
-    const PhiloxKey key(la.key0, la.key1);
     const unsigned long long t = ctl->t;
     const int r = label[(size_t)blockIdx.y * N + i];
-    const uint32_t w = potts_word((uint32_t)r, (uint32_t)t, (uint32_t)(t >> 32), TAG_FLIP, key);
+    const uint32_t w = potts_word((uint32_t)r, (uint32_t)t, (uint32_t)(t >> 32), TAG_FLIP, la.key0, la.key1);
     colours[(size_t)blockIdx.y * N + i] = (int8_t)__umulhi(w, (uint32_t)q);
 }
 
@@ -124,7 +139,7 @@ k_bond_rows_potts(const int8_t* __restrict__ colours, uint32_t* __restrict__ bon
 // Also counts the clusters that span tiles and maximises their sizes, as k_flip16 does.
 // ---------------------------------------------------------------------------------------------------
 template <int NW, int TH>
-__global__ void __launch_bounds__(NW * TH)
+__global__ void __launch_bounds__(NW * TH, 1536 / (NW * TH))
 k_assign16_potts(int8_t* __restrict__ colours, const uint16_t* __restrict__ lab16, const int4* __restrict__ nodes,
                  const int* __restrict__ ocount, Rec* __restrict__ rec, const Lat* __restrict__ lat,
                  const Ctl* __restrict__ ctl, DivL dv, int q, int L, int N, int nb) {
@@ -133,6 +148,7 @@ k_assign16_potts(int8_t* __restrict__ colours, const uint16_t* __restrict__ lab1
     constexpr int OSTEPS = SITES / 8 / THREADS;      // = 4
     constexpr int LOG_TW = ilog2_c(TW);
     __shared__ uint8_t col[SITES];                   // colour of the tile root with local index l
+    __shared__ uint4 sv[SITES / 8];                  // my sites' 16-bit roots, parked while the colours are drawn
 
     const int tid = threadIdx.x;
     const int tilesX = L / TW;
@@ -149,7 +165,6 @@ k_assign16_potts(int8_t* __restrict__ colours, const uint16_t* __restrict__ lab1
     }
     const int n = ocount[tile];
     const Lat la = lat[blockIdx.y];
-    const PhiloxKey key(la.key0, la.key1);
     const unsigned long long t = ctl->t;
     const uint32_t tlo = (uint32_t)t, thi = (uint32_t)(t >> 32);
 
@@ -164,13 +179,14 @@ k_assign16_potts(int8_t* __restrict__ colours, const uint16_t* __restrict__ lab1
             const uint32_t r = (u & 1) ? (w4[u >> 1] >> 16) : (w4[u >> 1] & 0xFFFFu);
             rootmask |= (r == (uint32_t)(l + u) ? 1u : 0u) << (8 * k + u);
         }
+        sv[k * THREADS + tid] = v[k];
     }
     while (rootmask) {                               // one Philox call per tile root
         const int b = __ffs(rootmask) - 1;
         rootmask &= rootmask - 1;
         const int l = 8 * ((b >> 3) * THREADS + tid) + (b & 7);
         const int g = tilebase + (l >> LOG_TW) * L + (l & (TW - 1));
-        col[l] = (uint8_t)__umulhi(potts_word((uint32_t)g, tlo, thi, TAG_FLIP, key), (uint32_t)q);
+        col[l] = (uint8_t)__umulhi(potts_word((uint32_t)g, tlo, thi, TAG_FLIP, la.key0, la.key1), (uint32_t)q);
     }
     __syncthreads();
     {   // open tile roots take the colour of their cluster root = the minimum site index under their root node
@@ -183,7 +199,7 @@ k_assign16_potts(int8_t* __restrict__ colours, const uint16_t* __restrict__ lab1
             if (me.x == nodebase + e) { ++nroot; big = max(big, me.y); }
             const int delta = me.w - tilebase;
             const int ry = div_l(delta, dv);
-            col[ry * TW + (delta - ry * L)] = (uint8_t)__umulhi(potts_word((uint32_t)R, tlo, thi, TAG_FLIP, key), (uint32_t)q);
+            col[ry * TW + (delta - ry * L)] = (uint8_t)__umulhi(potts_word((uint32_t)R, tlo, thi, TAG_FLIP, la.key0, la.key1), (uint32_t)q);
         }
         if (tid < ((n + 31) & ~31)) {                                  // (whole warps)
             nroot = warp_sum_i(nroot); big = warp_max_i(big);
@@ -198,7 +214,8 @@ k_assign16_potts(int8_t* __restrict__ colours, const uint16_t* __restrict__ lab1
 #pragma unroll
     for (int k = 0; k < OSTEPS; ++k) {
         const int l = 8 * (k * THREADS + tid);
-        const uint32_t w4[4] = { v[k].x, v[k].y, v[k].z, v[k].w };
+        const uint4 vk = sv[k * THREADS + tid];
+        const uint32_t w4[4] = { vk.x, vk.y, vk.z, vk.w };
         uint32_t out[2] = { 0u, 0u };
 #pragma unroll
         for (int u = 0; u < 8; ++u) {
