@@ -141,6 +141,12 @@ int        sw_set_graphs(sw_handle* h, int on);
 int        sw_set_spins(sw_handle* h, const int8_t* spins, int is_host);
 int        sw_set_cold(sw_handle* h);                      /* all +1 (BASELINE config 3) */
 int        sw_get_spins(sw_handle* h, int8_t* out_host);   /* synchronising copy, nb*N bytes */
+/* The same two transfers with BIT-PACKED host buffers (north_star: "int8 or bit-packed spins"): nb * ceil(N/32)
+ * uint32 words, lattice b at word b*ceil(N/32), site i of a lattice in bit (i & 31) of its word (i >> 5), bit 1 = spin +1,
+ * padding bits of the last word ignored / zero.  1/8 of the bytes of the int8 plane cross PCIe; packing and unpacking
+ * run on the device.  Both synchronise.  Ising handles only (SW_ESTATE for a Potts handle).  PAPER.md:71 (Fig. 1). */
+int        sw_set_spins_bits(sw_handle* h, const uint32_t* bits_host);
+int        sw_get_spins_bits(sw_handle* h, uint32_t* out_host);
 int        sw_get_labels(sw_handle* h, int32_t* out_host); /* synchronising copy, nb*N int32 */
 
 /* Next sweep uses sweep index t (checkpoint / resume, one-step parity at large L). */

@@ -62,6 +62,8 @@ PROTOTYPES = {
     "sw_set_spins": (C.c_int, [_VP, _VP, C.c_int]),
     "sw_set_cold": (C.c_int, [_VP]),
     "sw_get_spins": (C.c_int, [_VP, _VP]),
+    "sw_set_spins_bits": (C.c_int, [_VP, _VP]),
+    "sw_get_spins_bits": (C.c_int, [_VP, _VP]),
     "sw_get_labels": (C.c_int, [_VP, _VP]),
     "sw_set_sweep_index": (C.c_int, [_VP, _U64]),
     "sw_sweep_index": (_U64, [_VP]),
@@ -234,6 +236,12 @@ def sw_set_cold(h) -> None:
 
 def sw_get_spins(h, host_ptr: int) -> None:
     _check(lib().sw_get_spins(_ptr(h), host_ptr))
+
+def sw_set_spins_bits(h, host_ptr: int) -> None:
+    _check(lib().sw_set_spins_bits(_ptr(h), host_ptr))
+
+def sw_get_spins_bits(h, host_ptr: int) -> None:
+    _check(lib().sw_get_spins_bits(_ptr(h), host_ptr))
 
 def sw_get_labels(h, host_ptr: int) -> None:
     _check(lib().sw_get_labels(_ptr(h), host_ptr))

@@ -863,6 +863,28 @@ int sw_set_cold(sw_handle* h) {
     return SW_OK;
 }
 
+// bit-packed host interface: staged through the decision plane D (nb * words uint32), which every sweep rewrites
+int sw_set_spins_bits(sw_handle* h, const uint32_t* bits_host) {
+    if (!h || !bits_host) { set_err("sw_set_spins_bits: null argument"); return SW_EINVAL; }
+    if (h->q) { set_err("sw_set_spins_bits: Ising handles only (a Potts colour does not fit a bit)"); return SW_ESTATE; }
+    SW_CUDA(cudaMemcpyAsync(h->D, bits_host, (size_t)h->nb * h->words * 4, cudaMemcpyHostToDevice, h->stream));
+    k_unpack_spins<<<grid1(h->words, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(h->spins, h->D, h->N, h->words);
+    SW_CUDA(cudaGetLastError());
+    SW_CUDA(cudaStreamSynchronize(h->stream));          // the caller may reuse its buffer
+    h->have_sweep = false; h->rec_valid = false;
+    return SW_OK;
+}
+
+int sw_get_spins_bits(sw_handle* h, uint32_t* out_host) {
+    if (!h || !out_host) { set_err("sw_get_spins_bits: null argument"); return SW_EINVAL; }
+    if (h->q) { set_err("sw_get_spins_bits: Ising handles only"); return SW_ESTATE; }
+    k_pack_spins<<<grid1(h->words, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(h->spins, h->D, h->N, h->words);
+    SW_CUDA(cudaGetLastError());
+    SW_CUDA(cudaMemcpyAsync(out_host, h->D, (size_t)h->nb * h->words * 4, cudaMemcpyDeviceToHost, h->stream));
+    SW_CUDA(cudaStreamSynchronize(h->stream));
+    return SW_OK;
+}
+
 int sw_get_spins(sw_handle* h, int8_t* out_host) {
     if (!h || !out_host) { set_err("sw_get_spins: null argument"); return SW_EINVAL; }
     SW_CUDA(cudaMemcpyAsync(out_host, h->spins, (size_t)h->nb * h->N, cudaMemcpyDeviceToHost, h->stream));

@@ -187,6 +187,39 @@ k_observe_generic(const int8_t* __restrict__ spins, Rec* __restrict__ rec, const
     }
 }
 
+// ---- bit-packed host interface (north_star: "int8 or bit-packed spins"): word w holds sites 32w .. 32w+31 of a
+//      lattice, bit = 1 for spin +1; 8x fewer bytes over PCIe than the int8 plane -------------------------------
+__global__ void __launch_bounds__(GEN_THREADS)
+k_unpack_spins(int8_t* __restrict__ spins, const uint32_t* __restrict__ bits, int N, int words) {
+    const int w = blockIdx.x * GEN_THREADS + threadIdx.x;
+    if (w >= words) return;
+    const uint32_t b = bits[(size_t)blockIdx.y * words + w];
+    int8_t* s = spins + (size_t)blockIdx.y * N + (size_t)w * 32;
+    if ((N & 31) == 0) {                              // whole words, 16-byte aligned rows of 32 sites
+        reinterpret_cast<uint4*>(s)[0] = make_uint4(spin_bytes4(b & 15u), spin_bytes4((b >> 4) & 15u),
+                                                    spin_bytes4((b >> 8) & 15u), spin_bytes4((b >> 12) & 15u));
+        reinterpret_cast<uint4*>(s)[1] = make_uint4(spin_bytes4((b >> 16) & 15u), spin_bytes4((b >> 20) & 15u),
+                                                    spin_bytes4((b >> 24) & 15u), spin_bytes4(b >> 28));
+    } else {
+        const int n = min(32, N - w * 32);
+        for (int k = 0; k < n; ++k) s[k] = ((b >> k) & 1u) ? (int8_t)1 : (int8_t)-1;
+    }
+}
+__global__ void __launch_bounds__(GEN_THREADS)
+k_pack_spins(const int8_t* __restrict__ spins, uint32_t* __restrict__ bits, int N, int words) {
+    const int w = blockIdx.x * GEN_THREADS + threadIdx.x;
+    if (w >= words) return;
+    const int8_t* s = spins + (size_t)blockIdx.y * N + (size_t)w * 32;
+    uint32_t b = 0;
+    if ((N & 31) == 0) {
+        b = ~neg_mask32(reinterpret_cast<const uint4*>(s)[0], reinterpret_cast<const uint4*>(s)[1]);
+    } else {
+        const int n = min(32, N - w * 32);
+        for (int k = 0; k < n; ++k) b |= (s[k] > 0 ? 1u : 0u) << k;
+    }
+    bits[(size_t)blockIdx.y * words + w] = b;
+}
+
 // ---- sweep control -------------------------------------------------------------------------------
 __global__ void k_set_ctl(Ctl* ctl, unsigned long long t, uint32_t slot, uint32_t cap) {
     ctl->t = t; ctl->slot = slot; ctl->cap = cap;

@@ -575,3 +575,38 @@ def test_potts_argument_errors(B):
     with pytest.raises(Exception):
         B.sw_set_path(h, 2)                          # tiled Ising kernels read sign bits
     B.sw_destroy(h)
+
+
+# ------------------------------------------------------------------------------------------------
+# bit-packed host interface (sw_set_spins_bits / sw_get_spins_bits): the same spins, 1 bit per site
+@pytest.mark.parametrize("L,nb", [(64, 1), (13, 1), (27, 3), (128, 2), (5, 1)])
+def test_bit_packed_host_interface(B, L, nb):
+    N, words = L * L, (L * L + 31) // 32
+    Ts, seeds = [T_C] * nb, [40 + b for b in range(nb)]
+    sw = B.SwendsenWang(L, Ts, seeds)
+    bits = np.zeros(nb * words, dtype=np.uint32)
+    B.sw_get_spins_bits(sw.h, bits.ctypes.data)
+    s0 = sw.spins_host()
+    for b in range(nb):
+        assert np.array_equal(bits[b * words:(b + 1) * words], wl.pack_bits((s0[b] > 0).astype(np.uint8)))
+        assert np.array_equal(s0[b], oracle.init_random(L, seeds[b]))
+    # inject a different state through the packed interface, sweep, read back both ways
+    rng = np.random.default_rng(L)
+    s = [np.where(rng.random(N) < 0.4, 1, -1).astype(np.int8) for _ in range(nb)]
+    inj = np.concatenate([wl.pack_bits((x > 0).astype(np.uint8)) for x in s]).astype(np.uint32)
+    B.sw_set_spins_bits(sw.h, inj.ctypes.data)
+    got = sw.spins_host()
+    for b in range(nb):
+        assert np.array_equal(got[b], s[b])
+    sw.sweep(1)
+    B.sw_get_spins_bits(sw.h, bits.ctypes.data)
+    got = sw.spins_host()
+    for b in range(nb):
+        s1 = oracle.sweep(L, Ts[b], seeds[b], 0, s[b])[0]
+        assert np.array_equal(got[b], s1)
+        assert np.array_equal(bits[b * words:(b + 1) * words], wl.pack_bits((s1 > 0).astype(np.uint8)))
+    sw.close()
+    swp = B.SwendsenWang(16, 1.0, 1, q=3)
+    with pytest.raises(Exception):
+        B.sw_get_spins_bits(swp.h, bits.ctypes.data)
+    swp.close()
