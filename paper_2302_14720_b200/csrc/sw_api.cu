@@ -64,7 +64,7 @@ using Cfg64 = TileCfg<64, 64>;
 using Cfg256 = TileCfg<256, 32>;
 
 struct Layout {        // byte offsets into the workspace
-    size_t spins, bondE, bondS, D, label, lab16, gsize, olist, ocount, nodes, bslot, lat, ctl, rec_now, mom, series, total;
+    size_t spins, sbits, bondE, bondS, D, label, lab16, gsize, olist, ocount, nodes, bslot, lat, ctl, rec_now, mom, series, total;
 };
 
 size_t olist_entries(int L) {          // per lattice, maximum over the tile shapes usable for this L
@@ -89,6 +89,7 @@ Layout make_layout(int L, int nb) {
     const size_t N = (size_t)L * L, words = (N + 31) / 32;
     Layout o; size_t p = 0;
     o.spins = p;   p = align_up(p + (size_t)nb * N);
+    o.sbits = p;   p = align_up(p + (size_t)nb * words * 4);     // bit-packed spins (fused scan path, packed host interface)
     o.bondE = p;   p = align_up(p + (size_t)nb * words * 4);
     o.bondS = p;   p = align_up(p + (size_t)nb * words * 4);
     o.D = p;       p = align_up(p + (size_t)nb * ((words + 3) / 4 * 4) * 4);
@@ -136,6 +137,8 @@ struct sw_handle {
     int L = 0, nb = 0, N = 0, words = 0;
     bool owns_ws = false;
     char* ws = nullptr; size_t ws_bytes = 0;
+    uint32_t* sbits = nullptr;       // bit-packed spins: bit 1 = +1.  The fused scan path keeps the state HERE
+    bool i8_valid = true, bits_valid = false;      // which of the two spin planes holds the current configuration
     int8_t* spins = nullptr; uint32_t *bondE = nullptr, *bondS = nullptr, *D = nullptr;
     int *label = nullptr, *gsize = nullptr, *ocount = nullptr; int2* olist = nullptr;
     uint16_t* lab16 = nullptr;       // tile-local root index of every site (scan path)
@@ -194,6 +197,23 @@ TileKind pick_tile(int L, int path) {
 TileKind potts_tile(int L, int path) { return (path == 0 && L % 128 == 0) ? SCAN_4x64 : TILE_NONE; }
 
 inline dim3 grid1(size_t n, int threads, int nb) { return dim3((unsigned)((n + threads - 1) / threads), (unsigned)nb); }
+
+// the two spin planes: the fused scan path sweeps on the bit plane, everything else on the int8 plane
+bool sweeps_on_bits(const sw_handle* h) { return scan_nw(h->tile) && h->path != 6 && !h->q; }
+int ensure_i8(sw_handle* h) {
+    if (h->i8_valid) return SW_OK;
+    k_unpack_spins<<<grid1(h->words, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(h->spins, h->sbits, h->N, h->words);
+    SW_CUDA(cudaGetLastError());
+    h->i8_valid = true;
+    return SW_OK;
+}
+int ensure_bits(sw_handle* h) {
+    if (h->bits_valid) return SW_OK;
+    k_pack_spins<<<grid1(h->words, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(h->spins, h->sbits, h->N, h->words);
+    SW_CUDA(cudaGetLastError());
+    h->bits_valid = true;
+    return SW_OK;
+}
 
 // timing mode: an event before kernel `kid` of sweep h->cur_sweep (kid == K_COUNT closes the sweep)
 int mark(sw_handle* h, int kid) {
@@ -255,13 +275,13 @@ int launch_bond_label_scan(sw_handle* h, bool fused, bool obs_prev) {
     if (fused) {
         SW_MARK(h, K_BONDLABEL);
         k_bond_label<NW, TH, true><<<dim3(tiles, h->nb), NW * TH, smem, h->stream>>>(
-            h->spins, h->bondE, h->bondS, h->lab16, h->nodes, h->ocount, h->bslot,
+            h->sbits, h->bondE, h->bondS, h->lab16, h->nodes, h->ocount, h->bslot,
             h->series, h->lat, h->ctl,
             h->L, h->N, h->words, h->nb, obs_prev ? 1 : 0);
     } else {
         SW_MARK(h, K_TILE);
         k_bond_label<NW, TH, false><<<dim3(tiles, h->nb), NW * TH, smem, h->stream>>>(
-            h->spins, h->bondE, h->bondS, h->lab16, h->nodes, h->ocount, h->bslot,
+            nullptr, h->bondE, h->bondS, h->lab16, h->nodes, h->ocount, h->bslot,
             h->series, h->lat, h->ctl,
             h->L, h->N, h->words, h->nb, obs_prev ? 1 : 0);
     }
@@ -307,8 +327,13 @@ int launch_flip_scan(sw_handle* h) {
     constexpr int TW = 32 * NW;
     const int tiles = h->N / (TW * TH);
     SW_MARK(h, K_FLIPTILE);
-    k_flip16<NW, TH><<<dim3(tiles, h->nb), NW * TH, 0, h->stream>>>(
-        h->spins, h->lab16, h->D, h->nodes, h->ocount, h->series, h->ctl, make_div(h->L),
+    if (sweeps_on_bits(h))
+        k_flip16<NW, TH, true><<<dim3(tiles, h->nb), NW * TH, 0, h->stream>>>(
+            h->spins, h->sbits, h->lab16, h->D, h->nodes, h->ocount, h->series, h->ctl, make_div(h->L),
+            h->L, h->N, h->words, h->nb);
+    else
+    k_flip16<NW, TH, false><<<dim3(tiles, h->nb), NW * TH, 0, h->stream>>>(
+        h->spins, h->sbits, h->lab16, h->D, h->nodes, h->ocount, h->series, h->ctl, make_div(h->L),
         h->L, h->N, h->words, h->nb);
     h->launches += 1;
     if (h->eager_labels) {                          // a4 every sweep instead of on demand
@@ -516,6 +541,7 @@ int init_handle(sw_handle* h, const double* T, const uint64_t* seed) {
     const Layout o = make_layout(h->L, h->nb);
     char* w = h->ws;
     h->spins = (int8_t*)(w + o.spins);
+    h->sbits = (uint32_t*)(w + o.sbits);
     h->bondE = (uint32_t*)(w + o.bondE); h->bondS = (uint32_t*)(w + o.bondS); h->D = (uint32_t*)(w + o.D);
     h->label = (int*)(w + o.label); h->gsize = (int*)(w + o.gsize); h->lab16 = (uint16_t*)(w + o.lab16);
     h->nodes = (int4*)(w + o.nodes); h->bslot = (uint16_t*)(w + o.bslot);
@@ -672,6 +698,10 @@ int sw_sweep(sw_handle* h, int64_t n) {
     if (!h || n < 0) { set_err("sw_sweep: invalid argument"); return SW_EINVAL; }
     if (n == 0) return SW_OK;
     h->launches = 0;
+    {   // the configuration must sit in the plane this path sweeps on
+        const int rc = sweeps_on_bits(h) ? ensure_bits(h) : ensure_i8(h);
+        if (rc) return rc;
+    }
     // graph replay: scan path, no per-kernel timing, enough sweeps to pay for the two stream hops
     cudaStream_t const user = h->stream;
     bool graphs = h->use_graphs && !h->graph_failed && !h->timing && scan_nw(h->tile) && n >= 4 && !h->q;
@@ -724,6 +754,10 @@ int sw_sweep(sw_handle* h, int64_t n) {
     }
     if (scan_nw(h->tile) && !h->q) {                    // a7 of the configuration the call ends with
         if (h->timing) SW_CUDA(cudaEventRecord(h->ev_tail[0], h->stream));
+        if (sweeps_on_bits(h))
+            k_observe_bits<<<grid1(h->words, 256, h->nb), 256, 0, h->stream>>>(
+                h->sbits, h->series, h->ctl, h->L, h->N, h->words, h->nb);
+        else
         k_observe_rows<<<grid1(h->words, 256, h->nb), 256, 0, h->stream>>>(
             h->spins, h->series, h->ctl, h->L, h->N, h->words, h->nb);
         k_moments_last<<<1, 64, 0, h->stream>>>(h->ctl, h->series, h->nb, h->mom, h->N);
@@ -740,6 +774,8 @@ int sw_sweep(sw_handle* h, int64_t n) {
     h->last_n = n;
     h->timed_sweeps = h->timing ? std::min<int64_t>(n, MAX_TIMED_SWEEPS) : 0;
     h->have_sweep = true; h->rec_valid = true;
+    if (sweeps_on_bits(h)) { h->bits_valid = true; h->i8_valid = false; }
+    else                   { h->i8_valid = true; h->bits_valid = false; }
     return SW_OK;
 }
 
@@ -762,6 +798,7 @@ int sw_bonds(sw_handle* h, const uint32_t** bondE, const uint32_t** bondS) {
 
 const int8_t* sw_spins(sw_handle* h) {
     if (!h) { set_err("sw_spins: null handle"); return nullptr; }
+    if (ensure_i8(h) != SW_OK) return nullptr;         // the fused path sweeps on the bit plane: int8 on demand
     return h->spins;
 }
 
@@ -773,6 +810,7 @@ int sw_observables(sw_handle* h, sw_obs* out) {
         SW_CUDA(cudaMemcpyAsync(r.data(), h->series + (size_t)slot * h->nb, sizeof(Rec) * h->nb,
                                 cudaMemcpyDeviceToHost, h->stream));
     } else {
+        { const int rc = ensure_i8(h); if (rc) return rc; }
         SW_CUDA(cudaMemsetAsync(h->rec_now, 0, sizeof(Rec) * h->nb, h->stream));
         if (h->q) {
             k_observe_potts<<<grid1(h->N, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(
@@ -850,6 +888,7 @@ int sw_set_spins(sw_handle* h, const int8_t* spins, int is_host) {
     SW_CUDA(cudaMemcpyAsync(h->spins, spins, (size_t)h->nb * h->N,
                             is_host ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice, h->stream));
     if (is_host) SW_CUDA(cudaStreamSynchronize(h->stream));
+    h->i8_valid = true; h->bits_valid = false;
     h->have_sweep = false; h->rec_valid = false;
     return SW_OK;
 }
@@ -859,18 +898,18 @@ int sw_set_cold(sw_handle* h) {
     const size_t n = (size_t)h->nb * h->N;
     k_fill_i8<<<(unsigned)((n + GEN_THREADS - 1) / GEN_THREADS), GEN_THREADS, 0, h->stream>>>(h->spins, n, (int8_t)(h->q ? 0 : 1));
     SW_CUDA(cudaGetLastError());
+    h->i8_valid = true; h->bits_valid = false;
     h->have_sweep = false; h->rec_valid = false;
     return SW_OK;
 }
 
-// bit-packed host interface: staged through the decision plane D (nb * words uint32), which every sweep rewrites
+// bit-packed host interface: straight into / out of the bit plane the fused path sweeps on
 int sw_set_spins_bits(sw_handle* h, const uint32_t* bits_host) {
     if (!h || !bits_host) { set_err("sw_set_spins_bits: null argument"); return SW_EINVAL; }
     if (h->q) { set_err("sw_set_spins_bits: Ising handles only (a Potts colour does not fit a bit)"); return SW_ESTATE; }
-    SW_CUDA(cudaMemcpyAsync(h->D, bits_host, (size_t)h->nb * h->words * 4, cudaMemcpyHostToDevice, h->stream));
-    k_unpack_spins<<<grid1(h->words, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(h->spins, h->D, h->N, h->words);
-    SW_CUDA(cudaGetLastError());
+    SW_CUDA(cudaMemcpyAsync(h->sbits, bits_host, (size_t)h->nb * h->words * 4, cudaMemcpyHostToDevice, h->stream));
     SW_CUDA(cudaStreamSynchronize(h->stream));          // the caller may reuse its buffer
+    h->bits_valid = true; h->i8_valid = false;
     h->have_sweep = false; h->rec_valid = false;
     return SW_OK;
 }
@@ -878,15 +917,15 @@ int sw_set_spins_bits(sw_handle* h, const uint32_t* bits_host) {
 int sw_get_spins_bits(sw_handle* h, uint32_t* out_host) {
     if (!h || !out_host) { set_err("sw_get_spins_bits: null argument"); return SW_EINVAL; }
     if (h->q) { set_err("sw_get_spins_bits: Ising handles only"); return SW_ESTATE; }
-    k_pack_spins<<<grid1(h->words, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(h->spins, h->D, h->N, h->words);
-    SW_CUDA(cudaGetLastError());
-    SW_CUDA(cudaMemcpyAsync(out_host, h->D, (size_t)h->nb * h->words * 4, cudaMemcpyDeviceToHost, h->stream));
+    { const int rc = ensure_bits(h); if (rc) return rc; }
+    SW_CUDA(cudaMemcpyAsync(out_host, h->sbits, (size_t)h->nb * h->words * 4, cudaMemcpyDeviceToHost, h->stream));
     SW_CUDA(cudaStreamSynchronize(h->stream));
     return SW_OK;
 }
 
 int sw_get_spins(sw_handle* h, int8_t* out_host) {
     if (!h || !out_host) { set_err("sw_get_spins: null argument"); return SW_EINVAL; }
+    { const int rc = ensure_i8(h); if (rc) return rc; }
     SW_CUDA(cudaMemcpyAsync(out_host, h->spins, (size_t)h->nb * h->N, cudaMemcpyDeviceToHost, h->stream));
     SW_CUDA(cudaStreamSynchronize(h->stream));
     return SW_OK;

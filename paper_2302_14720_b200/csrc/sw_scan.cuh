@@ -62,7 +62,7 @@ __device__ __forceinline__ int div_l(int v, const DivL& D) {
 // that k_bond_rows (or a test) wrote -- per-stage timing (BASELINE config 3) and labelling-only tests.
 template <int NW, int TH, bool FUSE>
 __global__ void __launch_bounds__(NW * TH)
-k_bond_label(const int8_t* __restrict__ spins, uint32_t* bondE, uint32_t* bondS,
+k_bond_label(const uint32_t* __restrict__ sbits, uint32_t* bondE, uint32_t* bondS,
              uint16_t* __restrict__ lab16, int4* __restrict__ nodes, int* __restrict__ ocount,
              uint16_t* __restrict__ bslot,
              Rec* __restrict__ rec, const Lat* __restrict__ lat, const Ctl* __restrict__ ctl,
@@ -82,7 +82,8 @@ k_bond_label(const int8_t* __restrict__ spins, uint32_t* bondE, uint32_t* bondS,
     const int ty = blockIdx.x / tilesX, tx = blockIdx.x - ty * tilesX;
     const int y0 = ty * TH, x0 = tx * TW;
     const int wprL = L >> 5;
-    const int8_t* s = spins + (size_t)blockIdx.y * N;
+    // FUSE: the spins come bit-packed (bit 1 = +1; word w = sites 32w .. 32w+31), 1/8 of the int8 plane's bytes
+    const uint32_t* sb = sbits + (size_t)blockIdx.y * words;
     const Lat la = lat[blockIdx.y];
     const unsigned long long t = ctl->t;
     const uint32_t tlo = (uint32_t)t, thi = (uint32_t)(t >> 32);
@@ -110,13 +111,9 @@ k_bond_label(const int8_t* __restrict__ spins, uint32_t* bondE, uint32_t* bondS,
             const int y = y0 + row;
             const int xw = (x0 >> 5) + wx;
             const int w = y * wprL + xw;                              // word index within the lattice
-            const int8_t* r0 = s + (size_t)y * L + xw * 32;
-            const int8_t* r1 = s + (size_t)(y + 1 == L ? 0 : y + 1) * L + xw * 32;
-            const uint4 a0 = *reinterpret_cast<const uint4*>(r0), a1 = *reinterpret_cast<const uint4*>(r0 + 16);
-            const uint4 b0 = *reinterpret_cast<const uint4*>(r1), b1 = *reinterpret_cast<const uint4*>(r1 + 16);
-            const int8_t nx = s[(size_t)y * L + (xw + 1 == wprL ? 0 : (xw + 1) * 32)];
-            const uint32_t own = neg_mask32(a0, a1), south = neg_mask32(b0, b1);
-            const uint32_t eastm = (own >> 1) | (nx < 0 ? 0x80000000u : 0u);
+            const uint32_t own = ~sb[w], south = ~sb[(y + 1 == L ? 0 : y + 1) * wprL + xw];   // bit = 1: spin -1
+            const uint32_t nxw = sb[y * wprL + (xw + 1 == wprL ? 0 : xw + 1)];
+            const uint32_t eastm = (own >> 1) | ((~nxw & 1u) << 31);
             const uint32_t eqE = ~(own ^ eastm), eqS = ~(own ^ south);
             if (obs_prev) {
                 // a7 for free: the equal-pair masks of the bond test are the energy of the
@@ -145,16 +142,18 @@ k_bond_label(const int8_t* __restrict__ spins, uint32_t* bondE, uint32_t* bondS,
                 const int x = x0 + 2 * j;
                 const int i = yn * L + x;                                  // even site; call covers i, i + 1
                 const uint4 r = philox4x32_10((uint32_t)(i >> 1), tlo, thi, TAG_BOND, key);
-                const int8_t u0 = s[i], u1 = s[i + 1];
-                const int8_t d0 = s[(size_t)y0 * L + x], d1 = s[(size_t)y0 * L + x + 1];
-                const uint32_t bits = ((u0 == d0 && r.y < la.thr) ? 1u : 0u) | ((u1 == d1 && r.w < la.thr) ? 2u : 0u);
+                const int id = y0 * L + x;                                 // (x is even: both sites in one word)
+                const uint32_t eq = ~((sb[i >> 5] >> (i & 31)) ^ (sb[id >> 5] >> (id & 31)));
+                const uint32_t bits = (eq & ((r.y < la.thr ? 1u : 0u) | (r.w < la.thr ? 2u : 0u))) & 3u;
                 if (bits) atomicOr(&nIn[(2 * j) >> 5], bits << ((2 * j) & 31));
             } else {
                 const int row = j - TW / 2;
                 const int xwst = x0 == 0 ? L - 1 : x0 - 1;                 // odd column
                 const int i = (y0 + row) * L + xwst;
                 const uint4 r = philox4x32_10((uint32_t)(i >> 1), tlo, thi, TAG_BOND, key);
-                if (s[i] == s[(size_t)(y0 + row) * L + x0] && r.z < la.thr) atomicOr(&wIn[row >> 5], 1u << (row & 31));
+                const int ie = (y0 + row) * L + x0;
+                if (!(((sb[i >> 5] >> (i & 31)) ^ (sb[ie >> 5] >> (ie & 31))) & 1u) && r.z < la.thr)
+                    atomicOr(&wIn[row >> 5], 1u << (row & 31));
             }
         }
     }
@@ -503,9 +502,11 @@ k_labels16(int* __restrict__ label, const uint16_t* __restrict__ lab16, const in
 // Then every site reads its 16-bit tile-local root index (2 B / site, written by k_bond_label) and looks the
 // bit up in shared memory: no global gather, no index arithmetic per site.
 // ---------------------------------------------------------------------------------------------------
-template <int NW, int TH>
+// BITS: the new spins go out bit-packed (one byte = 8 sites per thread and step, 32 MiB instead of 256 MiB at
+// L = 16384) into the plane k_bond_label<FUSE> reads; else as the int8 plane (unfused path 6).
+template <int NW, int TH, bool BITS>
 __global__ void __launch_bounds__(NW * TH, 1536 / (NW * TH))
-k_flip16(int8_t* __restrict__ spins, const uint16_t* __restrict__ lab16, const uint32_t* __restrict__ D,
+k_flip16(int8_t* __restrict__ spins, uint32_t* __restrict__ sbits, const uint16_t* __restrict__ lab16, const uint32_t* __restrict__ D,
          const int4* __restrict__ nodes, const int* __restrict__ ocount, Rec* __restrict__ rec, const Ctl* __restrict__ ctl,
          DivL dv, int L, int N, int words, int nb) {
     constexpr int TW = 32 * NW, SITES = TW * TH, THREADS = NW * TH;
@@ -573,8 +574,9 @@ k_flip16(int8_t* __restrict__ spins, const uint16_t* __restrict__ lab16, const u
             const uint32_t r = (u & 1) ? (w4[u >> 1] >> 16) : (w4[u >> 1] & 0xFFFFu);
             b8 |= (__funnelshift_r(dec[r >> 5], 0u, r) & 1u) << u;
         }
-        *reinterpret_cast<uint2*>(spins + (size_t)blockIdx.y * N + (size_t)(y0 + (l >> LOG_TW)) * L + x0 + (l & (TW - 1))) =
-            make_uint2(spin_bytes4(b8 & 15u), spin_bytes4(b8 >> 4));
+        const size_t gsite = (size_t)blockIdx.y * N + (size_t)(y0 + (l >> LOG_TW)) * L + x0 + (l & (TW - 1));
+        if (BITS) reinterpret_cast<uint8_t*>(sbits)[gsite >> 3] = (uint8_t)b8;
+        else *reinterpret_cast<uint2*>(spins + gsite) = make_uint2(spin_bytes4(b8 & 15u), spin_bytes4(b8 >> 4));
     }
 }
 
@@ -596,6 +598,34 @@ k_observe_rows(const int8_t* __restrict__ spins, Rec* __restrict__ rec, const Ct
         const int8_t nx = s[(size_t)y * L + (xw + 1 == wpr ? 0 : (xw + 1) * 32)];
         const uint32_t own = neg_mask32(a0, a1), south = neg_mask32(b0, b1);
         const uint32_t eastm = (own >> 1) | (nx < 0 ? 0x80000000u : 0u);
+        e = 64 - 2 * (__popc(~(own ^ eastm)) + __popc(~(own ^ south)));
+        m = 32 - 2 * __popc(own);
+    }
+    e = warp_sum_i(e); m = warp_sum_i(m);
+    __shared__ int se[8], sm[8];
+    if ((threadIdx.x & 31) == 0) { se[threadIdx.x >> 5] = e; sm[threadIdx.x >> 5] = m; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int te = 0, tm = 0;
+        for (int k = 0; k < 8; ++k) { te += se[k]; tm += sm[k]; }
+        Rec* r = rec + (size_t)(ctl->slot == 0 ? ctl->cap - 1 : ctl->slot - 1) * nb + blockIdx.y;
+        if (te) atomic_add_ll(&r->E, te);
+        if (tm) atomic_add_ll(&r->M, tm);
+    }
+}
+
+// the same from the bit-packed plane (fused path): one word per thread
+__global__ void __launch_bounds__(256)
+k_observe_bits(const uint32_t* __restrict__ sbits, Rec* __restrict__ rec, const Ctl* __restrict__ ctl,
+               int L, int N, int words, int nb) {
+    const int w = blockIdx.x * 256 + threadIdx.x;
+    int e = 0, m = 0;
+    if (w < words) {
+        const int wpr = L >> 5;
+        const int y = w / wpr, xw = w - y * wpr;
+        const uint32_t* sb = sbits + (size_t)blockIdx.y * words;
+        const uint32_t own = ~sb[w], south = ~sb[(y + 1 == L ? 0 : y + 1) * wpr + xw];
+        const uint32_t eastm = (own >> 1) | ((~sb[y * wpr + (xw + 1 == wpr ? 0 : xw + 1)] & 1u) << 31);
         e = 64 - 2 * (__popc(~(own ^ eastm)) + __popc(~(own ^ south)));
         m = 32 - 2 * __popc(own);
     }
