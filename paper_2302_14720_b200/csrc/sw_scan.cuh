@@ -3,7 +3,8 @@
 // Stage map; one CTA per tile of TW x TH sites, TW = 32 * NW, TH = 32 or 64; the tile is
 // NW x TH/32 blocks of 32 x 32 sites, one warp each; NW * TH threads = one thread per 32-site word.
 //   a1+a2 k_bond_label<NW, TH, FUSE>
-//       phase 1  thread per 32-site word: sign masks of the int8 spins, 16 Philox4x32-10 calls, bond words to
+//       phase 1  thread per 32-site word: the word's spins from the BIT-PACKED plane (FUSE; bit 1 = +1; the int8 plane
+//                is derived on demand, sw_spins), 16 Philox4x32-10 calls, bond words to
 //                shared memory and to the canonical global bit-planes; E, M of the previous sweep's
 //                configuration from the same equal-pair masks; the bonds that enter the tile from its North
 //                and West neighbours are recomputed (TW/2 + TH extra calls)
@@ -20,9 +21,10 @@
 //       phase 6  per border site with a bond across the tile edge: the slot of its root
 //   a3    k_merge_nodes (union-find over the nodes of neighbouring tiles), k_roots_nodes (sizes and minimum
 //         site index of the clusters that span tiles)
-//   a4-a6 k_flip16<NW, TH>: one decision bit per tile root in shared memory, spins = lookup by 16-bit root;
+//   a4-a6 k_flip16<NW, TH, BITS>: one decision bit per tile root in shared memory, spins = lookup by 16-bit root,
+//         written bit-packed (BITS: a byte per 8 sites) or as int8 (unfused path 6);
 //         k_labels16<NW, TH>: flat int32 labels from the 16-bit roots, on demand (sw_labels)
-//   a7    E, M: by-product of the next sweep's bond test, k_observe_rows at the end of a call; cluster count
+//   a7    E, M: by-product of the next sweep's bond test, k_observe_bits / k_observe_rows at the end of a call; cluster count
 //         and largest cluster: k_bond_label (closed) + k_flip16 (root nodes)
 #pragma once
 #include "sw_common.cuh"
