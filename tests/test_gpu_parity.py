@@ -610,3 +610,42 @@ def test_bit_packed_host_interface(B, L, nb):
     with pytest.raises(Exception):
         B.sw_get_spins_bits(swp.h, bits.ctypes.data)
     swp.close()
+
+
+def test_switching_paths_keeps_one_state(B):
+    """The fused path sweeps on the bit-packed plane, the others on the int8 plane: one handle walked through the
+    paths must follow the oracle without a break (the planes are converted on demand)."""
+    L, T, seed = 256, T_C, 77
+    sw = B.SwendsenWang(L, T, seed)
+    s = oracle.init_random(L, seed)
+    t = 0
+    for path, n in ((0, 2), (1, 2), (0, 1), (6, 2), (11, 1), (0, 2), (2, 1), (9, 2)):
+        B.sw_set_path(sw.h, path)
+        for _ in range(n):
+            s, bE, bS, lab, obs = oracle.sweep(L, T, seed, t, s)
+            sw.sweep(1)
+            t += 1
+            assert np.array_equal(sw.labels_host()[0], lab), (path, t)
+            assert _obs_tuple(sw.observables()[0]) == obs, (path, t)
+        assert np.array_equal(sw.spins_host()[0], s), (path, t)
+    # several sweeps per call across a switch, spins read only at the end
+    B.sw_set_path(sw.h, 0); sw.sweep(5)
+    B.sw_set_path(sw.h, 1); sw.sweep(2)
+    B.sw_set_path(sw.h, 0); sw.sweep(4)
+    s, _ = oracle.run(L, T, seed, 11, spins=s, t0=t)
+    assert np.array_equal(sw.spins_host()[0], s)
+    sw.close()
+
+
+def test_observables_of_an_injected_packed_state(B):
+    L = 128
+    sw = B.SwendsenWang(L, T_C, 3)
+    s = wl.spins_numpy_random(L, 5, 0.3)
+    bits = wl.pack_bits((s > 0).astype(np.uint8)).astype(np.uint32)
+    B.sw_set_spins_bits(sw.h, bits.ctypes.data)
+    o = sw.observables()[0]                          # no sweep yet: E, M of the injected state, no clusters
+    assert _obs_tuple(o) == oracle.observables(L, s)[:2] + (0, 0)
+    s1, bE, bS, lab, obs = oracle.sweep(L, T_C, 3, 0, s)
+    sw.sweep(1)
+    assert _obs_tuple(sw.observables()[0]) == obs and np.array_equal(sw.spins_host()[0], s1)
+    sw.close()
