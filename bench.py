@@ -303,6 +303,20 @@ def main():
                 "issue_active_pct": issue,      # ncu smsp__issue_active of this kernel (profiles/): what really binds it
                 "bytes_per_site": kb.get(dom), "ms_per_launch": dom_ms,
                 "share_of_step": kms[dom] / max(1e-9, sum(kms.values()))}
+    # the same kernel against the bound that really holds it: instruction issue.  peak = 148 SMs x
+    # 4 schedulers x 32 lanes x SM clock (one warp instruction per scheduler and cycle; guide: B200_PROFILING.md unit
+    # counts); achieved = thread-instruction slots the kernel executes per site (committed ncu count, profiles/) x N /
+    # its live CUDA-event time; algorithmic = the Philox4x32-10 draws alone (24 integer instructions per site).
+    tips = (ncu_traffic("_thread_instr_slots_per_site") or {}).get(dom)
+    sm_ghz = (clk.get("sm_mhz") or 1965.0) / 1e3
+    alu_peak = 148 * 4 * 32 * sm_ghz / 1e3                               # T thread-instruction slots / s
+    roofline_alu = None
+    if tips:
+        ach = tips * N / (dom_ms * 1e-3) / 1e12
+        roofline_alu = {"bound": "alu", "kernel": dom, "achieved": ach, "peak": alu_peak, "unit": "T thread-instr/s",
+                        "frac": ach / alu_peak, "thread_instr_slots_per_site": tips,
+                        "algorithmic_instr_per_site": 24, "algorithmic_frac": 24 * N / (dom_ms * 1e-3) / 1e12 / alu_peak,
+                        "peak_source": "148 SMs x 4 schedulers x 32 lanes x measured SM clock"}
     stages = {}
     for s, v in stage.items():
         sms = v / timed
@@ -399,7 +413,7 @@ def main():
         "clocks": clk,
         "e2e": e2e, "e2e_int8": e2e_int8,
         "gpu_launches": int(launches),
-        "roofline": roofline,
+        "roofline": roofline, "roofline_alu": roofline_alu,
         "sweep_model": {"bytes_per_site": SWEEP_MODEL_BYTES_PER_SITE, "achieved_GBps": sweep_gbs,
                         "frac_of_peak": sweep_gbs / peak, "frac_of_8TBps_nominal": sweep_gbs / 8000.0},
         "stages": stages, "stages_unfused": unfused, "label_equivalence": equiv, "potts": potts, "kernels": kernels,
