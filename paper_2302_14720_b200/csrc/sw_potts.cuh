@@ -239,25 +239,41 @@ k_observe_potts_rows(const int8_t* __restrict__ colours, Rec* __restrict__ rec, 
     __syncthreads();
     const int g = blockIdx.x * GEN_THREADS + threadIdx.x;              // group of 16 sites (N / 16 is a multiple of 32)
     int e = 0;
-    if (g * 16 < N) {
+    const bool on = g * 16 < N;                                        // (warp-uniform: N / 16 is a multiple of 32)
+    uint32_t w[4] = { 0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu };   // 0xFF: no colour
+    if (on) {
         const int8_t* s = colours + (size_t)blockIdx.y * N;
         const int i = g * 16;
         const int y = i / L, x = i - y * L;
         const uint4 a = *reinterpret_cast<const uint4*>(s + i);
         const uint4 b = *reinterpret_cast<const uint4*>(s + (size_t)(y + 1 == L ? 0 : y + 1) * L + x);
         const uint32_t nx = (uint8_t)s[(size_t)y * L + (x + 16 == L ? 0 : x + 16)];
-        const uint32_t w[4] = { a.x, a.y, a.z, a.w }, so[4] = { b.x, b.y, b.z, b.w };
+        const uint32_t so[4] = { b.x, b.y, b.z, b.w };
+        w[0] = a.x; w[1] = a.y; w[2] = a.z; w[3] = a.w;
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
             const uint32_t east = __funnelshift_r(w[k], k < 3 ? w[k < 3 ? k + 1 : 3] : nx, 8);
             e -= (__popc(__vcmpeq4(w[k], east)) + __popc(__vcmpeq4(w[k], so[k]))) >> 3;
+        }
+    }
+    if (q <= 8) {
+        // few colours: sites of colour c among my 16 = equal bytes against the splat of c; one add per warp and colour
+        for (int c = 0; c < q; ++c) {
+            const uint32_t pat = (uint32_t)c * 0x01010101u;
+            int n = (__popc(__vcmpeq4(w[0], pat)) + __popc(__vcmpeq4(w[1], pat)) +
+                     __popc(__vcmpeq4(w[2], pat)) + __popc(__vcmpeq4(w[3], pat))) >> 3;
+            n = warp_sum_i(n);
+            if ((threadIdx.x & 31) == 0 && n) atomicAdd(&s_cnt[c], n);
+        }
+    } else if (on) {
+#pragma unroll
+        for (int k = 0; k < 4; ++k)
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
                 const int c = (w[k] >> (8 * u)) & POTTS_MAX_Q;
                 const unsigned grp = __match_any_sync(0xffffffffu, c);
                 if ((threadIdx.x & 31) == __ffs(grp) - 1) atomicAdd(&s_cnt[c], __popc(grp));
             }
-        }
     }
     e = warp_sum_i(e);
     if ((threadIdx.x & 31) == 0 && e) atomicAdd(&s_e, e);
