@@ -649,3 +649,55 @@ def test_observables_of_an_injected_packed_state(B):
     sw.sweep(1)
     assert _obs_tuple(sw.observables()[0]) == obs and np.array_equal(sw.spins_host()[0], s1)
     sw.close()
+
+
+# ------------------------------------------------------------------------------------------------
+# The GPU path against what the physics fixes, without the oracle in between
+import exact_ising as ex
+
+
+def _golden_kaufman(L):
+    import os
+    with open(os.path.join(os.path.dirname(__file__), "golden", "kaufman_u.txt")) as f:
+        for line in f:
+            if line.startswith("#") or not line.strip():
+                continue
+            v = line.split()
+            if int(v[0]) == L:
+                return dict(zip((2.0, 2.26919, "Tc", 2.5, 3.0), (float(x) for x in v[1:])))
+    raise KeyError(L)
+
+
+@pytest.mark.parametrize("T,seed", [(2.0, 1), (2.26919, 2), (3.0, 3)])
+def test_config2_L1024_energy_against_kaufman_on_the_gpu(B, T, seed):
+    L, therm, n = 1024, 200, 2000
+    sw = B.SwendsenWang(L, T, seed)
+    sw.sweep(therm)
+    sw.sweep(n)
+    ser = sw.series()[:, 0, :]
+    assert ser.shape[0] == n
+    u, du = ex.binned_mean_err(ser[:, 0] / (L * L), nbins=40)
+    exact = _golden_kaufman(L)[T]
+    assert abs(u - exact) <= 4 * du and du < 2e-3, (u, du, exact)
+    if T == 2.0:                                     # Yang's spontaneous magnetisation (finite-size shift << error bar)
+        m, dm = ex.binned_mean_err(np.abs(ser[:, 1]) / (L * L), nbins=40)
+        assert abs(m - 0.911319) <= 4 * dm + 1e-5, (m, dm)
+    sw.close()
+
+
+@pytest.mark.parametrize("T,seed", [(1.5, 7), (2.269, 8), (3.5, 9)])
+def test_config1_4x4_against_exact_enumeration_on_the_gpu(B, T, seed):
+    L, calls, per = 4, 25, 4000
+    r = ex.exact_small(L, T)
+    sw = B.SwendsenWang(L, T, seed)
+    sw.sweep(100)
+    E, M = [], []
+    for _ in range(calls):
+        sw.sweep(per)
+        ser = sw.series()[:, 0, :]
+        E.append(ser[:, 0]); M.append(np.abs(ser[:, 1]))
+    u, du = ex.binned_mean_err(np.concatenate(E) / 16.0)
+    m, dm = ex.binned_mean_err(np.concatenate(M) / 16.0)
+    assert abs(u - float(r["u"])) <= 4 * du, (u, du, float(r["u"]))
+    assert abs(m - float(r["abs_m"])) <= 4 * dm, (m, dm, float(r["abs_m"]))
+    sw.close()
