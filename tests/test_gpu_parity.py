@@ -701,3 +701,45 @@ def test_config1_4x4_against_exact_enumeration_on_the_gpu(B, T, seed):
     assert abs(u - float(r["u"])) <= 4 * du, (u, du, float(r["u"]))
     assert abs(m - float(r["abs_m"])) <= 4 * dm, (m, dm, float(r["abs_m"]))
     sw.close()
+
+
+def test_specific_heat_against_kaufman_on_the_gpu(B):
+    """The paper's own validation (Fig. 6: the specific-heat peak), with the on-device moments
+    (NEXT-1): 16 independent L = 64 lattices at T_c, C/N of each from sw_moments, mean +- standard error against
+    Kaufman's exact finite-lattice value."""
+    L, nb, therm, n = 64, 16, 500, 20000
+    T = T_C
+    sw = B.SwendsenWang(L, [T] * nb, [900 + b for b in range(nb)])
+    sw.sweep(therm)
+    sw.moments_reset()
+    sw.sweep(n)
+    mom = sw.moments()
+    c = np.array([m["specific_heat"] for m in mom])
+    u = np.array([m["e_mean"] for m in mom])
+    assert all(m["n"] == n for m in mom)
+    c_exact, u_exact = float(ex.kaufman_c(L, T)), float(ex.kaufman_u(L, T))
+    assert abs(c.mean() - c_exact) <= 4 * c.std(ddof=1) / np.sqrt(nb), (c.mean(), c.std(ddof=1) / np.sqrt(nb), c_exact)
+    assert abs(u.mean() - u_exact) <= 4 * u.std(ddof=1) / np.sqrt(nb), (u.mean(), u_exact)
+    assert c.std(ddof=1) / np.sqrt(nb) < 0.03 * c_exact
+    sw.close()
+
+
+@pytest.mark.parametrize("T,seed", [(0.7, 7), (0.995, 8)])
+def test_potts_3x3_against_exact_enumeration_on_the_gpu(B, T, seed):
+    from test_oracle_potts import _potts_enumeration
+    L, q, calls, per = 3, 3, 20, 4000
+    E, M = _potts_enumeration(L, q)
+    w = np.exp(-(E - E.min()) / T)
+    exact_E, exact_M = float((E * w).sum() / w.sum()), float((M * w).sum() / w.sum())
+    sw = B.SwendsenWang(L, T, seed, q=q)
+    sw.sweep(100)
+    es, ms = [], []
+    for _ in range(calls):
+        sw.sweep(per)
+        ser = sw.series()[:, 0, :]
+        es.append(ser[:, 0]); ms.append(ser[:, 1])
+    e, de = ex.binned_mean_err(np.concatenate(es))
+    m, dm = ex.binned_mean_err(np.concatenate(ms))
+    assert abs(e - exact_E) <= 4 * de and de < 0.06, (e, de, exact_E)
+    assert abs(m - exact_M) <= 4 * dm and dm < 0.06, (m, dm, exact_M)
+    sw.close()
