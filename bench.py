@@ -406,7 +406,7 @@ def main():
         "config": {"workload": f"2D Ising Swendsen-Wang, L={L} periodic, J=1, T=T_c=2/ln(1+sqrt2), random start "
                                f"seed {6}+rank, one sweep per step (BASELINE configs[3])",
                    "sites_per_gpu": N, "tile": f"{tw}x{th}", "parallelism": f"replicas x{world}",
-                   "l2_policy": "inputs larger than L2 (1.3 GB of spins+labels per sweep vs 126 MB L2)",
+                   "l2_policy": "working set larger than L2: every sweep streams the 512 MiB 16-bit root plane out and in, plus bond planes, bit-packed spins and node arrays (~0.7 GB) vs 126 MB L2",
                    "state_after": {"sweep": int(obs.sweep), "e_per_site": obs.e_per_site,
                                    "abs_m_per_site": obs.abs_m_per_site, "n_clusters": int(obs.n_clusters),
                                    "largest_cluster": int(obs.largest_cluster)}},
