@@ -17,6 +17,8 @@ import argparse
 import json
 import math
 import os
+
+import numpy as np
 import statistics
 import subprocess
 import sys
@@ -240,6 +242,12 @@ def main():
     launches = sw.launch_count()
     kms = sw.kernel_ms()
     stage = sw.stage_ms()
+    per = sw.sweep_ms()                               # the per-sweep time series of the timed run
+    per_sweep = {"n": int(len(per)), "median_ms": float(np.median(per)), "mean_ms": float(per.mean()),
+                 "mean_last_half_ms": float(per[len(per) // 2:].mean()), "min_ms": float(per.min()),
+                 "max_ms": float(per.max()), "first_ms": float(per[0]), "last_ms": float(per[-1]),
+                 "every_5th_ms": [round(float(v), 4) for v in per[::5]],
+                 "note": "CUDA events around each sweep of the timed call (sweeps W .. W+K-1 after the random start)"}
     timed = min(K, 1024)
     sw.set_stage_timing(False)
     obs = sw.observables()[0]
@@ -416,7 +424,7 @@ def main():
         "roofline": roofline, "roofline_alu": roofline_alu,
         "sweep_model": {"bytes_per_site": SWEEP_MODEL_BYTES_PER_SITE, "achieved_GBps": sweep_gbs,
                         "frac_of_peak": sweep_gbs / peak, "frac_of_8TBps_nominal": sweep_gbs / 8000.0},
-        "stages": stages, "stages_unfused": unfused, "label_equivalence": equiv, "potts": potts, "kernels": kernels,
+        "per_sweep": per_sweep, "stages": stages, "stages_unfused": unfused, "label_equivalence": equiv, "potts": potts, "kernels": kernels,
         "cpu_baseline": cpu,
         "paper_context": "paper: 17x (SW) / 90x (Wolff) over serial, Haswell E5-2695 vs Tesla P100; "
                          "SW GPU rate 1.25e8 site-updates/s at L=4096 (PAPER.md:127,142)",

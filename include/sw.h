@@ -188,6 +188,10 @@ int        sw_stage_ms(sw_handle* h, float out[4]);
  * "flip16" (a4 + a6 fused), ...; "" past the end). */
 int        sw_kernel_ms(sw_handle* h, float* out, int32_t cap);
 const char* sw_kernel_name(int32_t i);
+/* The same measurement per SWEEP, as a time series (a random start is not equilibrated quickly, so the
+ * cost of a sweep drifts): out[k] = ms from the first to the last event of timed sweep k, k < min(cap, timed sweeps);
+ * returns the number of timed sweeps of the last call (or a negative code). */
+int64_t    sw_sweep_ms(sw_handle* h, float* out, int64_t cap);
 
 /* Select the kernel path.  Results are identical on every path.
  *   0  automatic: the fused scan-line path when L is a multiple of 64 (tiles of 256, 128 or 64 x 32 sites,

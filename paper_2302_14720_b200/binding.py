@@ -78,6 +78,7 @@ PROTOTYPES = {
     "sw_kernel_name": (C.c_char_p, [_I32]),
     "sw_set_path": (C.c_int, [_VP, C.c_int]),
     "sw_label_passes": (C.c_int, [_VP, C.POINTER(C.c_int32)]),
+    "sw_sweep_ms": (C.c_int64, [_VP, C.POINTER(C.c_float), C.c_int64]),
     "sw_create_potts": (_VP, [C.c_int32, C.c_int32, C.c_double, C.c_uint64]),
     "sw_create_potts_in": (_VP, [_VP, C.c_uint64, C.c_int32, C.c_int32, C.c_int32, C.POINTER(C.c_double), C.POINTER(C.c_uint64)]),
     "sw_q": (C.c_int32, [_VP]),
@@ -268,6 +269,13 @@ def sw_kernel_ms(h):
     n = _check(lib().sw_kernel_ms(_ptr(h), out, 32))
     return {lib().sw_kernel_name(i).decode(): float(out[i]) for i in range(n)}
 
+def sw_sweep_ms(h) -> np.ndarray:
+    """ms of every timed sweep of the last sw_sweep call (stage timing on), in order."""
+    n = _check(lib().sw_sweep_ms(_ptr(h), (C.c_float * 1)(), 0))
+    out = (C.c_float * max(1, n))()
+    _check(lib().sw_sweep_ms(_ptr(h), out, n))
+    return np.array(out[:n], dtype=np.float64)
+
 def sw_set_path(h, path: int) -> None:
     _check(lib().sw_set_path(_ptr(h), path))
 
@@ -411,6 +419,9 @@ class SwendsenWang:
 
     def kernel_ms(self):
         return sw_kernel_ms(self.h)
+
+    def sweep_ms(self):
+        return sw_sweep_ms(self.h)
 
     def threshold(self, b: int = 0) -> int:
         return sw_threshold(self.h, b)

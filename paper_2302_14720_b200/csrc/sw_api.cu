@@ -981,6 +981,17 @@ int sw_kernel_ms(sw_handle* h, float* out, int32_t cap) {
     return K_COUNT;
 }
 
+int64_t sw_sweep_ms(sw_handle* h, float* out, int64_t cap) {
+    if (!h || !out || cap < 0) { set_err("sw_sweep_ms: invalid argument"); return SW_EINVAL; }
+    if (h->timed_sweeps == 0) { set_err("sw_sweep_ms: the last sw_sweep ran without stage timing"); return SW_ESTATE; }
+    SW_CUDA(cudaStreamSynchronize(h->stream));
+    const int ns = (int)h->ev_seq.size();            // marks per sweep, the closing one included
+    const int64_t n = std::min<int64_t>(h->timed_sweeps, cap);
+    for (int64_t k = 0; k < n; ++k)
+        SW_CUDA(cudaEventElapsedTime(out + k, h->ev[(size_t)k * EV_PER_SWEEP], h->ev[(size_t)k * EV_PER_SWEEP + ns - 1]));
+    return h->timed_sweeps;
+}
+
 const char* sw_kernel_name(int32_t i) { return (i >= 0 && i < K_COUNT) ? KERNEL_NAMES[i] : ""; }
 
 int sw_stage_ms(sw_handle* h, float out[4]) {

@@ -743,3 +743,16 @@ def test_potts_3x3_against_exact_enumeration_on_the_gpu(B, T, seed):
     assert abs(e - exact_E) <= 4 * de and de < 0.06, (e, de, exact_E)
     assert abs(m - exact_M) <= 4 * dm and dm < 0.06, (m, dm, exact_M)
     sw.close()
+
+
+def test_per_sweep_time_series(B):
+    sw = B.SwendsenWang(256, T_C, 1)
+    with pytest.raises(Exception):
+        sw.sweep(2); sw.sweep_ms()                   # no stage timing: SW_ESTATE
+    sw.set_stage_timing(True)
+    sw.sweep(7)
+    per = sw.sweep_ms()
+    assert per.shape == (7,) and np.all(per > 0)
+    km = sw.kernel_ms()                              # (on this path the "energy" slot is the pass after the last sweep)
+    assert abs(per.sum() - (sum(km.values()) - km["energy"])) < 1e-3 * per.sum() + 1e-3
+    sw.close()
