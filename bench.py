@@ -350,6 +350,13 @@ def main():
             unfused = {s_: {"ms": v / K6, "model_bytes_per_site": STAGE_MODEL[s_],
                             "hbm_frac": (STAGE_MODEL[s_] * N / (v / K6 * 1e-3) / 1e9 / peak) if v > 0 else None}
                        for s_, v in st6.items()}
+            # the bond stage against max(HBM time, measured Philox-only ALU ceiling)
+            alu_ms = B.sw_test_philox_ceiling(N, 20)
+            hbm_ms = STAGE_MODEL["bond"] * N / (peak * 1e9) * 1e3
+            bond_ms = unfused["bond"]["ms"]
+            unfused["bond"].update({"philox_only_ms": alu_ms, "hbm_ms_at_peak": hbm_ms,
+                                    "frac_of_binding_bound": max(alu_ms, hbm_ms) / bond_ms if bond_ms > 0 else None,
+                                    "binding_bound": "alu (Philox4x32-10)" if alu_ms > hbm_ms else "hbm"})
             unfused["note"] = ("stand-alone bond kernel: bound by the Philox4x32-10 integer work (>= 24 instructions per site), "
                                "not by its 1.25 B/site")
         except Exception as e:                       # never lose the headline line over the side measurement

@@ -226,6 +226,11 @@ int32_t    sw_batch(const sw_handle* h);
  * Philox4x32-10 of n (ctr, key) pairs, HOST arrays ctr[4n], key[2n] -> out[4n], computed ON THE GPU
  * by the same device function the kernels use. */
 int        sw_test_philox(const uint32_t* ctr, const uint32_t* key, uint32_t* out, int64_t n);
+/* The measured integer-ALU ceiling of the bond stage: ms per launch (mean of `reps`, after 3 warm-up
+ * launches, CUDA events on the default stream) of a kernel that makes the sites/2 Philox4x32-10 calls of one sweep of
+ * `sites` sites -- 16 per thread, as the bond kernels do -- XOR-reduces the words and stores one word per warp: no
+ * other memory traffic.  Synchronises. */
+int        sw_test_philox_ceiling(int64_t sites, int32_t reps, float* ms_out);
 /* Label injected bond planes: bondE/bondS HOST canonical bit-planes of one L x L lattice ->
  * labels_out[N] (HOST), through the handle's labelling kernels (h must have the same L, nb = 1). */
 int        sw_test_label(sw_handle* h, const uint32_t* bondE, const uint32_t* bondS, int32_t* labels_out);

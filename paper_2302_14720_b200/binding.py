@@ -90,6 +90,7 @@ PROTOTYPES = {
     "sw_batch": (_I32, [_VP]),
     "sw_test_philox": (C.c_int, [_VP, _VP, _VP, _I64]),
     "sw_test_label": (C.c_int, [_VP, _VP, _VP, _VP]),
+    "sw_test_philox_ceiling": (C.c_int, [C.c_int64, C.c_int32, C.POINTER(C.c_float)]),
     "sw_last_error": (C.c_char_p, []),
     "sw_version": (C.c_char_p, []),
 }
@@ -299,6 +300,12 @@ def sw_test_philox(ctr: np.ndarray, key: np.ndarray) -> np.ndarray:
     out = np.zeros_like(ctr)
     _check(lib().sw_test_philox(ctr.ctypes.data, key.ctypes.data, out.ctypes.data, len(ctr)))
     return out
+
+def sw_test_philox_ceiling(sites: int, reps: int = 20) -> float:
+    """ms per launch of the Philox-only kernel for one sweep of `sites` sites (the bond stage's ALU ceiling)."""
+    out = C.c_float(0.0)
+    _check(lib().sw_test_philox_ceiling(sites, reps, C.byref(out)))
+    return float(out.value)
 
 def sw_test_label(h, bondE_words: np.ndarray, bondS_words: np.ndarray) -> np.ndarray:
     L = lib().sw_L(_ptr(h))

@@ -1062,6 +1062,28 @@ int sw_label_passes(sw_handle* h, int32_t* passes) {
     return SW_OK;
 }
 
+int sw_test_philox_ceiling(int64_t sites, int32_t reps, float* ms_out) {
+    if (sites < 32 || sites > (1ll << 40) || reps < 1 || !ms_out) { set_err("sw_test_philox_ceiling: invalid argument"); return SW_EINVAL; }
+    const long long words = sites / 32;
+    const long long blocks = (words + GEN_THREADS - 1) / GEN_THREADS;
+    if (blocks > 0x7fffffffll) { set_err("sw_test_philox_ceiling: too many sites"); return SW_EINVAL; }
+    uint32_t* sink = nullptr;
+    SW_CUDA(cudaMalloc((void**)&sink, (size_t)(blocks * GEN_THREADS / 32) * 4));
+    cudaEvent_t e0, e1;
+    SW_CUDA(cudaEventCreate(&e0)); SW_CUDA(cudaEventCreate(&e1));
+    for (int i = 0; i < 3; ++i) k_philox_only<<<(unsigned)blocks, GEN_THREADS>>>(sink, 6u, 0u, (uint32_t)i, words);
+    SW_CUDA(cudaEventRecord(e0));
+    for (int i = 0; i < reps; ++i) k_philox_only<<<(unsigned)blocks, GEN_THREADS>>>(sink, 6u, 0u, 100u + (uint32_t)i, words);
+    SW_CUDA(cudaEventRecord(e1));
+    SW_CUDA(cudaEventSynchronize(e1));
+    float ms = 0.f;
+    SW_CUDA(cudaEventElapsedTime(&ms, e0, e1));
+    *ms_out = ms / (float)reps;
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(sink);
+    SW_CUDA(cudaGetLastError());
+    return SW_OK;
+}
+
 int sw_test_label(sw_handle* h, const uint32_t* bondE, const uint32_t* bondS, int32_t* labels_out) {
     if (!h || !bondE || !bondS || !labels_out || h->nb != 1) { set_err("sw_test_label: invalid argument"); return SW_EINVAL; }
     SW_CUDA(cudaMemcpyAsync(h->bondE, bondE, (size_t)h->words * 4, cudaMemcpyHostToDevice, h->stream));

@@ -220,6 +220,25 @@ k_pack_spins(const int8_t* __restrict__ spins, uint32_t* __restrict__ bits, int 
     bits[(size_t)blockIdx.y * words + w] = b;
 }
 
+// ---- the ALU ceiling of the bond stage: the Philox4x32-10 draws of a sweep and nothing else.
+//      One thread per 32-site word = 16 calls, as in the bond kernels; the words are XOR-reduced and stored once per
+//      warp (so the calls cannot be removed), no other memory traffic ------------------------------------------------
+__global__ void __launch_bounds__(GEN_THREADS)
+k_philox_only(uint32_t* __restrict__ sink, uint32_t key0, uint32_t key1, uint32_t tlo, long long words) {
+    const long long w = (long long)blockIdx.x * GEN_THREADS + threadIdx.x;
+    uint32_t acc = 0;
+    if (w < words) {
+        const PhiloxKey key(key0, key1);
+#pragma unroll
+        for (int c = 0; c < 16; ++c) {
+            const uint4 r = philox4x32_10((uint32_t)w * 16u + c, tlo, 0u, TAG_BOND, key);
+            acc ^= r.x ^ r.y ^ r.z ^ r.w;
+        }
+    }
+    acc = __reduce_xor_sync(0xffffffffu, acc);
+    if ((threadIdx.x & 31) == 0) sink[w >> 5] = acc;
+}
+
 // ---- sweep control -------------------------------------------------------------------------------
 __global__ void k_set_ctl(Ctl* ctl, unsigned long long t, uint32_t slot, uint32_t cap) {
     ctl->t = t; ctl->slot = slot; ctl->cap = cap;

@@ -756,3 +756,10 @@ def test_per_sweep_time_series(B):
     km = sw.kernel_ms()                              # (on this path the "energy" slot is the pass after the last sweep)
     assert abs(per.sum() - (sum(km.values()) - km["energy"])) < 1e-3 * per.sum() + 1e-3
     sw.close()
+
+
+def test_philox_ceiling_hook(B):
+    ms = B.sw_test_philox_ceiling(1 << 22, 5)
+    assert 0.0 < ms < 50.0
+    with pytest.raises(Exception):
+        B.sw_test_philox_ceiling(8, 1)
