@@ -419,22 +419,43 @@ int launch_label(sw_handle* h) {
     }
 }
 
+// Potts fast path: k_bond_label<4, 64, FUSE, POTTS> (equal-colour masks from the int8 plane), then the node merge
+int launch_bond_label_potts(sw_handle* h) {
+    constexpr int NW = 4, TH = 64, TW = 32 * NW, CAP = 2 * (TW + TH);
+    const int tiles = h->N / (TW * TH);
+    constexpr size_t smem = (size_t)TW * TH * sizeof(int);
+    static bool attr_done = false;
+    if (!attr_done) {
+        SW_CUDA(cudaFuncSetAttribute(k_bond_label<NW, TH, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr_done = true;
+    }
+    SW_MARK(h, K_BONDLABEL);
+    k_bond_label<NW, TH, true, true><<<dim3(tiles, h->nb), NW * TH, smem, h->stream>>>(
+        reinterpret_cast<const uint32_t*>(h->spins), h->bondE, h->bondS, h->lab16, h->nodes, h->ocount, h->bslot,
+        h->series, h->lat, h->ctl, h->L, h->N, h->words, h->nb, 0);
+    const size_t nedge = (size_t)h->L * (h->L / TW + h->L / TH);
+    SW_MARK(h, K_MERGE);
+    k_merge_nodes<TW, TH><<<grid1(nedge, 256, h->nb), 256, 0, h->stream>>>(h->nodes, h->bslot, h->L / TW, h->L / TH);
+    SW_MARK(h, K_SIZES);
+    k_roots_nodes<CAP><<<grid1((size_t)tiles * 32, 256, h->nb), 256, 0, h->stream>>>(h->nodes, h->ocount, tiles);
+    h->launches += 3;
+    return SW_OK;
+}
+
 // Potts sweep (sw_potts.cuh): bonds between equal colours, labels (generic union-find, or path 11), a colour per
 // cluster, observables
 int launch_sweep_potts(sw_handle* h, int64_t k) {
     int rc;
     h->cur_sweep = k; h->ev_cursor = 0;
-    SW_MARK(h, K_BOND);
-    if (h->tile == SCAN_4x64)
-        k_bond_rows_potts<<<grid1(h->words, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(
-            h->spins, h->bondE, h->bondS, h->lat, h->ctl, h->L, h->N, h->words);
-    else
+    if (h->tile != SCAN_4x64) {
+        SW_MARK(h, K_BOND);
         k_bond_generic<<<grid1(h->words, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(
             h->spins, h->bondE, h->bondS, h->lat, h->ctl, h->L, h->N, h->words);
-    h->launches += 1;
+        h->launches += 1;
+    }
     if (h->tile == SCAN_4x64) {
-        // fast path: scan-line tile labelling from the bond planes + node merge, colour per tile root
-        if ((rc = launch_bond_label_scan<4, 64>(h, false, false))) return rc;
+        // fast path: fused bond draw + scan-line tile labelling, node merge, colour per tile root
+        if ((rc = launch_bond_label_potts(h))) return rc;
         SW_MARK(h, K_FLIPTILE);
         k_assign16_potts<4, 64><<<dim3(h->N / (128 * 64), h->nb), 256, 0, h->stream>>>(
             h->spins, h->lab16, h->nodes, h->ocount, h->series, h->lat, h->ctl, make_div(h->L), h->q, h->L, h->N, h->nb);

@@ -98,42 +98,11 @@ k_observe_potts(const int8_t* __restrict__ colours, Rec* __restrict__ rec, int* 
     }
 }
 
-// bond formation on rows (L a multiple of 32), PAPER.md:37-39 generalised: thread w owns sites 32w .. 32w+31 of one
-// row; equal-colour masks from byte-wise compares with the East-shifted and the South bytes, draws as bond_draws
-__global__ void __launch_bounds__(GEN_THREADS)
-k_bond_rows_potts(const int8_t* __restrict__ colours, uint32_t* __restrict__ bondE, uint32_t* __restrict__ bondS,
-                  const Lat* __restrict__ lat, const Ctl* __restrict__ ctl, int L, int N, int words) {
-    const int w = blockIdx.x * GEN_THREADS + threadIdx.x;
-    if (w >= words) return;
-    const int wpr = L >> 5;
-    const int y = w / wpr, xw = w - y * wpr;
-    const int8_t* s = colours + (size_t)blockIdx.y * N;
-    const int8_t* row  = s + (size_t)y * L + xw * 32;
-    const int8_t* rowS = s + (size_t)(y + 1 == L ? 0 : y + 1) * L + xw * 32;
-    const uint4 a0 = *reinterpret_cast<const uint4*>(row),  a1 = *reinterpret_cast<const uint4*>(row + 16);
-    const uint4 b0 = *reinterpret_cast<const uint4*>(rowS), b1 = *reinterpret_cast<const uint4*>(rowS + 16);
-    const uint32_t nx = (uint8_t)s[(size_t)y * L + (xw + 1 == wpr ? 0 : (xw + 1) * 32)];
-    const uint32_t a[9] = { a0.x, a0.y, a0.z, a0.w, a1.x, a1.y, a1.z, a1.w, nx };
-    const uint32_t b[8] = { b0.x, b0.y, b0.z, b0.w, b1.x, b1.y, b1.z, b1.w };
-    uint32_t eqE = 0, eqS = 0;
-#pragma unroll
-    for (int k = 0; k < 8; ++k) {
-        eqE |= neg_nibble(__vcmpeq4(a[k], __funnelshift_r(a[k], a[k + 1], 8))) << (4 * k);
-        eqS |= neg_nibble(__vcmpeq4(a[k], b[k])) << (4 * k);
-    }
-    const Lat la = lat[blockIdx.y];
-    const PhiloxKey key(la.key0, la.key1);
-    const unsigned long long t = ctl->t;
-    uint32_t dE, dS;
-    bond_draws((uint32_t)w, (uint32_t)t, (uint32_t)(t >> 32), la.thr, key, dE, dS);
-    bondE[(size_t)blockIdx.y * words + w] = eqE & dE;
-    bondS[(size_t)blockIdx.y * words + w] = eqS & dS;
-}
-
 // ---------------------------------------------------------------------------------------------------
-// Fast path (L a multiple of 128): the scan-line labelling of sw_scan.cuh runs on the Potts bond planes
-// (k_bond_label<4, 64, FUSE = false>, k_merge_nodes, k_roots_nodes), leaving the 16-bit tile-local root of every
-// site and the node array of the open tile roots.  k_assign16_potts is the Potts counterpart of k_flip16: one
+// Fast path (L a multiple of 128): the fused bond + scan-line labelling kernel of sw_scan.cuh in its POTTS variant
+// (k_bond_label<4, 64, FUSE, POTTS>: equal-colour masks by byte-wise compares of the int8 plane, same draws), then
+// k_merge_nodes and k_roots_nodes, leaving the 16-bit tile-local root of every site and the node array of the open
+// tile roots.  k_assign16_potts is the Potts counterpart of k_flip16: one
 // colour per TILE ROOT in shared memory (a Philox call per root: closed roots draw for their own site index, open
 // ones for the minimum site index under their root node), then every site looks its colour up by its 16-bit root.
 // Also counts the clusters that span tiles and maximises their sizes, as k_flip16 does.

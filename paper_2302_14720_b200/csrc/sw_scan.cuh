@@ -62,7 +62,8 @@ __device__ __forceinline__ int div_l(int v, const DivL& D) {
 
 // FUSE = true: phase 1 draws the bonds (a1 fused into a2).  FUSE = false: phase 1 reads the bond planes
 // that k_bond_rows (or a test) wrote -- per-stage timing (BASELINE config 3) and labelling-only tests.
-template <int NW, int TH, bool FUSE>
+// POTTS (with FUSE; sw_potts.cuh): `sbits` is the int8 COLOUR plane; a bond needs equal colours (byte compares).
+template <int NW, int TH, bool FUSE, bool POTTS = false>
 __global__ void __launch_bounds__(NW * TH)
 k_bond_label(const uint32_t* __restrict__ sbits, uint32_t* bondE, uint32_t* bondS,
              uint16_t* __restrict__ lab16, int4* __restrict__ nodes, int* __restrict__ ocount,
@@ -86,6 +87,7 @@ k_bond_label(const uint32_t* __restrict__ sbits, uint32_t* bondE, uint32_t* bond
     const int wprL = L >> 5;
     // FUSE: the spins come bit-packed (bit 1 = +1; word w = sites 32w .. 32w+31), 1/8 of the int8 plane's bytes
     const uint32_t* sb = sbits + (size_t)blockIdx.y * words;
+    const int8_t* col = reinterpret_cast<const int8_t*>(sbits) + (size_t)blockIdx.y * N;   // (POTTS)
     const Lat la = lat[blockIdx.y];
     const unsigned long long t = ctl->t;
     const uint32_t tlo = (uint32_t)t, thi = (uint32_t)(t >> 32);
@@ -113,11 +115,28 @@ k_bond_label(const uint32_t* __restrict__ sbits, uint32_t* bondE, uint32_t* bond
             const int y = y0 + row;
             const int xw = (x0 >> 5) + wx;
             const int w = y * wprL + xw;                              // word index within the lattice
-            const uint32_t own = ~sb[w], south = ~sb[(y + 1 == L ? 0 : y + 1) * wprL + xw];   // bit = 1: spin -1
-            const uint32_t nxw = sb[y * wprL + (xw + 1 == wprL ? 0 : xw + 1)];
-            const uint32_t eastm = (own >> 1) | ((~nxw & 1u) << 31);
-            const uint32_t eqE = ~(own ^ eastm), eqS = ~(own ^ south);
-            if (obs_prev) {
+            uint32_t own = 0, eqE = 0, eqS = 0;
+            if (POTTS) {
+                const int8_t* r0 = col + (size_t)y * L + xw * 32;
+                const int8_t* r1 = col + (size_t)(y + 1 == L ? 0 : y + 1) * L + xw * 32;
+                const uint4 a0 = *reinterpret_cast<const uint4*>(r0), a1 = *reinterpret_cast<const uint4*>(r0 + 16);
+                const uint4 b0 = *reinterpret_cast<const uint4*>(r1), b1 = *reinterpret_cast<const uint4*>(r1 + 16);
+                const uint32_t nx = (uint8_t)col[(size_t)y * L + (xw + 1 == wprL ? 0 : (xw + 1) * 32)];
+                const uint32_t a[9] = { a0.x, a0.y, a0.z, a0.w, a1.x, a1.y, a1.z, a1.w, nx };
+                const uint32_t b[8] = { b0.x, b0.y, b0.z, b0.w, b1.x, b1.y, b1.z, b1.w };
+#pragma unroll
+                for (int k = 0; k < 8; ++k) {
+                    eqE |= neg_nibble(__vcmpeq4(a[k], __funnelshift_r(a[k], a[k + 1], 8))) << (4 * k);
+                    eqS |= neg_nibble(__vcmpeq4(a[k], b[k])) << (4 * k);
+                }
+            } else {
+                own = ~sb[w];                                            // bit = 1: spin -1
+                const uint32_t south = ~sb[(y + 1 == L ? 0 : y + 1) * wprL + xw];
+                const uint32_t nxw = sb[y * wprL + (xw + 1 == wprL ? 0 : xw + 1)];
+                const uint32_t eastm = (own >> 1) | ((~nxw & 1u) << 31);
+                eqE = ~(own ^ eastm); eqS = ~(own ^ south);
+            }
+            if (!POTTS && obs_prev) {
                 // a7 for free: the equal-pair masks of the bond test are the energy of the
                 // configuration the previous sweep left: E = (#edges) - 2 (#equal pairs), M = N - 2 (#down)
                 const int eo = warp_sum_i(64 - 2 * (__popc(eqE) + __popc(eqS)));
@@ -145,7 +164,8 @@ k_bond_label(const uint32_t* __restrict__ sbits, uint32_t* bondE, uint32_t* bond
                 const int i = yn * L + x;                                  // even site; call covers i, i + 1
                 const uint4 r = philox4x32_10((uint32_t)(i >> 1), tlo, thi, TAG_BOND, key);
                 const int id = y0 * L + x;                                 // (x is even: both sites in one word)
-                const uint32_t eq = ~((sb[i >> 5] >> (i & 31)) ^ (sb[id >> 5] >> (id & 31)));
+                const uint32_t eq = POTTS ? ((col[i] == col[id] ? 1u : 0u) | (col[i + 1] == col[id + 1] ? 2u : 0u))
+                                          : ~((sb[i >> 5] >> (i & 31)) ^ (sb[id >> 5] >> (id & 31)));
                 const uint32_t bits = (eq & ((r.y < la.thr ? 1u : 0u) | (r.w < la.thr ? 2u : 0u))) & 3u;
                 if (bits) atomicOr(&nIn[(2 * j) >> 5], bits << ((2 * j) & 31));
             } else {
@@ -154,7 +174,8 @@ k_bond_label(const uint32_t* __restrict__ sbits, uint32_t* bondE, uint32_t* bond
                 const int i = (y0 + row) * L + xwst;
                 const uint4 r = philox4x32_10((uint32_t)(i >> 1), tlo, thi, TAG_BOND, key);
                 const int ie = (y0 + row) * L + x0;
-                if (!(((sb[i >> 5] >> (i & 31)) ^ (sb[ie >> 5] >> (ie & 31))) & 1u) && r.z < la.thr)
+                const bool same = POTTS ? col[i] == col[ie] : !(((sb[i >> 5] >> (i & 31)) ^ (sb[ie >> 5] >> (ie & 31))) & 1u);
+                if (same && r.z < la.thr)
                     atomicOr(&wIn[row >> 5], 1u << (row & 31));
             }
         }
