@@ -260,6 +260,9 @@ int launch_label_tiled(sw_handle* h) {
     return SW_OK;
 }
 
+// k_roots_nodes: 4 warps per tile while the whole batch has fewer tiles than the GPU holds warps
+inline int roots_warps_per_tile(const sw_handle* h, int tiles) { return (long long)tiles * h->nb < 4096 ? 4 : 1; }
+
 // fast path: fused bond + scan-line tile labelling, global merge, open roots (a1-a3)
 template <int NW, int TH>
 int launch_bond_label_scan(sw_handle* h, bool fused, bool obs_prev) {
@@ -290,8 +293,9 @@ int launch_bond_label_scan(sw_handle* h, bool fused, bool obs_prev) {
     k_merge_nodes<TW, TH><<<grid1(nedge, 256, h->nb), 256, 0, h->stream>>>(
         h->nodes, h->bslot, h->L / TW, h->L / TH);
     SW_MARK(h, K_SIZES);
-    k_roots_nodes<CAP><<<grid1((size_t)tiles * 32, 256, h->nb), 256, 0, h->stream>>>(
-        h->nodes, h->ocount, tiles);
+    const int wpt = roots_warps_per_tile(h, tiles);
+    k_roots_nodes<CAP><<<grid1((size_t)tiles * wpt * 32, 256, h->nb), 256, 0, h->stream>>>(
+        h->nodes, h->ocount, tiles, wpt);
     h->launches += 3;
     return SW_OK;
 }
@@ -437,7 +441,8 @@ int launch_bond_label_potts(sw_handle* h) {
     SW_MARK(h, K_MERGE);
     k_merge_nodes<TW, TH><<<grid1(nedge, 256, h->nb), 256, 0, h->stream>>>(h->nodes, h->bslot, h->L / TW, h->L / TH);
     SW_MARK(h, K_SIZES);
-    k_roots_nodes<CAP><<<grid1((size_t)tiles * 32, 256, h->nb), 256, 0, h->stream>>>(h->nodes, h->ocount, tiles);
+    const int wpt = roots_warps_per_tile(h, tiles);
+    k_roots_nodes<CAP><<<grid1((size_t)tiles * wpt * 32, 256, h->nb), 256, 0, h->stream>>>(h->nodes, h->ocount, tiles, wpt);
     h->launches += 3;
     return SW_OK;
 }

@@ -423,17 +423,19 @@ k_merge_nodes(int4* nodes, const uint16_t* __restrict__ bslot, int tilesX, int t
 // After the merge: every open piece adds its size and its site index to the node it hangs under (sum -> cluster
 // size, min -> canonical label) and points straight at it.  Pieces are combined per root inside the warp first,
 // and the root with the largest sum of the first round is carried in registers across rounds: at T_c one cluster
-// owns many pieces in every tile.  One warp per tile.
+// owns many pieces in every tile.  wpt warps per tile (1 for large lattices; 4 for small ones, where the kernel is
+// the latency of one warp walking its tile's ~100 pieces 32 at a time): warp `sub` takes rounds sub, sub + wpt, ...
 template <int CAP>
 __global__ void __launch_bounds__(256)
-k_roots_nodes(int4* nodes, const int* __restrict__ ocount, int tiles) {
-    const int tile = blockIdx.x * 8 + (threadIdx.x >> 5);
+k_roots_nodes(int4* nodes, const int* __restrict__ ocount, int tiles, int wpt) {
+    const int gw = blockIdx.x * 8 + (threadIdx.x >> 5);
+    const int tile = gw / wpt, sub = gw - tile * wpt;
     const int lane = threadIdx.x & 31;
     if (tile >= tiles) return;                              // (warp-uniform)
     int4* nd = nodes + (size_t)blockIdx.y * tiles * CAP;
     const int n = ocount[(size_t)blockIdx.y * tiles + tile];
     int hot = -1, hotacc = 0, hotmin = 0x7fffffff;
-    for (int e0 = 0; e0 < n; e0 += 32) {
+    for (int e0 = 32 * sub; e0 < n; e0 += 32 * wpt) {
         const int e = e0 + lane;
         const bool on = e < n;
         int root = -1 - lane, add = 0, g = 0x7fffffff;      // idle lanes: distinct keys, nothing to add
@@ -451,7 +453,7 @@ k_roots_nodes(int4* nodes, const int* __restrict__ ocount, int tiles) {
         const unsigned grp = __match_any_sync(0xffffffffu, root);
         const int tot = __reduce_add_sync(grp, add);
         const int gm = __reduce_min_sync(grp, g);
-        if (e0 == 0) {                                      // choose the hot root
+        if (e0 == 32 * sub) {                               // (my first round) choose the hot root
             const int best = __reduce_max_sync(0xffffffffu, tot);
             const unsigned who = __ballot_sync(0xffffffffu, tot == best && on);
             if (who) hot = __shfl_sync(0xffffffffu, root, __ffs(who) - 1);
