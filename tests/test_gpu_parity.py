@@ -763,3 +763,23 @@ def test_philox_ceiling_hook(B):
     assert 0.0 < ms < 50.0
     with pytest.raises(Exception):
         B.sw_test_philox_ceiling(8, 1)
+
+
+def test_temperature_scan_batch_against_kaufman_on_the_gpu(B):
+    """BASELINE configs[4] in small (the paper's Fig. 5): a batch of lattices at temperatures across the
+    transition, one launch per stage; the mean energy of every lattice against Kaufman's exact finite-lattice value."""
+    L, nb, therm, n = 128, 16, 300, 3000
+    Ts = [1.5 + b * 2.0 / (nb - 1) for b in range(nb)]
+    sw = B.SwendsenWang(L, Ts, [1000 + b for b in range(nb)])
+    sw.sweep(therm)
+    sw.sweep(n)
+    ser = sw.series()
+    assert ser.shape == (n, nb, 4)
+    worst = 0.0
+    for b, T in enumerate(Ts):
+        u, du = ex.binned_mean_err(ser[:, b, 0] / (L * L), nbins=30)
+        exact = float(ex.kaufman_u(L, T))
+        worst = max(worst, abs(u - exact) / du)
+        assert abs(u - exact) <= 4.5 * du and du < 3e-3, (T, u, du, exact)
+    assert worst > 0.0
+    sw.close()
