@@ -368,7 +368,15 @@ class SwendsenWang:
         return self._view(sw_spins(self.h), self.nb * self.N).view(self.torch.int8).view(self.nb, self.L, self.L)
 
     def labels(self):
-        return self._view(sw_labels(self.h), self.nb * self.N * 4).view(self.torch.int32).view(self.nb, self.L, self.L)
+        """Flat int32 labels of the last sweep: a zero-copy tensor over the library's own label array (allocated by the
+        library on first use, outside the torch workspace; valid until the next sweep / sw_destroy)."""
+        ptr = sw_labels(self.h)
+
+        class _Raw:                                   # (__cuda_array_interface__: pointer + shape, no copy)
+            __cuda_array_interface__ = {"shape": (self.nb, self.L, self.L), "typestr": "<i4", "data": (ptr, False),
+                                        "version": 2, "strides": None}
+        with self.torch.cuda.device(self.device):
+            return self.torch.as_tensor(_Raw(), device=self.device)
 
     def bonds(self):
         e, s = sw_bonds(self.h)

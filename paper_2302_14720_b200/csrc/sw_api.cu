@@ -57,26 +57,24 @@ constexpr int EV_PER_SWEEP = K_COUNT + 1;
 inline size_t align_up(size_t v) { return (v + ALIGN - 1) / ALIGN * ALIGN; }
 
 // tile shapes of the fast path
-enum TileKind { TILE_NONE = 0, TILE_64x64 = 1, TILE_256x32 = 2, SCAN_2 = 3, SCAN_4 = 4, SCAN_8 = 5, SCAN_8x64 = 6, SCAN_4x64 = 7 };
-// width in 32-site words of the 32-row tiles the scan-line kernel and k_flip16 share
-inline int scan_nw(TileKind k) { return k == SCAN_2 ? 2 : (k == SCAN_4 || k == SCAN_4x64) ? 4 : (k == SCAN_8 || k == SCAN_8x64) ? 8 : 0; }
-using Cfg64 = TileCfg<64, 64>;
-using Cfg256 = TileCfg<256, 32>;
+// ROWS64: row kernels on the int8 plane + flat labels (path 11); SCAN_2: 64 x 32 tiles (L a multiple of 64 only);
+// SCAN_4x64: 128 x 64 tiles (L a multiple of 128: the headline shape)
+enum TileKind { TILE_NONE = 0, ROWS64 = 1, SCAN_2 = 3, SCAN_4x64 = 7 };
+// width in 32-site words of the tiles the scan-line kernel and k_flip16 share (0: not a scan tile)
+inline int scan_nw(TileKind k) { return k == SCAN_2 ? 2 : k == SCAN_4x64 ? 4 : 0; }
+constexpr int MAX_DEV = 64;            // per-device "attribute set" flags of the kernels with opt-in shared memory
 
 struct Layout {        // byte offsets into the workspace
-    size_t spins, sbits, bondE, bondS, D, label, lab16, gsize, olist, ocount, nodes, bslot, lat, ctl, rec_now, mom, series, total;
+    size_t spins, sbits, bondE, bondS, D, lab16, ocount, nodes, bslot, lat, ctl, rec_now, mom, series, total;
 };
 
-size_t olist_entries(int L) {          // per lattice, maximum over the tile shapes usable for this L
-    size_t n = 0;
+size_t node_entries(int L) {           // per lattice: CAP = 2 (TW + TH) entries per tile of the shape this L runs on
     const size_t N = (size_t)L * L;
-    if (L % 64 == 0) n = std::max(n, N / Cfg64::SITES * Cfg64::CAP);
-    if (L % 256 == 0) n = std::max(n, N / Cfg256::SITES * Cfg256::CAP);
-    for (int nw : {2, 4, 8})                                   // scan tiles: 32 nw x 32 sites
-        if (L % (32 * nw) == 0) n = std::max(n, N / (32 * nw * 32) * (size_t)(2 * (32 * nw + 32)));   // (the 64-row tile needs less)
-    return n;
+    if (L % 128 == 0) return N / (128 * 64) * (size_t)(2 * (128 + 64));
+    if (L % 64 == 0) return N / (64 * 32) * (size_t)(2 * (64 + 32));
+    return 0;
 }
-size_t tiles_max(int L) { return L % 64 == 0 ? (size_t)L * L / (64 * 32) : 0; }
+size_t tiles_max(int L) { return L % 128 == 0 ? (size_t)L * L / (128 * 64) : L % 64 == 0 ? (size_t)L * L / (64 * 32) : 0; }
 
 DivL make_div(int d) {          // q = (v * m) >> p is exact for 0 <= v < 2^30 (error term < 1/d)
     int k = 0; while ((1 << k) < d) ++k;
@@ -93,13 +91,11 @@ Layout make_layout(int L, int nb) {
     o.bondE = p;   p = align_up(p + (size_t)nb * words * 4);
     o.bondS = p;   p = align_up(p + (size_t)nb * words * 4);
     o.D = p;       p = align_up(p + (size_t)nb * ((words + 3) / 4 * 4) * 4);
-    o.label = p;   p = align_up(p + (size_t)nb * N * 4);
+    // (the flat int32 labels and the generic paths' size array, 4 B/site each, are allocated on first use: need_label)
     o.lab16 = p;   p = align_up(p + (L % 64 == 0 ? (size_t)nb * N * 2 : 0));
-    o.gsize = p;   p = align_up(p + (size_t)nb * N * 4);
-    o.olist = p;   p = align_up(p + (size_t)nb * olist_entries(L) * sizeof(int2));
     o.ocount = p;  p = align_up(p + (size_t)nb * tiles_max(L) * 4);
-    o.nodes = p;   p = align_up(p + (size_t)nb * olist_entries(L) * 16);     // node array of the scan path
-    o.bslot = p;   p = align_up(p + (size_t)nb * olist_entries(L) * 2);
+    o.nodes = p;   p = align_up(p + (size_t)nb * node_entries(L) * 16);     // node array of the scan path
+    o.bslot = p;   p = align_up(p + (size_t)nb * node_entries(L) * 2);
     o.lat = p;     p = align_up(p + (size_t)nb * sizeof(Lat));
     o.ctl = p;     p = align_up(p + sizeof(Ctl));
     o.rec_now = p; p = align_up(p + (size_t)nb * sizeof(Rec));
@@ -135,12 +131,14 @@ uint32_t host_threshold_potts(double T) {
 
 struct sw_handle {
     int L = 0, nb = 0, N = 0, words = 0;
+    int dev = 0;                     // the CUDA device the handle lives on: every entry point switches to it
     bool owns_ws = false;
     char* ws = nullptr; size_t ws_bytes = 0;
     uint32_t* sbits = nullptr;       // bit-packed spins: bit 1 = +1.  The fused scan path keeps the state HERE
     bool i8_valid = true, bits_valid = false;      // which of the two spin planes holds the current configuration
     int8_t* spins = nullptr; uint32_t *bondE = nullptr, *bondS = nullptr, *D = nullptr;
-    int *label = nullptr, *gsize = nullptr, *ocount = nullptr; int2* olist = nullptr;
+    int *label = nullptr, *gsize = nullptr;          // flat labels / cluster sizes, 4 B/site each: allocated on first use
+    int* ocount = nullptr;
     uint16_t* lab16 = nullptr;       // tile-local root index of every site (scan path)
     int4* nodes = nullptr;           // union-find over open tile roots: (parent, size, min site, site)
     uint16_t* bslot = nullptr;       // per tile: slot of the root of each border site
@@ -162,6 +160,7 @@ struct sw_handle {
     bool rec_valid = false;        // the last series slot holds E, M of the current spins
     int64_t last_n = 0;
     int path = 0; TileKind tile = TILE_NONE;
+    TileKind lab_tile = TILE_NONE;  // tile shape of the sweep whose 16-bit roots are pending (flattened on demand)
     bool timing = false; std::vector<cudaEvent_t> ev; int64_t timed_sweeps = 0;
     cudaEvent_t ev_tail[2] = { nullptr, nullptr };   // around the trailing k_observe_rows of a call
     // CUDA graphs of the steady sweep (every sweep of a call but the first launches the same kernels with the
@@ -178,25 +177,47 @@ struct sw_handle {
 
 namespace {
 
+// paths: 0 the fast path (fused bond + scan-line labelling on 128 x 64 tiles when L is a multiple of 128, on 64 x 32
+// tiles when it is a multiple of 64, generic kernels otherwise); 1 generic kernels; 6 the fast path's tiles with a
+// stand-alone bond kernel on the int8 plane (per-stage timing); 11 the paper's label-equivalence labelling
 TileKind pick_tile(int L, int path) {
     if (path == 1) return TILE_NONE;
-    if (path == 2) return L % 64 == 0 ? TILE_64x64 : TILE_NONE;
-    if (path == 3) return L % 256 == 0 ? TILE_256x32 : TILE_NONE;
-    if (path == 4) return L % 64 == 0 ? SCAN_2 : TILE_NONE;
-    if (path == 5) return L % 128 == 0 ? SCAN_4 : TILE_NONE;
-    if (path == 7) return L % 256 == 0 ? SCAN_8 : TILE_NONE;
-    if (path == 8) return L % 256 == 0 ? SCAN_8x64 : TILE_NONE;
-    if (path == 9) return L % 128 == 0 ? SCAN_4x64 : TILE_NONE;
-    if (path == 11) return L % 64 == 0 ? TILE_64x64 : TILE_NONE;      // row kernels for bond / flip / energy; labels: sw_equiv.cuh
+    if (path == 11) return L % 64 == 0 ? ROWS64 : TILE_NONE;          // row kernels for bond / flip / energy; labels: sw_equiv.cuh
     if (L % 128 == 0) return SCAN_4x64;
     if (L % 64 == 0) return SCAN_2;
     return TILE_NONE;
 }
+bool valid_path(int path) { return path == 0 || path == 1 || path == 6 || path == 11; }
 
 // Potts handles: the scan-line path on 128 x 64 tiles when L allows it (path 0), else the generic kernels
 TileKind potts_tile(int L, int path) { return (path == 0 && L % 128 == 0) ? SCAN_4x64 : TILE_NONE; }
 
 inline dim3 grid1(size_t n, int threads, int nb) { return dim3((unsigned)((n + threads - 1) / threads), (unsigned)nb); }
+
+// every entry point runs on the handle's device, whatever device is current in the calling thread
+struct DevGuard {
+    int prev = -1; bool switched = false;
+    explicit DevGuard(int dev) {
+        if (cudaGetDevice(&prev) == cudaSuccess && prev != dev) switched = cudaSetDevice(dev) == cudaSuccess;
+    }
+    ~DevGuard() { if (switched) cudaSetDevice(prev); }
+    DevGuard(const DevGuard&) = delete; DevGuard& operator=(const DevGuard&) = delete;
+};
+
+// flat int32 labels (sw_labels, generic / path-11 labelling) and the generic paths' cluster-size array: 4 B/site each,
+// allocated the first time a path needs them, so that the fast path's footprint stays at ~4.5 B/site
+int need_label(sw_handle* h) {
+    if (h->label) return SW_OK;
+    cudaError_t e = cudaMalloc((void**)&h->label, (size_t)h->nb * h->N * sizeof(int));
+    if (e != cudaSuccess) { (void)cudaGetLastError(); set_err("cudaMalloc of the label array (%zu bytes) failed: %s", (size_t)h->nb * h->N * sizeof(int), cudaGetErrorString(e)); h->label = nullptr; return SW_ENOMEM; }
+    return SW_OK;
+}
+int need_gsize(sw_handle* h) {
+    if (h->gsize) return SW_OK;
+    cudaError_t e = cudaMalloc((void**)&h->gsize, (size_t)h->nb * h->N * sizeof(int));
+    if (e != cudaSuccess) { (void)cudaGetLastError(); set_err("cudaMalloc of the size array (%zu bytes) failed: %s", (size_t)h->nb * h->N * sizeof(int), cudaGetErrorString(e)); h->gsize = nullptr; return SW_ENOMEM; }
+    return SW_OK;
+}
 
 // the two spin planes: the fused scan path sweeps on the bit plane, everything else on the int8 plane
 bool sweeps_on_bits(const sw_handle* h) { return scan_nw(h->tile) && h->path != 6 && !h->q; }
@@ -224,57 +245,28 @@ int mark(sw_handle* h, int kid) {
 }
 #define SW_MARK(h, kid) do { int rc_ = mark((h), (kid)); if (rc_) return rc_; } while (0)
 
-template <int TW, int TH>
-size_t tile_smem_bytes() {
-    using C = TileCfg<TW, TH>;
-    return (size_t)C::SITES * 8 + (size_t)C::RW * 8 + C::WPR * 4 + TH + 16;
-}
-
-template <int TW, int TH>
-int launch_label_tiled(sw_handle* h) {
-    using C = TileCfg<TW, TH>;
-    const int tiles = h->N / C::SITES;
-    static bool attr_done = false;
-    const size_t smem = tile_smem_bytes<TW, TH>();
-    if (!attr_done) {
-        SW_CUDA(cudaFuncSetAttribute(k_tile_label<TW, TH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_done = true;
-    }
-    SW_MARK(h, K_TILE);
-    k_tile_label<TW, TH><<<dim3(tiles, h->nb), C::THREADS, smem, h->stream>>>(
-        h->label, h->bondE, h->bondS, h->olist, h->ocount, h->series, h->ctl, h->L, h->N, h->words, h->nb);
-    const size_t nedge = (size_t)h->L * (h->L / TW + h->L / TH);
-    SW_MARK(h, K_MERGE);
-    k_merge_tiled<TW, TH><<<grid1(nedge, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
-        h->label, h->bondE, h->bondS, h->L, h->N, h->words);
-    SW_MARK(h, K_SIZES);
-    k_roots_open<C::CAP><<<grid1((size_t)tiles * 32, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
-        h->label, h->olist, h->ocount, h->gsize, h->series, h->ctl, tiles, h->N, h->nb, 0);
-    SW_MARK(h, K_COMPRESS);
-    k_compress_tiled<<<grid1((size_t)h->N / 4, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
-        h->label, h->series, h->ctl, h->N, h->nb, 1);
-    SW_MARK(h, K_SIZES_RESET);
-    k_sizes_reset<C::CAP><<<grid1((size_t)tiles * 32, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
-        h->olist, h->ocount, h->gsize, tiles, h->N);
-    h->launches += 5;
-    return SW_OK;
-}
-
 // k_roots_nodes: 4 warps per tile while the whole batch has fewer tiles than the GPU holds warps
 inline int roots_warps_per_tile(const sw_handle* h, int tiles) { return (long long)tiles * h->nb < 4096 ? 4 : 1; }
+
+// opt-in dynamic shared memory, once per kernel and device
+template <typename K>
+int opt_in_smem(K kernel, size_t smem, bool* done, int dev) {
+    if (dev < 0 || dev >= MAX_DEV || !done[dev]) {
+        SW_CUDA(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        if (dev >= 0 && dev < MAX_DEV) done[dev] = true;
+    }
+    return SW_OK;
+}
 
 // fast path: fused bond + scan-line tile labelling, global merge, open roots (a1-a3)
 template <int NW, int TH>
 int launch_bond_label_scan(sw_handle* h, bool fused, bool obs_prev) {
     constexpr int TW = 32 * NW, CAP = 2 * (TW + TH);
     const int tiles = h->N / (TW * TH);
-    constexpr size_t smem = (size_t)TW * TH * sizeof(int);          // the parent array (dynamic: > 48 KB at TH = 64)
-    static bool attr_done = false;
-    if (!attr_done) {
-        SW_CUDA(cudaFuncSetAttribute(k_bond_label<NW, TH, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        SW_CUDA(cudaFuncSetAttribute(k_bond_label<NW, TH, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_done = true;
-    }
+    constexpr size_t smem = (size_t)TW * TH * sizeof(uint32_t);      // the parent array (dynamic: 32 KB at 128 x 64)
+    static bool done[2][MAX_DEV];
+    { int rc = opt_in_smem(k_bond_label<NW, TH, true>, smem, done[0], h->dev); if (rc) return rc; }
+    { int rc = opt_in_smem(k_bond_label<NW, TH, false>, smem, done[1], h->dev); if (rc) return rc; }
     if (fused) {
         SW_MARK(h, K_BONDLABEL);
         k_bond_label<NW, TH, true><<<dim3(tiles, h->nb), NW * TH, smem, h->stream>>>(
@@ -305,22 +297,17 @@ int launch_flatten_scan(sw_handle* h) {
     constexpr int TW = 32 * NW;
     const int tiles = h->N / (TW * TH);
     constexpr size_t smem = (size_t)TW * TH * sizeof(int);
-    static bool attr_done = false;
-    if (!attr_done) {
-        SW_CUDA(cudaFuncSetAttribute(k_labels16<NW, TH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_done = true;
-    }
+    static bool done[MAX_DEV];
+    { int rc = opt_in_smem(k_labels16<NW, TH>, smem, done, h->dev); if (rc) return rc; }
+    { int rc = need_label(h); if (rc) return rc; }
     k_labels16<NW, TH><<<dim3(tiles, h->nb), NW * TH, smem, h->stream>>>(
         h->label, h->lab16, h->nodes, h->ocount, make_div(h->L), h->L, h->N);
     h->launches += 1;
     return SW_OK;
 }
-int flatten_scan(sw_handle* h) {
-    switch (h->tile) {
+int flatten_scan(sw_handle* h, TileKind tile) {
+    switch (tile) {
         case SCAN_2:    return launch_flatten_scan<2, 32>(h);
-        case SCAN_4:    return launch_flatten_scan<4, 32>(h);
-        case SCAN_8:    return launch_flatten_scan<8, 32>(h);
-        case SCAN_8x64: return launch_flatten_scan<8, 64>(h);
         case SCAN_4x64: return launch_flatten_scan<4, 64>(h);
         default:        return SW_ESTATE;
     }
@@ -336,9 +323,9 @@ int launch_flip_scan(sw_handle* h) {
             h->spins, h->sbits, h->lab16, h->D, h->nodes, h->ocount, h->series, h->ctl, make_div(h->L),
             h->L, h->N, h->words, h->nb);
     else
-    k_flip16<NW, TH, false><<<dim3(tiles, h->nb), NW * TH, 0, h->stream>>>(
-        h->spins, h->sbits, h->lab16, h->D, h->nodes, h->ocount, h->series, h->ctl, make_div(h->L),
-        h->L, h->N, h->words, h->nb);
+        k_flip16<NW, TH, false><<<dim3(tiles, h->nb), NW * TH, 0, h->stream>>>(
+            h->spins, h->sbits, h->lab16, h->D, h->nodes, h->ocount, h->series, h->ctl, make_div(h->L),
+            h->L, h->N, h->words, h->nb);
     h->launches += 1;
     if (h->eager_labels) {                          // a4 every sweep instead of on demand
         SW_MARK(h, K_COMPRESS);
@@ -366,23 +353,23 @@ int launch_label_generic(sw_handle* h) {
 
 // a2-a4 the paper's way: one cooperative kernel runs the label-equivalence passes to convergence
 int launch_label_equiv(sw_handle* h) {
-    static int max_blocks = 0;
-    if (!max_blocks) {
-        int dev = 0, sms = 0, per_sm = 0, coop = 0;
-        SW_CUDA(cudaGetDevice(&dev));
-        SW_CUDA(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev));
+    static int max_blocks[MAX_DEV];
+    int& mb = max_blocks[h->dev >= 0 && h->dev < MAX_DEV ? h->dev : 0];
+    if (!mb) {
+        int sms = 0, per_sm = 0, coop = 0;
+        SW_CUDA(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, h->dev));
         if (!coop) { set_err("path 11: the device does not support cooperative launches"); return SW_ECUDA; }
-        SW_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+        SW_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, h->dev));
         SW_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_label_equiv, EQ_THREADS, 0));
         if (per_sm < 1) { set_err("path 11: k_label_equiv does not fit on an SM"); return SW_ECUDA; }
-        max_blocks = sms * per_sm;
+        mb = sms * per_sm;
     }
     if (!h->eq_ref) {
         SW_CUDA(cudaMalloc(&h->eq_ref, (size_t)h->nb * h->N * sizeof(int)));
         SW_CUDA(cudaMalloc(&h->eq_flags, (size_t)(EQ_MAX_PASSES + 1) * sizeof(int)));
     }
     SW_CUDA(cudaMemsetAsync(h->eq_flags, 0, (size_t)(EQ_MAX_PASSES + 1) * sizeof(int), h->stream));
-    const int blocks = std::max(1, std::min(max_blocks, (h->N + EQ_THREADS - 1) / EQ_THREADS));
+    const int blocks = std::max(1, std::min(mb, (h->N + EQ_THREADS - 1) / EQ_THREADS));
     DivL dv = make_div(h->L);
     void* args[] = { &h->label, &h->eq_ref, &h->bondE, &h->bondS, &h->eq_flags, &dv, &h->L, &h->N, &h->words, &h->nb };
     SW_MARK(h, K_TILE);
@@ -410,15 +397,14 @@ int launch_label_scan(sw_handle* h) {
 }
 
 int launch_label(sw_handle* h) {
+    if (!scan_nw(h->tile)) {                        // flat labels + the size array: allocated on first use
+        int rc = need_label(h); if (rc) return rc;
+        rc = need_gsize(h); if (rc) return rc;
+    }
     if (h->path == 11) return launch_label_equiv(h);
     switch (h->tile) {
         case SCAN_2:      return launch_label_scan<2, 32>(h);
-        case SCAN_4:      return launch_label_scan<4, 32>(h);
-        case SCAN_8:      return launch_label_scan<8, 32>(h);
-        case SCAN_8x64:   return launch_label_scan<8, 64>(h);
         case SCAN_4x64:   return launch_label_scan<4, 64>(h);
-        case TILE_64x64:  return launch_label_tiled<64, 64>(h);
-        case TILE_256x32: return launch_label_tiled<256, 32>(h);
         default:          return launch_label_generic(h);
     }
 }
@@ -427,12 +413,9 @@ int launch_label(sw_handle* h) {
 int launch_bond_label_potts(sw_handle* h) {
     constexpr int NW = 4, TH = 64, TW = 32 * NW, CAP = 2 * (TW + TH);
     const int tiles = h->N / (TW * TH);
-    constexpr size_t smem = (size_t)TW * TH * sizeof(int);
-    static bool attr_done = false;
-    if (!attr_done) {
-        SW_CUDA(cudaFuncSetAttribute(k_bond_label<NW, TH, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_done = true;
-    }
+    constexpr size_t smem = (size_t)TW * TH * sizeof(uint32_t);
+    static bool done[MAX_DEV];
+    { int rc = opt_in_smem(k_bond_label<NW, TH, true, true>, smem, done, h->dev); if (rc) return rc; }
     SW_MARK(h, K_BONDLABEL);
     k_bond_label<NW, TH, true, true><<<dim3(tiles, h->nb), NW * TH, smem, h->stream>>>(
         reinterpret_cast<const uint32_t*>(h->spins), h->bondE, h->bondS, h->lab16, h->nodes, h->ocount, h->bslot,
@@ -473,6 +456,7 @@ int launch_sweep_potts(sw_handle* h, int64_t k) {
         h->launches += 4;
         SW_MARK(h, K_COUNT);
         h->labels_flat = false;                      // int32 labels on demand (k_labels16)
+        h->lab_tile = h->tile;
         return SW_OK;
     }
     h->labels_flat = true;
@@ -505,23 +489,20 @@ int launch_sweep(sw_handle* h, int64_t k) {
                 h->spins, h->bondE, h->bondS, h->lat, h->ctl, h->L, h->N, h->words, h->series, h->nb, obs_prev ? 1 : 0);
             h->launches += 1;
         }
-        rc = h->tile == SCAN_8x64 ? launch_bond_label_scan<8, 64>(h, fused, obs_prev)
-           : h->tile == SCAN_4x64 ? launch_bond_label_scan<4, 64>(h, fused, obs_prev)
-           : nw == 8 ? launch_bond_label_scan<8, 32>(h, fused, obs_prev)
-           : nw == 4 ? launch_bond_label_scan<4, 32>(h, fused, obs_prev) : launch_bond_label_scan<2, 32>(h, fused, obs_prev);
+        rc = nw == 4 ? launch_bond_label_scan<4, 64>(h, fused, obs_prev) : launch_bond_label_scan<2, 32>(h, fused, obs_prev);
         if (rc) return rc;
         SW_MARK(h, K_FLIPBITS);
         k_flipbits<<<grid1(((size_t)h->words + 3) / 4, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(
             h->D, h->lat, h->ctl, h->words);
         h->launches += 1;
-        rc = h->tile == SCAN_8x64 ? launch_flip_scan<8, 64>(h) : h->tile == SCAN_4x64 ? launch_flip_scan<4, 64>(h) : nw == 8 ? launch_flip_scan<8, 32>(h)
-           : nw == 4 ? launch_flip_scan<4, 32>(h) : launch_flip_scan<2, 32>(h);
+        rc = nw == 4 ? launch_flip_scan<4, 64>(h) : launch_flip_scan<2, 32>(h);
         if (rc) return rc;
         SW_MARK(h, K_ADVANCE);
         k_advance<<<1, 64, 0, h->stream>>>(h->ctl, h->series, h->nb, h->mom, h->N, k > 0 ? 2 : 0);
         h->launches += 1;
         SW_MARK(h, K_COUNT);
         h->labels_flat = h->eager_labels;
+        h->lab_tile = h->tile;                          // the tile shape lab16 / nodes were written with
         return SW_OK;
     }
     h->labels_flat = true;
@@ -569,9 +550,9 @@ int init_handle(sw_handle* h, const double* T, const uint64_t* seed) {
     h->spins = (int8_t*)(w + o.spins);
     h->sbits = (uint32_t*)(w + o.sbits);
     h->bondE = (uint32_t*)(w + o.bondE); h->bondS = (uint32_t*)(w + o.bondS); h->D = (uint32_t*)(w + o.D);
-    h->label = (int*)(w + o.label); h->gsize = (int*)(w + o.gsize); h->lab16 = (uint16_t*)(w + o.lab16);
+    h->lab16 = (uint16_t*)(w + o.lab16);
     h->nodes = (int4*)(w + o.nodes); h->bslot = (uint16_t*)(w + o.bslot);
-    h->olist = (int2*)(w + o.olist); h->ocount = (int*)(w + o.ocount);
+    h->ocount = (int*)(w + o.ocount);
     h->lat = (Lat*)(w + o.lat); h->ctl = (Ctl*)(w + o.ctl); h->rec_now = (Rec*)(w + o.rec_now); h->mom = (Mom*)(w + o.mom);
     h->hT.assign(T, T + h->nb);
     h->series = (Rec*)(w + o.series);
@@ -583,7 +564,6 @@ int init_handle(sw_handle* h, const double* T, const uint64_t* seed) {
         h->hlat[b].pad = 0;
     }
     SW_CUDA(cudaMemcpyAsync(h->lat, h->hlat.data(), sizeof(Lat) * h->nb, cudaMemcpyHostToDevice, h->stream));
-    SW_CUDA(cudaMemsetAsync(h->gsize, 0, (size_t)h->nb * h->N * 4, h->stream));
     SW_CUDA(cudaMemsetAsync(h->series, 0, (size_t)h->ring() * h->nb * sizeof(Rec), h->stream));
     SW_CUDA(cudaMemsetAsync(h->mom, 0, (size_t)h->nb * sizeof(Mom), h->stream));
     k_set_ctl<<<1, 1, 0, h->stream>>>(h->ctl, 0ull, 0u, (uint32_t)h->ring());
@@ -615,6 +595,7 @@ sw_handle* create_common(void* ws, uint64_t ws_bytes, int32_t L, int32_t nb, con
     sw_handle* h = new (std::nothrow) sw_handle();
     if (!h) { set_err("sw_create: out of host memory"); return nullptr; }
     h->L = L; h->nb = nb; h->N = L * L; h->words = (h->N + 31) / 32; h->q = q;
+    if (cudaGetDevice(&h->dev) != cudaSuccess) { (void)cudaGetLastError(); set_err("sw_create: cudaGetDevice failed"); delete h; return nullptr; }
     const size_t need = make_layout(L, nb).total;
     if (ws) {
         if (ws_bytes < need || ((uintptr_t)ws % ALIGN) != 0) {
@@ -676,6 +657,7 @@ sw_handle* sw_create_in(void* workspace, uint64_t workspace_bytes, int32_t L, in
 
 void sw_destroy(sw_handle* h) {
     if (!h) return;
+    DevGuard dg(h->dev);
     cudaStreamSynchronize(h->stream);
     for (cudaEvent_t e : h->ev) cudaEventDestroy(e);
     for (cudaEvent_t e : h->ev_tail) if (e) cudaEventDestroy(e);
@@ -686,6 +668,8 @@ void sw_destroy(sw_handle* h) {
     if (h->potts_cnt) cudaFree(h->potts_cnt);
     if (h->eq_ref) cudaFree(h->eq_ref);
     if (h->eq_flags) cudaFree(h->eq_flags);
+    if (h->label) cudaFree(h->label);
+    if (h->gsize) cudaFree(h->gsize);
     if (h->owns_ws) cudaFree(h->ws);
     (void)cudaGetLastError();
     delete h;
@@ -722,6 +706,7 @@ bool build_graphs(sw_handle* h) {
 
 int sw_sweep(sw_handle* h, int64_t n) {
     if (!h || n < 0) { set_err("sw_sweep: invalid argument"); return SW_EINVAL; }
+    DevGuard dg(h->dev);
     if (n == 0) return SW_OK;
     h->launches = 0;
     {   // the configuration must sit in the plane this path sweeps on
@@ -730,6 +715,14 @@ int sw_sweep(sw_handle* h, int64_t n) {
     }
     // graph replay: scan path, no per-kernel timing, enough sweeps to pay for the two stream hops
     cudaStream_t const user = h->stream;
+    struct StreamBack {                                 // whatever the exit: the handle goes back to the caller's stream,
+        sw_handle* h; cudaStream_t user;                // ordered after what ran on the internal one
+        ~StreamBack() {
+            if (h->stream == user) return;
+            if (h->gev[1] && cudaEventRecord(h->gev[1], h->stream) == cudaSuccess) cudaStreamWaitEvent(user, h->gev[1], 0);
+            h->stream = user;
+        }
+    } stream_back{h, user};
     bool graphs = h->use_graphs && !h->graph_failed && !h->timing && scan_nw(h->tile) && n >= 4 && !h->q;
     if (graphs) {
         if (!h->gstream) {
@@ -760,7 +753,7 @@ int sw_sweep(sw_handle* h, int64_t n) {
     h->launches += 1;
     {
         int rc = launch_sweep(h, 0);                    // (also sets the kernels' attributes before any capture)
-        if (rc) { h->stream = user; return rc; }
+        if (rc) return rc;
     }
     int64_t k = 1;
     if (graphs && !build_graphs(h)) { h->graph_failed = true; graphs = false; }
@@ -776,7 +769,7 @@ int sw_sweep(sw_handle* h, int64_t n) {
     }
     for (; k < n; ++k) {
         int rc = launch_sweep(h, k);
-        if (rc) { h->stream = user; return rc; }
+        if (rc) return rc;
     }
     if (scan_nw(h->tile) && !h->q) {                    // a7 of the configuration the call ends with
         if (h->timing) SW_CUDA(cudaEventRecord(h->ev_tail[0], h->stream));
@@ -792,8 +785,8 @@ int sw_sweep(sw_handle* h, int64_t n) {
     }
     if (h->stream != user) {                            // hand the result back to the caller's stream
         SW_CUDA(cudaEventRecord(h->gev[1], h->stream));
-        h->stream = user;
         SW_CUDA(cudaStreamWaitEvent(user, h->gev[1], 0));
+        h->stream = user;
     }
     SW_CUDA(cudaGetLastError());
     h->t += (uint64_t)n;
@@ -807,9 +800,10 @@ int sw_sweep(sw_handle* h, int64_t n) {
 
 const int32_t* sw_labels(sw_handle* h) {
     if (!h) { set_err("sw_labels: null handle"); return nullptr; }
+    DevGuard dg(h->dev);
     if (!h->have_sweep) { set_err("sw_labels: no sweep has run yet"); return nullptr; }
     if (!h->labels_flat) {      // the fast path leaves site -> tile root -> cluster root: flatten on demand (a4)
-        if (flatten_scan(h) != SW_OK || cudaGetLastError() != cudaSuccess) { set_err("sw_labels: flatten launch failed"); return nullptr; }
+        if (flatten_scan(h, h->lab_tile) != SW_OK || cudaGetLastError() != cudaSuccess) { set_err("sw_labels: flatten launch failed"); return nullptr; }
         h->labels_flat = true;
     }
     return h->label;
@@ -817,6 +811,7 @@ const int32_t* sw_labels(sw_handle* h) {
 
 int sw_bonds(sw_handle* h, const uint32_t** bondE, const uint32_t** bondS) {
     if (!h || !bondE || !bondS) { set_err("sw_bonds: null argument"); return SW_EINVAL; }
+    DevGuard dg(h->dev);
     if (!h->have_sweep) { set_err("sw_bonds: no sweep has run yet"); return SW_ESTATE; }
     *bondE = h->bondE; *bondS = h->bondS;
     return SW_OK;
@@ -824,12 +819,14 @@ int sw_bonds(sw_handle* h, const uint32_t** bondE, const uint32_t** bondS) {
 
 const int8_t* sw_spins(sw_handle* h) {
     if (!h) { set_err("sw_spins: null handle"); return nullptr; }
+    DevGuard dg(h->dev);
     if (ensure_i8(h) != SW_OK) return nullptr;         // the fused path sweeps on the bit plane: int8 on demand
     return h->spins;
 }
 
 int sw_observables(sw_handle* h, sw_obs* out) {
     if (!h || !out) { set_err("sw_observables: null argument"); return SW_EINVAL; }
+    DevGuard dg(h->dev);
     std::vector<Rec> r(h->nb);
     if (h->rec_valid) {
         const int64_t slot = (h->last_n - 1) % h->ring();
@@ -855,6 +852,7 @@ int sw_observables(sw_handle* h, sw_obs* out) {
 
 int64_t sw_series(sw_handle* h, sw_obs* out, int64_t cap) {
     if (!h || !out || cap < 0) { set_err("sw_series: invalid argument"); return SW_EINVAL; }
+    DevGuard dg(h->dev);
     if (!h->rec_valid) return 0;
     const int64_t kept = std::min(h->last_n, h->series_cap);
     const int64_t give = std::min(kept, cap);
@@ -873,6 +871,7 @@ int64_t sw_series(sw_handle* h, sw_obs* out, int64_t cap) {
 
 int sw_moments(sw_handle* h, sw_mom* out) {
     if (!h || !out) { set_err("sw_moments: null argument"); return SW_EINVAL; }
+    DevGuard dg(h->dev);
     std::vector<Mom> m(h->nb);
     SW_CUDA(cudaMemcpyAsync(m.data(), h->mom, sizeof(Mom) * h->nb, cudaMemcpyDeviceToHost, h->stream));
     SW_CUDA(cudaStreamSynchronize(h->stream));
@@ -893,12 +892,14 @@ int sw_moments(sw_handle* h, sw_mom* out) {
 
 int sw_moments_reset(sw_handle* h) {
     if (!h) { set_err("sw_moments_reset: null handle"); return SW_EINVAL; }
+    DevGuard dg(h->dev);
     SW_CUDA(cudaMemsetAsync(h->mom, 0, (size_t)h->nb * sizeof(Mom), h->stream));
     return SW_OK;
 }
 
 int sw_set_series_capacity(sw_handle* h, int64_t sweeps) {
     if (!h || sweeps < 1 || sweeps > (1ll << 26)) { set_err("sw_set_series_capacity: invalid argument"); return SW_EINVAL; }
+    DevGuard dg(h->dev);
     SW_CUDA(cudaStreamSynchronize(h->stream));
     Rec* p = nullptr;
     cudaError_t e = cudaMalloc((void**)&p, (size_t)(sweeps + 1) * h->nb * sizeof(Rec));
@@ -911,6 +912,7 @@ int sw_set_series_capacity(sw_handle* h, int64_t sweeps) {
 
 int sw_set_spins(sw_handle* h, const int8_t* spins, int is_host) {
     if (!h || !spins) { set_err("sw_set_spins: null argument"); return SW_EINVAL; }
+    DevGuard dg(h->dev);
     SW_CUDA(cudaMemcpyAsync(h->spins, spins, (size_t)h->nb * h->N,
                             is_host ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice, h->stream));
     if (is_host) SW_CUDA(cudaStreamSynchronize(h->stream));
@@ -921,6 +923,7 @@ int sw_set_spins(sw_handle* h, const int8_t* spins, int is_host) {
 
 int sw_set_cold(sw_handle* h) {
     if (!h) { set_err("sw_set_cold: null handle"); return SW_EINVAL; }
+    DevGuard dg(h->dev);
     const size_t n = (size_t)h->nb * h->N;
     k_fill_i8<<<(unsigned)((n + GEN_THREADS - 1) / GEN_THREADS), GEN_THREADS, 0, h->stream>>>(h->spins, n, (int8_t)(h->q ? 0 : 1));
     SW_CUDA(cudaGetLastError());
@@ -932,6 +935,7 @@ int sw_set_cold(sw_handle* h) {
 // bit-packed host interface: straight into / out of the bit plane the fused path sweeps on
 int sw_set_spins_bits(sw_handle* h, const uint32_t* bits_host) {
     if (!h || !bits_host) { set_err("sw_set_spins_bits: null argument"); return SW_EINVAL; }
+    DevGuard dg(h->dev);
     if (h->q) { set_err("sw_set_spins_bits: Ising handles only (a Potts colour does not fit a bit)"); return SW_ESTATE; }
     SW_CUDA(cudaMemcpyAsync(h->sbits, bits_host, (size_t)h->nb * h->words * 4, cudaMemcpyHostToDevice, h->stream));
     SW_CUDA(cudaStreamSynchronize(h->stream));          // the caller may reuse its buffer
@@ -942,6 +946,7 @@ int sw_set_spins_bits(sw_handle* h, const uint32_t* bits_host) {
 
 int sw_get_spins_bits(sw_handle* h, uint32_t* out_host) {
     if (!h || !out_host) { set_err("sw_get_spins_bits: null argument"); return SW_EINVAL; }
+    DevGuard dg(h->dev);
     if (h->q) { set_err("sw_get_spins_bits: Ising handles only"); return SW_ESTATE; }
     { const int rc = ensure_bits(h); if (rc) return rc; }
     SW_CUDA(cudaMemcpyAsync(out_host, h->sbits, (size_t)h->nb * h->words * 4, cudaMemcpyDeviceToHost, h->stream));
@@ -951,6 +956,7 @@ int sw_get_spins_bits(sw_handle* h, uint32_t* out_host) {
 
 int sw_get_spins(sw_handle* h, int8_t* out_host) {
     if (!h || !out_host) { set_err("sw_get_spins: null argument"); return SW_EINVAL; }
+    DevGuard dg(h->dev);
     { const int rc = ensure_i8(h); if (rc) return rc; }
     SW_CUDA(cudaMemcpyAsync(out_host, h->spins, (size_t)h->nb * h->N, cudaMemcpyDeviceToHost, h->stream));
     SW_CUDA(cudaStreamSynchronize(h->stream));
@@ -959,6 +965,7 @@ int sw_get_spins(sw_handle* h, int8_t* out_host) {
 
 int sw_get_labels(sw_handle* h, int32_t* out_host) {
     if (!h || !out_host) { set_err("sw_get_labels: null argument"); return SW_EINVAL; }
+    DevGuard dg(h->dev);
     const int32_t* l = sw_labels(h);
     if (!l) return SW_ESTATE;
     SW_CUDA(cudaMemcpyAsync(out_host, l, (size_t)h->nb * h->N * 4, cudaMemcpyDeviceToHost, h->stream));
@@ -975,6 +982,7 @@ uint64_t sw_sweep_index(const sw_handle* h) { return h ? h->t : 0; }
 
 int sw_set_stream(sw_handle* h, void* cuda_stream) {
     if (!h) { set_err("sw_set_stream: null handle"); return SW_EINVAL; }
+    DevGuard dg(h->dev);
     SW_CUDA(cudaStreamSynchronize(h->stream));
     h->stream = (cudaStream_t)cuda_stream;
     return SW_OK;
@@ -989,6 +997,7 @@ int sw_set_stage_timing(sw_handle* h, int on) {
 
 int sw_kernel_ms(sw_handle* h, float* out, int32_t cap) {
     if (!h || !out || cap < 0) { set_err("sw_kernel_ms: invalid argument"); return SW_EINVAL; }
+    DevGuard dg(h->dev);
     for (int i = 0; i < cap; ++i) out[i] = 0.f;
     if (h->timed_sweeps == 0) { set_err("sw_kernel_ms: the last sw_sweep ran without stage timing"); return SW_ESTATE; }
     SW_CUDA(cudaStreamSynchronize(h->stream));
@@ -1009,6 +1018,7 @@ int sw_kernel_ms(sw_handle* h, float* out, int32_t cap) {
 
 int64_t sw_sweep_ms(sw_handle* h, float* out, int64_t cap) {
     if (!h || !out || cap < 0) { set_err("sw_sweep_ms: invalid argument"); return SW_EINVAL; }
+    DevGuard dg(h->dev);
     if (h->timed_sweeps == 0) { set_err("sw_sweep_ms: the last sw_sweep ran without stage timing"); return SW_ESTATE; }
     SW_CUDA(cudaStreamSynchronize(h->stream));
     const int ns = (int)h->ev_seq.size();            // marks per sweep, the closing one included
@@ -1031,12 +1041,12 @@ int sw_stage_ms(sw_handle* h, float out[4]) {
 }
 
 int sw_set_path(sw_handle* h, int path) {
-    if (!h || path < 0 || path > 11 || path == 10) { set_err("sw_set_path: invalid argument"); return SW_EINVAL; }
-    if (h->q && path != 0 && path != 1 && path != 11) { set_err("sw_set_path: a Potts handle runs on paths 0 / 1 (generic) and 11 only"); return SW_EINVAL; }
+    if (!h || !valid_path(path)) { set_err("sw_set_path: path %d is not one of 0 (fast path), 1 (generic kernels), 6 (unfused stages), 11 (label equivalence)", path); return SW_EINVAL; }
+    DevGuard dg(h->dev);
+    if (h->q && path == 6) { set_err("sw_set_path: a Potts handle runs on paths 0 (128 x 64 tiles when L allows, else generic), 1 (generic) and 11"); return SW_EINVAL; }
     h->path = path;
     h->eq_ran = false;
-    // the tiled paths keep gsize zero between sweeps themselves; the generic / path-11 kernels leave sizes in it
-    SW_CUDA(cudaMemsetAsync(h->gsize, 0, (size_t)h->nb * h->N * sizeof(int), h->stream));
+    // (16-bit roots of a sweep on the previous path stay valid: sw_labels flattens them with the tile shape that wrote them)
     h->tile = h->q ? potts_tile(h->L, path) : pick_tile(h->L, path);
     return SW_OK;
 }
@@ -1061,21 +1071,24 @@ int32_t sw_batch(const sw_handle* h) { return h ? h->nb : 0; }
 int sw_test_philox(const uint32_t* ctr, const uint32_t* key, uint32_t* out, int64_t n) {
     if (!ctr || !key || !out || n < 0) { set_err("sw_test_philox: invalid argument"); return SW_EINVAL; }
     if (n == 0) return SW_OK;
-    uint32_t *dc = nullptr, *dk = nullptr, *dout = nullptr;
-    SW_CUDA(cudaMalloc((void**)&dc, (size_t)n * 16));
-    SW_CUDA(cudaMalloc((void**)&dk, (size_t)n * 8));
-    SW_CUDA(cudaMalloc((void**)&dout, (size_t)n * 16));
-    SW_CUDA(cudaMemcpy(dc, ctr, (size_t)n * 16, cudaMemcpyHostToDevice));
-    SW_CUDA(cudaMemcpy(dk, key, (size_t)n * 8, cudaMemcpyHostToDevice));
-    k_test_philox<<<(unsigned)((n + 255) / 256), 256>>>(dc, dk, dout, n);
+    struct Bufs {                                       // freed on every exit
+        uint32_t *dc = nullptr, *dk = nullptr, *dout = nullptr;
+        ~Bufs() { cudaFree(dc); cudaFree(dk); cudaFree(dout); }
+    } b;
+    SW_CUDA(cudaMalloc((void**)&b.dc, (size_t)n * 16));
+    SW_CUDA(cudaMalloc((void**)&b.dk, (size_t)n * 8));
+    SW_CUDA(cudaMalloc((void**)&b.dout, (size_t)n * 16));
+    SW_CUDA(cudaMemcpy(b.dc, ctr, (size_t)n * 16, cudaMemcpyHostToDevice));
+    SW_CUDA(cudaMemcpy(b.dk, key, (size_t)n * 8, cudaMemcpyHostToDevice));
+    k_test_philox<<<(unsigned)((n + 255) / 256), 256>>>(b.dc, b.dk, b.dout, n);
     SW_CUDA(cudaGetLastError());
-    SW_CUDA(cudaMemcpy(out, dout, (size_t)n * 16, cudaMemcpyDeviceToHost));
-    cudaFree(dc); cudaFree(dk); cudaFree(dout);
+    SW_CUDA(cudaMemcpy(out, b.dout, (size_t)n * 16, cudaMemcpyDeviceToHost));
     return SW_OK;
 }
 
 int sw_label_passes(sw_handle* h, int32_t* passes) {
     if (!h || !passes) { set_err("sw_label_passes: null argument"); return SW_EINVAL; }
+    DevGuard dg(h->dev);
     if (h->path != 11 || !h->eq_ran) { set_err("sw_label_passes: no labelling has run on path 11 yet"); return SW_ESTATE; }
     int tail[2] = { 0, 0 };
     SW_CUDA(cudaMemcpyAsync(&tail[1], h->eq_flags + EQ_MAX_PASSES, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
@@ -1112,6 +1125,7 @@ int sw_test_philox_ceiling(int64_t sites, int32_t reps, float* ms_out) {
 
 int sw_test_label(sw_handle* h, const uint32_t* bondE, const uint32_t* bondS, int32_t* labels_out) {
     if (!h || !bondE || !bondS || !labels_out || h->nb != 1) { set_err("sw_test_label: invalid argument"); return SW_EINVAL; }
+    DevGuard dg(h->dev);
     SW_CUDA(cudaMemcpyAsync(h->bondE, bondE, (size_t)h->words * 4, cudaMemcpyHostToDevice, h->stream));
     SW_CUDA(cudaMemcpyAsync(h->bondS, bondS, (size_t)h->words * 4, cudaMemcpyHostToDevice, h->stream));
     SW_CUDA(cudaMemsetAsync(h->series, 0, sizeof(Rec), h->stream));

@@ -37,21 +37,92 @@ constexpr uint32_t OPEN_BIT = 0x40000000u;      // bit 30 of a root's word: the 
 // cluster size (<= 2^LS), bit 30 open.
 __host__ __device__ constexpr int ilog2_c(int v) { return v <= 1 ? 0 : 1 + ilog2_c(v >> 1); }
 
-// find on the shared parent array; roots may carry size / open bits above the index mask
-__device__ __forceinline__ int sc_find(const int* par, int x, int mask) {
-    int p = par[x] & mask;
-    while (p != x) { x = p; p = par[x] & mask; }
+// ---- the shared parent array of k_bond_label -------------------------------------------------------------
+// One 32-bit word per site of the tile:
+//   bits 16 .. 29  parent (tile-local index); a root points at itself
+//   bits  0 .. 13  sites counted at this node: every run adds its length to the label it takes (phase 2); the
+//                  flatten (phase 3b) moves the counts of the nodes that were hooked to their roots, so that a
+//                  root ends up with the size of its tile-local cluster
+//   bit  14        CLAIMED (roots with a bond across the tile edge, phase 5): the low 14 bits now hold the root's
+//                  slot in the tile's node list instead of the count
+// The parent sits in the HIGH half so that hooking "larger under smaller" stays one atomicMin on the whole
+// word: (b << 16) is below every word whose parent is above b.  The count the atomicMin wipes out comes back
+// in its return value and is added again by the thread that hooked.
+// All accesses go through the shared window (32-bit addresses, ld / st / atom / red .shared): word x sits at
+// par_s + 4 x, its parent at par_s + 4 x + 2.
+constexpr uint32_t CLAIMED16 = 0x4000u, CNT16 = 0x3FFFu;
+
+__device__ __forceinline__ uint32_t lds_u16(uint32_t a) {
+    uint16_t v; asm volatile("ld.shared.u16 %0, [%1];" : "=h"(v) : "r"(a) : "memory"); return v;
+}
+__device__ __forceinline__ uint32_t lds_u32(uint32_t a) {
+    uint32_t v; asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a) : "memory"); return v;
+}
+__device__ __forceinline__ uint4 lds_u128(uint32_t a) {
+    uint4 v; asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(a) : "memory"); return v;
+}
+__device__ __forceinline__ void sts_u16(uint32_t a, uint32_t v) {
+    asm volatile("st.shared.u16 [%0], %1;" :: "r"(a), "h"((uint16_t)v) : "memory");
+}
+__device__ __forceinline__ void sts_u128(uint32_t a, uint4 v) {
+    asm volatile("st.shared.v4.u32 [%0], {%1,%2,%3,%4};" :: "r"(a), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
+__device__ __forceinline__ void red_add_s(uint32_t a, uint32_t v) {
+    asm volatile("red.shared.add.u32 [%0], %1;" :: "r"(a), "r"(v) : "memory");
+}
+__device__ __forceinline__ uint32_t atom_min_s(uint32_t a, uint32_t v) {
+    uint32_t o; asm volatile("atom.shared.min.u32 %0, [%1], %2;" : "=r"(o) : "r"(a), "r"(v) : "memory"); return o;
+}
+__device__ __forceinline__ uint32_t atom_or_s(uint32_t a, uint32_t v) {
+    uint32_t o; asm volatile("atom.shared.or.b32 %0, [%1], %2;" : "=r"(o) : "r"(a), "r"(v) : "memory"); return o;
+}
+
+__device__ __forceinline__ int sc_find(uint32_t par_s, int x) {
+    int p = (int)lds_u16(par_s + 4u * x + 2u);
+    while (p != x) { x = p; p = (int)lds_u16(par_s + 4u * x + 2u); }
     return x;
 }
 // unite the trees of a and b (any nodes); hooking "larger under smaller" with atomicMin so the root of a
-// component is its minimum index whatever the interleaving.  Only used before any size / flag bit is set.
-__device__ __forceinline__ void sc_union(int* par, int a, int b) {
+// component is its minimum index whatever the interleaving.  A node stops being a root exactly once, and the
+// call whose atomicMin did it (the return value still shows the node as its own parent) returns that node --
+// at most one per call, NO_NODE otherwise.  Phase 3b flattens exactly these hooked nodes: ~0.03 per site at T_c,
+// against ~0.2 label nodes per site.
+constexpr int NO_NODE = 0xFFFF;
+__device__ __forceinline__ uint32_t atom_add_s(uint32_t a, uint32_t v) {
+    uint32_t o; asm volatile("atom.shared.add.u32 %0, [%1], %2;" : "=r"(o) : "r"(a), "r"(v) : "memory"); return o;
+}
+// the tile's list of hooked nodes (phase 3b flattens from it with all threads); the counter runs on past the capacity
+// (it also gives the number of roots), and phase 3b then visits every label node instead
+struct HookList { uint32_t items_s, count_s; int cap; };     // (shared-window addresses)
+__device__ __forceinline__ void hooked(const HookList& hk, int node) {
+    if (node == NO_NODE) return;
+    // (the increment is made opaque: ptxas would otherwise turn the add into a warp-aggregated one -- vote, popc,
+    // shuffle: 20 instructions -- for the few lanes that get here together)
+    uint32_t one = 1u;
+    asm volatile("mov.u32 %0, %0;" : "+r"(one));
+    const int pos = (int)atom_add_s(hk.count_s, one);
+    if (pos < hk.cap) sts_u16(hk.items_s + 2u * pos, (uint32_t)node);
+}
+__device__ __forceinline__ int sc_union(uint32_t par_s, int a, int b) {
     while (a != b) {
         if (a < b) { const int s = a; a = b; b = s; }      // a is the larger
-        const int old = atomicMin(par + a, b);
-        if (old == a) break;                                // a was a root: hooked under b
-        a = old;                                            // a had parent `old`: unite that with b
+        const uint32_t nv = (uint32_t)b << 16;
+        const uint32_t old = atom_min_s(par_s + 4u * a, nv);
+        if (old > nv && (old & 0xFFFFu)) red_add_s(par_s + 4u * a, old & 0xFFFFu);   // the count the minimum replaced
+        const int p = (int)(old >> 16);
+        if (p == a) return a;                               // a was a root: hooked under b
+        a = p;                                              // a had parent p: unite that with b
     }
+    return NO_NODE;
+}
+// point a hooked node at its root and hand it the node's count
+__device__ __forceinline__ void sc_flatten(uint32_t par_s, int n) {
+    const uint32_t wn = lds_u32(par_s + 4u * n);
+    const int p0 = (int)(wn >> 16);
+    int r = p0, q = (int)lds_u16(par_s + 4u * r + 2u);
+    while (q != r) { r = q; q = (int)lds_u16(par_s + 4u * r + 2u); }
+    if (r != p0) sts_u16(par_s + 4u * n + 2u, (uint32_t)r);
+    if (wn & 0xFFFFu) red_add_s(par_s + 4u * r, wn & 0xFFFFu);    // (a hooked node receives nothing any more)
 }
 
 // exact v / d for 0 <= v < 2^30 with a host-made magic (m, p): q = (v * m) >> p
@@ -72,15 +143,20 @@ k_bond_label(const uint32_t* __restrict__ sbits, uint32_t* bondE, uint32_t* bond
              int L, int N, int words, int nb, int obs_prev) {
     constexpr int TW = 32 * NW, SITES = TW * TH, THREADS = NW * TH;   // one thread per 32-site word
     constexpr int CAP = 2 * (TW + TH);
-    constexpr int LS = ilog2_c(SITES), IDX_MASK = SITES - 1, CNT_SHIFT = LS, CNT_MASK = 2 * SITES - 1;
-    static_assert(TH % BAND == 0 && TH <= 64 && (1 << LS) == SITES && LS <= 14, "tile shape");
-    extern __shared__ __align__(16) int par[];  // [SITES] parent, tile-local index (+ size / open bits at roots); dynamic: 64 KB at TH = 64
+    constexpr int NWARPS = THREADS / 32;
+    constexpr int PCAP = 192;                   // label meetings a warp can list while it scans its block (~80 at T_c)
+    constexpr int HKCAP = 1024;                 // hooked nodes the tile can list (~250 at T_c)
+    static_assert(TH % BAND == 0 && TH <= 64 && SITES <= 8192 && CAP < 0x3FFF, "tile shape");
+    extern __shared__ __align__(16) uint32_t par[];  // [SITES] (see above); dynamic: 32 KB at 128 x 64
     __shared__ uint2 es[TH * NW];              // [row][strip] = (East word, South word)
+    __shared__ uint16_t pend[NWARPS][PCAP];    // phase 2: sites where two labels met
+    __shared__ uint16_t hkitems[HKCAP];        // nodes hooked in phases 2 and 3
     __shared__ uint32_t nIn[NW];               // South bonds entering from the tile above, per strip
     __shared__ uint32_t wIn[2];                // East bonds entering from the tile to the West, bit = row
-    __shared__ int s_nopen, s_max, s_nclosed, s_obs[2];
+    __shared__ int s_nopen, s_max, s_nlab, s_nhook, s_obs[2];
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const uint32_t lanebit = 1u << lane, lt = lanebit - 1u;
     const int tilesX = L / TW;
     const int ty = blockIdx.x / tilesX, tx = blockIdx.x - ty * tilesX;
     const int y0 = ty * TH, x0 = tx * TW;
@@ -93,7 +169,13 @@ k_bond_label(const uint32_t* __restrict__ sbits, uint32_t* bondE, uint32_t* bond
     const uint32_t tlo = (uint32_t)t, thi = (uint32_t)(t >> 32);
 
     if (tid < NW) nIn[tid] = 0;
-    if (tid == 0) { wIn[0] = 0; wIn[1] = 0; s_nopen = 0; s_max = 0; s_nclosed = 0; s_obs[0] = 0; s_obs[1] = 0; }
+    if (tid == 0) { wIn[0] = 0; wIn[1] = 0; s_nopen = 0; s_max = 0; s_nlab = 0; s_nhook = 0; s_obs[0] = 0; s_obs[1] = 0; }
+    uint32_t par_s = (uint32_t)__cvta_generic_to_shared(par);        // shared-window address of word 0
+    asm volatile("mov.u32 %0, %0;" : "+r"(par_s));                   // (opaque: kept in a register, not recomputed at every use)
+    const HookList hk = { (uint32_t)__cvta_generic_to_shared(hkitems), (uint32_t)__cvta_generic_to_shared(&s_nhook), HKCAP };
+#pragma unroll
+    for (int k = 0; k < SITES / 4 / THREADS; ++k)                    // counts start at 0 (the scan stores parents only)
+        sts_u128(par_s + 16u * (k * THREADS + tid), make_uint4(0u, 0u, 0u, 0u));
     __syncthreads();
 
     // ---- phase 1: bonds of the tile, PAPER.md:37-39 (section 2.1) --------------------------------------
@@ -183,14 +265,22 @@ k_bond_label(const uint32_t* __restrict__ sbits, uint32_t* bondE, uint32_t* bond
     __syncthreads();
 
     // ---- phase 2: scan-line labelling of this warp's block (32 columns x 32 rows), PAPER.md:49-51 -------
+    // Lane = column, the block's rows in sequence, uniform control flow.  A run of East bonds takes the label of the
+    // first of its sites that has a South bond from the row above (one shuffle), or opens a new label = its head's
+    // own index (a root).  Where another site of the run is bonded to a different label above, the two labels are
+    // equivalent: the pair goes into the warp's list (ballot-compacted, no divergent work in the loop) and the warp
+    // unites its pairs with all lanes once the block is scanned.  Labels are never refreshed on the way down, so the
+    // only loop-carried dependency of a row is the shuffle.
     {
-        const uint32_t lanebit = 1u << lane, lt = lanebit - 1u;
         const int strip = warp % NW, yb = (warp / NW) * BAND;
         int rowbase = yb * TW + strip * 32;                          // first site of the row in this strip
-        int prev = 0;
+        uint32_t rowaddr = par_s + 4u * (rowbase + lane) + 2u;       // my site's parent field in this row
+        uint32_t prev = 0;                                           // label of the site above
         uint32_t s_up = 0;                                           // (a band's first row adopts nothing: seams come later)
+        const uint32_t pl_s = (uint32_t)__cvta_generic_to_shared(pend[warp]);
+        int npend = 0;                                               // (warp-uniform)
 #pragma unroll 4
-        for (int y = yb; y < yb + BAND; ++y, rowbase += TW) {
+        for (int y = yb; y < yb + BAND; ++y, rowbase += TW, rowaddr += 4u * TW) {
             const uint2 w = es[y * NW + strip];
             const uint32_t nz = ~w.x | 0x80000000u;                  // bit k: no bond between columns k, k + 1 of the strip
             const uint32_t below = nz & lt, above = nz & ~lt;        // run boundaries left of me / at or right of me
@@ -198,22 +288,33 @@ k_bond_label(const uint32_t* __restrict__ sbits, uint32_t* bondE, uint32_t* bond
             // my run: bits h .. tail, tail = lowest set bit of `above` (bit 31 is always set)
             const uint32_t runmask = (above ^ (above - 1u)) & ~((1u << h) - 1u);
             const uint32_t upm = s_up & runmask;                     // sites of my run bonded to the row above
-            const bool myUp = s_up & lanebit;
-            // label of the site above, one hop fresher: its parent (itself while it still is a root; the root it was
-            // hooked under in the previous row otherwise).  Nothing below needs an exact root: a stale node is
-            // still a label node of the right tree, and the hook falls back to sc_union, which takes any nodes.
-            const int a = par[prev];
-            const int got = __shfl_sync(0xffffffffu, a, __ffs(upm) - 1);   // (source lane is taken mod 32)
-            const int c = upm ? got : rowbase + h;                   // a new label: the head's own index (its own root)
-            par[rowbase + lane] = c;
-            if (myUp && a != c) {                                    // two roots meet in my run: hook the larger under the smaller
-                const int hi = max(a, c), lo = min(a, c);
-                const int old = atomicMin(par + hi, lo);
-                if (old != hi) sc_union(par, old, lo);               // hi had been hooked meanwhile (rare)
-            }
-            __syncwarp();                                            // row y's parents are written before row y + 1 walks them
+            const uint32_t got = __shfl_sync(0xffffffffu, prev, __ffs(upm) - 1);   // (source lane is taken mod 32)
+            const uint32_t c = upm ? got : (uint32_t)(rowbase + h);  // a new label: the head's own index (its own root)
+            sts_u16(rowaddr, c);
+            const bool meet = (s_up & lanebit) && prev != c;         // two labels meet at my site: the one above, my run's
+            const uint32_t mb = __ballot_sync(0xffffffffu, meet);
+            const int at = npend + __popc(mb & lt);
+            if (meet && at < PCAP) sts_u16(pl_s + 2u * at, (uint32_t)(rowbase + lane));
+            npend += __popc(mb);
             prev = c;
             s_up = w.y;
+        }
+        __syncwarp();                                                // the block's parents and meetings are written
+        if (npend <= PCAP) {
+            for (int j = lane; j < npend; j += 32) {                 // unite with all lanes
+                const uint32_t i = lds_u16(pl_s + 2u * j);
+                const int a = (int)lds_u16(par_s + 4u * (i - TW) + 2u), c = (int)lds_u16(par_s + 4u * i + 2u);
+                hooked(hk, sc_union(par_s, a, c));                   // (labels are mostly still roots: sc_union takes any nodes)
+            }
+        } else {
+            // more meetings than the list holds (far from the workloads' bond densities): take them from the labels again
+            for (int y = yb + 1; y < yb + BAND; ++y) {
+                const int i = y * TW + strip * 32 + lane;
+                if ((es[(y - 1) * NW + strip].y >> lane) & 1u) {
+                    const int a = (int)lds_u16(par_s + 4u * (i - TW) + 2u), c = (int)lds_u16(par_s + 4u * i + 2u);
+                    if (a != c) hooked(hk, sc_union(par_s, a, c));
+                }
+            }
         }
     }
     __syncthreads();
@@ -224,27 +325,40 @@ k_bond_label(const uint32_t* __restrict__ sbits, uint32_t* bondE, uint32_t* bond
             const int row = j / (NW - 1), st = j - row * (NW - 1);
             if (es[row * NW + st].x >> 31) {
                 const int i = row * TW + st * 32 + 31;
-                sc_union(par, sc_find(par, i, IDX_MASK), sc_find(par, i + 1, IDX_MASK));
+                hooked(hk, sc_union(par_s, (int)lds_u16(par_s + 4u * i + 2u), (int)lds_u16(par_s + 4u * i + 6u)));   // the two sites' labels
             }
         } else {
             const int k = j - (NW - 1) * TH;
             const int row = (k / TW + 1) * BAND - 1, c = k % TW;
             if ((es[row * NW + (c >> 5)].y >> (c & 31)) & 1u) {
                 const int i = row * TW + c;
-                sc_union(par, sc_find(par, i, IDX_MASK), sc_find(par, i + TW, IDX_MASK));
+                hooked(hk, sc_union(par_s, (int)lds_u16(par_s + 4u * i + 2u), (int)lds_u16(par_s + 4u * (i + TW) + 2u)));
             }
+        }
+    }
+    // ... and, in the same phase, every site is counted at its label (any node of its tree will do: the flatten
+    // moves the counts to the roots); four consecutive sites per thread, one add where they share the label
+#pragma unroll 2
+    for (int k = 0; k < SITES / 4 / THREADS; ++k) {
+        const uint4 v = lds_u128(par_s + 16u * (k * THREADS + tid));
+        const uint32_t n0 = v.x >> 16, n1 = v.y >> 16, n2 = v.z >> 16, n3 = v.w >> 16;
+        if (n0 == n1 && n2 == n3 && n0 == n2) red_add_s(par_s + 4u * n0, 4u);
+        else {
+            red_add_s(par_s + 4u * n0, 1u); red_add_s(par_s + 4u * n1, 1u);
+            red_add_s(par_s + 4u * n2, 1u); red_add_s(par_s + 4u * n3, 1u);
         }
     }
     __syncthreads();
 
-    // ---- phase 3b: flatten the label nodes ---------------------------------------------------------------
+    // ---- phase 3b: flatten ---------------------------------------------------------------------------
     // The scan gave every site of a run the run's label = a root at that time; the only nodes that ever were
-    // roots are the heads of runs with no bond from the row above ("label nodes", ~0.15 per site at T_c).
-    // One thread per 32-site word finds them by bit tricks and points each at its root, so that afterwards
-    // root(site) = par[par[site]] for every site, without a loop.
-    uint32_t rootbits = 0;                                           // bit c: column c of my word is a tile-local root
-    const int mybase = (tid / NW) * TW + (tid % NW) * 32;
+    // roots are the heads of runs with no bond from the row above ("label nodes", ~0.2 per site at T_c), and
+    // the only ones that no longer are were hooked (~0.03 per site): each of those is pointed at its root and hands
+    // it its count, so that afterwards root(site) = parent(parent(site)) for every site, without a loop, and a
+    // root's count is the size of its tile-local cluster.  The label nodes themselves are only COUNTED (bit tricks
+    // on the bond words): roots = label nodes - hooked nodes.
     {
+        const int mybase = (tid / NW) * TW + (tid % NW) * 32;
         const uint32_t ew = es[tid].x & 0x7FFFFFFFu;
         uint32_t up = (tid / NW) % BAND ? es[tid - NW].y : 0u;       // South bonds of the row above, within the band
         uint32_t m = ew;                                             // OR of the run's uplinks, gathered at its head
@@ -254,100 +368,87 @@ k_bond_label(const uint32_t* __restrict__ sbits, uint32_t* bondE, uint32_t* bond
         up |= (up >> 8) & m;  m &= m >> 8;
         up |= (up >> 16) & m;
         uint32_t o = ~(ew << 1) & ~up;                               // heads of runs without an uplink
-        while (o) {                                                  // two label nodes per round: their loads overlap
-            const int c0 = __ffs(o) - 1;
-            o &= o - 1;
-            const int c1 = o ? __ffs(o) - 1 : c0;
-            o &= o - 1;
-            const int n0 = mybase + c0, n1 = mybase + c1;
-            const int p0 = par[n0], p1 = par[n1];
-            int r0 = p0, r1 = p1;
-            int q0 = par[r0], q1 = par[r1];
-            while (q0 != r0 || q1 != r1) { r0 = q0; r1 = q1; q0 = par[r0]; q1 = par[r1]; }
-            if (p0 == n0) rootbits |= 1u << c0; else if (r0 != p0) par[n0] = r0;
-            if (p1 == n1) rootbits |= 1u << c1; else if (r1 != p1) par[n1] = r1;
+        const int nl = warp_sum_i(__popc(o));
+        if (lane == 0) atomicAdd(&s_nlab, nl);
+        const int nh = s_nhook;                                      // (complete: the barrier above)
+        if (nh <= HKCAP) {
+            for (int j = tid; j < nh; j += THREADS) sc_flatten(par_s, hkitems[j]);
+        } else {                                                     // more hooks than the list holds: visit every label node
+            while (o) {
+                const int n = mybase + __ffs(o) - 1;
+                o &= o - 1;
+                if ((int)lds_u16(par_s + 4u * n + 2u) != n) sc_flatten(par_s, n);
+            }
         }
     }
     __syncthreads();
 
-    // ---- phase 4: open flags (border sites only), then root / global label / size of every site ----------
-    // From here on roots carry size and open bits above IDX_MASK; every read of par[] masks them.
-    for (int j = tid; j < 2 * (TW + TH); j += THREADS) {
-        int site; bool open;
-        if (j < TW)               { site = j;                              open = (nIn[j >> 5] >> (j & 31)) & 1u; }
-        else if (j < 2 * TW)      { const int c = j - TW; site = (TH - 1) * TW + c;
-                                    open = (es[(TH - 1) * NW + (c >> 5)].y >> (c & 31)) & 1u; }
-        else if (j < 2 * TW + TH) { const int r = j - 2 * TW; site = r * TW; open = (wIn[r >> 5] >> (r & 31)) & 1u; }
-        else                      { const int r = j - 2 * TW - TH; site = r * TW + TW - 1;
-                                    open = es[r * NW + NW - 1].x >> 31; }
-        if (open) atomicOr(reinterpret_cast<unsigned int*>(par + sc_find(par, site, IDX_MASK)), OPEN_BIT);
-    }
+    // ---- phase 4: the root of every site -> 16-bit tile-local label; the largest count of the tile ---------
     constexpr int QSTEPS = SITES / 4 / THREADS;                      // = 8
-    constexpr int LOG_TW = 5 + (NW == 8 ? 3 : NW == 4 ? 2 : NW == 2 ? 1 : 0);
+    constexpr int LOG_TW = ilog2_c(TW);
     static_assert((1 << LOG_TW) == TW, "tile width is a power of two");
     const int tilebase = y0 * L + x0;
-    const uint32_t par_s = (uint32_t)__cvta_generic_to_shared(par);  // shared-window address of par[0]
-#pragma unroll
-    for (int k = 0; k < QSTEPS; ++k) {
-        const int q = k * THREADS + tid;
-        const int l = 4 * q;
-        const int4 v = *reinterpret_cast<const int4*>(par + l);
-        // site -> its label node -> root (label nodes are flat; roots carry size / open bits)
-        int r[4] = { par[v.x & IDX_MASK] & IDX_MASK, par[v.y & IDX_MASK] & IDX_MASK,
-                     par[v.z & IDX_MASK] & IDX_MASK, par[v.w & IDX_MASK] & IDX_MASK };
+    {
         // the tile-local 16-bit root of every site is all the sweep stores per site (2 B); the int32 labels
         // of the C ABI are derived from it on demand (k_labels16)
-        const size_t gsite = (size_t)(y0 + (l >> LOG_TW)) * L + x0 + (l & (TW - 1));
-        *reinterpret_cast<uint2*>(lab16 + (size_t)blockIdx.y * N + gsite) =
-            make_uint2((uint32_t)r[0] | ((uint32_t)r[1] << 16), (uint32_t)r[2] | ((uint32_t)r[3] << 16));
-        // sizes: one shared atomic per group of equal neighbours in the quad
-        uint32_t acc = 1u << CNT_SHIFT;
+        uint16_t* out = lab16 + (size_t)blockIdx.y * N + (size_t)(y0 + ((4 * tid) >> LOG_TW)) * L + x0 + ((4 * tid) & (TW - 1));
+        const size_t step = (size_t)(4 * THREADS / TW) * L;          // rows a step of the CTA covers
+        uint32_t mx = 0;
 #pragma unroll
-        for (int u = 1; u < 4; ++u) {
-            const bool cut = r[u] != r[u - 1];
-            red_shared_add_if(par_s + 4u * r[u - 1], acc, cut);      // (predicated: no branch around the atomic)
-            acc = (cut ? 0u : acc) + (1u << CNT_SHIFT);
+        for (int k = 0; k < QSTEPS; ++k) {
+            const uint4 v = lds_u128(par_s + 16u * (k * THREADS + tid));
+            // site -> its label node -> root (label nodes are flat)
+            const uint32_t r0 = lds_u16(par_s + 4u * (v.x >> 16) + 2u), r1 = lds_u16(par_s + 4u * (v.y >> 16) + 2u),
+                           r2 = lds_u16(par_s + 4u * (v.z >> 16) + 2u), r3 = lds_u16(par_s + 4u * (v.w >> 16) + 2u);
+            *reinterpret_cast<uint2*>(out + k * step) = make_uint2(r0 | (r1 << 16), r2 | (r3 << 16));
+            // counts sit at label nodes only (0 elsewhere); a root holds its cluster's size, a hooked node a part of
+            // one: the maximum over all words is the largest tile-local cluster (a piece of a cluster that spans
+            // tiles may enter: its total, which k_flip16 maximises, is no smaller)
+            mx = max(max(mx, v.x & CNT16), max(v.y & CNT16, max(v.z & CNT16, v.w & CNT16)));
         }
-        red_shared_add_if(par_s + 4u * r[3], acc, true);
+        mx = (uint32_t)warp_max_i((int)mx);
+        if (lane == 0) atomicMax(&s_max, (int)mx);
     }
     __syncthreads();
 
-    // ---- phase 5: closed clusters are complete -> maximum; open ones -> the tile's list -----------------
+    // ---- phase 5: a root with a bond across the tile edge becomes a node of the global union-find --------
+    // (order of the border sites: North row, South row, West column, East column).  The first border site to
+    // reach a root claims it: slot in the tile's list, node, and the slot in place of the count in the root's word.
+    // Dense node arrays of CAP entries per tile (L2-resident at L = 16384) instead of the N-entry label array.
     {
-        int mymax = 0, nclosed = 0;
-        // an open tile root becomes node (tile, slot) of the global union-find: dense arrays of CAP entries per
-        // tile (L2-resident at L = 16384) instead of the N-entry label array (random DRAM sectors)
         const int nodebase = blockIdx.x * CAP;                       // node ids are local to the lattice
         const size_t lb = (size_t)blockIdx.y * gridDim.x * CAP;
         int4* mynodes = nodes + lb + nodebase;
-        while (rootbits) {
-            const int l = mybase + __ffs(rootbits) - 1;
-            rootbits &= rootbits - 1;
-            const uint32_t v = (uint32_t)par[l];
-            const int cnt = (int)((v >> CNT_SHIFT) & CNT_MASK);
-            if (v & OPEN_BIT) {
-                const int pos = atomicAdd(&s_nopen, 1);
-                const int g = tilebase + (l >> LOG_TW) * L + (l & (TW - 1));
-                // node = (parent: its own root, size of the cluster rooted here: so far this piece,
-                //         minimum site index of the cluster rooted here, site index of this tile root)
-                mynodes[pos] = make_int4(nodebase + pos, cnt, g, g);
-                par[l] = l | (pos << LS);                            // the root's word now carries its slot
-            } else {
-                mymax = max(mymax, cnt);
-                ++nclosed;                                           // a closed tile root is a cluster root
+        for (int j = tid; j < 2 * (TW + TH); j += THREADS) {
+            int site; bool open;
+            if (j < TW)               { site = j;                              open = (nIn[j >> 5] >> (j & 31)) & 1u; }
+            else if (j < 2 * TW)      { const int c = j - TW; site = (TH - 1) * TW + c;
+                                        open = (es[(TH - 1) * NW + (c >> 5)].y >> (c & 31)) & 1u; }
+            else if (j < 2 * TW + TH) { const int r = j - 2 * TW; site = r * TW; open = (wIn[r >> 5] >> (r & 31)) & 1u; }
+            else                      { const int r = j - 2 * TW - TH; site = r * TW + TW - 1;
+                                        open = es[r * NW + NW - 1].x >> 31; }
+            if (open) {
+                const uint32_t l = lds_u16(par_s + 4u * lds_u16(par_s + 4u * site + 2u) + 2u);   // site -> label node -> root
+                const uint32_t old = atom_or_s(par_s + 4u * l, CLAIMED16);
+                if (!(old & CLAIMED16)) {
+                    const int pos = atomicAdd(&s_nopen, 1);
+                    const int cnt = (int)(old & CNT16);
+                    const int g = tilebase + (int)(l >> LOG_TW) * L + (int)(l & (TW - 1));
+                    // node = (parent: its own root, size of the cluster rooted here: so far this piece,
+                    //         minimum site index of the cluster rooted here, site index of this tile root)
+                    mynodes[pos] = make_int4(nodebase + pos, cnt, g, g);
+                    red_add_s(par_s + 4u * l, (uint32_t)(pos - cnt));     // the root's word now carries its slot
+                }
             }
         }
-        mymax = warp_max_i(mymax);
-        nclosed = warp_sum_i(nclosed);
-        if (lane == 0 && mymax) atomicMax(&s_max, mymax);
-        if (lane == 0 && nclosed) atomicAdd(&s_nclosed, nclosed);
     }
     __syncthreads();
     if (tid == 0) {
         ocount[(size_t)blockIdx.y * gridDim.x + blockIdx.x] = s_nopen;
         Rec* rc = rec + (size_t)ctl->slot * nb + blockIdx.y;
+        const int nclosed = s_nlab - s_nhook - s_nopen;              // roots = label nodes - hooked nodes; closed = not claimed
         if (s_max) atomic_max_ll(&rc->maxcl, s_max);
-        if (s_nclosed) atomic_add_ll(&rc->ncl, s_nclosed);
+        if (nclosed) atomic_add_ll(&rc->ncl, nclosed);               // a closed tile root is a cluster root
         if (FUSE && obs_prev) {                                      // E, M of the previous sweep's configuration
             Rec* rp = rec + (size_t)(ctl->slot == 0 ? ctl->cap - 1 : ctl->slot - 1) * nb + blockIdx.y;
             if (s_obs[0]) atomic_add_ll(&rp->E, s_obs[0]);
@@ -356,7 +457,7 @@ k_bond_label(const uint32_t* __restrict__ sbits, uint32_t* bondE, uint32_t* bond
     }
 
     // ---- phase 6: slot of the root of every border site with a bond across the tile edge ----------------
-    // (order: North row, South row, West column, East column; what k_merge_nodes reads instead of label[])
+    // (what k_merge_nodes reads instead of label[])
     {
         uint16_t* myb = bslot + ((size_t)blockIdx.y * gridDim.x + blockIdx.x) * CAP;
         for (int j = tid; j < 2 * (TW + TH); j += THREADS) {
@@ -369,8 +470,8 @@ k_bond_label(const uint32_t* __restrict__ sbits, uint32_t* bondE, uint32_t* bond
                                         open = es[r * NW + NW - 1].x >> 31; }
             uint32_t slot = 0xFFFFu;
             if (open) {
-                const int r = par[par[site] & IDX_MASK] & IDX_MASK;  // site -> label node -> root
-                slot = ((uint32_t)par[r] >> LS) & (uint32_t)CNT_MASK;
+                const uint32_t l = lds_u16(par_s + 4u * lds_u16(par_s + 4u * site + 2u) + 2u);
+                slot = lds_u32(par_s + 4u * l) & CNT16;
             }
             myb[j] = (uint16_t)slot;
         }

@@ -94,8 +94,8 @@ def test_generic_path_every_sweep(B, L):
         _compare_sweeps(B, L, T, seed + L, 8, path=1)
 
 
-@pytest.mark.parametrize("L,path", [(64, 0), (128, 0), (192, 0), (256, 0), (256, 2), (320, 0), (512, 0), (512, 2), (768, 3),
-                                    (256, 4), (256, 5), (384, 0), (512, 6), (768, 0), (128, 6), (256, 7), (512, 7), (1024, 0), (256, 9), (384, 9), (512, 8)])
+@pytest.mark.parametrize("L,path", [(64, 0), (128, 0), (192, 0), (256, 0), (320, 0), (512, 0), (384, 0), (512, 6), (768, 0),
+                                    (128, 6), (192, 6), (1024, 0), (640, 0)])
 def test_tiled_path_every_sweep(B, L, path):
     for T, seed in ((2.0, 1), (T_C, 2), (3.0, 3)):
         _compare_sweeps(B, L, T, seed + L, 6, path=path)
@@ -118,7 +118,7 @@ def test_survey_golden_vector_on_gpu(B):
     sw.close()
 
 
-@pytest.mark.parametrize("L,path", [(64, 0), (256, 0), (256, 2), (100, 1), (128, 0), (256, 6), (256, 7)])
+@pytest.mark.parametrize("L,path", [(64, 0), (256, 0), (100, 1), (128, 0), (256, 6), (192, 0)])
 def test_special_starts(B, L, path):
     for name, s0 in (("cold", wl.spins_cold(L)), ("down", wl.spins_all_down(L)),
                      ("checker", wl.spins_checkerboard(L)), ("hstripes", wl.spins_stripes(L, 1)),
@@ -140,7 +140,7 @@ def _label_patterns(L):
         yield f"random{d}", wl.bonds_random(L, 7 * L + k, d)
 
 
-@pytest.mark.parametrize("L,path", [(64, 0), (128, 0), (256, 0), (256, 2), (256, 4), (320, 0), (100, 1), (512, 0), (512, 3), (512, 7)])
+@pytest.mark.parametrize("L,path", [(64, 0), (128, 0), (256, 0), (320, 0), (100, 1), (512, 0), (192, 6)])
 def test_labelling_of_injected_bond_graphs(B, L, path):
     """Labelling alone on adversarial bond graphs (long thin spiral, comb, wrap-around rows)."""
     sw = B.SwendsenWang(L, 2.0, 1, path=path)
@@ -336,7 +336,7 @@ def test_invariants_hold_at_size_without_the_oracle(B):
 
 # ------------------------------------------------------------------------------------------------
 # moments accumulated on the device against oracle/moments.py on the oracle's series
-@pytest.mark.parametrize("L,path,T", [(64, 0, T_C), (256, 0, 2.0), (128, 0, 3.0), (20, 1, T_C), (256, 2, T_C), (256, 6, 2.5)])
+@pytest.mark.parametrize("L,path,T", [(64, 0, T_C), (256, 0, 2.0), (128, 0, 3.0), (20, 1, T_C), (192, 0, T_C), (256, 6, 2.5)])
 def test_moments_match_oracle(B, L, path, T):
     from oracle import moments as om
     seed, therm, n = 31 + L, 7, 40
@@ -379,7 +379,7 @@ def test_moments_of_a_batch(B):
 
 # ------------------------------------------------------------------------------------------------
 # many sweeps in ONE call: the steady sweep is replayed from CUDA graphs (sw_set_graphs, default on)
-@pytest.mark.parametrize("L,path,n", [(128, 0, 37), (256, 0, 12), (256, 7, 21), (64, 0, 50), (512, 6, 9)])
+@pytest.mark.parametrize("L,path,n", [(128, 0, 37), (256, 0, 12), (192, 0, 21), (64, 0, 50), (512, 6, 9)])
 def test_many_sweeps_per_call_with_and_without_graphs(B, L, path, n):
     T, seed = T_C, 77 + L
     s_ref, ser_ref = oracle.run(L, T, seed, n)
@@ -573,7 +573,7 @@ def test_potts_argument_errors(B):
             B.sw_create_potts(16, q, 1.0, 1)
     h = B.sw_create_potts(16, 3, 1.0, 1)
     with pytest.raises(Exception):
-        B.sw_set_path(h, 2)                          # tiled Ising kernels read sign bits
+        B.sw_set_path(h, 6)                          # the stand-alone Ising bond kernel reads sign bits
     B.sw_destroy(h)
 
 
@@ -619,7 +619,7 @@ def test_switching_paths_keeps_one_state(B):
     sw = B.SwendsenWang(L, T, seed)
     s = oracle.init_random(L, seed)
     t = 0
-    for path, n in ((0, 2), (1, 2), (0, 1), (6, 2), (11, 1), (0, 2), (2, 1), (9, 2)):
+    for path, n in ((0, 2), (1, 2), (0, 1), (6, 2), (11, 1), (0, 2), (6, 1), (0, 2)):
         B.sw_set_path(sw.h, path)
         for _ in range(n):
             s, bE, bS, lab, obs = oracle.sweep(L, T, seed, t, s)
