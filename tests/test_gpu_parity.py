@@ -102,8 +102,8 @@ def test_tiled_path_every_sweep(B, L, path):
 
 
 def test_config1_L64_many_sweeps(B):
-    # BASELINE configs[0]: L = 64, T = 2.26919, seed 2024 -- every sweep for the first 200, in full
-    _compare_sweeps(B, 64, wl.T_C_PRINTED, 2024, 200)
+    # BASELINE configs[0]: L = 64, T = 2.26919, seed 2024 -- every one of the 1000 sweeps, in full
+    _compare_sweeps(B, 64, wl.T_C_PRINTED, 2024, 1000)
 
 
 def test_survey_golden_vector_on_gpu(B):
@@ -314,9 +314,85 @@ def test_one_step_parity_headline_L16384(B):
     """BASELINE configs[3]: L = 16384, T_c, seed 6 -- in the launch configuration bench.py times."""
     L, T, seed = 16384, T_C, 6
     sw = B.SwendsenWang(L, T, seed)
+    for t in (0, 1, 2, 100, 199):         # SURVEY.md 8(d), config 4: the random start, then the state the bench times
+        sw.sweep(t - sw.sweep_index)
+        _one_step(B, sw, L, T, seed)
+    sw.close()
+
+
+def test_one_step_parity_headline_cold_start(B):
+    """L = 16384 from the cold start: the first sweep's bonds percolate (p = 0.586 per edge): one cluster holds most
+    sites, every tile has ~100 open roots hanging under one node."""
+    L, T, seed = 16384, T_C, 6
+    sw = B.SwendsenWang(L, T, seed)
+    sw.set_cold()
     _one_step(B, sw, L, T, seed)          # t = 0
-    sw.sweep(6)
-    _one_step(B, sw, L, T, seed)          # t = 7
+    _one_step(B, sw, L, T, seed)          # t = 1
+    sw.close()
+
+
+def test_one_step_parity_at_the_largest_side(B):
+    """SW_MAX_L = 32768: N = 2^30, the int32 edge the ABI advertises (labels up to 2^30 - 1, 32-bit word and site
+    indices in every kernel)."""
+    L, T, seed = 32768, T_C, 9
+    sw = B.SwendsenWang(L, T, seed)
+    _one_step(B, sw, L, T, seed)          # t = 0
+    sw.close()
+
+
+def test_config2_every_sweep(B):
+    """BASELINE configs[1]: L = 1024, T in {2.0, 2.26919, 3.0}, seeds 1, 2, 3 -- the first 200 sweeps, each in full."""
+    for T, seed in ((2.0, 1), (wl.T_C_PRINTED, 2), (3.0, 3)):
+        _compare_sweeps(B, 1024, T, seed, 200)
+
+
+@pytest.mark.parametrize("seed,start", [(4, "cold"), (5, "random")])
+def test_config3_sweeps_0_to_9_then_every_100th(B, seed, start):
+    """BASELINE configs[2]: L = 4096, T_c, 1000 sweeps -- sweeps 0 .. 9 in full, then one-step parity at every 100th."""
+    L, T = 4096, T_C
+    sw = B.SwendsenWang(L, T, seed)
+    if start == "cold":
+        sw.set_cold()
+    for t in list(range(10)) + list(range(100, 1001, 100)):
+        sw.sweep(t - sw.sweep_index)
+        _one_step(B, sw, L, T, seed)
+    sw.close()
+
+
+def test_config5_at_size(B):
+    """BASELINE configs[4]: 32 lattices of L = 2048, T_b = 1.5 + 2 b / 31, seeds 1000 + b, one launch per stage for the
+    batch.  Lattices b = 0, 12, 31 against three oracle runs, every sweep for 20 sweeps, then one step after 200."""
+    L, nb = 2048, 32
+    Ts, seeds = wl.scan_temperatures(nb), [1000 + b for b in range(nb)]
+    sw = B.SwendsenWang(L, Ts, seeds)
+    pick = (0, 12, 31)
+    ref = {b: oracle.init_random(L, seeds[b]) for b in pick}
+    g0 = sw.spins()
+    for b in pick:
+        assert np.array_equal(g0[b].cpu().numpy().reshape(-1), ref[b])
+
+    def check(t):
+        before = {b: ref[b] for b in pick}
+        sw.sweep(1)
+        gs, gl = sw.spins(), sw.labels()
+        gE, gS = sw.bonds()
+        obs = sw.observables()
+        for b in pick:
+            s1, bE, bS, lab, o = oracle.sweep(L, Ts[b], seeds[b], t, before[b])
+            assert np.array_equal(gE[b].cpu().numpy().view(np.uint32), wl.pack_bits(bE)), (b, t)
+            assert np.array_equal(gS[b].cpu().numpy().view(np.uint32), wl.pack_bits(bS)), (b, t)
+            assert np.array_equal(gl[b].cpu().numpy().reshape(-1), lab), (b, t)
+            assert np.array_equal(gs[b].cpu().numpy().reshape(-1), s1), (b, t)
+            assert _obs_tuple(obs[b]) == o, (b, t)
+            ref[b] = s1
+
+    for t in range(20):
+        check(t)
+    sw.sweep(180)
+    g = sw.spins()
+    for b in pick:
+        ref[b] = g[b].cpu().numpy().reshape(-1).copy()
+    check(200)
     sw.close()
 
 
@@ -352,11 +428,12 @@ def test_moments_match_oracle(B, L, path, T):
     _, ser = oracle.run(L, T, seed, therm + n)
     ref = om.moments(ser[therm:, 0], ser[therm:, 1], N, T)
     assert got["n"] == n
+    # the device adds the same doubles in the same order with unfused operations: the means are the oracle's to the
+    # last bit, and so are the derived quantities (same formula on the same doubles); the bar is north_star's 1e-12
     for k in ("e_mean", "e2_mean", "absm_mean", "m2_mean", "m4_mean"):
-        assert abs(got[k] - ref[k]) <= 1e-12 * max(1.0, abs(ref[k])), (k, got[k], ref[k])
-    # derived quantities subtract nearly equal means: same formula on the same doubles
+        assert got[k] == ref[k], (k, got[k], ref[k])
     for k in ("specific_heat", "susceptibility", "binder"):
-        assert abs(got[k] - ref[k]) <= 1e-12 * max(1.0, abs(ref[k])) * N, (k, got[k], ref[k])
+        assert abs(got[k] - ref[k]) <= 1e-12 * abs(ref[k]), (k, got[k], ref[k])
     sw.close()
 
 
@@ -780,6 +857,6 @@ def test_temperature_scan_batch_against_kaufman_on_the_gpu(B):
         u, du = ex.binned_mean_err(ser[:, b, 0] / (L * L), nbins=30)
         exact = float(ex.kaufman_u(L, T))
         worst = max(worst, abs(u - exact) / du)
-        assert abs(u - exact) <= 4.5 * du and du < 3e-3, (T, u, du, exact)
+        assert abs(u - exact) <= 4.0 * du and du < 3e-3, (T, u, du, exact)
     assert worst > 0.0
     sw.close()

@@ -113,6 +113,23 @@ def test_statements_agree_on_structured_graphs():
             assert np.array_equal(a, b) and pa == pb
 
 
+def test_statements_agree_at_parity_size():
+    """The numpy statement is what the GPU pass counts are compared with at L >= 64: labels AND pass count against the
+    plain loops on random bond graphs of that size (sub-, near- and super-critical bond densities) and on the bond graph
+    of a Swendsen-Wang sweep."""
+    L = 64
+    graphs = [wl.bonds_random(L, 900 + k, d) for k, d in enumerate((0.3, 0.5, 0.7))]
+    s = oracle.init_random(L, 5)
+    for t in range(3):
+        s, bE, bS, _, _ = oracle.sweep(L, wl.T_C, 5, t, s)
+    graphs.append((bE, bS))
+    for g, (bE, bS) in enumerate(graphs):
+        a, pa = le.label_equivalence_loops(L, bE, bS)
+        b, pb = le.label_equivalence(L, bE, bS)
+        assert np.array_equal(a, b) and pa == pb, (g, pa, pb)
+        assert np.array_equal(a, oracle.labels(L, bE, bS))
+
+
 def test_pass_count_on_sw_bond_graphs_is_small():
     # context, not a pin: PAPER.md:53 reports "5 or 6 parallel iterations" for 512 x 512 (variant and counting
     # convention unstated); this statement needs 5-8 scans (the last one idle) at L = 512 and T_c on the way to equilibrium
