@@ -64,17 +64,6 @@ def measured_peaks():
     return 6650.0, "fallback (B200_PROFILING.md)"
 
 
-def ncu_traffic(kernel: str):
-    """Per-launch DRAM bytes of `kernel` from the committed ncu --set full summary, or None."""
-    p = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(p):
-        try:
-            return json.load(open(p)).get(kernel)
-        except Exception:
-            return None
-    return None
-
-
 class ClockSampler:
     QUERY = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
              "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
@@ -123,19 +112,68 @@ class ClockSampler:
         return out
 
 
-def cpu_oracle_baseline(L_sample: int, T: float, seed: int, sweeps: int):
-    """The serial oracle, as it stands, on one host core: site-updates/s on a bounded sample."""
+def _pin_one_core():
+    """Pin this process to one host core (what `taskset -c` does) for the oracle leg; returns the previous affinity."""
+    try:
+        prev = os.sched_getaffinity(0)
+        core = sorted(prev)[-1]
+        os.sched_setaffinity(0, {core})
+        return prev, core
+    except Exception:
+        return None, None
+
+
+def _unpin(prev):
+    if prev:
+        try:
+            os.sched_setaffinity(0, prev)
+        except Exception:
+            pass
+
+
+def cpu_oracle_baseline(L: int, T: float, seed: int, sweeps: int, scaling_Ls=()):
+    """The serial oracle, as it stands, on ONE pinned host core: `sweeps` full sweeps (t = 0 ..) of the L x L workload
+    from its random start, stage by stage through the oracle's own entry points (bond / label / assign / observe), plus
+    one sweep at each side of `scaling_Ls` so that the size dependence of the rate is on the record."""
     import oracle
     oracle.lib()
-    s = oracle.init_random(L_sample, seed)
-    t0 = time.perf_counter()
-    oracle.run(L_sample, T, seed, sweeps, spins=s, series=False)
-    dt = time.perf_counter() - t0
-    return L_sample * L_sample * sweeps / dt, dt
+    prev, core = _pin_one_core()
+    try:
+        thr = oracle.threshold(T)
+        N = L * L
+        s = oracle.init_random(L, seed)
+        st = {"bond": 0.0, "label": 0.0, "assign": 0.0, "observe": 0.0}
+        t_all = time.perf_counter()
+        for t in range(sweeps):
+            t0 = time.perf_counter(); bE, bS = oracle.bonds(L, thr, seed, t, s)
+            t1 = time.perf_counter(); lab = oracle.labels(L, bE, bS)
+            t2 = time.perf_counter(); s = oracle.assign(L, seed, t, lab)
+            t3 = time.perf_counter(); oracle.observables(L, s, lab)
+            t4 = time.perf_counter()
+            st["bond"] += t1 - t0; st["label"] += t2 - t1; st["assign"] += t3 - t2; st["observe"] += t4 - t3
+        dt = time.perf_counter() - t_all
+        scaling = []
+        for Ls in scaling_Ls:
+            ss = oracle.init_random(Ls, seed)
+            t0 = time.perf_counter()
+            oracle.run(Ls, T, seed, 1, spins=ss, series=False)
+            scaling.append({"L": Ls, "site_updates_per_s": Ls * Ls / (time.perf_counter() - t0), "sweeps": 1})
+    finally:
+        _unpin(prev)
+    return {"value": N * sweeps / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
+            "sample": f"{sweeps} full sweeps (t = 0 .. {sweeps - 1}, random start) of the L={L} lattice at T_c, {dt:.1f} s of CPU "
+                      f"work, serial C oracle (gcc -O2), one core (sched_setaffinity to core {core}) of {os.cpu_count()}",
+            "L": L, "sweeps": sweeps, "seconds": dt,
+            "stage_ns_per_site": {k: 1e9 * v / (N * sweeps) for k, v in st.items()},
+            "stage_site_updates_per_s": {k: (N * sweeps / v if v > 0 else None) for k, v in st.items()},
+            "scaling": scaling}
 
 
 def run_reference(args):
-    """--impl reference: the oracle timed on the host cores (rank 0 only)."""
+    """--impl reference: the oracle timed on the host cores (rank 0 only).  Each step is one full sweep of an
+    L = --ref-L sample of the workload, so that K + W steps end within a few minutes (a sweep of the full L = 16384
+    lattice takes ~17 s on one core: the default bench's cpu_baseline leg times three of those and prints the size
+    dependence)."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return 0
@@ -144,28 +182,221 @@ def run_reference(args):
     oracle.lib()
     Ls = args.ref_L
     T, seed = wl.T_C, 6
-    s = oracle.init_random(Ls, seed)
-    t = 0
-    for _ in range(args.warmup):
-        s, _ = oracle.run(Ls, T, seed, 1, spins=s, t0=t, series=False); t += 1
-    t0 = time.perf_counter()
-    for _ in range(args.steps):
-        s, _ = oracle.run(Ls, T, seed, 1, spins=s, t0=t, series=False); t += 1
-    dt = time.perf_counter() - t0
+    prev, core = _pin_one_core()
+    try:
+        s = oracle.init_random(Ls, seed)
+        t = 0
+        for _ in range(args.warmup):
+            s, _ = oracle.run(Ls, T, seed, 1, spins=s, t0=t, series=False); t += 1
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            s, _ = oracle.run(Ls, T, seed, 1, spins=s, t0=t, series=False); t += 1
+        dt = time.perf_counter() - t0
+    finally:
+        _unpin(prev)
     val = Ls * Ls * args.steps / dt
     sample = (f"each step = one full sweep of an L={Ls} lattice at T_c (a {Ls}x{Ls} sample of the "
-              f"L={args.L} workload), serial C oracle, gcc -O2, 1 thread")
+              f"L={args.L} workload), serial C oracle, gcc -O2, one pinned core (core {core})")
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
-        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int8/int32",
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int8 spins / int32 labels / uint32 Philox",
         "data": "synthetic",
         "config": {"workload": f"2D Ising SW sweep, L={args.L}, T=T_c, random start (BASELINE configs[3])",
-                   "reference_sample_L": Ls},
+                   "reference_sample_L": Ls, "same_config": Ls == args.L},
         "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }))
     return 0
+
+
+def profile_numbers():
+    """Numbers that come from the committed ncu capture (profiles/traffic.json), not from this run: per-launch DRAM bytes,
+    issue-slot occupancy, executed instruction slots per site.  Everything taken from here is labelled with its source."""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    try:
+        j = json.load(open(p))
+    except Exception:
+        return {}
+    return {"source": j.get("_source"), "sites": j.get("_sites", 268435456),
+            "dram_bytes_per_launch": {k: v for k, v in j.items() if not k.startswith("_")},
+            "issue_active_pct": j.get("_issue_active_pct"), "thread_instr_slots_per_site": j.get("_thread_instr_slots_per_site")}
+
+
+def _timed_sweeps(sw, n):
+    """ms per sweep of one sw_sweep(n) call on the handle's stream (graphs on), CUDA events."""
+    import torch
+    st = torch.cuda.current_stream(sw.device)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize(sw.device)
+    e0.record(st); sw.sweep(n); e1.record(st)
+    torch.cuda.synchronize(sw.device)
+    return e0.elapsed_time(e1) / n
+
+
+def block_unfused(B, L, T, seed, dev, W, K, peak, philox_ms):
+    """The per-stage split with a stand-alone bond kernel (BASELINE config 3 asks for bond / label / flip): the same lattice on
+    path 6 (k_bond_rows, then labelling from the bond planes), a few sweeps; the bond stage against max(HBM, Philox ALU)."""
+    N = L * L
+    sw6 = B.SwendsenWang(L, T, seed, device=str(dev), path=6)
+    sw6.sweep(W)
+    sw6.set_stage_timing(True)
+    K6 = min(K, 10)
+    sw6.sweep(K6)
+    st6 = sw6.stage_ms()
+    sw6.close()
+    out = {s_: {"ms": v / K6, "model_bytes_per_site": STAGE_MODEL[s_],
+                "model_frac_of_peak": (STAGE_MODEL[s_] * N / (v / K6 * 1e-3) / 1e9 / peak) if v > 0 else None}
+           for s_, v in st6.items()}
+    hbm_ms = STAGE_MODEL["bond"] * N / (peak * 1e9) * 1e3
+    bond_ms = out["bond"]["ms"]
+    if philox_ms:
+        out["bond"].update({"philox_only_ms": philox_ms, "hbm_ms_at_peak": hbm_ms,
+                            "frac_of_binding_bound": max(philox_ms, hbm_ms) / bond_ms if bond_ms > 0 else None,
+                            "binding_bound": "alu (Philox4x32-10)" if philox_ms > hbm_ms else "hbm"})
+    out["note"] = ("model_frac_of_peak charges the SURVEY.md 8(d) model bytes: the observe stage reads bit-packed spins (1/8 of the "
+                   "model's bytes), so its model fraction can exceed 1 -- it is not a bandwidth; the stand-alone bond kernel is bound by "
+                   "the Philox4x32-10 integer work, not by its 1.25 B/site")
+    return out
+
+
+def block_label_equivalence(B, L, T, seed, dev, W, K, stages):
+    """A/B: the paper's own labelling (label equivalence; path 11) on the same lattice and sweeps."""
+    sw11 = B.SwendsenWang(L, T, seed, device=str(dev), path=11)
+    sw11.sweep(W)
+    sw11.set_stage_timing(True)
+    K11 = min(K, 5)
+    sw11.sweep(K11)
+    st11, km11 = sw11.stage_ms(), sw11.kernel_ms()
+    passes = sw11.label_passes()
+    sw11.close()
+    return {"label_ms": st11["label"] / K11, "k_label_equiv_ms": km11.get("tile_label", 0.0) / K11,
+            "passes_last_sweep": passes, "sweeps": K11,
+            "kernels_ms": {k_: v_ / K11 for k_, v_ in km11.items() if v_ > 0},
+            "label_ms_union_find": stages["label"]["ms"],
+            "note": "label stage of the paper's iteration (scan -> collapse -> relabel until no reference forms) "
+                    "vs the tile union-find path's bond_label + merge + roots (which also draws the bonds)"}
+
+
+def block_potts(B, L, seed, dev, W, K):
+    """The q-state Potts model on the same sweep: q = 3 at its T_c, fast path (128 x 64 tiles)."""
+    qp, Tp = 3, 1.0 / math.log(1.0 + math.sqrt(3.0))
+    N = L * L
+    swp = B.SwendsenWang(L, Tp, seed, device=str(dev), q=qp)
+    swp.sweep(W)
+    swp.set_stage_timing(True)
+    Kp = min(K, 10)
+    swp.sweep(Kp)
+    stp, kmp = swp.stage_ms(), swp.kernel_ms()
+    op = swp.observables()[0]
+    swp.close()
+    tot = sum(stp.values()) / Kp
+    return {"q": qp, "T": Tp, "ms_per_sweep": tot, "site_updates_per_s": N / (tot * 1e-3), "sweeps": Kp,
+            "stages_ms": {k_: v_ / Kp for k_, v_ in stp.items()},
+            "kernels_ms": {k_: v_ / Kp for k_, v_ in kmp.items() if v_ > 0},
+            "state_after": {"e_per_site": op.e_per_site, "order_parameter": op.abs_m_per_site / (qp - 1),
+                            "n_clusters": int(op.n_clusters), "largest_cluster": int(op.largest_cluster)}}
+
+
+def block_eager_labels(B, L, T, seed, dev, W, K):
+    """The same run with the flat int32 labels materialised EVERY sweep (sw_set_eager_labels): what the lazy k_labels16 saves."""
+    N = L * L
+    swe = B.SwendsenWang(L, T, seed, device=str(dev))
+    B.sw_set_eager_labels(swe.h, True)
+    swe.sweep(W)
+    ms = _timed_sweeps(swe, min(K, 20))
+    swe.close()
+    return {"ms_per_sweep": ms, "site_updates_per_s": N / (ms * 1e-3), "sweeps": min(K, 20),
+            "note": "every sweep also writes the 4 B/site canonical labels (k_labels16); the headline leaves them to sw_labels"}
+
+
+def block_equilibrated(B, sw, N):
+    """BASELINE configs[3] is 200 sweeps and the state drifts: the lattice of the timed run is taken to sweep 200, then 20 more
+    sweeps are timed (graphs on, as in the headline)."""
+    sw.set_stage_timing(False)
+    done = int(sw.sweep_index)
+    if done < 200:
+        sw.sweep(200 - done)
+    first = int(sw.sweep_index)
+    ms = _timed_sweeps(sw, 20)
+    o = sw.observables()[0]
+    return {"ms_per_sweep": ms, "site_updates_per_s": N / (ms * 1e-3), "timed_sweeps": f"{first} .. {first + 19}",
+            "state_after": {"sweep": int(o.sweep), "e_per_site": o.e_per_site, "abs_m_per_site": o.abs_m_per_site,
+                            "n_clusters": int(o.n_clusters), "largest_cluster": int(o.largest_cluster)}}
+
+
+def block_config3(B, wl, dev):
+    """BASELINE configs[2]: L = 4096, T_c, cold (seed 4) and random (seed 5) start: per-stage ms from the unfused path 6, and the
+    fused path's ms per sweep over the first 300 sweeps (first / mean / last-half mean)."""
+    L, T, N = 4096, wl.T_C, 4096 * 4096
+    out = {}
+    for name, seed in (("cold", 4), ("random", 5)):
+        r = {}
+        s6 = B.SwendsenWang(L, T, seed, device=str(dev), path=6)
+        if name == "cold":
+            s6.set_cold()
+        s6.set_stage_timing(True)
+        s6.sweep(100)
+        r["stages_ms_unfused"] = {k: v / 100 for k, v in s6.stage_ms().items()}
+        s6.close()
+        s0 = B.SwendsenWang(L, T, seed, device=str(dev))
+        if name == "cold":
+            s0.set_cold()
+        s0.set_stage_timing(True)
+        s0.sweep(300)
+        per = s0.sweep_ms()
+        r["fused_ms_per_sweep"] = {"first": float(per[0]), "mean": float(per.mean()), "mean_last_half": float(per[len(per) // 2:].mean()),
+                                   "sweeps": int(len(per)), "note": "per-kernel CUDA events (no graph replay)"}
+        s0.set_stage_timing(False)
+        ms = _timed_sweeps(s0, 200)
+        r["fused_ms_per_sweep_graphs"] = ms
+        r["site_updates_per_s"] = N / (ms * 1e-3)
+        s0.close()
+        out[name] = r
+    return out
+
+
+def block_config5(B, wl, dev):
+    """BASELINE configs[4]: 32 lattices of L = 2048, T = 1.5 .. 3.5, seeds 1000 + b, one launch per stage for the batch."""
+    L, nb = 2048, 32
+    sw = B.SwendsenWang(L, wl.scan_temperatures(nb), [1000 + b for b in range(nb)], device=str(dev))
+    sw.sweep(50)
+    ms = _timed_sweeps(sw, 200)
+    sw.close()
+    return {"ms_per_batch_sweep": ms, "lattices": nb, "L": L, "site_updates_per_s": nb * L * L / (ms * 1e-3), "sweeps": 200,
+            "note": "sweeps 50 .. 249 of the 1000; aggregate over the 32 lattices"}
+
+
+def block_paper_sizes(B, dev):
+    """The paper's own table (Fig. 8): L = 128 .. 4096 at k_B T = 2.5, time per sweep (graphs on)."""
+    paper_gpu_min = {128: 0.112, 256: 0.151, 512: 0.390, 1024: 1.472, 2048: 5.483, 4096: 22.440}     # 10,000 iterations, Tesla P100
+    paper_cpu_min = {128: 0.339, 256: 1.369, 512: 5.367, 1024: 21.497, 2048: 89.504, 4096: 400.372}   # Haswell E5-2695, serial
+    out = {}
+    for L in (128, 256, 512, 1024, 2048, 4096):
+        sw = B.SwendsenWang(L, 2.5, 10 + L, device=str(dev))
+        sw.sweep(100)
+        ms = _timed_sweeps(sw, 400)
+        sw.close()
+        out[str(L)] = {"us_per_sweep": 1e3 * ms, "site_updates_per_s": L * L / (ms * 1e-3),
+                       "paper_gpu_us_per_sweep": paper_gpu_min[L] * 60e6 / 1e4, "paper_cpu_us_per_sweep": paper_cpu_min[L] * 60e6 / 1e4}
+    out["note"] = "paper_*: PAPER.md:137-142 (another machine: context, not a target); ours: 400 sweeps after 100, one sw_sweep call"
+    return out
+
+
+def block_config2_moments(B, wl, dev):
+    """BASELINE configs[1] (L = 1024, T = 2.0 / 2.26919 / 3.0, 200 + 2000 sweeps) with the on-device error analysis: <e> with its
+    binned error and the integrated autocorrelation time of e and |m| (the paper's motivation)."""
+    L = 1024
+    Ts = [2.0, wl.T_C_PRINTED, 3.0]
+    sw = B.SwendsenWang(L, Ts, [1, 2, 3], device=str(dev))
+    sw.sweep(200)
+    ms = _timed_sweeps(sw, 2000)
+    be, te, tm = sw.bins(0, 50), sw.autocorr(0, 200), sw.autocorr(1, 200)
+    sw.close()
+    return {"ms_per_batch_sweep": ms, "per_temperature": [
+        {"T": Ts[b], "e_mean": be[b]["mean"], "e_binned_err": be[b]["err"], "bins": be[b]["n_bins"],
+         "tau_int_e": te[b]["tau_int"], "window_e": te[b]["window"], "tau_int_absm": tm[b]["tau_int"], "window_absm": tm[b]["window"]}
+        for b in range(3)]}
 
 
 def main():
@@ -176,11 +407,12 @@ def main():
     ap.add_argument("--L", type=int, default=16384)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-unfused", action="store_true", help="skip the short unfused (path 6) per-stage measurement")
-    ap.add_argument("--ref-L", type=int, default=2048, help="sample lattice side for --impl reference")
-    ap.add_argument("--cpu-sample-L", type=int, default=8192, help="sample side for the cpu_baseline leg")
+    ap.add_argument("--ref-L", type=int, default=4096, help="sample lattice side for --impl reference (one sweep per step)")
+    ap.add_argument("--cpu-sample-L", type=int, default=16384, help="lattice side for the cpu_baseline leg")
+    ap.add_argument("--cpu-sweeps", type=int, default=3, help="oracle sweeps (t = 0 ..) the cpu_baseline leg times")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--path", type=int, default=0, help="0 auto (fused scan-line, 256x64 tiles), 1 generic, 2/3 first-generation tiles 64x64 / 256x32, 4/5 scan 64/128 wide, 6 unfused, 7 scan 256x32")
+    ap.add_argument("--path", type=int, default=0, help="0 the fast path (fused bond + scan-line labelling, 128x64 tiles), 1 generic kernels, 6 unfused stages, 11 the paper's label equivalence")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
 
@@ -211,12 +443,7 @@ def main():
     N = L * L
     seed = rp.replica_seed(rank)                      # configs[3] uses seed 6; replicas take 6 + rank
     sw = B.SwendsenWang(L, T, seed, device=str(dev), path=args.path)
-    if args.path in (0, 4, 5, 6, 7, 8, 9):
-        tw, th = (64 if args.path == 4 else 256 if (args.path in (7, 8) and L % 256 == 0) else 128 if L % 128 == 0 else 64), 32
-        if args.path == 8 or (tw == 128 and args.path != 5):
-            th = 64
-    else:
-        tw, th = (256, 32) if (L % 256 == 0 and args.path == 3) else (64, 64)
+    tw, th = (128, 64) if L % 128 == 0 else (64, 32)
 
     def barrier():
         if dist is not None:
@@ -302,125 +529,123 @@ def main():
     # ---- roofline of the dominant kernel, per-stage split
     peak, peak_src = measured_peaks()
     kb = kernel_bytes_per_site(tw, th)
+    prof = profile_numbers()
     dom = max(kms, key=lambda k: kms[k])
     dom_ms = kms[dom] / timed
     achieved = kb.get(dom, 0.0) * N / (dom_ms * 1e-3) / 1e9
-    issue = (ncu_traffic("_issue_active_pct") or {}).get(dom)
+
+    def real(kernel, ms_launch):
+        """DRAM bytes the kernel really moves per launch (ncu --set full capture committed under profiles/), the bandwidth
+        that is at its live CUDA-event time, and the fraction of the measured peak -- or Nones without a capture."""
+        rb = (prof.get("dram_bytes_per_launch") or {}).get(kernel)
+        if not rb or ms_launch <= 0:
+            return {"real_bytes": None, "real_GBps": None, "real_frac_of_peak": None}
+        g = rb * (N / prof.get("sites", N)) / (ms_launch * 1e-3) / 1e9
+        return {"real_bytes": rb * (N / prof.get("sites", N)), "real_GBps": g, "real_frac_of_peak": g / peak}
+
     roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": ncu_traffic(dom), "peak_source": peak_src,
-                "issue_active_pct": issue,      # ncu smsp__issue_active of this kernel (profiles/): what really binds it
+                "frac": achieved / peak, "traffic": (prof.get("dram_bytes_per_launch") or {}).get(dom),
+                "traffic_source": prof.get("source"), "peak_source": peak_src,
+                "note": "achieved = ALGORITHMIC bytes (SURVEY.md 8(d) model, bytes_per_site x sites) / live CUDA-event time; traffic = "
+                        "DRAM bytes of one launch from the committed ncu capture (real_* below are computed from it): the kernel moves "
+                        "less than the model charges (bit-packed spins, 16-bit roots) and is bound by instruction issue, not by HBM",
                 "bytes_per_site": kb.get(dom), "ms_per_launch": dom_ms,
-                "share_of_step": kms[dom] / max(1e-9, sum(kms.values()))}
-    # the same kernel against the bound that really holds it: instruction issue.  peak = 148 SMs x
-    # 4 schedulers x 32 lanes x SM clock (one warp instruction per scheduler and cycle; guide: B200_PROFILING.md unit
-    # counts); achieved = thread-instruction slots the kernel executes per site (committed ncu count, profiles/) x N /
-    # its live CUDA-event time; algorithmic = the Philox4x32-10 draws alone (24 integer instructions per site).
-    tips = (ncu_traffic("_thread_instr_slots_per_site") or {}).get(dom)
+                "share_of_step": kms[dom] / max(1e-9, sum(kms.values())),
+                "issue_active_pct": (prof.get("issue_active_pct") or {}).get(dom),
+                "issue_active_source": prof.get("source")}
+    roofline.update(real(dom, dom_ms))
+    # the same kernel against the bound that really holds it (DESIGN.md section 7): integer issue.  The binding floor is the
+    # Philox4x32-10 draws the RNG convention fixes: a kernel that makes only those (sw_test_philox_ceiling, measured live, here)
     sm_ghz = (clk.get("sm_mhz") or 1965.0) / 1e3
     alu_peak = 148 * 4 * 32 * sm_ghz / 1e3                               # T thread-instruction slots / s
-    roofline_alu = None
-    if tips:
-        ach = tips * N / (dom_ms * 1e-3) / 1e12
-        roofline_alu = {"bound": "alu", "kernel": dom, "achieved": ach, "peak": alu_peak, "unit": "T thread-instr/s",
-                        "frac": ach / alu_peak, "thread_instr_slots_per_site": tips,
-                        "algorithmic_instr_per_site": 24, "algorithmic_frac": 24 * N / (dom_ms * 1e-3) / 1e12 / alu_peak,
-                        "peak_source": "148 SMs x 4 schedulers x 32 lanes x measured SM clock"}
+    philox_ms = None
+    try:
+        philox_ms = B.sw_test_philox_ceiling(N, 20)
+    except Exception:
+        pass
+    tips = (prof.get("thread_instr_slots_per_site") or {}).get(dom)
+    roofline_alu = {"bound": "alu", "kernel": dom, "unit": "T thread-instr/s", "peak": alu_peak,
+                    "peak_source": "148 SMs x 4 schedulers x 32 lanes x SM clock sampled in this run (one warp instruction per scheduler and cycle)",
+                    "philox_only_ms": philox_ms,
+                    "frac": (philox_ms / dom_ms) if philox_ms else None,
+                    "frac_note": "measured time of the sweep's Philox draws alone / this kernel's time: the share of the kernel that the "
+                                 "RNG convention makes unavoidable",
+                    "achieved": (24 * N / (dom_ms * 1e-3) / 1e12),
+                    "achieved_note": "24 Philox instructions per site (20 per call of 40, + compares) x sites / kernel time",
+                    "issue_slot_occupancy": (tips * N / (dom_ms * 1e-3) / 1e12 / alu_peak) if tips else None,
+                    "thread_instr_slots_per_site": tips, "slots_source": prof.get("source")}
     stages = {}
     for s, v in stage.items():
         sms = v / timed
         stages[s] = {"ms": sms, "site_updates_per_s": N / (sms * 1e-3) if sms > 0 else None,
                      "model_bytes_per_site": STAGE_MODEL[s],
-                     "hbm_frac": (STAGE_MODEL[s] * N / (sms * 1e-3) / 1e9 / peak) if sms > 0 else None}
-    kernels = {k: {"ms": v / timed, "GBps_model": (kb.get(k, 0.0) * N / (v / timed * 1e-3) / 1e9) if v > 0 else None}
-               for k, v in kms.items()}
+                     "model_frac_of_peak": (STAGE_MODEL[s] * N / (sms * 1e-3) / 1e9 / peak) if sms > 0 else None}
+        if s == "observe":                          # one pass over the bit-packed plane per sw_sweep CALL, spread over its sweeps
+            stages[s].update({"model_frac_of_peak": None, "amortised_over_sweeps": timed,
+                              "ms_per_call": v, "real_bytes_per_call": 3 * N // 8,
+                              "real_GBps_per_call": (3 * N / 8 / (v * 1e-3) / 1e9) if v > 0 else None,
+                              "note": "E and M of a sweep come out of the NEXT sweep's bond test; only the last sweep of a call "
+                                      "needs this pass (own word + South word + East bit of the 1 bit/site plane, mostly L2 hits)"})
+    # real bytes of a stage = those of its kernels
+    stage_kernels = {"label": ("bond_label", "merge", "roots_open"), "flip": ("flipbits", "flip16")}
+    for st_, ks_ in stage_kernels.items():
+        rb = [(prof.get("dram_bytes_per_launch") or {}).get(k_) for k_ in ks_]
+        if st_ in stages and all(v is not None for v in rb) and stages[st_]["ms"] > 0:
+            g = sum(rb) * (N / prof.get("sites", N)) / (stages[st_]["ms"] * 1e-3) / 1e9
+            stages[st_].update({"real_bytes": sum(rb), "real_GBps": g, "real_frac_of_peak": g / peak})
+    kernels = {}
+    for k, v in kms.items():
+        if v <= 0:
+            continue
+        e = {"ms": v / timed, "model_bytes_per_site": kb.get(k, 0.0),
+             "model_GBps": kb.get(k, 0.0) * N / (v / timed * 1e-3) / 1e9}
+        e["model_frac_of_peak"] = e["model_GBps"] / peak
+        e.update(real(k, v / timed))
+        if k == "energy":                           # (see stages.observe: once per call, amortised)
+            e.update({"model_GBps": None, "model_frac_of_peak": None, "amortised_over_sweeps": timed})
+        kernels[k] = e
     sweep_gbs = SWEEP_MODEL_BYTES_PER_SITE * N / (ms / K * 1e-3) / 1e9
+    real_sweep = sum(v for v in (prof.get("dram_bytes_per_launch") or {}).values() if isinstance(v, (int, float)))
+    sweep_model = {"bytes_per_site": SWEEP_MODEL_BYTES_PER_SITE, "achieved_GBps": sweep_gbs,
+                   "frac_of_peak": sweep_gbs / peak, "frac_of_8TBps_nominal": sweep_gbs / 8000.0,
+                   "real_bytes_per_sweep": real_sweep or None,
+                   "real_GBps": (real_sweep / (ms / K * 1e-3) / 1e9) if real_sweep else None,
+                   "real_frac_of_peak": (real_sweep / (ms / K * 1e-3) / 1e9 / peak) if real_sweep else None,
+                   "real_source": prof.get("source")}
 
-    # ---- the per-stage split with a stand-alone bond kernel (BASELINE config 3 asks for bond / label / flip):
-    # the same lattice on path 6 (k_bond_rows, then labelling from the bond planes), a few sweeps
-    unfused = None
-    if not args.no_unfused:
+    def side(fn):                                   # never lose the headline line over a side measurement
         try:
-            sw6 = B.SwendsenWang(L, T, seed, device=str(dev), path=6)
-            sw6.sweep(W)
-            sw6.set_stage_timing(True)
-            K6 = min(K, 10)
-            sw6.sweep(K6)
-            st6 = sw6.stage_ms()
-            sw6.close()
-            unfused = {s_: {"ms": v / K6, "model_bytes_per_site": STAGE_MODEL[s_],
-                            "hbm_frac": (STAGE_MODEL[s_] * N / (v / K6 * 1e-3) / 1e9 / peak) if v > 0 else None}
-                       for s_, v in st6.items()}
-            # the bond stage against max(HBM time, measured Philox-only ALU ceiling)
-            alu_ms = B.sw_test_philox_ceiling(N, 20)
-            hbm_ms = STAGE_MODEL["bond"] * N / (peak * 1e9) * 1e3
-            bond_ms = unfused["bond"]["ms"]
-            unfused["bond"].update({"philox_only_ms": alu_ms, "hbm_ms_at_peak": hbm_ms,
-                                    "frac_of_binding_bound": max(alu_ms, hbm_ms) / bond_ms if bond_ms > 0 else None,
-                                    "binding_bound": "alu (Philox4x32-10)" if alu_ms > hbm_ms else "hbm"})
-            unfused["note"] = ("stand-alone bond kernel: bound by the Philox4x32-10 integer work (>= 24 instructions per site), "
-                               "not by its 1.25 B/site")
-        except Exception as e:                       # never lose the headline line over the side measurement
-            unfused = {"error": str(e)}
-
-    # ---- A/B: the paper's own labelling (label equivalence) on the same lattice and sweeps
-    # (path 11: one cooperative kernel runs the passes to convergence)
-    equiv = None
-    if not args.no_unfused:
-        try:
-            sw11 = B.SwendsenWang(L, T, seed, device=str(dev), path=11)
-            sw11.sweep(W)
-            sw11.set_stage_timing(True)
-            K11 = min(K, 10)
-            sw11.sweep(K11)
-            st11, km11 = sw11.stage_ms(), sw11.kernel_ms()
-            passes = sw11.label_passes()
-            sw11.close()
-            equiv = {"label_ms": st11["label"] / K11, "k_label_equiv_ms": km11.get("tile_label", 0.0) / K11,
-                     "passes_last_sweep": passes, "sweeps": K11,
-                     "kernels_ms": {k_: v_ / K11 for k_, v_ in km11.items() if v_ > 0},
-                     "label_ms_union_find": stages["label"]["ms"],
-                     "note": "label stage of the paper's iteration (scan -> collapse -> relabel until no reference forms) "
-                             "vs the tile union-find path's bond_label + merge + roots (which also draws the bonds)"}
+            return fn()
         except Exception as e:
-            equiv = {"error": str(e)}
+            return {"error": repr(e)}
 
-    # ---- the q-state Potts model on the same sweep (generic kernels): q = 3 at its T_c
-    potts = None
+    extras = {}
     if not args.no_unfused:
-        try:
-            qp, Tp = 3, 1.0 / math.log(1.0 + math.sqrt(3.0))
-            swp = B.SwendsenWang(L, Tp, seed, device=str(dev), q=qp)
-            swp.sweep(W)
-            swp.set_stage_timing(True)
-            Kp = min(K, 10)
-            swp.sweep(Kp)
-            stp, kmp = swp.stage_ms(), swp.kernel_ms()
-            op = swp.observables()[0]
-            swp.close()
-            tot = sum(stp.values()) / Kp
-            potts = {"q": qp, "T": Tp, "ms_per_sweep": tot, "site_updates_per_s": N / (tot * 1e-3), "sweeps": Kp,
-                     "stages_ms": {k_: v_ / Kp for k_, v_ in stp.items()},
-                     "kernels_ms": {k_: v_ / Kp for k_, v_ in kmp.items() if v_ > 0},
-                     "state_after": {"e_per_site": op.e_per_site, "order_parameter": op.abs_m_per_site / (qp - 1),
-                                     "n_clusters": int(op.n_clusters), "largest_cluster": int(op.largest_cluster)}}
-        except Exception as e:
-            potts = {"error": str(e)}
+        extras["stages_unfused"] = side(lambda: block_unfused(B, L, T, seed, dev, W, K, peak, philox_ms))
+        extras["label_equivalence"] = side(lambda: block_label_equivalence(B, L, T, seed, dev, W, K, stages))
+        extras["potts"] = side(lambda: block_potts(B, L, seed, dev, W, K))
+        extras["value_eager_labels"] = side(lambda: block_eager_labels(B, L, T, seed, dev, W, K))
+        extras["equilibrated"] = side(lambda: block_equilibrated(B, sw, N))
+        sw.close()
+        extras["config3"] = side(lambda: block_config3(B, wl, dev))
+        extras["config5"] = side(lambda: block_config5(B, wl, dev))
+        extras["paper_sizes"] = side(lambda: block_paper_sizes(B, dev))
+        extras["config2_moments"] = side(lambda: block_config2_moments(B, wl, dev))
 
     cpu = None
     if not args.no_cpu_baseline:
-        Ls = min(args.cpu_sample_L, L)
-        v, dt = cpu_oracle_baseline(Ls, T, 6, 1)
-        cpu = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle",
-               "sample": f"1 full sweep (t=0, random start) of an L={Ls} lattice at T_c, {dt:.1f} s of CPU work, "
-                         f"serial C oracle (gcc -O2), 1 of {os.cpu_count()} host cores"}
+        cpu = side(lambda: cpu_oracle_baseline(min(args.cpu_sample_L, L), T, 6, args.cpu_sweeps, scaling_Ls=(2048, 4096)))
 
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "int8 spins / int32 labels / uint32 Philox", "data": "synthetic",
+        "dtype": "bit-packed spins (1 bit/site) and uint16 tile-local roots on the device; int8 spins / int32 labels at the C ABI "
+                 "(derived on demand: see value_eager_labels); uint32 Philox4x32-10 words compared as integers",
+        "data": "synthetic",
         "config": {"workload": f"2D Ising Swendsen-Wang, L={L} periodic, J=1, T=T_c=2/ln(1+sqrt2), random start "
                                f"seed {6}+rank, one sweep per step (BASELINE configs[3])",
                    "sites_per_gpu": N, "tile": f"{tw}x{th}", "parallelism": f"replicas x{world}",
+                   "timed_sweeps": f"sweeps {W} .. {W + K - 1} after the random start (see `equilibrated` for the state after 200)",
                    "l2_policy": "working set larger than L2: every sweep streams the 512 MiB 16-bit root plane out and in, plus bond planes, bit-packed spins and node arrays (~0.7 GB) vs 126 MB L2",
                    "state_after": {"sweep": int(obs.sweep), "e_per_site": obs.e_per_site,
                                    "abs_m_per_site": obs.abs_m_per_site, "n_clusters": int(obs.n_clusters),
@@ -429,13 +654,13 @@ def main():
         "e2e": e2e, "e2e_int8": e2e_int8,
         "gpu_launches": int(launches),
         "roofline": roofline, "roofline_alu": roofline_alu,
-        "sweep_model": {"bytes_per_site": SWEEP_MODEL_BYTES_PER_SITE, "achieved_GBps": sweep_gbs,
-                        "frac_of_peak": sweep_gbs / peak, "frac_of_8TBps_nominal": sweep_gbs / 8000.0},
-        "per_sweep": per_sweep, "stages": stages, "stages_unfused": unfused, "label_equivalence": equiv, "potts": potts, "kernels": kernels,
+        "sweep_model": sweep_model,
+        "per_sweep": per_sweep, "stages": stages, "kernels": kernels,
         "cpu_baseline": cpu,
         "paper_context": "paper: 17x (SW) / 90x (Wolff) over serial, Haswell E5-2695 vs Tesla P100; "
                          "SW GPU rate 1.25e8 site-updates/s at L=4096 (PAPER.md:127,142)",
     }
+    out.update(extras)
     print(json.dumps(out))
     if dist is not None:
         dist.destroy_process_group()

@@ -48,7 +48,7 @@ extern "C" {
 #define SW_OK       0
 #define SW_EINVAL  -1   /* L < 2, L > 32768, T <= 0 or not finite, n < 0, nb < 1, null pointer, bad size */
 #define SW_ENOMEM  -2   /* host or device allocation failed / workspace too small */
-#define SW_ECUDA   -3   /* CUDA error (sticky); text in sw_last_error() */
+#define SW_ECUDA   -3   /* CUDA error; text in sw_last_error() */
 #define SW_ESTATE  -4   /* labels / bonds asked for before the first sweep, etc. */
 
 #define SW_MAX_L   32768      /* int32 labels: N <= 2^30 */
@@ -97,8 +97,8 @@ void       sw_destroy(sw_handle* h);                       /* NULL is a no-op */
  * label >> 2, word label & 3); random start: the same with TAG_INIT, t = 0, field = site index.
  * q in 2 .. 127.  A Potts handle answers every call of this header; differences: sw_obs.energy = -#(equal East /
  * South pairs), sw_obs.magnetisation = q * max_c n_c - N (n_c = sites of colour c), abs_m_per_site =
- * magnetisation / N; sw_set_cold sets colour 0; sw_set_spins takes colours; paths 0 / 1 (generic kernels, any L) and
- * 11 only.  sw_create_potts allocates its own workspace; sw_create_potts_in takes one of sw_workspace_bytes(L, nb)
+ * magnetisation / N; sw_set_cold sets colour 0; sw_set_spins takes colours; paths 0 (128 x 64 tiles when L is a
+ * multiple of 128, else the generic kernels), 1 (generic kernels) and 11 only.  sw_create_potts allocates its own workspace; sw_create_potts_in takes one of sw_workspace_bytes(L, nb)
  * bytes like sw_create_in (plus nb*q*4 bytes the library allocates itself for the colour counts).
  * NULL + error text on invalid arguments (q outside 2 .. 127, and as for sw_create). */
 sw_handle* sw_create_potts(int32_t L, int32_t q, double T, uint64_t seed);
@@ -155,9 +155,10 @@ uint64_t   sw_sweep_index(const sw_handle* h);
 
 int        sw_set_stream(sw_handle* h, void* cuda_stream); /* a cudaStream_t; NULL = default stream */
 
-/* Per-sweep history of the LAST sw_sweep call, oldest first: entry (k*nb + b) is lattice b after the
- * k-th retained sweep.  At most `cap` entries are written; returns the number of sweeps retained
- * (<= the series capacity, default 4096 sweeps, see sw_set_series_capacity) or a negative code. */
+/* Per-sweep history of the LAST sw_sweep call, oldest first: record (k*nb + b) is lattice b after the
+ * k-th retained sweep.  `cap` counts SWEEPS: `out` (HOST) must hold cap * nb records, and min(retained, cap) * nb
+ * are written; returns the number of sweeps retained (<= the series capacity, default 4096 sweeps, see
+ * sw_set_series_capacity) or a negative code. */
 int64_t    sw_series(sw_handle* h, sw_obs* out, int64_t cap);
 int        sw_set_series_capacity(sw_handle* h, int64_t sweeps);
 
@@ -177,6 +178,26 @@ typedef struct {
 int        sw_moments(sw_handle* h, sw_mom* out);
 int        sw_moments_reset(sw_handle* h);
 
+/* Error analysis of the per-sweep series the LAST sw_sweep call left on the device (the sweeps sw_series returns),
+ * binning and the integrated autocorrelation time -- the quantity the paper's motivation is
+ * about (tau ~ |g - g*|^(-z) for local updates; cluster updates keep it small; section 4).
+ * The paper gives no formulas; the textbook definitions are taken:
+ *   series x_k = E_k / N (which = 0) or |M_k| / N (which = 1), retained sweeps in order, n of them;
+ *   sw_bins: n_bins = floor(n / bin_len) bins of consecutive sweeps (a remainder at the end is dropped); a bin mean is
+ *     the exact integer sum of its E_k (or |M_k|) divided once by bin_len * N; mean = mean of the bin means;
+ *     err = sqrt( sum (b_j - mean)^2 / (n_bins (n_bins - 1)) ), 0 with fewer than two bins;
+ *   sw_autocorr: C(t) = (1/(n-t)) sum_k (x_k - xbar)(x_{k+t} - xbar), rho(t) = C(t) / C(0), t = 0 .. min(tmax, n-1);
+ *     tau_int = 1/2 + sum_{t=1}^{W} rho(t) with the self-consistent window W = smallest W >= 1 with W >= c * tau(W)
+ *     (c = 6 is customary), else the last lag; a constant series has rho = 0, tau_int = 1/2, window = 0.
+ * All sums run on the device in index order in double with unfused operations.  Both calls synchronise.
+ * out[0..nb-1] (HOST).  bin_means: NULL or HOST [nb][cap] (the first min(n_bins, cap) bin means of each lattice);
+ * rho: NULL or HOST [nb][tmax + 1] (0 beyond lag n - 1); sw_taustat.tmax = the last lag computed, c0 = C(0).
+ * SW_ESTATE when there is no series (no sweep since the state was set), SW_EINVAL on bad arguments. */
+typedef struct { int64_t n_bins; double mean, err; } sw_binstat;
+typedef struct { double tau_int; int64_t window, tmax; double c0; } sw_taustat;
+int        sw_bins(sw_handle* h, int32_t which, int64_t bin_len, double* bin_means, int64_t cap, sw_binstat* out);
+int        sw_autocorr(sw_handle* h, int32_t which, int64_t tmax, double c, double* rho, sw_taustat* out);
+
 /* Per-stage device time in ms, summed over the sweeps of the last sw_sweep call that ran with stage
  * timing on: out = {bond, label, flip, observe}.  Stage timing brackets each stage with CUDA events
  * (it serialises nothing but adds event records; off by default).  BASELINE config 3. */
@@ -194,19 +215,18 @@ const char* sw_kernel_name(int32_t i);
 int64_t    sw_sweep_ms(sw_handle* h, float* out, int64_t cap);
 
 /* Select the kernel path.  Results are identical on every path.
- *   0  automatic: the fused scan-line path when L is a multiple of 64 (tiles of 256, 128 or 64 x 32 sites,
- *      the widest that divides L), the generic path otherwise
+ *   0  the fast path: fused bond draw + scan-line tile labelling on 128 x 64 tiles when L is a multiple of 128, on
+ *      64 x 32 tiles when it is a multiple of 64, the generic kernels otherwise
  *   1  generic any-L path (global union-find, no tiles)
- *   2, 3  the first-generation tiled kernels (64 x 64 / 256 x 32 tiles, thread-per-site union-find), kept for A/B timing
- *   4, 5  scan-line path forced to 64- / 128-wide tiles
- *   6  as 0 but UNFUSED: stand-alone bond kernel, then labelling from the bond planes (per-stage timing of
- *      bond / label / flip, BASELINE config 3)
- *   7, 8, 9  scan-line path forced to 256 x 32, 256 x 64, 128 x 64 tiles
+ *   6  as 0 but UNFUSED, on the int8 spin plane: stand-alone bond kernel, then labelling from the bond planes
+ *      (per-stage timing of bond / label / flip, BASELINE config 3); Ising handles only
  *   11 the paper's own labelling (section 2.3): the label-equivalence iteration scan -> collapse
  *      -> relabel, repeated until a scan forms no reference, run to convergence by ONE cooperative kernel (in
  *      place of the paper's dynamic-parallelism maintenance kernel); any L; kept for A/B timing
  *      against the union-find paths.  Allocates nb*N*4 extra bytes with cudaMalloc on first use (freed by
- *      sw_destroy). */
+ *      sw_destroy).
+ * Any other value: SW_EINVAL.  (The flat int32 labels of sw_labels and the size array of paths 1 / 11, nb*N*4 bytes
+ * each, are allocated by the library on first use, outside a caller-supplied workspace, and freed by sw_destroy.) */
 int        sw_set_path(sw_handle* h, int path);
 
 /* Path 11 only: number of passes (scans, including the last one that formed no reference) the label-equivalence

@@ -38,6 +38,16 @@ class sw_mom(C.Structure):
         return {k: getattr(self, k) for k, _ in self._fields_}
 
 
+class sw_binstat(C.Structure):
+    """Mirror of include/sw.h sw_binstat."""
+    _fields_ = [("n_bins", C.c_int64), ("mean", C.c_double), ("err", C.c_double)]
+
+
+class sw_taustat(C.Structure):
+    """Mirror of include/sw.h sw_taustat."""
+    _fields_ = [("tau_int", C.c_double), ("window", C.c_int64), ("tmax", C.c_int64), ("c0", C.c_double)]
+
+
 class SwError(RuntimeError):
     def __init__(self, code: int, text: str):
         super().__init__(f"sw error {code}: {text}")
@@ -72,6 +82,8 @@ PROTOTYPES = {
     "sw_set_series_capacity": (C.c_int, [_VP, _I64]),
     "sw_moments": (C.c_int, [_VP, C.POINTER(sw_mom)]),
     "sw_moments_reset": (C.c_int, [_VP]),
+    "sw_bins": (C.c_int, [_VP, _I32, C.c_int64, C.POINTER(C.c_double), C.c_int64, C.POINTER(sw_binstat)]),
+    "sw_autocorr": (C.c_int, [_VP, _I32, C.c_int64, C.c_double, C.POINTER(C.c_double), C.POINTER(sw_taustat)]),
     "sw_set_stage_timing": (C.c_int, [_VP, C.c_int]),
     "sw_stage_ms": (C.c_int, [_VP, C.POINTER(C.c_float)]),
     "sw_kernel_ms": (C.c_int, [_VP, C.POINTER(C.c_float), _I32]),
@@ -223,6 +235,26 @@ def sw_moments(h) -> List[dict]:
 
 def sw_moments_reset(h) -> None:
     _check(lib().sw_moments_reset(_ptr(h)))
+
+def sw_bins(h, which: int, bin_len: int, want_means: bool = True):
+    """Binning of the last call's series (which: 0 = E/N, 1 = |M|/N): per lattice (n_bins, mean, err[, bin means])."""
+    nb = lib().sw_batch(_ptr(h))
+    out = (sw_binstat * nb)()
+    _check(lib().sw_bins(h, which, bin_len, None, 0, out))           # first the number of bins
+    nbins = int(out[0].n_bins)
+    means = np.zeros((nb, max(nbins, 1)), dtype=np.float64)
+    if want_means and nbins > 0:
+        _check(lib().sw_bins(h, which, bin_len, means.ctypes.data_as(C.POINTER(C.c_double)), means.shape[1], out))
+    return [{"n_bins": int(o.n_bins), "mean": o.mean, "err": o.err, "bin_means": means[b, :nbins].copy()} for b, o in enumerate(out)]
+
+def sw_autocorr(h, which: int, tmax: int, c: float = 6.0):
+    """Normalised autocorrelation rho(0 .. tmax) of the last call's series and the windowed tau_int, per lattice."""
+    nb = lib().sw_batch(_ptr(h))
+    out = (sw_taustat * nb)()
+    rho = np.zeros((nb, tmax + 1), dtype=np.float64)
+    _check(lib().sw_autocorr(h, which, tmax, c, rho.ctypes.data_as(C.POINTER(C.c_double)), out))
+    return [{"tau_int": o.tau_int, "window": int(o.window), "tmax": int(o.tmax), "c0": o.c0, "rho": rho[b, :int(o.tmax) + 1].copy()}
+            for b, o in enumerate(out)]
 
 def sw_set_graphs(h, on: bool) -> None:
     _check(lib().sw_set_graphs(_ptr(h), 1 if on else 0))
@@ -405,6 +437,12 @@ class SwendsenWang:
 
     def moments_reset(self):
         sw_moments_reset(self.h)
+
+    def bins(self, which: int, bin_len: int):
+        return sw_bins(self.h, which, bin_len)
+
+    def autocorr(self, which: int, tmax: int, c: float = 6.0):
+        return sw_autocorr(self.h, which, tmax, c)
 
     # -- state
     def set_spins(self, spins):

@@ -7,6 +7,7 @@
 #include "sw_scan.cuh"
 #include "sw_equiv.cuh"
 #include "sw_potts.cuh"
+#include "sw_series.cuh"
 
 #include <algorithm>
 #include <cmath>
@@ -894,6 +895,83 @@ int sw_moments_reset(sw_handle* h) {
     if (!h) { set_err("sw_moments_reset: null handle"); return SW_EINVAL; }
     DevGuard dg(h->dev);
     SW_CUDA(cudaMemsetAsync(h->mom, 0, (size_t)h->nb * sizeof(Mom), h->stream));
+    return SW_OK;
+}
+
+namespace {
+// the retained sweeps of the last sw_sweep call, as the kernels of sw_series.cuh see them
+bool series_view(const sw_handle* h, int32_t which, SeriesView* v) {
+    if (!h->rec_valid || h->last_n <= 0) return false;
+    const int64_t kept = std::min(h->last_n, h->series_cap);
+    v->rec = h->series; v->first = h->last_n - kept; v->ring = h->ring(); v->n = kept; v->nb = h->nb; v->which = which;
+    return true;
+}
+struct DevBuf {                 // scratch of one analysis call, freed on every exit
+    void* p = nullptr;
+    ~DevBuf() { if (p) cudaFree(p); }
+    cudaError_t alloc(size_t bytes) { return cudaMalloc(&p, bytes ? bytes : 1); }
+};
+} // namespace
+
+int sw_bins(sw_handle* h, int32_t which, int64_t bin_len, double* bin_means, int64_t cap, sw_binstat* out) {
+    if (!h || !out || (which != 0 && which != 1) || bin_len < 1 || cap < 0) { set_err("sw_bins: invalid argument"); return SW_EINVAL; }
+    DevGuard dg(h->dev);
+    SeriesView v;
+    if (!series_view(h, which, &v)) { set_err("sw_bins: no series (no sw_sweep since the last state change)"); return SW_ESTATE; }
+    const long long nbins = v.n / bin_len;
+    DevBuf bins, stat;
+    if (bins.alloc((size_t)h->nb * nbins * sizeof(double)) != cudaSuccess || stat.alloc((size_t)h->nb * sizeof(BinStat)) != cudaSuccess) {
+        (void)cudaGetLastError(); set_err("sw_bins: cudaMalloc failed"); return SW_ENOMEM;
+    }
+    if (nbins > 0)
+        k_series_bins<<<grid1((size_t)nbins, 256, h->nb), 256, 0, h->stream>>>(v, (double*)bins.p, bin_len, nbins, h->N);
+    k_series_binerr<<<(h->nb + 63) / 64, 64, 0, h->stream>>>((const double*)bins.p, (BinStat*)stat.p, nbins, h->nb);
+    SW_CUDA(cudaGetLastError());
+    std::vector<BinStat> hs(h->nb);
+    SW_CUDA(cudaMemcpyAsync(hs.data(), stat.p, sizeof(BinStat) * h->nb, cudaMemcpyDeviceToHost, h->stream));
+    std::vector<double> hb;
+    if (bin_means && nbins > 0) {
+        hb.resize((size_t)h->nb * nbins);
+        SW_CUDA(cudaMemcpyAsync(hb.data(), bins.p, hb.size() * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    }
+    SW_CUDA(cudaStreamSynchronize(h->stream));
+    const int64_t give = std::min<int64_t>(nbins, cap);
+    for (int b = 0; b < h->nb; ++b) {
+        out[b].n_bins = hs[b].n_bins; out[b].mean = hs[b].mean; out[b].err = hs[b].err;
+        if (bin_means) for (int64_t j = 0; j < give; ++j) bin_means[(size_t)b * cap + j] = hb[(size_t)b * nbins + j];
+    }
+    return SW_OK;
+}
+
+int sw_autocorr(sw_handle* h, int32_t which, int64_t tmax, double c, double* rho, sw_taustat* out) {
+    if (!h || !out || (which != 0 && which != 1) || tmax < 0 || !(c > 0.0)) { set_err("sw_autocorr: invalid argument"); return SW_EINVAL; }
+    DevGuard dg(h->dev);
+    SeriesView v;
+    if (!series_view(h, which, &v)) { set_err("sw_autocorr: no series (no sw_sweep since the last state change)"); return SW_ESTATE; }
+    const long long tm = std::min<long long>(tmax, v.n - 1);            // (rho is still written with stride tmax + 1)
+    DevBuf x, xbar, C, R, stat;
+    if (x.alloc((size_t)h->nb * v.n * sizeof(double)) != cudaSuccess || xbar.alloc((size_t)h->nb * sizeof(double)) != cudaSuccess ||
+        C.alloc((size_t)h->nb * (tm + 1) * sizeof(double)) != cudaSuccess || R.alloc((size_t)h->nb * (tm + 1) * sizeof(double)) != cudaSuccess ||
+        stat.alloc((size_t)h->nb * sizeof(TauStat)) != cudaSuccess) {
+        (void)cudaGetLastError(); set_err("sw_autocorr: cudaMalloc failed"); return SW_ENOMEM;
+    }
+    k_series_x<<<grid1((size_t)v.n, 256, h->nb), 256, 0, h->stream>>>(v, (double*)x.p, h->N);
+    k_series_mean<<<(h->nb + 63) / 64, 64, 0, h->stream>>>((const double*)x.p, (double*)xbar.p, v.n, h->nb);
+    k_series_autocov<<<grid1((size_t)(tm + 1), 128, h->nb), 128, 0, h->stream>>>((const double*)x.p, (const double*)xbar.p, (double*)C.p, v.n, tm);
+    k_series_tau<<<(h->nb + 63) / 64, 64, 0, h->stream>>>((const double*)C.p, (double*)R.p, (TauStat*)stat.p, tm, c, h->nb);
+    SW_CUDA(cudaGetLastError());
+    std::vector<TauStat> hs(h->nb);
+    SW_CUDA(cudaMemcpyAsync(hs.data(), stat.p, sizeof(TauStat) * h->nb, cudaMemcpyDeviceToHost, h->stream));
+    std::vector<double> hr;
+    if (rho) {
+        hr.resize((size_t)h->nb * (tm + 1));
+        SW_CUDA(cudaMemcpyAsync(hr.data(), R.p, hr.size() * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    }
+    SW_CUDA(cudaStreamSynchronize(h->stream));
+    for (int b = 0; b < h->nb; ++b) {
+        out[b].tau_int = hs[b].tau_int; out[b].window = hs[b].window; out[b].tmax = hs[b].tmax; out[b].c0 = hs[b].c0;
+        if (rho) for (int64_t t = 0; t <= tmax; ++t) rho[(size_t)b * (tmax + 1) + t] = t <= tm ? hr[(size_t)b * (tm + 1) + t] : 0.0;
+    }
     return SW_OK;
 }
 

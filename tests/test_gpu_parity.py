@@ -454,6 +454,71 @@ def test_moments_of_a_batch(B):
     sw.close()
 
 
+# SURVEY.md 8(f) NEXT-1, second half: binning and the integrated autocorrelation time over the device series ring
+@pytest.mark.parametrize("L,path,T,n,cap", [(64, 0, T_C, 400, None), (128, 0, 2.0, 300, None), (20, 1, T_C, 257, None),
+                                            (64, 0, 3.0, 300, 128)])
+def test_binning_and_autocorrelation_match_oracle(B, L, path, T, n, cap):
+    from oracle import moments as om
+    seed, N = 900 + L, L * L
+    sw = B.SwendsenWang(L, T, seed, path=path)
+    if cap:
+        B.sw_set_series_capacity(sw.h, cap)          # the ring keeps the last `cap` sweeps of the call
+    sw.sweep(n)
+    _, ser = oracle.run(L, T, seed, n)
+    ser = ser[-cap:] if cap else ser
+    E, M = ser[:, 0], ser[:, 1]
+    for which in (0, 1):
+        for bl in (1, 7, 50, len(E), len(E) + 1):
+            got = sw.bins(which, bl)[0]
+            means = om.bin_means(E, M, N, which, bl)
+            mean, err, nb = om.binned_error(E, M, N, which, bl)
+            assert got["n_bins"] == nb == len(means)
+            assert got["bin_means"].tolist() == means                      # exact integer sums, one division
+            assert abs(got["mean"] - mean) <= 1e-12 * abs(mean) and abs(got["err"] - err) <= 1e-12 * err
+        for tmax, c in ((60, 6.0), (5, 6.0), (len(E) + 10, 4.0)):
+            got = sw.autocorr(which, tmax, c)[0]
+            tau, W, rho = om.tau_int(E, M, N, which, tmax, c)
+            assert got["window"] == W and got["tmax"] == len(rho) - 1
+            assert abs(got["tau_int"] - tau) <= 1e-12 * abs(tau)
+            assert np.all(np.abs(got["rho"] - np.array(rho)) <= 1e-12 * np.maximum(1.0, np.abs(rho)))
+            assert abs(got["c0"] - om.autocovariance(E, M, N, which, 0)[0]) <= 1e-12 * got["c0"]
+    sw.close()
+
+
+def test_binning_of_a_batch_and_without_a_series(B):
+    from oracle import moments as om
+    L, Ts, seeds, n = 64, [2.0, T_C, 3.0], [31, 32, 33], 200
+    sw = B.SwendsenWang(L, Ts, seeds)
+    with pytest.raises(B.SwError):
+        sw.bins(0, 10)                               # no sweep yet
+    sw.sweep(n)
+    gb, gt = sw.bins(1, 20), sw.autocorr(0, 30)
+    for b in range(3):
+        _, ser = oracle.run(L, Ts[b], seeds[b], n)
+        mean, err, nb = om.binned_error(ser[:, 0], ser[:, 1], L * L, 1, 20)
+        assert gb[b]["n_bins"] == nb and abs(gb[b]["mean"] - mean) <= 1e-12 * mean and abs(gb[b]["err"] - err) <= 1e-12 * err
+        tau, W, _ = om.tau_int(ser[:, 0], ser[:, 1], L * L, 0, 30)
+        assert gt[b]["window"] == W and abs(gt[b]["tau_int"] - tau) <= 1e-12 * tau
+    with pytest.raises(B.SwError):
+        sw.bins(2, 10)
+    with pytest.raises(B.SwError):
+        sw.autocorr(0, 10, c=0.0)
+    sw.close()
+
+
+def test_critical_slowing_down_is_absent(B):
+    """The paper's motivation made visible: tau_int of the energy stays of order one for cluster updates,
+    at T_c as away from it (config 2's temperatures, L = 256)."""
+    L, n = 256, 2000
+    sw = B.SwendsenWang(L, [2.0, T_C, 3.0], [1, 2, 3])
+    sw.sweep(200)
+    sw.sweep(n)
+    taus = [r["tau_int"] for r in sw.autocorr(0, 100)]
+    assert all(0.4 < t < 12.0 for t in taus), taus
+    assert taus[1] > taus[0] and taus[1] > taus[2]   # largest at the critical point, but small (z ~ 0.2)
+    sw.close()
+
+
 # ------------------------------------------------------------------------------------------------
 # many sweeps in ONE call: the steady sweep is replayed from CUDA graphs (sw_set_graphs, default on)
 @pytest.mark.parametrize("L,path,n", [(128, 0, 37), (256, 0, 12), (192, 0, 21), (64, 0, 50), (512, 6, 9)])
