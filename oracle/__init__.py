@@ -25,13 +25,17 @@ _SO = os.path.join(_HERE, "liboracle_sw.so")
 TAG_INIT, TAG_BOND, TAG_FLIP = 0, 1, 2
 
 
+_SRC4 = os.path.join(os.path.dirname(os.path.abspath(__file__)), "phi4_oracle.c")
+
+
 def build(force: bool = False) -> str:
-    """Compile sw_oracle.c -> liboracle_sw.so with gcc -O2 (no tuning flags)."""
-    stale = (not os.path.exists(_SO)) or os.path.getmtime(_SO) < os.path.getmtime(_SRC)
+    """Compile sw_oracle.c + phi4_oracle.c -> liboracle_sw.so with gcc -O2 (no tuning flags; -std=c99 keeps
+    floating-point contraction off, stated explicitly: no fused multiply-add anywhere)."""
+    stale = (not os.path.exists(_SO)) or os.path.getmtime(_SO) < max(os.path.getmtime(_SRC), os.path.getmtime(_SRC4))
     if force or stale:
         tmp = _SO + ".tmp%d" % os.getpid()
         subprocess.check_call(
-            ["gcc", "-O2", "-std=c99", "-fPIC", "-shared", "-o", tmp, _SRC, "-lm"])
+            ["gcc", "-O2", "-std=c99", "-ffp-contract=off", "-fPIC", "-shared", "-o", tmp, _SRC, _SRC4, "-lm"])
         os.replace(tmp, _SO)
     return _SO
 
