@@ -383,6 +383,34 @@ def block_paper_sizes(B, dev):
     return out
 
 
+def block_phi4(dev):
+    """The paper's second workload (Fig. 9): the Wolff-type embedded cluster update for O(4) phi^4 in four
+    dimensions at kappa = 0.304, L = 16 .. 28, time per update (one phi4_sweep call of 1000 updates after 200, graphs on)."""
+    import torch
+    from paper_2302_14720_b200 import phi4
+    paper_gpu_min = {16: 0.186, 20: 0.305, 24: 0.619, 28: 1.188}           # 10,000 iterations, Tesla P100
+    paper_cpu_min = {16: 11.246, 20: 26.931, 24: 57.939, 28: 106.821}      # Haswell E5-2695, serial
+    out = {}
+    for L in (16, 20, 24, 28):
+        g = phi4.Phi4(L, 0.304, 1, device=str(dev))
+        g.sweep(200)
+        st = torch.cuda.current_stream(dev)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize(dev)
+        e0.record(st); g.sweep(1000); e1.record(st)
+        torch.cuda.synchronize(dev)
+        us = 1e3 * e0.elapsed_time(e1) / 1000
+        o = g.observables()
+        g.close()
+        out[str(L)] = {"us_per_update": us, "site_updates_per_s": L ** 4 / (us * 1e-6),
+                       "paper_gpu_us_per_update": paper_gpu_min[L] * 60e6 / 1e4, "paper_cpu_us_per_update": paper_cpu_min[L] * 60e6 / 1e4,
+                       "state_after": {"link_per_link": o.link_per_link, "abs_m_per_site": o.abs_m_per_site,
+                                       "n_clusters": int(o.n_clusters), "largest_cluster": int(o.largest_cluster)}}
+    out["note"] = ("paper_*: PAPER.md:152-156 (another machine: context, not a target); the update is the cluster step only (Eq. 2-3), "
+                   "double precision, 6 launches per update replayed from a CUDA graph")
+    return out
+
+
 def block_config2_moments(B, wl, dev):
     """BASELINE configs[1] (L = 1024, T = 2.0 / 2.26919 / 3.0, 200 + 2000 sweeps) with the on-device error analysis: <e> with its
     binned error and the integrated autocorrelation time of e and |m| (the paper's motivation)."""
@@ -631,6 +659,7 @@ def main():
         extras["config5"] = side(lambda: block_config5(B, wl, dev))
         extras["paper_sizes"] = side(lambda: block_paper_sizes(B, dev))
         extras["config2_moments"] = side(lambda: block_config2_moments(B, wl, dev))
+        extras["phi4"] = side(lambda: block_phi4(dev))
 
     cpu = None
     if not args.no_cpu_baseline:

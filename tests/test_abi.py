@@ -38,6 +38,30 @@ def test_library_exports_every_declared_symbol(binding):
     assert sorted(binding.PROTOTYPES) == _declared()
 
 
+def _declared4():
+    txt = open(os.path.join(ROOT, "include", "phi4.h")).read()
+    txt = re.sub(r"/\*.*?\*/", "", txt, flags=re.S)
+    return sorted(set(re.findall(r"\b(phi4_[a-z_A-Z0-9]+)\s*\(", txt)))
+
+
+def test_phi4_header_exports_and_binding_agree(binding):
+    """include/phi4.h (the second workload): every declared call is exported and marshalled."""
+    from paper_2302_14720_b200 import phi4
+    so = ctypes.CDLL(os.path.join(ROOT, "paper_2302_14720_b200", "libsw_b200.so"))
+    names = _declared4()
+    assert "phi4_create" in names and "phi4_sweep" in names and "phi4_observables" in names
+    for name in names:
+        assert hasattr(so, name), f"{name} declared in phi4.h but not exported"
+    assert sorted(phi4.PROTOTYPES) == names
+    assert ctypes.sizeof(phi4.phi4_obs) == 88
+    phi4.lib()
+    import torch
+    if not torch.cuda.is_available():
+        assert not phi4.lib().phi4_create(4, 0.3, 1)
+        assert b"no CPU path" in phi4.lib().phi4_last_error()
+        assert not phi4.lib().phi4_create(1, 0.3, 1) and not phi4.lib().phi4_create(4, -1.0, 1)
+
+
 def test_struct_layout_matches_header(binding):
     assert ctypes.sizeof(binding.sw_obs) == 56
     assert [f[0] for f in binding.sw_obs._fields_] == ["energy", "magnetisation", "n_clusters", "largest_cluster",
