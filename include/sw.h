@@ -229,6 +229,12 @@ int64_t    sw_sweep_ms(sw_handle* h, float* out, int64_t cap);
  * each, are allocated by the library on first use, outside a caller-supplied workspace, and freed by sw_destroy.) */
 int        sw_set_path(sw_handle* h, int path);
 
+/* Default 1: on the fast path with 128 x 64 tiles the assignment kernel stages the 16-bit root plane through the TMA
+ * engine (cp.async.bulk.tensor.2d boxes of one tile into a ring of shared-memory stages, persistent CTAs:
+ * k_flip16_tma); 0: the direct-load kernel k_flip16 (also used when the driver cannot encode the tensor map, and for
+ * lattices of fewer than 8 tiles).  Same results. */
+int        sw_set_tma(sw_handle* h, int on);
+
 /* Path 11 only: number of passes (scans, including the last one that formed no reference) the label-equivalence
  * iteration of the last sweep / sw_test_label took -- a deterministic function of the bond graph (PAPER.md:53
  * reports "5 or 6" for 512 x 512).  Synchronises.  SW_ESTATE on another path, before any labelling, or if the

@@ -89,6 +89,7 @@ PROTOTYPES = {
     "sw_kernel_ms": (C.c_int, [_VP, C.POINTER(C.c_float), _I32]),
     "sw_kernel_name": (C.c_char_p, [_I32]),
     "sw_set_path": (C.c_int, [_VP, C.c_int]),
+    "sw_set_tma": (C.c_int, [_VP, C.c_int]),
     "sw_label_passes": (C.c_int, [_VP, C.POINTER(C.c_int32)]),
     "sw_sweep_ms": (C.c_int64, [_VP, C.POINTER(C.c_float), C.c_int64]),
     "sw_create_potts": (_VP, [C.c_int32, C.c_int32, C.c_double, C.c_uint64]),
@@ -308,6 +309,9 @@ def sw_sweep_ms(h) -> np.ndarray:
     out = (C.c_float * max(1, n))()
     _check(lib().sw_sweep_ms(_ptr(h), out, n))
     return np.array(out[:n], dtype=np.float64)
+
+def sw_set_tma(h, on: bool) -> None:
+    _check(lib().sw_set_tma(_ptr(h), 1 if on else 0))
 
 def sw_set_path(h, path: int) -> None:
     _check(lib().sw_set_path(_ptr(h), path))

@@ -5,6 +5,7 @@
 #include "sw_generic.cuh"
 #include "sw_tiled.cuh"
 #include "sw_scan.cuh"
+#include "sw_flip_tma.cuh"
 #include "sw_equiv.cuh"
 #include "sw_potts.cuh"
 #include "sw_series.cuh"
@@ -174,6 +175,9 @@ struct sw_handle {
     int ev_cursor = 0; std::vector<int> ev_seq;   // kernel ids in launch order within one sweep
     int64_t cur_sweep = 0;
     int64_t launches = 0;
+    // TMA staging of the 16-bit root plane in the assignment kernel (sw_flip_tma.cuh): tensor map of lab16, made on first use
+    CUtensorMap tmap, tmap_d; int tmap_state = 0;   // 0: not tried, 1: ready, -1: unavailable (k_flip16 is used)
+    bool use_tma = true;
 };
 
 namespace {
@@ -313,13 +317,54 @@ int flatten_scan(sw_handle* h, TileKind tile) {
         default:        return SW_ESTATE;
     }
 }
+// tensor map of the 16-bit root plane: [nb * L rows][L columns] uint16, boxes of 128 x 64 (one tile)
+bool make_lab16_tmap(sw_handle* h) {
+    if (h->tmap_state) return h->tmap_state > 0;
+    h->tmap_state = -1;
+    typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                 const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                 CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qr;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr) != cudaSuccess || !fn || qr != cudaDriverEntryPointSuccess) {
+        (void)cudaGetLastError();
+        return false;
+    }
+    const cuuint64_t dims[2] = { (cuuint64_t)h->L, (cuuint64_t)h->L * (cuuint64_t)h->nb };
+    const cuuint64_t strides[1] = { (cuuint64_t)h->L * 2 };
+    const cuuint32_t box[2] = { 128, 64 }, estr[2] = { 1, 1 };
+    if (((EncodeFn)fn)(&h->tmap, CU_TENSOR_MAP_DATA_TYPE_UINT16, 2, h->lab16, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                       CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+        return false;
+    // the decision plane: [nb * L rows][L / 32 words] uint32, boxes of 4 x 64 (a tile's own words)
+    const cuuint64_t ddims[2] = { (cuuint64_t)(h->L / 32), (cuuint64_t)h->L * (cuuint64_t)h->nb };
+    const cuuint64_t dstrides[1] = { (cuuint64_t)(h->L / 32) * 4 };
+    const cuuint32_t dbox[2] = { 4, 64 };
+    if (((size_t)h->words * 4) % 16 != 0 ||
+        ((EncodeFn)fn)(&h->tmap_d, CU_TENSOR_MAP_DATA_TYPE_UINT32, 2, h->D, ddims, dstrides, dbox, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                       CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+        return false;
+    h->tmap_state = 1;
+    return true;
+}
+
 // a4-a6 fused (+ count and largest of the clusters that span tiles)
 template <int NW, int TH>
 int launch_flip_scan(sw_handle* h) {
     constexpr int TW = 32 * NW;
     const int tiles = h->N / (TW * TH);
     SW_MARK(h, K_FLIPTILE);
-    if (sweeps_on_bits(h))
+    if (NW == 4 && TH == 64 && sweeps_on_bits(h) && h->use_tma && tiles >= 512 && make_lab16_tmap(h)) {
+        constexpr size_t smem = (size_t)FT_NSTAGE * FT_STAGE_BYTES + 128;
+        static bool done[MAX_DEV];
+        { int rc = opt_in_smem(k_flip16_tma, smem, done, h->dev); if (rc) return rc; }
+        static int sms[MAX_DEV];
+        int& nsm = sms[h->dev >= 0 && h->dev < MAX_DEV ? h->dev : 0];
+        if (!nsm) SW_CUDA(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, h->dev));
+        const int ctas = std::max(1, std::min(tiles, 3 * nsm / std::max(1, std::min(h->nb, 3))));   // persistent: ~3 CTAs per SM in all
+        k_flip16_tma<<<dim3(ctas, h->nb), 256 + 32 * FT_PROD_WARPS, smem, h->stream>>>(
+            h->tmap, h->tmap_d, h->sbits, h->D, h->nodes, h->ocount, h->series, h->ctl, make_div(h->L), h->L, h->N, h->words, h->nb, tiles);
+    } else if (sweeps_on_bits(h))
         k_flip16<NW, TH, true><<<dim3(tiles, h->nb), NW * TH, 0, h->stream>>>(
             h->spins, h->sbits, h->lab16, h->D, h->nodes, h->ocount, h->series, h->ctl, make_div(h->L),
             h->L, h->N, h->words, h->nb);
@@ -1132,6 +1177,13 @@ int sw_set_path(sw_handle* h, int path) {
 int sw_set_graphs(sw_handle* h, int on) {
     if (!h) { set_err("sw_set_graphs: null handle"); return SW_EINVAL; }
     h->use_graphs = on != 0;
+    return SW_OK;
+}
+
+int sw_set_tma(sw_handle* h, int on) {
+    if (!h) { set_err("sw_set_tma: null handle"); return SW_EINVAL; }
+    h->use_tma = on != 0;
+    h->gkey_path = -1;                              // (the captured sweep holds the other kernel: capture again)
     return SW_OK;
 }
 

@@ -151,6 +151,34 @@ def test_labelling_of_injected_bond_graphs(B, L, path):
     sw.close()
 
 
+@pytest.mark.parametrize("L,nb", [(2048, 1), (4096, 1), (2048, 2)])
+def test_assignment_kernel_with_and_without_tma_staging(B, L, nb):
+    """k_flip16_tma (16-bit root plane staged by cp.async.bulk.tensor boxes, persistent CTAs) against the oracle, and the
+    direct-load kernel on the same handle: identical spins and observables, every sweep."""
+    Ts, seeds = [T_C, 2.0, 3.0][:nb], [71, 72, 73][:nb]
+    sw = B.SwendsenWang(L, Ts, seeds)
+    refs = [oracle.init_random(L, s) for s in seeds]
+    for t in range(6):
+        B.sw_set_tma(sw.h, t % 2 == 0)
+        sw.sweep(1)
+        gs, obs = sw.spins_host(), sw.observables()
+        for b in range(nb):
+            s1, _, _, _, o = oracle.sweep(L, Ts[b], seeds[b], t, refs[b])
+            assert np.array_equal(gs[b], s1), (t, b)
+            assert _obs_tuple(obs[b]) == o, (t, b)
+            refs[b] = s1
+    # many sweeps in one call (graph replay) on either kernel
+    for on in (True, False):
+        B.sw_set_tma(sw.h, on)
+        t0 = sw.sweep_index
+        sw.sweep(9)
+        gs = sw.spins_host()
+        for b in range(nb):
+            refs[b], _ = oracle.run(L, Ts[b], seeds[b], 9, spins=refs[b], t0=t0, series=False)
+            assert np.array_equal(gs[b], refs[b]), (on, b)
+    sw.close()
+
+
 def test_race_order_independence(B):
     """Same state, same sweep index, repeated: identical bits every time (min-index labels)."""
     L, T, seed = 512, T_C, 3
