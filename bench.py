@@ -471,7 +471,7 @@ def main():
     N = L * L
     seed = rp.replica_seed(rank)                      # configs[3] uses seed 6; replicas take 6 + rank
     sw = B.SwendsenWang(L, T, seed, device=str(dev), path=args.path)
-    tw, th = (128, 64) if L % 128 == 0 else (64, 32)
+    tw, th = (128, 64) if (L % 128 == 0 and L > 1024) else (64, 32)      # (the library's choice: 64 x 32 tiles up to L = 1024)
 
     def barrier():
         if dist is not None:

@@ -64,6 +64,7 @@ inline size_t align_up(size_t v) { return (v + ALIGN - 1) / ALIGN * ALIGN; }
 enum TileKind { TILE_NONE = 0, ROWS64 = 1, SCAN_2 = 3, SCAN_4x64 = 7 };
 // width in 32-site words of the tiles the scan-line kernel and k_flip16 share (0: not a scan tile)
 inline int scan_nw(TileKind k) { return k == SCAN_2 ? 2 : k == SCAN_4x64 ? 4 : 0; }
+constexpr int SMALL_L = 1024;          // up to this side the fast path runs on 64 x 32 tiles
 constexpr int MAX_DEV = 64;            // per-device "attribute set" flags of the kernels with opt-in shared memory
 
 struct Layout {        // byte offsets into the workspace
@@ -72,11 +73,11 @@ struct Layout {        // byte offsets into the workspace
 
 size_t node_entries(int L) {           // per lattice: CAP = 2 (TW + TH) entries per tile of the shape this L runs on
     const size_t N = (size_t)L * L;
-    if (L % 128 == 0) return N / (128 * 64) * (size_t)(2 * (128 + 64));
+    if (L % 128 == 0 && L > SMALL_L) return N / (128 * 64) * (size_t)(2 * (128 + 64));
     if (L % 64 == 0) return N / (64 * 32) * (size_t)(2 * (64 + 32));
     return 0;
 }
-size_t tiles_max(int L) { return L % 128 == 0 ? (size_t)L * L / (128 * 64) : L % 64 == 0 ? (size_t)L * L / (64 * 32) : 0; }
+size_t tiles_max(int L) { return (L % 128 == 0 && L > SMALL_L) ? (size_t)L * L / (128 * 64) : L % 64 == 0 ? (size_t)L * L / (64 * 32) : 0; }
 
 DivL make_div(int d) {          // q = (v * m) >> p is exact for 0 <= v < 2^30 (error term < 1/d)
     int k = 0; while ((1 << k) < d) ++k;
@@ -188,7 +189,8 @@ namespace {
 TileKind pick_tile(int L, int path) {
     if (path == 1) return TILE_NONE;
     if (path == 11) return L % 64 == 0 ? ROWS64 : TILE_NONE;          // row kernels for bond / flip / energy; labels: sw_equiv.cuh
-    if (L % 128 == 0) return SCAN_4x64;
+    // small lattices wait for the latency of ONE tile: 64 x 32 tiles (8 warps each on 32 x 8 blocks) up to L = 1024
+    if (L % 128 == 0 && L > SMALL_L) return SCAN_4x64;
     if (L % 64 == 0) return SCAN_2;
     return TILE_NONE;
 }
@@ -264,23 +266,23 @@ int opt_in_smem(K kernel, size_t smem, bool* done, int dev) {
 }
 
 // fast path: fused bond + scan-line tile labelling, global merge, open roots (a1-a3)
-template <int NW, int TH>
+template <int NW, int TH, int BAND_T = 32>
 int launch_bond_label_scan(sw_handle* h, bool fused, bool obs_prev) {
-    constexpr int TW = 32 * NW, CAP = 2 * (TW + TH);
+    constexpr int TW = 32 * NW, CAP = 2 * (TW + TH), THREADS = NW * TH * (32 / BAND_T);
     const int tiles = h->N / (TW * TH);
     constexpr size_t smem = (size_t)TW * TH * sizeof(uint32_t);      // the parent array (dynamic: 32 KB at 128 x 64)
     static bool done[2][MAX_DEV];
-    { int rc = opt_in_smem(k_bond_label<NW, TH, true>, smem, done[0], h->dev); if (rc) return rc; }
-    { int rc = opt_in_smem(k_bond_label<NW, TH, false>, smem, done[1], h->dev); if (rc) return rc; }
+    { int rc = opt_in_smem(k_bond_label<NW, TH, true, false, BAND_T>, smem, done[0], h->dev); if (rc) return rc; }
+    { int rc = opt_in_smem(k_bond_label<NW, TH, false, false, BAND_T>, smem, done[1], h->dev); if (rc) return rc; }
     if (fused) {
         SW_MARK(h, K_BONDLABEL);
-        k_bond_label<NW, TH, true><<<dim3(tiles, h->nb), NW * TH, smem, h->stream>>>(
+        k_bond_label<NW, TH, true, false, BAND_T><<<dim3(tiles, h->nb), THREADS, smem, h->stream>>>(
             h->sbits, h->bondE, h->bondS, h->lab16, h->nodes, h->ocount, h->bslot,
             h->series, h->lat, h->ctl,
             h->L, h->N, h->words, h->nb, obs_prev ? 1 : 0);
     } else {
         SW_MARK(h, K_TILE);
-        k_bond_label<NW, TH, false><<<dim3(tiles, h->nb), NW * TH, smem, h->stream>>>(
+        k_bond_label<NW, TH, false, false, BAND_T><<<dim3(tiles, h->nb), THREADS, smem, h->stream>>>(
             nullptr, h->bondE, h->bondS, h->lab16, h->nodes, h->ocount, h->bslot,
             h->series, h->lat, h->ctl,
             h->L, h->N, h->words, h->nb, obs_prev ? 1 : 0);
@@ -349,8 +351,11 @@ bool make_lab16_tmap(sw_handle* h) {
 }
 
 // a4-a6 fused (+ count and largest of the clusters that span tiles)
+// small lattices on 64 x 32 tiles: decision words drawn inside the assignment kernel, sweep advanced by its last CTA
+bool flip_fused(const sw_handle* h) { return h->tile == SCAN_2 && sweeps_on_bits(h); }
+
 template <int NW, int TH>
-int launch_flip_scan(sw_handle* h) {
+int launch_flip_scan(sw_handle* h, int adv_acc) {
     constexpr int TW = 32 * NW;
     const int tiles = h->N / (TW * TH);
     SW_MARK(h, K_FLIPTILE);
@@ -364,14 +369,18 @@ int launch_flip_scan(sw_handle* h) {
         const int ctas = std::max(1, std::min(tiles, 3 * nsm / std::max(1, std::min(h->nb, 3))));   // persistent: ~3 CTAs per SM in all
         k_flip16_tma<<<dim3(ctas, h->nb), 256 + 32 * FT_PROD_WARPS, smem, h->stream>>>(
             h->tmap, h->tmap_d, h->sbits, h->D, h->nodes, h->ocount, h->series, h->ctl, make_div(h->L), h->L, h->N, h->words, h->nb, tiles);
-    } else if (sweeps_on_bits(h))
+    } else if (flip_fused(h))
+        k_flip16<NW, TH, true, true><<<dim3(tiles, h->nb), NW * TH, 0, h->stream>>>(
+            h->spins, h->sbits, h->lab16, nullptr, h->nodes, h->ocount, h->series, h->ctl, h->lat, h->mom, adv_acc,
+            make_div(h->L), h->L, h->N, h->words, h->nb);
+    else if (sweeps_on_bits(h))
         k_flip16<NW, TH, true><<<dim3(tiles, h->nb), NW * TH, 0, h->stream>>>(
-            h->spins, h->sbits, h->lab16, h->D, h->nodes, h->ocount, h->series, h->ctl, make_div(h->L),
-            h->L, h->N, h->words, h->nb);
+            h->spins, h->sbits, h->lab16, h->D, h->nodes, h->ocount, h->series, h->ctl, h->lat, h->mom, adv_acc,
+            make_div(h->L), h->L, h->N, h->words, h->nb);
     else
         k_flip16<NW, TH, false><<<dim3(tiles, h->nb), NW * TH, 0, h->stream>>>(
-            h->spins, h->sbits, h->lab16, h->D, h->nodes, h->ocount, h->series, h->ctl, make_div(h->L),
-            h->L, h->N, h->words, h->nb);
+            h->spins, h->sbits, h->lab16, h->D, h->nodes, h->ocount, h->series, h->ctl, h->lat, h->mom, adv_acc,
+            make_div(h->L), h->L, h->N, h->words, h->nb);
     h->launches += 1;
     if (h->eager_labels) {                          // a4 every sweep instead of on demand
         SW_MARK(h, K_COMPRESS);
@@ -436,7 +445,7 @@ int launch_label_equiv(sw_handle* h) {
 // labelling alone from the bond planes, leaving flat labels (the unfused order; sw_test_label)
 template <int NW, int TH>
 int launch_label_scan(sw_handle* h) {
-    int rc = launch_bond_label_scan<NW, TH>(h, false, false);
+    int rc = NW == 2 ? launch_bond_label_scan<NW, TH, 8>(h, false, false) : launch_bond_label_scan<NW, TH>(h, false, false);
     if (rc) return rc;
     SW_MARK(h, K_COMPRESS);
     return launch_flatten_scan<NW, TH>(h);
@@ -535,17 +544,24 @@ int launch_sweep(sw_handle* h, int64_t k) {
                 h->spins, h->bondE, h->bondS, h->lat, h->ctl, h->L, h->N, h->words, h->series, h->nb, obs_prev ? 1 : 0);
             h->launches += 1;
         }
-        rc = nw == 4 ? launch_bond_label_scan<4, 64>(h, fused, obs_prev) : launch_bond_label_scan<2, 32>(h, fused, obs_prev);
+        // (64 x 32 tiles: 8 warps per tile, each scanning 32 x 8 sites -- the latency of one tile is what small lattices wait for)
+        rc = nw == 4 ? launch_bond_label_scan<4, 64>(h, fused, obs_prev) : launch_bond_label_scan<2, 32, 8>(h, fused, obs_prev);
         if (rc) return rc;
-        SW_MARK(h, K_FLIPBITS);
-        k_flipbits<<<grid1(((size_t)h->words + 3) / 4, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(
-            h->D, h->lat, h->ctl, h->words);
-        h->launches += 1;
-        rc = nw == 4 ? launch_flip_scan<4, 64>(h) : launch_flip_scan<2, 32>(h);
+        const int adv_acc = k > 0 ? 2 : 0;              // (E, M of a sweep arrive with the next sweep's bond test)
+        const bool ff = flip_fused(h);
+        if (!ff) {
+            SW_MARK(h, K_FLIPBITS);
+            k_flipbits<<<grid1(((size_t)h->words + 3) / 4, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(
+                h->D, h->lat, h->ctl, h->words);
+            h->launches += 1;
+        }
+        rc = nw == 4 ? launch_flip_scan<4, 64>(h, adv_acc) : launch_flip_scan<2, 32>(h, adv_acc);
         if (rc) return rc;
-        SW_MARK(h, K_ADVANCE);
-        k_advance<<<1, 64, 0, h->stream>>>(h->ctl, h->series, h->nb, h->mom, h->N, k > 0 ? 2 : 0);
-        h->launches += 1;
+        if (!ff) {
+            SW_MARK(h, K_ADVANCE);
+            k_advance<<<1, 64, 0, h->stream>>>(h->ctl, h->series, h->nb, h->mom, h->N, adv_acc);
+            h->launches += 1;
+        }
         SW_MARK(h, K_COUNT);
         h->labels_flat = h->eager_labels;
         h->lab_tile = h->tile;                          // the tile shape lab16 / nodes were written with

@@ -21,6 +21,8 @@ struct Ctl {
     unsigned long long t;  // sweep index the next sweep uses
     uint32_t slot;         // series slot the running sweep accumulates into
     uint32_t cap;          // number of series slots (ring)
+    uint32_t done;         // CTAs of the sweep's last kernel that have finished (k_flip16<FUSED>: the last one advances the sweep)
+    uint32_t pad;
 };
 
 // one per (series slot, lattice); accumulated with atomics during the sweep

@@ -241,12 +241,12 @@ k_philox_only(uint32_t* __restrict__ sink, uint32_t key0, uint32_t key1, uint32_
 
 // ---- sweep control -------------------------------------------------------------------------------
 __global__ void k_set_ctl(Ctl* ctl, unsigned long long t, uint32_t slot, uint32_t cap) {
-    ctl->t = t; ctl->slot = slot; ctl->cap = cap;
+    ctl->t = t; ctl->slot = slot; ctl->cap = cap; ctl->done = 0; ctl->pad = 0;
 }
 // end of a sweep: t += 1, move to the next series slot and zero it.  acc: which record feeds the running
 // moments -- 1: this sweep's (its E, M are complete), 2: the previous sweep's (scan path: E, M of a sweep
 // arrive with the next sweep's bond test), 0: none.  One thread per lattice: sweep order, fixed arithmetic.
-__global__ void k_advance(Ctl* ctl, Rec* rec, int nb, Mom* mom, int N, int acc) {
+__device__ __forceinline__ void advance_sweep(Ctl* ctl, Rec* rec, int nb, Mom* mom, int N, int acc) {   // (a whole block)
     const uint32_t cur = ctl->slot;
     const uint32_t next = (cur + 1 == ctl->cap) ? 0u : cur + 1;
     const uint32_t from = acc == 2 ? (cur == 0 ? ctl->cap - 1 : cur - 1) : cur;
@@ -262,6 +262,7 @@ __global__ void k_advance(Ctl* ctl, Rec* rec, int nb, Mom* mom, int N, int acc) 
     __syncthreads();
     if (threadIdx.x == 0) { ctl->t += 1; ctl->slot = next; }
 }
+__global__ void k_advance(Ctl* ctl, Rec* rec, int nb, Mom* mom, int N, int acc) { advance_sweep(ctl, rec, nb, mom, N, acc); }
 // scan path, end of a sw_sweep call (after k_observe_rows): the last sweep's record, now complete
 __global__ void k_moments_last(const Ctl* ctl, const Rec* rec, int nb, Mom* mom, int N) {
     const uint32_t from = ctl->slot == 0 ? ctl->cap - 1 : ctl->slot - 1;

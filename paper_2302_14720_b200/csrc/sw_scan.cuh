@@ -31,7 +31,7 @@
 
 namespace sw {
 
-constexpr int BAND = 32;                        // rows a warp walks; a tile is TH / 32 bands of NW strips
+constexpr int BAND = 32;                        // rows a warp walks by default; a tile is TH / BAND bands of NW strips
 constexpr uint32_t OPEN_BIT = 0x40000000u;      // bit 30 of a root's word: the cluster has a bond across the tile edge
 // A root's word: bits 0 .. LS-1 tile-local index (LS = log2 of the sites per tile <= 14), bits LS .. 2 LS the
 // cluster size (<= 2^LS), bit 30 open.
@@ -134,16 +134,22 @@ __device__ __forceinline__ int div_l(int v, const DivL& D) {
 // FUSE = true: phase 1 draws the bonds (a1 fused into a2).  FUSE = false: phase 1 reads the bond planes
 // that k_bond_rows (or a test) wrote -- per-stage timing (BASELINE config 3) and labelling-only tests.
 // POTTS (with FUSE; sw_potts.cuh): `sbits` is the int8 COLOUR plane; a bond needs equal colours (byte compares).
-template <int NW, int TH, bool FUSE, bool POTTS = false>
-__global__ void __launch_bounds__(NW * TH)
+// BAND_T: rows of the block a warp scans (32: one thread per 32-site word; 8: four threads per word, each with a quarter
+// of the word's Philox calls -- the variant for small lattices, whose sweep time is the latency of ONE tile through this
+// kernel: 4 x less serial work per warp).
+template <int NW, int TH, bool FUSE, bool POTTS = false, int BAND_T = 32>
+__global__ void __launch_bounds__(NW * TH * (32 / BAND_T))
 k_bond_label(const uint32_t* __restrict__ sbits, uint32_t* bondE, uint32_t* bondS,
              uint16_t* __restrict__ lab16, int4* __restrict__ nodes, int* __restrict__ ocount,
              uint16_t* __restrict__ bslot,
              Rec* __restrict__ rec, const Lat* __restrict__ lat, const Ctl* __restrict__ ctl,
              int L, int N, int words, int nb, int obs_prev) {
-    constexpr int TW = 32 * NW, SITES = TW * TH, THREADS = NW * TH;   // one thread per 32-site word
+    constexpr int BAND = BAND_T;                // (shadows the default: rows per warp block in this instantiation)
+    constexpr int TPW = 32 / BAND;              // threads per 32-site word (one warp per 32 x BAND block)
+    constexpr int TW = 32 * NW, SITES = TW * TH, WORDS = NW * TH, THREADS = WORDS * TPW;
     constexpr int CAP = 2 * (TW + TH);
     constexpr int NWARPS = THREADS / 32;
+    static_assert(TPW == 1 || TPW == 2 || TPW == 4, "threads per word");
     constexpr int PCAP = 192;                   // label meetings a warp can list while it scans its block (~80 at T_c)
     constexpr int HKCAP = 1024;                 // hooked nodes the tile can list (~250 at T_c)
     static_assert(TH % BAND == 0 && TH <= 64 && SITES <= 8192 && CAP < 0x3FFF, "tile shape");
@@ -182,9 +188,11 @@ k_bond_label(const uint32_t* __restrict__ sbits, uint32_t* bondE, uint32_t* bond
     if (!FUSE) {
         const uint32_t* bE = bondE + (size_t)blockIdx.y * words;
         const uint32_t* bS = bondS + (size_t)blockIdx.y * words;
-        const int row = tid / NW, wx = tid - row * NW;
-        const size_t gw = (size_t)(y0 + row) * wprL + (x0 >> 5) + wx;
-        es[tid] = make_uint2(bE[gw], bS[gw]);
+        if (tid < WORDS) {
+            const int row = tid / NW, wx = tid - row * NW;
+            const size_t gw = (size_t)(y0 + row) * wprL + (x0 >> 5) + wx;
+            es[tid] = make_uint2(bE[gw], bS[gw]);
+        }
         if (tid < NW) nIn[tid] = bS[(size_t)(y0 == 0 ? L - 1 : y0 - 1) * wprL + (x0 >> 5) + tid];
         if (tid < TH) {
             const int wl = (x0 >> 5) == 0 ? wprL - 1 : (x0 >> 5) - 1;
@@ -193,7 +201,8 @@ k_bond_label(const uint32_t* __restrict__ sbits, uint32_t* bondE, uint32_t* bond
     } else {
         const PhiloxKey key(la.key0, la.key1);
         {
-            const int row = tid / NW, wx = tid - row * NW;          // this thread's 32-site word
+            const int wid = tid / TPW, part = tid - wid * TPW;      // this thread's 32-site word (and which part of its draws)
+            const int row = wid / NW, wx = wid - row * NW;
             const int y = y0 + row;
             const int xw = (x0 >> 5) + wx;
             const int w = y * wprL + xw;                              // word index within the lattice
@@ -221,21 +230,29 @@ k_bond_label(const uint32_t* __restrict__ sbits, uint32_t* bondE, uint32_t* bond
             if (!POTTS && obs_prev) {
                 // a7 for free: the equal-pair masks of the bond test are the energy of the
                 // configuration the previous sweep left: E = (#edges) - 2 (#equal pairs), M = N - 2 (#down)
-                const int eo = warp_sum_i(64 - 2 * (__popc(eqE) + __popc(eqS)));
-                const int mo = warp_sum_i(32 - 2 * __popc(own));
+                const int eo = warp_sum_i(part == 0 ? 64 - 2 * (__popc(eqE) + __popc(eqS)) : 0);
+                const int mo = warp_sum_i(part == 0 ? 32 - 2 * __popc(own) : 0);
                 if (lane == 0) { atomicAdd(&s_obs[0], eo); atomicAdd(&s_obs[1], mo); }
             }
             uint32_t dE = 0, dS = 0;
 #pragma unroll
-            for (int c = 0; c < 16; ++c) {
+            for (int cc = 0; cc < 16 / TPW; ++cc) {
+                const int c = part * (16 / TPW) + cc;
                 const uint4 r = philox4x32_10((uint32_t)w * 16u + c, tlo, thi, TAG_BOND, key);
-                dE |= (r.x < la.thr ? 1u : 0u) << (2 * c) | (r.z < la.thr ? 1u : 0u) << (2 * c + 1);
-                dS |= (r.y < la.thr ? 1u : 0u) << (2 * c) | (r.w < la.thr ? 1u : 0u) << (2 * c + 1);
+                dE |= ((r.x < la.thr ? 1u : 0u) | (r.z < la.thr ? 2u : 0u)) << (2 * c);
+                dS |= ((r.y < la.thr ? 1u : 0u) | (r.w < la.thr ? 2u : 0u)) << (2 * c);
+            }
+#pragma unroll
+            for (int o = 1; o < TPW; o <<= 1) {                      // the word's TPW threads are neighbouring lanes
+                dE |= __shfl_xor_sync(0xffffffffu, dE, o);
+                dS |= __shfl_xor_sync(0xffffffffu, dS, o);
             }
             const uint32_t e = eqE & dE, so = eqS & dS;
-            es[tid] = make_uint2(e, so);
-            bondE[(size_t)blockIdx.y * words + w] = e;
-            bondS[(size_t)blockIdx.y * words + w] = so;
+            if (part == 0) {
+                es[wid] = make_uint2(e, so);
+                bondE[(size_t)blockIdx.y * words + w] = e;
+                bondS[(size_t)blockIdx.y * words + w] = so;
+            }
         }
         // bonds entering the tile: South bonds of the row above (TW / 2 calls), East bonds of the column to
         // the West (32 calls).  They are owned by the neighbouring tiles; recomputed here from the same draws.
@@ -358,9 +375,10 @@ k_bond_label(const uint32_t* __restrict__ sbits, uint32_t* bondE, uint32_t* bond
     // root's count is the size of its tile-local cluster.  The label nodes themselves are only COUNTED (bit tricks
     // on the bond words): roots = label nodes - hooked nodes.
     {
-        const int mybase = (tid / NW) * TW + (tid % NW) * 32;
-        const uint32_t ew = es[tid].x & 0x7FFFFFFFu;
-        uint32_t up = (tid / NW) % BAND ? es[tid - NW].y : 0u;       // South bonds of the row above, within the band
+        const int wd = tid < WORDS ? tid : 0;                        // (with several threads per word the first WORDS threads count)
+        const int mybase = (wd / NW) * TW + (wd % NW) * 32;
+        const uint32_t ew = es[wd].x & 0x7FFFFFFFu;
+        uint32_t up = (wd / NW) % BAND ? es[wd - NW].y : 0u;         // South bonds of the row above, within the band
         uint32_t m = ew;                                             // OR of the run's uplinks, gathered at its head
         up |= (up >> 1) & m;  m &= m >> 1;
         up |= (up >> 2) & m;  m &= m >> 2;
@@ -368,6 +386,7 @@ k_bond_label(const uint32_t* __restrict__ sbits, uint32_t* bondE, uint32_t* bond
         up |= (up >> 8) & m;  m &= m >> 8;
         up |= (up >> 16) & m;
         uint32_t o = ~(ew << 1) & ~up;                               // heads of runs without an uplink
+        if (tid >= WORDS) o = 0;
         const int nl = warp_sum_i(__popc(o));
         if (lane == 0) atomicAdd(&s_nlab, nl);
         const int nh = s_nhook;                                      // (complete: the barrier above)
@@ -630,10 +649,16 @@ k_labels16(int* __restrict__ label, const uint16_t* __restrict__ lab16, const in
 // ---------------------------------------------------------------------------------------------------
 // BITS: the new spins go out bit-packed (one byte = 8 sites per thread and step, 32 MiB instead of 256 MiB at
 // L = 16384) into the plane k_bond_label<FUSE> reads; else as the int8 plane (unfused path 6).
-template <int NW, int TH, bool BITS>
+// FUSED (small lattices, where a sweep is the sum of its kernels' latencies): no decision plane and no separate end-of-sweep
+// kernel -- the decision words of the tile's own sites and of the cluster roots of its open tile roots are drawn here (word w
+// of the plane is word w & 3 of Philox call (w >> 2, t, TAG_FLIP): the same bits k_flipbits would have stored), and the CTA
+// that finishes last advances the sweep (advance_sweep).  4 launches per sweep instead of 6.  (At L = 16384 the extra draws
+// cost more than the two launches: not used there.)
+template <int NW, int TH, bool BITS, bool FUSED = false>
 __global__ void __launch_bounds__(NW * TH, 1536 / (NW * TH))
 k_flip16(int8_t* __restrict__ spins, uint32_t* __restrict__ sbits, const uint16_t* __restrict__ lab16, const uint32_t* __restrict__ D,
-         const int4* __restrict__ nodes, const int* __restrict__ ocount, Rec* __restrict__ rec, const Ctl* __restrict__ ctl,
+         const int4* __restrict__ nodes, const int* __restrict__ ocount, Rec* __restrict__ rec, Ctl* __restrict__ ctl,
+         const Lat* __restrict__ lat, Mom* __restrict__ mom, int adv_acc,
          DivL dv, int L, int N, int words, int nb) {
     constexpr int TW = 32 * NW, SITES = TW * TH, THREADS = NW * TH;
     constexpr int CAP = 2 * (TW + TH);
@@ -657,9 +682,19 @@ k_flip16(int8_t* __restrict__ spins, uint32_t* __restrict__ sbits, const uint16_
         v[k] = ld_stream_u4(lab16 + (size_t)blockIdx.y * N + (size_t)(y0 + (l >> LOG_TW)) * L + x0 + (l & (TW - 1)));
     }
     const int n = ocount[tile];
+    const Lat la = lat[blockIdx.y];
+    const unsigned long long t = ctl->t;
+    const uint32_t tlo = (uint32_t)t, thi = (uint32_t)(t >> 32);
     {
         const int row = tid / NW, wx = tid - row * NW;
-        dec[tid] = d[(size_t)(y0 + row) * (L >> 5) + (x0 >> 5) + wx];
+        const int w = (y0 + row) * (L >> 5) + (x0 >> 5) + wx;            // my word of the decision plane
+        if (FUSED) {
+            const PhiloxKey key(la.key0, la.key1);
+            const uint4 r = philox4x32_10((uint32_t)w >> 2, tlo, thi, TAG_FLIP, key);
+            dec[tid] = (w & 2) ? ((w & 1) ? r.w : r.z) : ((w & 1) ? r.y : r.x);
+        } else {
+            dec[tid] = d[w];
+        }
     }
     __syncthreads();
     // open tile roots take the decision of their cluster root = the minimum site index under their root node;
@@ -672,7 +707,15 @@ k_flip16(int8_t* __restrict__ spins, uint32_t* __restrict__ sbits, const uint16_
             const int4 me = nodes[lb + nodebase + e];                  // (root node, size, min site, site of the tile root)
             const int R = me.x == nodebase + e ? me.z : nodes[lb + me.x].z;
             if (me.x == nodebase + e) { ++nroot; big = max(big, me.y); }
-            const uint32_t up = (__ldg(d + (R >> 5)) >> (R & 31)) & 1u;
+            uint32_t up;
+            if (FUSED) {
+                const PhiloxKey key(la.key0, la.key1);
+                const uint4 r = philox4x32_10((uint32_t)R >> 7, tlo, thi, TAG_FLIP, key);
+                const uint32_t wsel = (R & 64) ? ((R & 32) ? r.w : r.z) : ((R & 32) ? r.y : r.x);
+                up = (wsel >> (R & 31)) & 1u;
+            } else {
+                up = (__ldg(d + (R >> 5)) >> (R & 31)) & 1u;
+            }
             const int delta = me.w - tilebase;
             const int ry = div_l(delta, dv);
             const int l = ry * TW + (delta - ry * L);
@@ -703,6 +746,21 @@ k_flip16(int8_t* __restrict__ spins, uint32_t* __restrict__ sbits, const uint16_
         const size_t gsite = (size_t)blockIdx.y * N + (size_t)(y0 + (l >> LOG_TW)) * L + x0 + (l & (TW - 1));
         if (BITS) reinterpret_cast<uint8_t*>(sbits)[gsite >> 3] = (uint8_t)b8;
         else *reinterpret_cast<uint2*>(spins + gsite) = make_uint2(spin_bytes4(b8 & 15u), spin_bytes4(b8 >> 4));
+    }
+    if (FUSED) {
+        // the CTA that finishes last closes the sweep (its own and every other CTA's record updates are done)
+        __shared__ int s_last;
+        __syncthreads();
+        if (tid == 0) {
+            __threadfence();
+            s_last = atomicAdd(&ctl->done, 1u) == gridDim.x * gridDim.y - 1;
+        }
+        __syncthreads();
+        if (s_last) {
+            __threadfence();
+            if (tid == 0) ctl->done = 0;
+            advance_sweep(ctl, rec, nb, mom, N, adv_acc);
+        }
     }
 }
 
