@@ -156,11 +156,16 @@ k4_reflect(double* __restrict__ phi, const double* __restrict__ r, int* label, i
            const Ctl4* __restrict__ ctl, long long* __restrict__ iacc, Geo g, uint32_t key0, uint32_t key1) {
     const int x = blockIdx.x * P4_THREADS + threadIdx.x;
     int isroot = 0;
+    int root = -1 - (int)(threadIdx.x & 31);                // (lanes past the end: distinct keys)
+    if (x < g.V) root = uf_find(label, x);
+    {   // sizes: one add per root and warp -- at kappa = 0.304 one cluster holds most of the lattice, and a site-by-site add
+        // would send every one of its sites to the same address
+        const unsigned grp = __match_any_sync(0xffffffffu, root);
+        if (x < g.V && (int)(threadIdx.x & 31) == __ffs(grp) - 1) atomicAdd(gsize + root, __popc(grp));
+    }
     if (x < g.V) {
-        const int root = uf_find(label, x);
         if (root != x) label[x] = root;                     // (only ever an ancestor: safe while others walk)
         isroot = root == x;
-        atomicAdd(gsize + root, 1);
         const uint4 w = draw4((uint32_t)root >> 7, ctl->t, TAG_SEL, key0, key1);
         const uint32_t ww[4] = { w.x, w.y, w.z, w.w };
         if ((ww[(root >> 5) & 3] >> (root & 31)) & 1u) {
