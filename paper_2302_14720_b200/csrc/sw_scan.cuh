@@ -31,6 +31,10 @@
 
 namespace sw {
 
+#ifndef SCAN_UNROLL_N
+#define SCAN_UNROLL_N 16
+#endif
+constexpr int SCAN_UNROLL = SCAN_UNROLL_N;      // rows of the scan loop unrolled together
 constexpr int BAND = 32;                        // rows a warp walks by default; a tile is TH / BAND bands of NW strips
 constexpr uint32_t OPEN_BIT = 0x40000000u;      // bit 30 of a root's word: the cluster has a bond across the tile edge
 // A root's word: bits 0 .. LS-1 tile-local index (LS = log2 of the sites per tile <= 14), bits LS .. 2 LS the
@@ -296,7 +300,7 @@ k_bond_label(const uint32_t* __restrict__ sbits, uint32_t* bondE, uint32_t* bond
         uint32_t s_up = 0;                                           // (a band's first row adopts nothing: seams come later)
         const uint32_t pl_s = (uint32_t)__cvta_generic_to_shared(pend[warp]);
         int npend = 0;                                               // (warp-uniform)
-#pragma unroll 4
+#pragma unroll SCAN_UNROLL
         for (int y = yb; y < yb + BAND; ++y, rowbase += TW, rowaddr += 4u * TW) {
             const uint2 w = es[y * NW + strip];
             const uint32_t nz = ~w.x | 0x80000000u;                  // bit k: no bond between columns k, k + 1 of the strip

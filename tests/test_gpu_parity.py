@@ -179,6 +179,60 @@ def test_assignment_kernel_with_and_without_tma_staging(B, L, nb):
     sw.close()
 
 
+def test_labels_of_a_sweep_survive_a_path_switch(B):
+    """sw_labels flattens the 16-bit roots of the LAST sweep with the tile shape that wrote them, whatever path is selected
+    afterwards (sw_set_path between the sweep and the first sw_labels call)."""
+    L, T, seed = 256, T_C, 19
+    for new_path in (1, 6, 11):
+        sw = B.SwendsenWang(L, T, seed)
+        s = oracle.init_random(L, seed)
+        for t in range(3):
+            s, _, _, lab, _ = oracle.sweep(L, T, seed, t, s)
+        sw.sweep(3)
+        B.sw_set_path(sw.h, new_path)
+        assert np.array_equal(sw.labels_host()[0], lab), new_path
+        sw.sweep(1)                                   # and the chain goes on, on the new path
+        s, _, _, lab, o = oracle.sweep(L, T, seed, 3, s)
+        assert np.array_equal(sw.labels_host()[0], lab) and np.array_equal(sw.spins_host()[0], s)
+        assert _obs_tuple(sw.observables()[0]) == o
+        sw.close()
+
+
+def test_series_through_the_raw_c_call_with_a_batch(B):
+    """include/sw.h: `cap` of sw_series counts SWEEPS; the caller's buffer holds cap * nb records."""
+    import ctypes
+    L, Ts, seeds, n = 64, [2.0, T_C, 3.0], [5, 6, 7], 9
+    sw = B.SwendsenWang(L, Ts, seeds)
+    sw.sweep(n)
+    cap = 4                                           # fewer sweeps than retained: only cap * nb records may be written
+    buf = (B.sw_obs * (cap * 3 + 1))()
+    buf[cap * 3].energy = 123456789
+    kept = B.lib().sw_series(sw.h, buf, cap)
+    assert kept == n and buf[cap * 3].energy == 123456789
+    for b in range(3):
+        _, ser = oracle.run(L, Ts[b], seeds[b], n)
+        for k in range(cap):
+            r = buf[k * 3 + b]
+            assert (r.energy, r.magnetisation, r.n_clusters, r.largest_cluster) == tuple(int(v) for v in ser[k]) and r.sweep == k + 1
+    sw.close()
+
+
+def test_handle_on_a_device_that_is_not_current(B):
+    """A handle lives on the device it was created on; every call switches to it (needs two GPUs)."""
+    import torch
+    if torch.cuda.device_count() < 2:
+        pytest.skip("one GPU")
+    L, T, seed = 256, T_C, 3
+    sw = B.SwendsenWang(L, T, seed, device="cuda:1")
+    torch.cuda.set_device(0)
+    s = oracle.init_random(L, seed)
+    for t in range(3):
+        s, _, _, lab, o = oracle.sweep(L, T, seed, t, s)
+        sw.sweep(1)
+    assert np.array_equal(sw.spins_host()[0], s) and np.array_equal(sw.labels_host()[0], lab) and _obs_tuple(sw.observables()[0]) == o
+    sw.close()
+
+
 def test_race_order_independence(B):
     """Same state, same sweep index, repeated: identical bits every time (min-index labels)."""
     L, T, seed = 512, T_C, 3
