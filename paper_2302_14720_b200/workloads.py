@@ -172,6 +172,39 @@ def bonds_comb(L: int):
     return bE, bS
 
 
+def bonds_ladder(L: int, every: int = 2, phase: int = 1):
+    """Every column bonded top to bottom (not around the torus), rungs of East bonds on every `every`-th row: at each
+    rung a whole row of distinct column labels meets at once -- far more label meetings and merges per 32 x 32 block than any
+    equilibrium bond graph has (the kernels' lists of meetings / hooked nodes overflow into their fallback paths)."""
+    bE, bS = bonds_none(L)
+    bS[: (L - 1) * L] = 1
+    for y in range(phase, L, every):
+        bE[y * L: y * L + L - 1] = 1
+    return bE, bS
+
+
+def bonds_u_shapes(L: int):
+    """Clusters of 2 x 3 sites: two columns of South bonds joined by one East bond at the bottom -- one merge of two labels
+    per six sites (more hooked nodes per tile than the kernels' list holds)."""
+    bE, bS = bonds_none(L)
+    y = np.arange(L * L) // L
+    x = np.arange(L * L) % L
+    bS[(y % 3 != 2) & (y < L - 1)] = 1
+    bE[(y % 3 == 2) & (x % 2 == 0) & (x < L - 1)] = 1
+    return bE, bS
+
+
+def bonds_dense_meetings(L: int, seed: int):
+    """Columns broken at random places, rungs on random rows: many meetings, many separate clusters."""
+    rng = np.random.default_rng(seed)
+    bE, bS = bonds_none(L)
+    bS[:] = (rng.random(L * L) < 0.9)
+    rows = rng.random(L) < 0.5
+    for y in np.nonzero(rows)[0]:
+        bE[y * L:(y + 1) * L] = (rng.random(L) < 0.95)
+    return bE, bS
+
+
 def pack_bits(bytes01: np.ndarray) -> np.ndarray:
     """Canonical bit-plane layout of the C ABI: bit (i & 31) of uint32 word (i >> 5)."""
     b = np.asarray(bytes01, dtype=np.uint8).reshape(-1)

@@ -136,11 +136,15 @@ def _label_patterns(L):
     yield "row0", wl.bonds_row_wrap(L, 0)
     yield "comb", wl.bonds_comb(L)
     yield "spiral", wl.bonds_spiral(L)
+    yield "ladder", wl.bonds_ladder(L)
+    yield "u_shapes", wl.bonds_u_shapes(L)
+    yield "ladder3", wl.bonds_ladder(L, 3, 0)
+    yield "dense_meetings", wl.bonds_dense_meetings(L, L)
     for k, d in enumerate((0.2, 0.45, 0.5, 0.55, 0.8)):
         yield f"random{d}", wl.bonds_random(L, 7 * L + k, d)
 
 
-@pytest.mark.parametrize("L,path", [(64, 0), (128, 0), (256, 0), (320, 0), (100, 1), (512, 0), (192, 6)])
+@pytest.mark.parametrize("L,path", [(64, 0), (128, 0), (256, 0), (320, 0), (100, 1), (512, 0), (192, 6), (1152, 0), (2048, 0)])
 def test_labelling_of_injected_bond_graphs(B, L, path):
     """Labelling alone on adversarial bond graphs (long thin spiral, comb, wrap-around rows)."""
     sw = B.SwendsenWang(L, 2.0, 1, path=path)
