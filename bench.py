@@ -74,10 +74,21 @@ class ClockSampler:
         self.p = None
         try:
             self.p = subprocess.Popen(["nvidia-smi", "-i", str(gpu_index), f"--query-gpu={self.QUERY}",
-                                       "--format=csv,noheader,nounits", "-lms", "100"],
+                                       "--format=csv,noheader,nounits", "-lms", "20"],
                                       stdout=self.f, stderr=subprocess.DEVNULL)
         except Exception:
             self.p = None
+
+    def wait_ready(self, timeout_s: float = 5.0):
+        """nvidia-smi takes a while to print its first line on a fresh box: wait for it, so that the samples cover the timed region."""
+        t0 = time.time()
+        while self.p is not None and time.time() - t0 < timeout_s:
+            try:
+                if os.path.getsize(self.f.name) > 0:
+                    return
+            except OSError:
+                return
+            time.sleep(0.05)
 
     def stop(self):
         out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
@@ -485,14 +496,14 @@ def main():
     stream = torch.cuda.current_stream(dev)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     clocks = ClockSampler(local)
-    time.sleep(0.3)
+    clocks.wait_ready()
     barrier()
     e0.record(stream)
     sw.sweep(K)
     e1.record(stream)
     barrier()
     ms = e0.elapsed_time(e1)
-    time.sleep(0.2)
+    time.sleep(0.05)
     clk = clocks.stop()
     launches = sw.launch_count()
     kms = sw.kernel_ms()
