@@ -465,7 +465,10 @@ int launch_label(sw_handle* h) {
 }
 
 // Potts fast path: k_bond_label<4, 64, FUSE, POTTS> (equal-colour masks from the int8 plane), then the node merge
-int launch_bond_label_potts(sw_handle* h) {
+// Potts fast path with few colours: E of a sweep from the next sweep's bond test, colour counts (for M) from the assignment kernel
+bool potts_folded(const sw_handle* h) { return h->q && h->q <= 8 && h->tile == SCAN_4x64; }
+
+int launch_bond_label_potts(sw_handle* h, bool obs_prev) {
     constexpr int NW = 4, TH = 64, TW = 32 * NW, CAP = 2 * (TW + TH);
     const int tiles = h->N / (TW * TH);
     constexpr size_t smem = (size_t)TW * TH * sizeof(uint32_t);
@@ -474,7 +477,7 @@ int launch_bond_label_potts(sw_handle* h) {
     SW_MARK(h, K_BONDLABEL);
     k_bond_label<NW, TH, true, true><<<dim3(tiles, h->nb), NW * TH, smem, h->stream>>>(
         reinterpret_cast<const uint32_t*>(h->spins), h->bondE, h->bondS, h->lab16, h->nodes, h->ocount, h->bslot,
-        h->series, h->lat, h->ctl, h->L, h->N, h->words, h->nb, 0);
+        h->series, h->lat, h->ctl, h->L, h->N, h->words, h->nb, obs_prev ? 1 : 0);
     const size_t nedge = (size_t)h->L * (h->L / TW + h->L / TH);
     SW_MARK(h, K_MERGE);
     k_merge_nodes<TW, TH><<<grid1(nedge, 256, h->nb), 256, 0, h->stream>>>(h->nodes, h->bslot, h->L / TW, h->L / TH);
@@ -498,17 +501,22 @@ int launch_sweep_potts(sw_handle* h, int64_t k) {
     }
     if (h->tile == SCAN_4x64) {
         // fast path: fused bond draw + scan-line tile labelling, node merge, colour per tile root
-        if ((rc = launch_bond_label_potts(h))) return rc;
+        const bool folded = potts_folded(h);          // E with the next sweep's bond test, colour counts in the assignment
+        if ((rc = launch_bond_label_potts(h, folded && k > 0))) return rc;
         SW_MARK(h, K_FLIPTILE);
         k_assign16_potts<4, 64><<<dim3(h->N / (128 * 64), h->nb), 256, 0, h->stream>>>(
-            h->spins, h->lab16, h->nodes, h->ocount, h->series, h->lat, h->ctl, make_div(h->L), h->q, h->L, h->N, h->nb);
+            h->spins, h->lab16, h->nodes, h->ocount, h->series, h->lat, h->ctl, make_div(h->L), h->q, h->L, h->N, h->nb,
+            folded ? h->potts_cnt : nullptr);
         SW_MARK(h, K_ENERGY);
-        k_observe_potts_rows<<<grid1((size_t)h->N / 16, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(
-            h->spins, h->series, h->potts_cnt, h->ctl, 1, h->q, h->L, h->N, h->nb);
+        if (!folded) {
+            k_observe_potts_rows<<<grid1((size_t)h->N / 16, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(
+                h->spins, h->series, h->potts_cnt, h->ctl, 1, h->q, h->L, h->N, h->nb);
+            h->launches += 1;
+        }
         k_potts_finish<<<1, 64, 0, h->stream>>>(h->series, h->potts_cnt, h->ctl, 1, h->q, h->N, h->nb);
         SW_MARK(h, K_ADVANCE);
-        k_advance<<<1, 64, 0, h->stream>>>(h->ctl, h->series, h->nb, h->mom, h->N, 1);
-        h->launches += 4;
+        k_advance<<<1, 64, 0, h->stream>>>(h->ctl, h->series, h->nb, h->mom, h->N, folded ? (k > 0 ? 2 : 0) : 1);
+        h->launches += 3;
         SW_MARK(h, K_COUNT);
         h->labels_flat = false;                      // int32 labels on demand (k_labels16)
         h->lab_tile = h->tile;
@@ -833,6 +841,14 @@ int sw_sweep(sw_handle* h, int64_t n) {
         int rc = launch_sweep(h, k);
         if (rc) return rc;
     }
+    if (potts_folded(h)) {                              // Potts fast path: E of the configuration the call ends with
+        if (h->timing) SW_CUDA(cudaEventRecord(h->ev_tail[0], h->stream));
+        k_observe_potts_rows<<<grid1((size_t)h->N / 16, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(
+            h->spins, h->series, h->potts_cnt, h->ctl, 2, h->q, h->L, h->N, h->nb);
+        k_moments_last<<<1, 64, 0, h->stream>>>(h->ctl, h->series, h->nb, h->mom, h->N);
+        if (h->timing) SW_CUDA(cudaEventRecord(h->ev_tail[1], h->stream));
+        h->launches += 2;
+    }
     if (scan_nw(h->tile) && !h->q) {                    // a7 of the configuration the call ends with
         if (h->timing) SW_CUDA(cudaEventRecord(h->ev_tail[0], h->stream));
         if (sweeps_on_bits(h))
@@ -1147,7 +1163,7 @@ int sw_kernel_ms(sw_handle* h, float* out, int32_t cap) {
             SW_CUDA(cudaEventElapsedTime(&ms, h->ev[(size_t)k * EV_PER_SWEEP + j], h->ev[(size_t)k * EV_PER_SWEEP + j + 1]));
             if (h->ev_seq[j] < cap) out[h->ev_seq[j]] += ms;
         }
-    if (scan_nw(h->tile) && !h->q && K_ENERGY < cap) {  // the trailing observables pass of the call
+    if (scan_nw(h->tile) && (!h->q || potts_folded(h)) && K_ENERGY < cap) {  // the trailing observables pass of the call
         float ms = 0.f;
         SW_CUDA(cudaEventElapsedTime(&ms, h->ev_tail[0], h->ev_tail[1]));
         out[K_ENERGY] += ms;

@@ -111,7 +111,7 @@ template <int NW, int TH>
 __global__ void __launch_bounds__(NW * TH, 1536 / (NW * TH))
 k_assign16_potts(int8_t* __restrict__ colours, const uint16_t* __restrict__ lab16, const int4* __restrict__ nodes,
                  const int* __restrict__ ocount, Rec* __restrict__ rec, const Lat* __restrict__ lat,
-                 const Ctl* __restrict__ ctl, DivL dv, int q, int L, int N, int nb) {
+                 const Ctl* __restrict__ ctl, DivL dv, int q, int L, int N, int nb, int* __restrict__ cnt) {
     constexpr int TW = 32 * NW, SITES = TW * TH, THREADS = NW * TH;
     constexpr int CAP = 2 * (TW + TH);
     constexpr int OSTEPS = SITES / 8 / THREADS;      // = 4
@@ -136,6 +136,7 @@ k_assign16_potts(int8_t* __restrict__ colours, const uint16_t* __restrict__ lab1
     const Lat la = lat[blockIdx.y];
     const unsigned long long t = ctl->t;
     const uint32_t tlo = (uint32_t)t, thi = (uint32_t)(t >> 32);
+    uint32_t ncol[2] = { 0u, 0u };                   // my sites per colour, a byte each (at most 32): colours 0-3, 4-7
 
     // which of my 32 sites are tile roots (their 16-bit root is their own local index)
     uint32_t rootmask = 0;
@@ -193,6 +194,29 @@ k_assign16_potts(int8_t* __restrict__ colours, const uint16_t* __restrict__ lab1
         }
         *reinterpret_cast<uint2*>(colours + (size_t)blockIdx.y * N + (size_t)(y0 + (l >> LOG_TW)) * L + x0 + (l & (TW - 1))) =
             make_uint2(out[0], out[1]);
+        if (cnt) {                                   // (q <= 8) sites per colour, for M: equal bytes against the splat of the colour
+#pragma unroll
+            for (int c = 0; c < 8; ++c)
+                if (c < q) {
+                    const uint32_t pat = (uint32_t)c * 0x01010101u;
+                    ncol[c >> 2] += (uint32_t)((__popc(__vcmpeq4(out[0], pat)) + __popc(__vcmpeq4(out[1], pat))) >> 3) << (8 * (c & 3));
+                }
+        }
+    }
+    if (cnt) {
+        // the colour counts of the new configuration, a7 (the order parameter needs max_c n_c): one add per warp and colour
+        // into shared memory, one per CTA into the lattice's counters (k_potts_finish turns them into M)
+        __shared__ int s_ncol[8];
+        if (tid < 8) s_ncol[tid] = 0;
+        __syncthreads();
+#pragma unroll
+        for (int c = 0; c < 8; ++c)
+            if (c < q) {
+                const int n_c = warp_sum_i((int)((ncol[c >> 2] >> (8 * (c & 3))) & 0xFFu));
+                if ((tid & 31) == 0 && n_c) atomicAdd(&s_ncol[c], n_c);
+            }
+        __syncthreads();
+        if (tid < q && s_ncol[tid]) atomicAdd(cnt + (size_t)blockIdx.y * q + tid, s_ncol[tid]);
     }
 }
 
@@ -201,6 +225,8 @@ k_assign16_potts(int8_t* __restrict__ colours, const uint16_t* __restrict__ lab1
 __global__ void __launch_bounds__(GEN_THREADS)
 k_observe_potts_rows(const int8_t* __restrict__ colours, Rec* __restrict__ rec, int* __restrict__ cnt,
                      const Ctl* __restrict__ ctl, int use_slot, int q, int L, int N, int nb) {
+    // use_slot: 0 record 0 (sw_observables of a state no sweep produced), 1 the running sweep's slot, 2 the slot BEFORE it and
+    // the energy only (end of a sw_sweep call on the fast path: E of a sweep otherwise comes out of the next sweep's bond test)
     __shared__ int s_cnt[POTTS_MAX_Q + 1];
     __shared__ int s_e;
     for (int c = threadIdx.x; c <= POTTS_MAX_Q; c += GEN_THREADS) s_cnt[c] = 0;
@@ -225,7 +251,9 @@ k_observe_potts_rows(const int8_t* __restrict__ colours, Rec* __restrict__ rec, 
             e -= (__popc(__vcmpeq4(w[k], east)) + __popc(__vcmpeq4(w[k], so[k]))) >> 3;
         }
     }
-    if (q <= 8) {
+    if (use_slot == 2) {
+        // (energy only)
+    } else if (q <= 8) {
         // few colours: sites of colour c among my 16 = equal bytes against the splat of c; one add per warp and colour
         for (int c = 0; c < q; ++c) {
             const uint32_t pat = (uint32_t)c * 0x01010101u;
@@ -248,9 +276,10 @@ k_observe_potts_rows(const int8_t* __restrict__ colours, Rec* __restrict__ rec, 
     if ((threadIdx.x & 31) == 0 && e) atomicAdd(&s_e, e);
     __syncthreads();
     for (int c = threadIdx.x; c < q; c += GEN_THREADS)
-        if (s_cnt[c]) atomicAdd(cnt + (size_t)blockIdx.y * q + c, s_cnt[c]);
+        if (use_slot != 2 && s_cnt[c]) atomicAdd(cnt + (size_t)blockIdx.y * q + c, s_cnt[c]);
     if (threadIdx.x == 0 && s_e) {
-        Rec* r = rec + (use_slot ? (size_t)ctl->slot * nb : 0) + blockIdx.y;
+        const uint32_t slot = use_slot == 2 ? (ctl->slot == 0 ? ctl->cap - 1 : ctl->slot - 1) : ctl->slot;
+        Rec* r = rec + (use_slot ? (size_t)slot * nb : 0) + blockIdx.y;
         atomic_add_ll(&r->E, s_e);
     }
 }

@@ -231,6 +231,12 @@ k_bond_label(const uint32_t* __restrict__ sbits, uint32_t* bondE, uint32_t* bond
                 const uint32_t eastm = (own >> 1) | ((~nxw & 1u) << 31);
                 eqE = ~(own ^ eastm); eqS = ~(own ^ south);
             }
+            if (POTTS && obs_prev) {
+                // Potts: E = -#(equal East / South pairs) of the configuration the previous sweep left (M comes from the colour
+                // counts of the assignment kernel)
+                const int eo = warp_sum_i(-(__popc(eqE) + __popc(eqS)));
+                if (lane == 0) atomicAdd(&s_obs[0], eo);
+            }
             if (!POTTS && obs_prev) {
                 // a7 for free: the equal-pair masks of the bond test are the energy of the
                 // configuration the previous sweep left: E = (#edges) - 2 (#equal pairs), M = N - 2 (#down)
