@@ -255,6 +255,18 @@ int mark(sw_handle* h, int kid) {
 // k_roots_nodes: 4 warps per tile while the whole batch has fewer tiles than the GPU holds warps
 inline int roots_warps_per_tile(const sw_handle* h, int tiles) { return (long long)tiles * h->nb < 4096 ? 4 : 1; }
 
+// launch with programmatic stream serialization (see pdl_wait in sw_common.cuh): the kernels of the fast path's sweep
+template <typename... KArgs, typename... Args>
+cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args&&... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
+}
+
 // opt-in dynamic shared memory, once per kernel and device
 template <typename K>
 int opt_in_smem(K kernel, size_t smem, bool* done, int dev) {
@@ -276,10 +288,10 @@ int launch_bond_label_scan(sw_handle* h, bool fused, bool obs_prev) {
     { int rc = opt_in_smem(k_bond_label<NW, TH, false, false, BAND_T>, smem, done[1], h->dev); if (rc) return rc; }
     if (fused) {
         SW_MARK(h, K_BONDLABEL);
-        k_bond_label<NW, TH, true, false, BAND_T><<<dim3(tiles, h->nb), THREADS, smem, h->stream>>>(
+        SW_CUDA(launch_pdl(k_bond_label<NW, TH, true, false, BAND_T>, dim3(tiles, h->nb), dim3(THREADS), smem, h->stream,
             h->sbits, h->bondE, h->bondS, h->lab16, h->nodes, h->ocount, h->bslot,
             h->series, h->lat, h->ctl,
-            h->L, h->N, h->words, h->nb, obs_prev ? 1 : 0);
+            h->L, h->N, h->words, h->nb, obs_prev ? 1 : 0));
     } else {
         SW_MARK(h, K_TILE);
         k_bond_label<NW, TH, false, false, BAND_T><<<dim3(tiles, h->nb), THREADS, smem, h->stream>>>(
@@ -289,12 +301,12 @@ int launch_bond_label_scan(sw_handle* h, bool fused, bool obs_prev) {
     }
     const size_t nedge = (size_t)h->L * (h->L / TW + h->L / TH);
     SW_MARK(h, K_MERGE);
-    k_merge_nodes<TW, TH><<<grid1(nedge, 256, h->nb), 256, 0, h->stream>>>(
-        h->nodes, h->bslot, h->L / TW, h->L / TH);
+    SW_CUDA(launch_pdl(k_merge_nodes<TW, TH>, grid1(nedge, 256, h->nb), dim3(256), 0, h->stream,
+        h->nodes, h->bslot, h->L / TW, h->L / TH));
     SW_MARK(h, K_SIZES);
     const int wpt = roots_warps_per_tile(h, tiles);
-    k_roots_nodes<CAP><<<grid1((size_t)tiles * wpt * 32, 256, h->nb), 256, 0, h->stream>>>(
-        h->nodes, h->ocount, tiles, wpt);
+    SW_CUDA(launch_pdl(k_roots_nodes<CAP>, grid1((size_t)tiles * wpt * 32, 256, h->nb), dim3(256), 0, h->stream,
+        h->nodes, h->ocount, tiles, wpt));
     h->launches += 3;
     return SW_OK;
 }
@@ -367,12 +379,12 @@ int launch_flip_scan(sw_handle* h, int adv_acc) {
         int& nsm = sms[h->dev >= 0 && h->dev < MAX_DEV ? h->dev : 0];
         if (!nsm) SW_CUDA(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, h->dev));
         const int ctas = std::max(1, std::min(tiles, 3 * nsm / std::max(1, std::min(h->nb, 3))));   // persistent: ~3 CTAs per SM in all
-        k_flip16_tma<<<dim3(ctas, h->nb), 256 + 32 * FT_PROD_WARPS, smem, h->stream>>>(
-            h->tmap, h->tmap_d, h->sbits, h->D, h->nodes, h->ocount, h->series, h->ctl, make_div(h->L), h->L, h->N, h->words, h->nb, tiles);
+        SW_CUDA(launch_pdl(k_flip16_tma, dim3(ctas, h->nb), dim3(256 + 32 * FT_PROD_WARPS), smem, h->stream,
+            h->tmap, h->tmap_d, h->sbits, h->D, h->nodes, h->ocount, h->series, h->ctl, make_div(h->L), h->L, h->N, h->words, h->nb, tiles));
     } else if (flip_fused(h))
-        k_flip16<NW, TH, true, true><<<dim3(tiles, h->nb), NW * TH, 0, h->stream>>>(
+        SW_CUDA(launch_pdl(k_flip16<NW, TH, true, true>, dim3(tiles, h->nb), dim3(NW * TH), 0, h->stream,
             h->spins, h->sbits, h->lab16, nullptr, h->nodes, h->ocount, h->series, h->ctl, h->lat, h->mom, adv_acc,
-            make_div(h->L), h->L, h->N, h->words, h->nb);
+            make_div(h->L), h->L, h->N, h->words, h->nb));
     else if (sweeps_on_bits(h))
         k_flip16<NW, TH, true><<<dim3(tiles, h->nb), NW * TH, 0, h->stream>>>(
             h->spins, h->sbits, h->lab16, h->D, h->nodes, h->ocount, h->series, h->ctl, h->lat, h->mom, adv_acc,
@@ -559,15 +571,15 @@ int launch_sweep(sw_handle* h, int64_t k) {
         const bool ff = flip_fused(h);
         if (!ff) {
             SW_MARK(h, K_FLIPBITS);
-            k_flipbits<<<grid1(((size_t)h->words + 3) / 4, GEN_THREADS, h->nb), GEN_THREADS, 0, h->stream>>>(
-                h->D, h->lat, h->ctl, h->words);
+            SW_CUDA(launch_pdl(k_flipbits, grid1(((size_t)h->words + 3) / 4, GEN_THREADS, h->nb), dim3(GEN_THREADS), 0, h->stream,
+                h->D, h->lat, h->ctl, h->words));
             h->launches += 1;
         }
         rc = nw == 4 ? launch_flip_scan<4, 64>(h, adv_acc) : launch_flip_scan<2, 32>(h, adv_acc);
         if (rc) return rc;
         if (!ff) {
             SW_MARK(h, K_ADVANCE);
-            k_advance<<<1, 64, 0, h->stream>>>(h->ctl, h->series, h->nb, h->mom, h->N, adv_acc);
+            SW_CUDA(launch_pdl(k_advance, dim3(1), dim3(64), 0, h->stream, h->ctl, h->series, h->nb, h->mom, h->N, adv_acc));
             h->launches += 1;
         }
         SW_MARK(h, K_COUNT);

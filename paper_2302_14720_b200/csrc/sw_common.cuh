@@ -50,6 +50,12 @@ __device__ __forceinline__ void mom_add(Mom& m, long long E, long long M, int N)
     m.n += 1;
 }
 
+// programmatic dependent launch: the kernels of a sweep are launched with the "programmatic stream serialization" attribute, so
+// that the next kernel's launch overlaps the tail of the running one; a kernel waits HERE -- before it reads anything an
+// earlier kernel of the stream wrote -- until that kernel has completed and its writes are visible (a no-op in a kernel that was
+// launched the ordinary way)
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
 // bit-plane layout shared by the bond planes and the decision plane D: bit (i & 31) of word (i >> 5)
 __device__ __forceinline__ uint32_t get_bit(const uint32_t* __restrict__ plane, int i) {
     return (plane[i >> 5] >> (i & 31)) & 1u;

@@ -72,6 +72,7 @@ k_flip16_tma(const __grid_constant__ CUtensorMap tm_lab, const __grid_constant__
              uint32_t* __restrict__ sbits, const uint32_t* __restrict__ D, const int4* __restrict__ nodes,
              const int* __restrict__ ocount, Rec* __restrict__ rec, const Ctl* __restrict__ ctl,
              DivL dv, int L, int N, int words, int nb, int tiles) {
+    pdl_wait();
     constexpr int NW = 4, TH = 64, TW = 128, OSTEPS = 4, LOG_TW = 7;
     extern __shared__ __align__(128) uint8_t stage_mem[];
     __shared__ __align__(8) uint64_t full[FT_NSTAGE], empty[FT_NSTAGE];

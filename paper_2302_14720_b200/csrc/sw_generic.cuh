@@ -134,6 +134,7 @@ k_maxsize_generic(const int* __restrict__ label, const int* __restrict__ gsize, 
 //      one thread per call = 4 words = 128 candidate root decisions ------------------------------
 __global__ void __launch_bounds__(GEN_THREADS)
 k_flipbits(uint32_t* __restrict__ D, const Lat* __restrict__ lat, const Ctl* __restrict__ ctl, int words) {
+    pdl_wait();
     const int c = blockIdx.x * GEN_THREADS + threadIdx.x;      // call index
     if (c * 4 >= words) return;
     const Lat la = lat[blockIdx.y];
@@ -241,6 +242,7 @@ k_philox_only(uint32_t* __restrict__ sink, uint32_t key0, uint32_t key1, uint32_
 
 // ---- sweep control -------------------------------------------------------------------------------
 __global__ void k_set_ctl(Ctl* ctl, unsigned long long t, uint32_t slot, uint32_t cap) {
+    pdl_wait();
     ctl->t = t; ctl->slot = slot; ctl->cap = cap; ctl->done = 0; ctl->pad = 0;
 }
 // end of a sweep: t += 1, move to the next series slot and zero it.  acc: which record feeds the running
@@ -265,6 +267,8 @@ __device__ __forceinline__ void advance_sweep(Ctl* ctl, Rec* rec, int nb, Mom* m
 __global__ void k_advance(Ctl* ctl, Rec* rec, int nb, Mom* mom, int N, int acc) { advance_sweep(ctl, rec, nb, mom, N, acc); }
 // scan path, end of a sw_sweep call (after k_observe_rows): the last sweep's record, now complete
 __global__ void k_moments_last(const Ctl* ctl, const Rec* rec, int nb, Mom* mom, int N) {
+    pdl_wait();
+    pdl_wait();
     const uint32_t from = ctl->slot == 0 ? ctl->cap - 1 : ctl->slot - 1;
     for (int b = threadIdx.x; b < nb; b += blockDim.x) {
         const Rec r = rec[(size_t)from * nb + b];

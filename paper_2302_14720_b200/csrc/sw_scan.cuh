@@ -148,6 +148,7 @@ k_bond_label(const uint32_t* __restrict__ sbits, uint32_t* bondE, uint32_t* bond
              uint16_t* __restrict__ bslot,
              Rec* __restrict__ rec, const Lat* __restrict__ lat, const Ctl* __restrict__ ctl,
              int L, int N, int words, int nb, int obs_prev) {
+    pdl_wait();
     constexpr int BAND = BAND_T;                // (shadows the default: rows per warp block in this instantiation)
     constexpr int TPW = 32 / BAND;              // threads per 32-site word (one warp per 32 x BAND block)
     constexpr int TW = 32 * NW, SITES = TW * TH, WORDS = NW * TH, THREADS = WORDS * TPW;
@@ -534,6 +535,7 @@ __device__ __forceinline__ void nd_union(int4* nodes, int a, int b) {
 template <int TW, int TH>
 __global__ void __launch_bounds__(256)
 k_merge_nodes(int4* nodes, const uint16_t* __restrict__ bslot, int tilesX, int tilesY) {
+    pdl_wait();
     constexpr int CAP = 2 * (TW + TH), PER = TW + TH;       // per tile: TW South-row sites, TH East-column sites
     const int idx = blockIdx.x * 256 + threadIdx.x;
     const int tiles = tilesX * tilesY;
@@ -558,6 +560,7 @@ k_merge_nodes(int4* nodes, const uint16_t* __restrict__ bslot, int tilesX, int t
 template <int CAP>
 __global__ void __launch_bounds__(256)
 k_roots_nodes(int4* nodes, const int* __restrict__ ocount, int tiles, int wpt) {
+    pdl_wait();
     const int gw = blockIdx.x * 8 + (threadIdx.x >> 5);
     const int tile = gw / wpt, sub = gw - tile * wpt;
     const int lane = threadIdx.x & 31;
@@ -605,6 +608,7 @@ template <int NW, int TH>
 __global__ void __launch_bounds__(NW * TH)
 k_labels16(int* __restrict__ label, const uint16_t* __restrict__ lab16, const int4* __restrict__ nodes,
            const int* __restrict__ ocount, DivL dv, int L, int N) {
+    pdl_wait();
     constexpr int TW = 32 * NW, SITES = TW * TH, THREADS = NW * TH, CAP = 2 * (TW + TH);
     constexpr int LOG_TW = ilog2_c(TW);
     extern __shared__ int tab[];                     // [SITES] canonical label of the open tile root with this local index, else -1
@@ -670,6 +674,7 @@ k_flip16(int8_t* __restrict__ spins, uint32_t* __restrict__ sbits, const uint16_
          const int4* __restrict__ nodes, const int* __restrict__ ocount, Rec* __restrict__ rec, Ctl* __restrict__ ctl,
          const Lat* __restrict__ lat, Mom* __restrict__ mom, int adv_acc,
          DivL dv, int L, int N, int words, int nb) {
+    pdl_wait();
     constexpr int TW = 32 * NW, SITES = TW * TH, THREADS = NW * TH;
     constexpr int CAP = 2 * (TW + TH);
     constexpr int OSTEPS = SITES / 8 / THREADS;      // = 4
@@ -779,6 +784,7 @@ k_flip16(int8_t* __restrict__ spins, uint32_t* __restrict__ sbits, const uint16_
 __global__ void __launch_bounds__(256)
 k_observe_rows(const int8_t* __restrict__ spins, Rec* __restrict__ rec, const Ctl* __restrict__ ctl,
                int L, int N, int words, int nb) {
+    pdl_wait();
     const int w = blockIdx.x * 256 + threadIdx.x;
     int e = 0, m = 0;
     if (w < words) {
@@ -812,6 +818,7 @@ k_observe_rows(const int8_t* __restrict__ spins, Rec* __restrict__ rec, const Ct
 __global__ void __launch_bounds__(256)
 k_observe_bits(const uint32_t* __restrict__ sbits, Rec* __restrict__ rec, const Ctl* __restrict__ ctl,
                int L, int N, int words, int nb) {
+    pdl_wait();
     const int w = blockIdx.x * 256 + threadIdx.x;
     int e = 0, m = 0;
     if (w < words) {
