@@ -179,6 +179,8 @@ struct sw_handle {
     // TMA staging of the 16-bit root plane in the assignment kernel (sw_flip_tma.cuh): tensor map of lab16, made on first use
     CUtensorMap tmap, tmap_d; int tmap_state = 0;   // 0: not tried, 1: ready, -1: unavailable (k_flip16 is used)
     bool use_tma = true;
+    // side branch of the sweep: the decision plane depends on nothing but the sweep index, so k_flipbits runs beside the labelling
+    cudaStream_t side = nullptr; cudaEvent_t ev_fork = nullptr, ev_join = nullptr; bool side_failed = false;
 };
 
 namespace {
@@ -558,6 +560,24 @@ int launch_sweep(sw_handle* h, int64_t k) {
     if (const int nw = scan_nw(h->tile)) {
         const bool fused = h->path != 6;
         const bool obs_prev = k > 0;                    // E, M of sweep k - 1 come out of this sweep's bond test
+        // the decision plane on a side branch (fork here, join before the assignment): under capture this becomes a parallel
+        // branch of the graph.  Not with per-kernel timing (the events of the split assume one stream).
+        bool side = fused && !flip_fused(h) && !h->timing && !h->side_failed;
+        if (side && !h->side) {
+            if (cudaStreamCreateWithFlags(&h->side, cudaStreamNonBlocking) != cudaSuccess ||
+                cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
+                cudaEventCreateWithFlags(&h->ev_join, cudaEventDisableTiming) != cudaSuccess) {
+                (void)cudaGetLastError(); h->side_failed = true; side = false;
+            }
+        }
+        if (side) {
+            SW_CUDA(cudaEventRecord(h->ev_fork, h->stream));
+            SW_CUDA(cudaStreamWaitEvent(h->side, h->ev_fork, 0));
+            k_flipbits<<<grid1(((size_t)h->words + 3) / 4, GEN_THREADS, h->nb), GEN_THREADS, 0, h->side>>>(
+                h->D, h->lat, h->ctl, h->words);
+            SW_CUDA(cudaEventRecord(h->ev_join, h->side));
+            h->launches += 1;
+        }
         if (!fused) {                                   // stand-alone a1 for the per-stage split
             SW_MARK(h, K_BOND);
             k_bond_rows<<<grid1(h->words, ROW_THREADS, h->nb), ROW_THREADS, 0, h->stream>>>(
@@ -569,7 +589,8 @@ int launch_sweep(sw_handle* h, int64_t k) {
         if (rc) return rc;
         const int adv_acc = k > 0 ? 2 : 0;              // (E, M of a sweep arrive with the next sweep's bond test)
         const bool ff = flip_fused(h);
-        if (!ff) {
+        if (side) SW_CUDA(cudaStreamWaitEvent(h->stream, h->ev_join, 0));
+        if (!ff && !side) {
             SW_MARK(h, K_FLIPBITS);
             SW_CUDA(launch_pdl(k_flipbits, grid1(((size_t)h->words + 3) / 4, GEN_THREADS, h->nb), dim3(GEN_THREADS), 0, h->stream,
                 h->D, h->lat, h->ctl, h->words));
@@ -746,6 +767,9 @@ void sw_destroy(sw_handle* h) {
     for (cudaGraphExec_t g : h->gexec) if (g) cudaGraphExecDestroy(g);
     for (cudaEvent_t e : h->gev) if (e) cudaEventDestroy(e);
     if (h->gstream) cudaStreamDestroy(h->gstream);
+    if (h->ev_fork) cudaEventDestroy(h->ev_fork);
+    if (h->ev_join) cudaEventDestroy(h->ev_join);
+    if (h->side) cudaStreamDestroy(h->side);
     if (h->series_owned) cudaFree(h->series_owned);
     if (h->potts_cnt) cudaFree(h->potts_cnt);
     if (h->eq_ref) cudaFree(h->eq_ref);
