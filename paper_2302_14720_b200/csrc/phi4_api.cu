@@ -3,14 +3,15 @@
 // Product code (CUDA path).  No CPU fallback.  Shares the device Philox and the lock-free union-find with the Ising path
 // (sw_common.cuh); nothing with oracle/.
 //
-// One update = 7 launches on one stream, no host synchronisation (the sweep index lives on the device, so the sequence is
+// One update = 4 launches on one stream, no host synchronisation (the sweep index lives on the device, so the sequence is
 // replayed from a CUDA graph):
-//   k4_direction   one thread: the update's direction r (rejection from the cube to the ball, IEEE-exact operations)
+//   (k4_direction  first update of a call only: the update's direction r, rejection from the cube to the ball, IEEE-exact
+//                  operations; afterwards the block that closes an update draws the next one's)
 //   k4_bonds       thread per site: projections, Eq. 2 thresholds, 4 Philox words -> bond byte; label[x] = x
 //   k4_union       thread per site: lock-free union-find over its bonds (atomicMin hooking: the root is the minimum index)
 //   k4_reflect     thread per site: root (stored: flat labels), cluster sizes, selection bit of the root, Eq. 3
-//   k4_observe     link and magnetisation sums of the new field (fixed tree inside a block, partials per block),
-//   k4_finish      partials summed in block order by one block; cluster count / largest / bonds; record; t += 1
+//   k4_observe     link and magnetisation sums of the new field (fixed tree inside a block, partials per block); the block that
+//                  finishes last sums the partials in block order, writes the record, advances t and draws the next direction
 // The lattices of the paper (L = 16 .. 28: 2 .. 20 MB of field) live in L2; the update is bound by launch latency and the
 // dependent walks of the union-find, not by HBM.
 #include "../../include/phi4.h"
@@ -82,12 +83,8 @@ __global__ void k4_init(double* __restrict__ phi, int V, uint32_t key0, uint32_t
 
 __global__ void k4_set_ctl(Ctl4* ctl, unsigned long long t, uint32_t slot, uint32_t cap) { ctl->t = t; ctl->slot = slot; ctl->cap = cap; }
 
-// step 1: the direction of this update, r . r = 1; also clears the integer accumulators of the record
-__global__ void k4_direction(double* __restrict__ r, const Ctl4* __restrict__ ctl, long long* __restrict__ iacc,
-                             uint32_t key0, uint32_t key1) {
-    if (threadIdx.x != 0) return;
-    iacc[0] = 0; iacc[1] = 0; iacc[2] = 0;
-    const unsigned long long t = ctl->t;
+// step 1: the direction of the update with sweep index t, r . r = 1 (one thread)
+__device__ __forceinline__ void draw_direction(double* __restrict__ r, unsigned long long t, uint32_t key0, uint32_t key1) {
     for (uint32_t j = 0; ; ++j) {
         const uint4 w = draw4(j, t, TAG_DIR, key0, key1);
         const double v0 = sym(w.x), v1 = sym(w.y), v2 = sym(w.z), v3 = sym(w.w);
@@ -98,6 +95,14 @@ __global__ void k4_direction(double* __restrict__ r, const Ctl4* __restrict__ ct
             return;
         }
     }
+}
+// first update of a phi4_sweep call: its direction, and the integer accumulators of its record cleared (the following
+// updates get both from the end of the update before them: k4_observe)
+__global__ void k4_direction(double* __restrict__ r, const Ctl4* __restrict__ ctl, long long* __restrict__ iacc,
+                             uint32_t key0, uint32_t key1) {
+    if (threadIdx.x != 0) return;
+    iacc[0] = 0; iacc[1] = 0; iacc[2] = 0; iacc[3] = 0;
+    draw_direction(r, ctl->t, key0, key1);
 }
 
 // Eq. 2 as an integer threshold on a 32-bit word
@@ -181,10 +186,45 @@ k4_reflect(double* __restrict__ phi, const double* __restrict__ r, int* label, i
     if ((threadIdx.x & 31) == 0 && isroot) atomic_add_ll(&iacc[0], isroot);
 }
 
-// observables of the new field: per block a fixed tree over its sites -> partial[block][5]; largest cluster
+// the block's partial sums in block order (fixed strided tree: the result does not depend on which block runs this), the
+// record of the update, t += 1; with `advance` also the NEXT update's direction and cleared accumulators (r_last keeps the
+// direction this update used, for phi4_direction)
+__device__ void finish_update(const double* __restrict__ partial, int nblocks, Rec4* __restrict__ rec, Ctl4* ctl,
+                              long long* __restrict__ iacc, double* __restrict__ r, double* __restrict__ r_last,
+                              uint32_t key0, uint32_t key1, int advance, double (*sh)[P4_THREADS]) {
+    double v[5] = { 0.0, 0.0, 0.0, 0.0, 0.0 };
+    for (int b = threadIdx.x; b < nblocks; b += P4_THREADS)
+#pragma unroll
+        for (int k = 0; k < 5; ++k) v[k] = __dadd_rn(v[k], __ldcg(partial + (size_t)b * 5 + k));
+#pragma unroll
+    for (int k = 0; k < 5; ++k) sh[k][threadIdx.x] = v[k];
+    __syncthreads();
+    for (int s = P4_THREADS / 2; s > 0; s >>= 1) {
+        if (threadIdx.x < s)
+#pragma unroll
+            for (int k = 0; k < 5; ++k) sh[k][threadIdx.x] = __dadd_rn(sh[k][threadIdx.x], sh[k][threadIdx.x + s]);
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) {
+        Rec4 rc;
+        rc.link = sh[0][0]; rc.m[0] = sh[1][0]; rc.m[1] = sh[2][0]; rc.m[2] = sh[3][0]; rc.m[3] = sh[4][0];
+        rc.ncl = advance ? iacc[0] : 0; rc.maxcl = advance ? iacc[1] : 0; rc.nbonds = advance ? iacc[2] : 0;
+        rec[advance ? ctl->slot : ctl->cap] = rc;                // (slot `cap` = the scratch record of phi4_observables)
+        if (advance) {
+            ctl->t += 1; ctl->slot = ctl->slot + 1 == ctl->cap ? 0u : ctl->slot + 1;
+            r_last[0] = r[0]; r_last[1] = r[1]; r_last[2] = r[2]; r_last[3] = r[3];
+            iacc[0] = 0; iacc[1] = 0; iacc[2] = 0;
+            draw_direction(r, ctl->t, key0, key1);
+        }
+    }
+}
+
+// observables of the new field: per block a fixed tree over its sites -> partial[block][5]; largest cluster; the block
+// that finishes last closes the update (finish_update)
 __global__ void __launch_bounds__(P4_THREADS)
 k4_observe(const double* __restrict__ phi, const int* __restrict__ gsize, double* __restrict__ partial,
-           long long* __restrict__ iacc, Geo g, int with_sizes) {
+           long long* __restrict__ iacc, Geo g, int with_sizes, Rec4* __restrict__ rec, Ctl4* ctl,
+           double* __restrict__ r, double* __restrict__ r_last, uint32_t key0, uint32_t key1, int advance) {
     const int x = blockIdx.x * P4_THREADS + threadIdx.x;
     double v[5] = { 0.0, 0.0, 0.0, 0.0, 0.0 };
     int big = 0;
@@ -200,7 +240,8 @@ k4_observe(const double* __restrict__ phi, const int* __restrict__ gsize, double
         v[1] = a.x; v[2] = a.y; v[3] = b.x; v[4] = b.y;
         if (with_sizes) big = gsize[x];
     }
-    __shared__ double sh[5][P4_THREADS / 32];
+    __shared__ double sh[5][P4_THREADS];
+    __shared__ int s_last;
 #pragma unroll
     for (int k = 0; k < 5; ++k) {
 #pragma unroll
@@ -215,32 +256,16 @@ k4_observe(const double* __restrict__ phi, const int* __restrict__ gsize, double
         for (int w = 0; w < P4_THREADS / 32; ++w) tot = __dadd_rn(tot, sh[threadIdx.x][w]);
         partial[(size_t)blockIdx.x * 5 + threadIdx.x] = tot;
     }
-}
-
-// one block: partials in block order (fixed strided tree), record of the update, t += 1
-__global__ void __launch_bounds__(P4_THREADS)
-k4_finish(const double* __restrict__ partial, int nblocks, Rec4* __restrict__ rec, Ctl4* ctl, const long long* __restrict__ iacc,
-          int advance) {
-    __shared__ double sh[5][P4_THREADS];
-    double v[5] = { 0.0, 0.0, 0.0, 0.0, 0.0 };
-    for (int b = threadIdx.x; b < nblocks; b += P4_THREADS)
-#pragma unroll
-        for (int k = 0; k < 5; ++k) v[k] = __dadd_rn(v[k], partial[(size_t)b * 5 + k]);
-#pragma unroll
-    for (int k = 0; k < 5; ++k) sh[k][threadIdx.x] = v[k];
     __syncthreads();
-    for (int s = P4_THREADS / 2; s > 0; s >>= 1) {
-        if (threadIdx.x < s)
-#pragma unroll
-            for (int k = 0; k < 5; ++k) sh[k][threadIdx.x] = __dadd_rn(sh[k][threadIdx.x], sh[k][threadIdx.x + s]);
-        __syncthreads();
-    }
     if (threadIdx.x == 0) {
-        Rec4 r;
-        r.link = sh[0][0]; r.m[0] = sh[1][0]; r.m[1] = sh[2][0]; r.m[2] = sh[3][0]; r.m[3] = sh[4][0];
-        r.ncl = advance ? iacc[0] : 0; r.maxcl = advance ? iacc[1] : 0; r.nbonds = advance ? iacc[2] : 0;
-        rec[advance ? ctl->slot : ctl->cap] = r;                 // (slot `cap` = the scratch record of phi4_observables)
-        if (advance) { ctl->t += 1; ctl->slot = ctl->slot + 1 == ctl->cap ? 0u : ctl->slot + 1; }
+        __threadfence();
+        s_last = atomicAdd(reinterpret_cast<unsigned long long*>(&iacc[3]), 1ull) == (unsigned long long)gridDim.x - 1;
+    }
+    __syncthreads();
+    if (s_last) {                                           // (every other block's partials and maximum are in)
+        __threadfence();
+        if (threadIdx.x == 0) iacc[3] = 0;
+        finish_update(partial, (int)gridDim.x, rec, ctl, iacc, r, r_last, key0, key1, advance, sh);
     }
 }
 
@@ -258,7 +283,7 @@ struct phi4_handle {
     double kappa = 0.0;
     uint32_t key0 = 0, key1 = 0;
     Geo g{};
-    double* phi = nullptr; double* r = nullptr; double* partial = nullptr;
+    double* phi = nullptr; double* r = nullptr; double* partial = nullptr;      // r: [0..3] the running update's direction, [4..7] the last one's
     uint8_t* bonds = nullptr; int* label = nullptr; int* gsize = nullptr;
     long long* iacc = nullptr; Ctl4* ctl = nullptr; Rec4* rec = nullptr;      // rec: P4_SERIES_CAP ring + 1 scratch
     uint64_t t = 0;
@@ -272,17 +297,17 @@ struct phi4_handle {
 
 namespace {
 
-int launch_update(phi4_handle* h) {
+int launch_update(phi4_handle* h, bool first) {
     const unsigned nb = (unsigned)h->nblocks;
-    k4_direction<<<1, 32, 0, h->stream>>>(h->r, h->ctl, h->iacc, h->key0, h->key1);
+    if (first) { k4_direction<<<1, 32, 0, h->stream>>>(h->r, h->ctl, h->iacc, h->key0, h->key1); h->launches += 1; }
     k4_bonds<<<nb, P4_THREADS, 0, h->stream>>>(h->phi, h->r, h->bonds, h->label, h->gsize, h->ctl, h->iacc, h->g,
                                                -4.0 * h->kappa, h->key0, h->key1);
     k4_union<<<nb, P4_THREADS, 0, h->stream>>>(h->label, h->bonds, h->g);
     k4_reflect<<<nb, P4_THREADS, 0, h->stream>>>(h->phi, h->r, h->label, h->gsize, h->ctl, h->iacc, h->g, h->key0, h->key1);
-    k4_observe<<<nb, P4_THREADS, 0, h->stream>>>(h->phi, h->gsize, h->partial, h->iacc, h->g, 1);
-    k4_finish<<<1, P4_THREADS, 0, h->stream>>>(h->partial, h->nblocks, h->rec, h->ctl, h->iacc, 1);
+    k4_observe<<<nb, P4_THREADS, 0, h->stream>>>(h->phi, h->gsize, h->partial, h->iacc, h->g, 1, h->rec, h->ctl, h->r, h->r + 4,
+                                                 h->key0, h->key1, 1);
     P4_CUDA(cudaGetLastError());
-    h->launches += 6;
+    h->launches += 4;
     return PHI4_OK;
 }
 
@@ -321,7 +346,7 @@ phi4_handle* phi4_create(int32_t L, double kappa, uint64_t seed) {
     bool ok = cudaGetDevice(&h->dev) == cudaSuccess;
     const size_t V = (size_t)h->V;
     ok = ok && cudaMalloc((void**)&h->phi, V * 4 * sizeof(double)) == cudaSuccess;
-    ok = ok && cudaMalloc((void**)&h->r, 4 * sizeof(double)) == cudaSuccess;
+    ok = ok && cudaMalloc((void**)&h->r, 8 * sizeof(double)) == cudaSuccess;
     ok = ok && cudaMalloc((void**)&h->partial, (size_t)h->nblocks * 5 * sizeof(double)) == cudaSuccess;
     ok = ok && cudaMalloc((void**)&h->bonds, V) == cudaSuccess;
     ok = ok && cudaMalloc((void**)&h->label, V * sizeof(int)) == cudaSuccess;
@@ -332,7 +357,7 @@ phi4_handle* phi4_create(int32_t L, double kappa, uint64_t seed) {
     if (ok) {
         k4_init<<<(unsigned)h->nblocks, P4_THREADS>>>(h->phi, h->V, h->key0, h->key1);
         k4_set_ctl<<<1, 1>>>(h->ctl, 0ull, 0u, (uint32_t)P4_SERIES_CAP);
-        ok = cudaMemset(h->r, 0, 4 * sizeof(double)) == cudaSuccess && cudaMemset(h->iacc, 0, 4 * sizeof(long long)) == cudaSuccess &&
+        ok = cudaMemset(h->r, 0, 8 * sizeof(double)) == cudaSuccess && cudaMemset(h->iacc, 0, 4 * sizeof(long long)) == cudaSuccess &&
              cudaDeviceSynchronize() == cudaSuccess;
     }
     if (!ok) {
@@ -385,14 +410,14 @@ int phi4_sweep(phi4_handle* h, int64_t n) {
     }
     k4_set_ctl<<<1, 1, 0, h->stream>>>(h->ctl, (unsigned long long)h->t, 0u, (uint32_t)P4_SERIES_CAP);
     h->launches += 1;
-    { int rc = launch_update(h); if (rc) return rc; }
+    { int rc = launch_update(h, true); if (rc) return rc; }
     int64_t k = 1;
     if (graphs && !h->gexec) {
         cudaGraph_t graph = nullptr;
         const int64_t keep = h->launches;
         bool ok = cudaStreamBeginCapture(h->stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
         if (ok) {
-            const int rc = launch_update(h);
+            const int rc = launch_update(h, false);
             ok = cudaStreamEndCapture(h->stream, &graph) == cudaSuccess && rc == PHI4_OK && graph;
         }
         if (ok) ok = cudaGraphInstantiate(&h->gexec, graph, 0) == cudaSuccess;
@@ -401,8 +426,8 @@ int phi4_sweep(phi4_handle* h, int64_t n) {
         if (!ok) { (void)cudaGetLastError(); h->gexec = nullptr; h->graph_failed = true; graphs = false; }
     }
     if (graphs)
-        for (; k < n; ++k) { P4_CUDA(cudaGraphLaunch(h->gexec, h->stream)); h->launches += 6; }
-    for (; k < n; ++k) { int rc = launch_update(h); if (rc) return rc; }
+        for (; k < n; ++k) { P4_CUDA(cudaGraphLaunch(h->gexec, h->stream)); h->launches += 4; }
+    for (; k < n; ++k) { int rc = launch_update(h, false); if (rc) return rc; }
     P4_CUDA(cudaGetLastError());
     h->t += (uint64_t)n; h->last_n = n; h->have_sweep = true; h->rec_valid = true;
     return PHI4_OK;
@@ -423,7 +448,7 @@ int phi4_direction(phi4_handle* h, double r[4]) {
     if (!h || !r) { set_err4("phi4_direction: null argument"); return PHI4_EINVAL; }
     if (!h->have_sweep) { set_err4("phi4_direction: no update has run yet"); return PHI4_ESTATE; }
     DevGuard4 dg(h->dev);
-    P4_CUDA(cudaMemcpyAsync(r, h->r, 4 * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    P4_CUDA(cudaMemcpyAsync(r, h->r + 4, 4 * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
     P4_CUDA(cudaStreamSynchronize(h->stream));
     return PHI4_OK;
 }
@@ -436,8 +461,8 @@ int phi4_observables(phi4_handle* h, phi4_obs* out) {
         const int64_t slot = (h->last_n - 1) % P4_SERIES_CAP;
         P4_CUDA(cudaMemcpyAsync(&r, h->rec + slot, sizeof(Rec4), cudaMemcpyDeviceToHost, h->stream));
     } else {
-        k4_observe<<<(unsigned)h->nblocks, P4_THREADS, 0, h->stream>>>(h->phi, h->gsize, h->partial, h->iacc, h->g, 0);
-        k4_finish<<<1, P4_THREADS, 0, h->stream>>>(h->partial, h->nblocks, h->rec, h->ctl, h->iacc, 0);
+        k4_observe<<<(unsigned)h->nblocks, P4_THREADS, 0, h->stream>>>(h->phi, h->gsize, h->partial, h->iacc, h->g, 0, h->rec, h->ctl,
+                                                                       h->r, h->r + 4, h->key0, h->key1, 0);
         P4_CUDA(cudaGetLastError());
         P4_CUDA(cudaMemcpyAsync(&r, h->rec + P4_SERIES_CAP, sizeof(Rec4), cudaMemcpyDeviceToHost, h->stream));
     }
