@@ -173,7 +173,7 @@ __device__ __forceinline__ int uf_find(const int* lab, int x) {
 }
 // the same walk through L1 (ld.global.ca).  A stale line can only show an older parent, which is still an
 // ancestor, so the walk ends at a node that was a root when its line was fetched; callers either run when no
-// root changes any more (k_roots_open) or let an atomic on the result arbitrate (uf_union_l1).  At T_c one
+// root changes any more (k_roots_nodes) or let an atomic on the result arbitrate (uf_union_l1).  At T_c one
 // cluster owns ~1/3 of all sites: its root's line would otherwise be fetched from one L2 slice by every walker.
 __device__ __forceinline__ int ld_ca(const int* p) {
     int v; asm volatile("ld.global.ca.s32 %0, [%1];" : "=r"(v) : "l"(p)); return v;

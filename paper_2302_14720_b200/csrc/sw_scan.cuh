@@ -1,31 +1,31 @@
-// sw_scan.cuh -- the fast path (lattice side a multiple of 64; the default tile is 128 x 64).
+// sw_scan.cuh -- the fast path (lattice side a multiple of 64): 128 x 64 tiles above L = 1024, 64 x 32 tiles up to it.
 //
-// Stage map; one CTA per tile of TW x TH sites, TW = 32 * NW, TH = 32 or 64; the tile is
-// NW x TH/32 blocks of 32 x 32 sites, one warp each; NW * TH threads = one thread per 32-site word.
-//   a1+a2 k_bond_label<NW, TH, FUSE>
-//       phase 1  thread per 32-site word: the word's spins from the BIT-PACKED plane (FUSE; bit 1 = +1; the int8 plane
-//                is derived on demand, sw_spins), 16 Philox4x32-10 calls, bond words to
-//                shared memory and to the canonical global bit-planes; E, M of the previous sweep's
-//                configuration from the same equal-pair masks; the bonds that enter the tile from its North
-//                and West neighbours are recomputed (TW/2 + TH extra calls)
-//       phase 2  scan-line labelling, lane = column, the block's rows in sequence, uniform control flow:
-//                runs of East bonds from bit tricks on the row's bond word; a run takes the label of the
-//                first of its sites that has a South bond from the row above (one shuffle), or opens a new
-//                label (its head's index); other sites of the run whose upper label differs hook the larger
-//                under the smaller (atomicMin)
-//       phase 3  seams between blocks (East bonds across strips, South bonds across the band seam)
-//       phase 3b thread per word: the label nodes (heads of runs with no bond from above) point at their roots
-//       phase 4  open flags (border sites), then per site: root = par[par[site]], 16-bit tile-local root to
-//                global memory (2 B / site), cluster sizes into spare bits of the root's word
-//       phase 5  closed roots -> count, running maximum; open roots -> nodes (parent, size, min site, site)
+// Stage map; one CTA per tile of TW x TH sites, TW = 32 * NW; the tile is NW x TH / BAND blocks of
+// 32 x BAND sites, one warp each (BAND = 32: one thread per 32-site word; BAND = 8: four threads per word -- small lattices).
+//   a1+a2 k_bond_label<NW, TH, FUSE, POTTS, BAND>
+//       phase 1  per 32-site word: the word's spins from the BIT-PACKED plane (FUSE; bit 1 = +1; the int8 plane is derived
+//                on demand, sw_spins), 16 Philox4x32-10 calls, bond words to shared memory and to the canonical global
+//                bit-planes; E, M of the previous sweep's configuration from the same equal-pair masks; the bonds that enter
+//                the tile from its North and West neighbours are recomputed (TW/2 + TH extra calls)
+//       phase 2  scan-line labelling, lane = column, the block's rows in sequence, uniform control flow: runs of East bonds
+//                from bit tricks on the row's bond word; a run takes the label of the first of its sites that has a South
+//                bond from the row above (one shuffle), or opens a new label (its head's index); where another site of the
+//                run is bonded to a different label above, the site is listed (ballot-compacted); after the block the warp
+//                unites the listed pairs with all lanes (atomicMin hooking; hooked nodes go into a tile-wide list)
+//       phase 3  seams between blocks (East bonds across strips, South bonds across band seams); every site counted at its label
+//       phase 3b the label nodes (heads of runs with no bond from above) are counted; the hooked ones point at their roots and
+//                hand them their counts
+//       phase 4  per site: root = parent(parent(site)) -> 16-bit tile-local root to global memory (2 B / site); largest count
+//       phase 5  border sites with a bond across the tile edge claim their root: node (parent, size, min site, site), slot
 //       phase 6  per border site with a bond across the tile edge: the slot of its root
 //   a3    k_merge_nodes (union-find over the nodes of neighbouring tiles), k_roots_nodes (sizes and minimum
 //         site index of the clusters that span tiles)
-//   a4-a6 k_flip16<NW, TH, BITS>: one decision bit per tile root in shared memory, spins = lookup by 16-bit root,
-//         written bit-packed (BITS: a byte per 8 sites) or as int8 (unfused path 6);
+//   a4-a6 k_flip16<NW, TH, BITS, FUSED>: one decision bit per tile root in shared memory, spins = lookup by 16-bit root,
+//         written bit-packed (BITS: a byte per 8 sites) or as int8 (unfused path 6); on 128 x 64 tiles of large lattices the
+//         TMA-staged, warp-specialised k_flip16_tma (sw_flip_tma.cuh) does the same;
 //         k_labels16<NW, TH>: flat int32 labels from the 16-bit roots, on demand (sw_labels)
 //   a7    E, M: by-product of the next sweep's bond test, k_observe_bits / k_observe_rows at the end of a call; cluster count
-//         and largest cluster: k_bond_label (closed) + k_flip16 (root nodes)
+//         and largest cluster: k_bond_label (closed roots, largest tile-local count) + the assignment kernel (root nodes)
 #pragma once
 #include "sw_common.cuh"
 
@@ -656,7 +656,7 @@ k_labels16(int* __restrict__ label, const uint16_t* __restrict__ lab16, const in
 // memory, one decision bit per TILE ROOT, indexed by the root's tile-local index:
 //   closed tile root g (cluster inside the tile): the cluster root is g itself -> bit D[g]: the tile's own
 //                      words of the decision plane, copied in bulk;
-//   open tile root g:  its cluster root R was found by k_roots_open and sits next to g in the tile's list ->
+//   open tile root g:  its cluster root R was found by k_roots_nodes and sits next to g in the tile's list ->
 //                      bit D[R] overwrites the copied bit (a few hundred per tile).
 // Then every site reads its 16-bit tile-local root index (2 B / site, written by k_bond_label) and looks the
 // bit up in shared memory: no global gather, no index arithmetic per site.
