@@ -250,8 +250,10 @@ k_bond_label(const uint32_t* __restrict__ sbits, uint32_t* bondE, uint32_t* bond
             for (int cc = 0; cc < 16 / TPW; ++cc) {
                 const int c = part * (16 / TPW) + cc;
                 const uint4 r = philox4x32_10((uint32_t)w * 16u + c, tlo, thi, TAG_BOND, key);
-                dE |= ((r.x < la.thr ? 1u : 0u) | (r.z < la.thr ? 2u : 0u)) << (2 * c);
-                dS |= ((r.y < la.thr ? 1u : 0u) | (r.w < la.thr ? 2u : 0u)) << (2 * c);
+                if (r.x < la.thr) dE |= 1u << (2 * c);               // (a compare and a predicated OR per word)
+                if (r.z < la.thr) dE |= 2u << (2 * c);
+                if (r.y < la.thr) dS |= 1u << (2 * c);
+                if (r.w < la.thr) dS |= 2u << (2 * c);
             }
 #pragma unroll
             for (int o = 1; o < TPW; o <<= 1) {                      // the word's TPW threads are neighbouring lanes
