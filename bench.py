@@ -378,6 +378,18 @@ def block_config5(B, wl, dev):
             "note": "sweeps 50 .. 249 of the 1000; aggregate over the 32 lattices"}
 
 
+def block_batch_small(B, wl, dev):
+    """Many small lattices in one handle (one launch per stage for the whole batch): 148 lattices of L = 256 at T_c -- what a
+    temperature / replica scan of the paper's sizes runs like when the lattices are batched instead of swept one by one."""
+    L, nb = 256, 148
+    sw = B.SwendsenWang(L, [wl.T_C] * nb, [3000 + b for b in range(nb)], device=str(dev))
+    sw.sweep(100)
+    ms = _timed_sweeps(sw, 400)
+    sw.close()
+    return {"L": L, "lattices": nb, "us_per_batch_sweep": 1e3 * ms, "us_per_lattice_sweep": 1e3 * ms / nb,
+            "site_updates_per_s": nb * L * L / (ms * 1e-3), "sweeps": 400}
+
+
 def block_paper_sizes(B, dev):
     """The paper's own table (Fig. 8): L = 128 .. 4096 at k_B T = 2.5, time per sweep (graphs on)."""
     paper_gpu_min = {128: 0.112, 256: 0.151, 512: 0.390, 1024: 1.472, 2048: 5.483, 4096: 22.440}     # 10,000 iterations, Tesla P100
@@ -678,6 +690,7 @@ def main():
         extras["config3"] = side(lambda: block_config3(B, wl, dev))
         extras["config5"] = side(lambda: block_config5(B, wl, dev))
         extras["paper_sizes"] = side(lambda: block_paper_sizes(B, dev))
+        extras["batch_small"] = side(lambda: block_batch_small(B, wl, dev))
         extras["config2_moments"] = side(lambda: block_config2_moments(B, wl, dev))
         extras["phi4"] = side(lambda: block_phi4(dev))
 
