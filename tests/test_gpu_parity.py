@@ -237,6 +237,17 @@ def test_handle_on_a_device_that_is_not_current(B):
     sw.close()
 
 
+def test_random_sizes_temperatures_and_seeds(B):
+    """A sweep of (L, T, seed) drawn from a fixed generator over both tile shapes and the generic path: every sweep in full."""
+    rng = np.random.default_rng(20260511)
+    sides = [64, 128, 192, 256, 320, 384, 448, 576, 704, 1088, 1152, 1280, 96, 160, 40]
+    for k in range(18):
+        L = int(sides[k % len(sides)])
+        T = float(rng.choice([0.9, 1.6, 2.1, T_C, 2.4, 2.9, 4.5, 9.0]))
+        seed = int(rng.integers(1, 2 ** 62))
+        _compare_sweeps(B, L, T, seed, 4 if L < 1000 else 3)
+
+
 def test_race_order_independence(B):
     """Same state, same sweep index, repeated: identical bits every time (min-index labels)."""
     L, T, seed = 512, T_C, 3
