@@ -153,14 +153,11 @@ k_bond_label(const uint32_t* __restrict__ sbits, uint32_t* bondE, uint32_t* bond
     constexpr int TPW = 32 / BAND;              // threads per 32-site word (one warp per 32 x BAND block)
     constexpr int TW = 32 * NW, SITES = TW * TH, WORDS = NW * TH, THREADS = WORDS * TPW;
     constexpr int CAP = 2 * (TW + TH);
-    constexpr int NWARPS = THREADS / 32;
     static_assert(TPW == 1 || TPW == 2 || TPW == 4, "threads per word");
-    constexpr int PCAP = 192;                   // label meetings a warp can list while it scans its block (~80 at T_c)
     constexpr int HKCAP = 1024;                 // hooked nodes the tile can list (~250 at T_c)
     static_assert(TH % BAND == 0 && TH <= 64 && SITES <= 8192 && CAP < 0x3FFF, "tile shape");
     extern __shared__ __align__(16) uint32_t par[];  // [SITES] (see above); dynamic: 32 KB at 128 x 64
     __shared__ uint2 es[TH * NW];              // [row][strip] = (East word, South word)
-    __shared__ uint16_t pend[NWARPS][PCAP];    // phase 2: sites where two labels met
     __shared__ uint16_t hkitems[HKCAP];        // nodes hooked in phases 2 and 3
     __shared__ uint32_t nIn[NW];               // South bonds entering from the tile above, per strip
     __shared__ uint32_t wIn[2];                // East bonds entering from the tile to the West, bit = row
@@ -307,7 +304,9 @@ k_bond_label(const uint32_t* __restrict__ sbits, uint32_t* bondE, uint32_t* bond
         uint32_t rowaddr = par_s + 4u * (rowbase + lane) + 2u;       // my site's parent field in this row
         uint32_t prev = 0;                                           // label of the site above
         uint32_t s_up = 0;                                           // (a band's first row adopts nothing: seams come later)
-        const uint32_t pl_s = (uint32_t)__cvta_generic_to_shared(pend[warp]);
+        // the warp's list of meetings lives in the (still unused) count fields of its own block: entry k in the low half of
+        // the block's word (k >> 5, k & 31).  No capacity to overflow (a block has fewer meetings than sites), no memory of its own.
+        const uint32_t pl_s = par_s + 4u * rowbase;
         int npend = 0;                                               // (warp-uniform)
 #pragma unroll SCAN_UNROLL
         for (int y = yb; y < yb + BAND; ++y, rowbase += TW, rowaddr += 4u * TW) {
@@ -324,26 +323,24 @@ k_bond_label(const uint32_t* __restrict__ sbits, uint32_t* bondE, uint32_t* bond
             const bool meet = (s_up & lanebit) && prev != c;         // two labels meet at my site: the one above, my run's
             const uint32_t mb = __ballot_sync(0xffffffffu, meet);
             const int at = npend + __popc(mb & lt);
-            if (meet && at < PCAP) sts_u16(pl_s + 2u * at, (uint32_t)(rowbase + lane));
+            if (meet) sts_u16(pl_s + 4u * (uint32_t)((at >> 5) * TW + (at & 31)), (uint32_t)(rowbase + lane));
             npend += __popc(mb);
             prev = c;
             s_up = w.y;
         }
-        __syncwarp();                                                // the block's parents and meetings are written
-        if (npend <= PCAP) {
-            for (int j = lane; j < npend; j += 32) {                 // unite with all lanes
-                const uint32_t i = lds_u16(pl_s + 2u * j);
+        // unite with all lanes, 32 meetings at a time.  An entry is read and its field cleared (the counts start at 0 in
+        // phase 3) while no union of this warp is in flight: a hook wipes the low half of the word it replaces and adds it
+        // back, and only this warp's unions touch this block's words before the barrier below.
+        for (int j0 = 0; j0 < npend; j0 += 32) {
+            __syncwarp();
+            const int j = j0 + lane;
+            const uint32_t slot = pl_s + 4u * (uint32_t)((j >> 5) * TW + (j & 31));
+            uint32_t i = 0;
+            if (j < npend) { i = lds_u16(slot); sts_u16(slot, 0u); }
+            __syncwarp();
+            if (j < npend) {
                 const int a = (int)lds_u16(par_s + 4u * (i - TW) + 2u), c = (int)lds_u16(par_s + 4u * i + 2u);
                 hooked(hk, sc_union(par_s, a, c));                   // (labels are mostly still roots: sc_union takes any nodes)
-            }
-        } else {
-            // more meetings than the list holds (far from the workloads' bond densities): take them from the labels again
-            for (int y = yb + 1; y < yb + BAND; ++y) {
-                const int i = y * TW + strip * 32 + lane;
-                if ((es[(y - 1) * NW + strip].y >> lane) & 1u) {
-                    const int a = (int)lds_u16(par_s + 4u * (i - TW) + 2u), c = (int)lds_u16(par_s + 4u * i + 2u);
-                    if (a != c) hooked(hk, sc_union(par_s, a, c));
-                }
             }
         }
     }
