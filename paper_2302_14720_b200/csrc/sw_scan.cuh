@@ -10,8 +10,8 @@
 //       phase 2  scan-line labelling, lane = column, the block's rows in sequence, uniform control flow: runs of East bonds
 //                from bit tricks on the row's bond word; a run takes the label of the first of its sites that has a South
 //                bond from the row above (one shuffle), or opens a new label (its head's index); where another site of the
-//                run is bonded to a different label above, the site is listed (ballot-compacted); after the block the warp
-//                unites the listed pairs with all lanes (atomicMin hooking; hooked nodes go into a tile-wide list)
+//                run is bonded to a different label above, the lane notes the row in a bit mask; after the block every lane
+//                unites the pairs of its column (atomicMin hooking; hooked nodes go into a tile-wide list)
 //       phase 3  seams between blocks (East bonds across strips, South bonds across band seams); every site counted at its label
 //       phase 3b the label nodes (heads of runs with no bond from above) are counted; the hooked ones point at their roots and
 //                hand them their counts
@@ -97,14 +97,13 @@ __device__ __forceinline__ uint32_t atom_add_s(uint32_t a, uint32_t v) {
 }
 // the tile's list of hooked nodes (phase 3b flattens from it with all threads); the counter runs on past the capacity
 // (it also gives the number of roots), and phase 3b then visits every label node instead
-struct HookList { uint32_t items_s, count_s; int cap; };     // (shared-window addresses)
+struct HookList { uint32_t items_s, count_s; int cap; uint32_t one; };     // (shared-window addresses; one = 1)
 __device__ __forceinline__ void hooked(const HookList& hk, int node) {
     if (node == NO_NODE) return;
-    // (the increment is made opaque: ptxas would otherwise turn the add into a warp-aggregated one -- vote, popc,
-    // shuffle: 20 instructions -- for the few lanes that get here together)
-    uint32_t one = 1u;
-    asm volatile("mov.u32 %0, %0;" : "+r"(one));
-    const int pos = (int)atom_add_s(hk.count_s, one);
+    // (the increment is a 1 that ptxas cannot prove to be one -- `one` comes from a kernel argument: it would otherwise
+    // turn the add into a warp-aggregated one -- vote, popc, shuffle: 20 instructions -- for the few lanes that get here
+    // together)
+    const int pos = (int)atom_add_s(hk.count_s, hk.one);
     if (pos < hk.cap) sts_u16(hk.items_s + 2u * pos, (uint32_t)node);
 }
 __device__ __forceinline__ int sc_union(uint32_t par_s, int a, int b) {
@@ -180,7 +179,7 @@ k_bond_label(const uint32_t* __restrict__ sbits, uint32_t* bondE, uint32_t* bond
     if (tid == 0) { wIn[0] = 0; wIn[1] = 0; s_nopen = 0; s_max = 0; s_nlab = 0; s_nhook = 0; s_obs[0] = 0; s_obs[1] = 0; }
     uint32_t par_s = (uint32_t)__cvta_generic_to_shared(par);        // shared-window address of word 0
     asm volatile("mov.u32 %0, %0;" : "+r"(par_s));                   // (opaque: kept in a register, not recomputed at every use)
-    const HookList hk = { (uint32_t)__cvta_generic_to_shared(hkitems), (uint32_t)__cvta_generic_to_shared(&s_nhook), HKCAP };
+    const HookList hk = { (uint32_t)__cvta_generic_to_shared(hkitems), (uint32_t)__cvta_generic_to_shared(&s_nhook), HKCAP, (uint32_t)(L > -tid) };   // (1, but neither constant nor warp-uniform for ptxas)
 #pragma unroll
     for (int k = 0; k < SITES / 4 / THREADS; ++k)                    // counts start at 0 (the scan stores parents only)
         sts_u128(par_s + 16u * (k * THREADS + tid), make_uint4(0u, 0u, 0u, 0u));
@@ -295,19 +294,16 @@ k_bond_label(const uint32_t* __restrict__ sbits, uint32_t* bondE, uint32_t* bond
     // Lane = column, the block's rows in sequence, uniform control flow.  A run of East bonds takes the label of the
     // first of its sites that has a South bond from the row above (one shuffle), or opens a new label = its head's
     // own index (a root).  Where another site of the run is bonded to a different label above, the two labels are
-    // equivalent: the pair goes into the warp's list (ballot-compacted, no divergent work in the loop) and the warp
-    // unites its pairs with all lanes once the block is scanned.  Labels are never refreshed on the way down, so the
-    // only loop-carried dependency of a row is the shuffle.
+    // equivalent: the lane notes the row in a bit mask (no divergent work in the loop, no list) and unites the pairs of
+    // its column once the block is scanned.  Labels are never refreshed on the way down, so the only loop-carried
+    // dependency of a row is the shuffle.
     {
         const int strip = warp % NW, yb = (warp / NW) * BAND;
         int rowbase = yb * TW + strip * 32;                          // first site of the row in this strip
         uint32_t rowaddr = par_s + 4u * (rowbase + lane) + 2u;       // my site's parent field in this row
         uint32_t prev = 0;                                           // label of the site above
         uint32_t s_up = 0;                                           // (a band's first row adopts nothing: seams come later)
-        // the warp's list of meetings lives in the (still unused) count fields of its own block: entry k in the low half of
-        // the block's word (k >> 5, k & 31).  No capacity to overflow (a block has fewer meetings than sites), no memory of its own.
-        const uint32_t pl_s = par_s + 4u * rowbase;
-        int npend = 0;                                               // (warp-uniform)
+        uint32_t mymeet = 0;                                         // rows of the block where two labels met at my column
 #pragma unroll SCAN_UNROLL
         for (int y = yb; y < yb + BAND; ++y, rowbase += TW, rowaddr += 4u * TW) {
             const uint2 w = es[y * NW + strip];
@@ -321,16 +317,36 @@ k_bond_label(const uint32_t* __restrict__ sbits, uint32_t* bondE, uint32_t* bond
             const uint32_t c = upm ? got : (uint32_t)(rowbase + h);  // a new label: the head's own index (its own root)
             sts_u16(rowaddr, c);
             const bool meet = (s_up & lanebit) && prev != c;         // two labels meet at my site: the one above, my run's
-            const uint32_t mb = __ballot_sync(0xffffffffu, meet);
-            const int at = npend + __popc(mb & lt);
-            if (meet) sts_u16(pl_s + 4u * (uint32_t)((at >> 5) * TW + (at & 31)), (uint32_t)(rowbase + lane));
-            npend += __popc(mb);
+            mymeet = (mymeet >> 1) | (meet ? 0x80000000u : 0u);
             prev = c;
             s_up = w.y;
         }
-        // unite with all lanes, 32 meetings at a time.  An entry is read and its field cleared (the counts start at 0 in
-        // phase 3) while no union of this warp is in flight: a hook wipes the low half of the word it replaces and adds it
-        // back, and only this warp's unions touch this block's words before the barrier below.
+        __syncwarp();                                                // the block's parents are written
+        // The meetings (~2.5 per lane at T_c, up to ~7) are united by all lanes, 32 at a time: every lane writes the sites of
+        // its column into the warp's list at the positions a prefix sum gives it.  The list lives in the (still unused)
+        // count fields of the warp's own block: entry k in the low half of the block's word (k >> 5, k & 31) -- no memory of
+        // its own (6 CTAs per SM), no capacity to overflow (a block has fewer meetings than sites).
+        mymeet >>= 32 - BAND;                                        // bit r: row yb + r
+        const uint32_t pl_s = par_s + 4u * (uint32_t)(yb * TW + strip * 32);
+        const int cnt = __popc(mymeet);
+        int pos = cnt;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int v = __shfl_up_sync(0xffffffffu, pos, o);
+            if (lane >= o) pos += v;
+        }
+        const int npend = __shfl_sync(0xffffffffu, pos, 31);
+        pos -= cnt;
+        const int colbase = yb * TW + strip * 32 + lane;
+        while (mymeet) {
+            const int i = colbase + (__ffs(mymeet) - 1) * TW;
+            mymeet &= mymeet - 1u;
+            sts_u16(pl_s + 4u * (uint32_t)((pos >> 5) * TW + (pos & 31)), (uint32_t)i);
+            ++pos;
+        }
+        // An entry is read and its field cleared (the counts start at 0 in phase 3) while no union of this warp is in
+        // flight: a hook wipes the low half of the word it replaces and adds it back, and only this warp's unions touch
+        // this block's words before the barrier below.
         for (int j0 = 0; j0 < npend; j0 += 32) {
             __syncwarp();
             const int j = j0 + lane;
