@@ -380,7 +380,7 @@ int launch_flip_scan(sw_handle* h, int adv_acc) {
         static int sms[MAX_DEV];
         int& nsm = sms[h->dev >= 0 && h->dev < MAX_DEV ? h->dev : 0];
         if (!nsm) SW_CUDA(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, h->dev));
-        const int ctas = std::max(1, std::min(tiles, 3 * nsm / std::max(1, std::min(h->nb, 3))));   // persistent: ~3 CTAs per SM in all
+        const int ctas = std::max(1, std::min(tiles, FT_CTAS_PER_SM * nsm / std::max(1, std::min(h->nb, FT_CTAS_PER_SM))));   // persistent: FT_CTAS_PER_SM CTAs per SM in all
         SW_CUDA(launch_pdl(k_flip16_tma, dim3(ctas, h->nb), dim3(256 + 32 * FT_PROD_WARPS), smem, h->stream,
             h->tmap, h->tmap_d, h->sbits, h->D, h->nodes, h->ocount, h->series, h->ctl, make_div(h->L), h->L, h->N, h->words, h->nb, tiles));
     } else if (flip_fused(h))

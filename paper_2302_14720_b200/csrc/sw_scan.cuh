@@ -32,7 +32,7 @@
 namespace sw {
 
 #ifndef SCAN_UNROLL_N
-#define SCAN_UNROLL_N 16
+#define SCAN_UNROLL_N 32
 #endif
 constexpr int SCAN_UNROLL = SCAN_UNROLL_N;      // rows of the scan loop unrolled together
 constexpr int BAND = 32;                        // rows a warp walks by default; a tile is TH / BAND bands of NW strips
