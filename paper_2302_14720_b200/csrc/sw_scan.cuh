@@ -391,6 +391,25 @@ k_bond_label(const uint32_t* __restrict__ sbits, uint32_t* bondE, uint32_t* bond
             red_add_s(par_s + 4u * n2, 1u); red_add_s(par_s + 4u * n3, 1u);
         }
     }
+    // (the label nodes are counted here, in front of the barrier: bit tricks on the bond words only)
+    uint32_t o;                                                      // heads of runs without an uplink in this thread's word
+    int mybase;
+    {
+        const int wd = tid < WORDS ? tid : 0;                        // (with several threads per word the first WORDS threads count)
+        mybase = (wd / NW) * TW + (wd % NW) * 32;
+        const uint32_t ew = es[wd].x & 0x7FFFFFFFu;
+        uint32_t up = (wd / NW) % BAND ? es[wd - NW].y : 0u;         // South bonds of the row above, within the band
+        uint32_t m = ew;                                             // OR of the run's uplinks, gathered at its head
+        up |= (up >> 1) & m;  m &= m >> 1;
+        up |= (up >> 2) & m;  m &= m >> 2;
+        up |= (up >> 4) & m;  m &= m >> 4;
+        up |= (up >> 8) & m;  m &= m >> 8;
+        up |= (up >> 16) & m;
+        o = ~(ew << 1) & ~up;
+        if (tid >= WORDS) o = 0;
+        const int nl = warp_sum_i(__popc(o));
+        if (lane == 0) atomicAdd(&s_nlab, nl);
+    }
     __syncthreads();
 
     // ---- phase 3b: flatten ---------------------------------------------------------------------------
@@ -401,20 +420,6 @@ k_bond_label(const uint32_t* __restrict__ sbits, uint32_t* bondE, uint32_t* bond
     // root's count is the size of its tile-local cluster.  The label nodes themselves are only COUNTED (bit tricks
     // on the bond words): roots = label nodes - hooked nodes.
     {
-        const int wd = tid < WORDS ? tid : 0;                        // (with several threads per word the first WORDS threads count)
-        const int mybase = (wd / NW) * TW + (wd % NW) * 32;
-        const uint32_t ew = es[wd].x & 0x7FFFFFFFu;
-        uint32_t up = (wd / NW) % BAND ? es[wd - NW].y : 0u;         // South bonds of the row above, within the band
-        uint32_t m = ew;                                             // OR of the run's uplinks, gathered at its head
-        up |= (up >> 1) & m;  m &= m >> 1;
-        up |= (up >> 2) & m;  m &= m >> 2;
-        up |= (up >> 4) & m;  m &= m >> 4;
-        up |= (up >> 8) & m;  m &= m >> 8;
-        up |= (up >> 16) & m;
-        uint32_t o = ~(ew << 1) & ~up;                               // heads of runs without an uplink
-        if (tid >= WORDS) o = 0;
-        const int nl = warp_sum_i(__popc(o));
-        if (lane == 0) atomicAdd(&s_nlab, nl);
         const int nh = s_nhook;                                      // (complete: the barrier above)
         if (nh <= HKCAP) {
             for (int j = tid; j < nh; j += THREADS) sc_flatten(par_s, hkitems[j]);
