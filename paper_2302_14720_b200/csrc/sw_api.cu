@@ -255,7 +255,10 @@ int mark(sw_handle* h, int kid) {
 #define SW_MARK(h, kid) do { int rc_ = mark((h), (kid)); if (rc_) return rc_; } while (0)
 
 // k_roots_nodes: 4 warps per tile while the whole batch has fewer tiles than the GPU holds warps
-inline int roots_warps_per_tile(const sw_handle* h, int tiles) { return (long long)tiles * h->nb < 4096 ? 4 : 1; }
+#ifndef ROOTS_WPT
+#define ROOTS_WPT 1
+#endif
+inline int roots_warps_per_tile(const sw_handle* h, int tiles) { return (long long)tiles * h->nb < 4096 ? 4 : ROOTS_WPT; }
 
 // launch with programmatic stream serialization (see pdl_wait in sw_common.cuh): the kernels of the fast path's sweep
 template <typename... KArgs, typename... Args>

@@ -567,15 +567,17 @@ k_merge_nodes(int4* nodes, const uint16_t* __restrict__ bslot, int tilesX, int t
     int ka, tb, kb;
     if (j < TW) { ka = TW + j;                tb = (r + 1 == tilesY ? 0 : r + 1) * tilesX + c; kb = j; }            // South row -> North row below
     else        { ka = 2 * TW + TH + (j - TW); tb = r * tilesX + (c + 1 == tilesX ? 0 : c + 1); kb = 2 * TW + (j - TW); }  // East column -> West column
-    const int sa = bs[(size_t)ta * CAP + ka];
+    const int sa = bs[(size_t)ta * CAP + ka], sb = bs[(size_t)tb * CAP + kb];   // (both loads in flight before the test)
     if (sa == 0xFFFF) return;                               // no bond across the edge here
-    nd_union(nodes + lb, ta * CAP + sa, tb * CAP + (int)bs[(size_t)tb * CAP + kb]);
+    nd_union(nodes + lb, ta * CAP + sa, tb * CAP + sb);
 }
 
 // After the merge: every open piece adds its size and its site index to the node it hangs under (sum -> cluster
-// size, min -> canonical label) and points straight at it.  Pieces are combined per root inside the warp first,
-// and the root with the largest sum of the first round is carried in registers across rounds: at T_c one cluster
-// owns many pieces in every tile.  wpt warps per tile (1 for large lattices; 4 for small ones, where the kernel is
+// size, min -> canonical label) and points straight at it.  The root of the largest piece of a warp's first round is
+// carried in registers across rounds (at T_c one cluster owns many pieces in every tile); the other pieces go to
+// their roots with one pair of reductions each (no return value to wait for; combining them per root inside the
+// warp first -- __match_any_sync and reductions over the groups' masks, which run group after group -- took half of
+// this kernel's time).  wpt warps per tile (1 for large lattices; 4 for small ones, where the kernel is
 // the latency of one warp walking its tile's ~100 pieces 32 at a time): warp `sub` takes rounds sub, sub + wpt, ...
 template <int CAP>
 __global__ void __launch_bounds__(256)
@@ -603,17 +605,14 @@ k_roots_nodes(int4* nodes, const int* __restrict__ ocount, int tiles, int wpt) {
             }
             g = me.w;
         }
-        const unsigned grp = __match_any_sync(0xffffffffu, root);
-        const int tot = __reduce_add_sync(grp, add);
-        const int gm = __reduce_min_sync(grp, g);
-        if (e0 == 32 * sub) {                               // (my first round) choose the hot root
-            const int best = __reduce_max_sync(0xffffffffu, tot);
-            const unsigned who = __ballot_sync(0xffffffffu, tot == best && on);
+        if (e0 == 32 * sub) {                               // (my first round) the hot root: the one of the round's largest piece
+            const int best = __reduce_max_sync(0xffffffffu, add);
+            const unsigned who = __ballot_sync(0xffffffffu, add == best && on);
             if (who) hot = __shfl_sync(0xffffffffu, root, __ffs(who) - 1);
         }
-        if (on && lane == __ffs(grp) - 1) {                 // one lane per root and round
-            if (root == hot) { hotacc += tot; hotmin = min(hotmin, gm); }
-            else if (tot) { atomicAdd(&nd[root].y, tot); atomicMin(&nd[root].z, gm); }
+        if (on) {
+            if (root == hot) { hotacc += add; hotmin = min(hotmin, g); }
+            else if (add) { atomicAdd(&nd[root].y, add); atomicMin(&nd[root].z, g); }     // (fire and forget: L2 combines)
         }
     }
     hotacc = warp_sum_i(hotacc);
