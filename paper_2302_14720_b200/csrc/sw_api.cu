@@ -260,7 +260,9 @@ int mark(sw_handle* h, int kid) {
 #endif
 inline int roots_warps_per_tile(const sw_handle* h, int tiles) { return (long long)tiles * h->nb < 4096 ? 4 : ROOTS_WPT; }
 
-// launch with programmatic stream serialization (see pdl_wait in sw_common.cuh): the kernels of the fast path's sweep
+// launch with programmatic stream serialization (see pdl_wait in sw_common.cuh): the kernels of the fast path's sweep.
+// Not with per-kernel timing: an event between two overlapping launches does not separate them (sw_sweep sets t_pdl).
+thread_local bool t_pdl = true;
 template <typename... KArgs, typename... Args>
 cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args&&... args) {
     cudaLaunchConfig_t cfg = {};
@@ -268,7 +270,7 @@ cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t s
     cudaLaunchAttribute at[1];
     at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     at[0].val.programmaticStreamSerializationAllowed = 1;
-    cfg.attrs = at; cfg.numAttrs = 1;
+    cfg.attrs = at; cfg.numAttrs = t_pdl ? 1 : 0;
     return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
 }
 
@@ -818,6 +820,7 @@ int sw_sweep(sw_handle* h, int64_t n) {
     DevGuard dg(h->dev);
     if (n == 0) return SW_OK;
     h->launches = 0;
+    t_pdl = !h->timing;
     {   // the configuration must sit in the plane this path sweeps on
         const int rc = sweeps_on_bits(h) ? ensure_bits(h) : ensure_i8(h);
         if (rc) return rc;
