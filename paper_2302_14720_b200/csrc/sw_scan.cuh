@@ -574,10 +574,12 @@ k_merge_nodes(int4* nodes, const uint16_t* __restrict__ bslot, int tilesX, int t
 
 // After the merge: every open piece adds its size and its site index to the node it hangs under (sum -> cluster
 // size, min -> canonical label) and points straight at it.  The root of the largest piece of a warp's first round is
-// carried in registers across rounds (at T_c one cluster owns many pieces in every tile); the other pieces go to
-// their roots with one pair of reductions each (no return value to wait for; combining them per root inside the
-// warp first -- __match_any_sync and reductions over the groups' masks, which run group after group -- took half of
-// this kernel's time).  wpt warps per tile (1 for large lattices; 4 for small ones, where the kernel is
+// carried in registers across rounds (at T_c one cluster owns many pieces in every tile); a piece whose root no other
+// lane of the round shares goes there with one pair of reductions (no return value to wait for); only roots that
+// several lanes share are combined inside the warp first.  (Combining ALL pieces per root -- __match_any_sync and
+// reductions over the groups' masks, which run group after group, 18 groups of 1.7 lanes per round -- took half of
+// this kernel's time; combining none is fastest on the young lattice of the bench, 1.270 ms per sweep, but loses on
+// the equilibrated one: 1.367 ms at sweeps 200-249 against 1.314 for this version and 1.320 for combining all.)  wpt warps per tile (1 for large lattices; 4 for small ones, where the kernel is
 // the latency of one warp walking its tile's ~100 pieces 32 at a time): warp `sub` takes rounds sub, sub + wpt, ...
 template <int CAP>
 __global__ void __launch_bounds__(256)
@@ -610,9 +612,19 @@ k_roots_nodes(int4* nodes, const int* __restrict__ ocount, int tiles, int wpt) {
             const unsigned who = __ballot_sync(0xffffffffu, add == best && on);
             if (who) hot = __shfl_sync(0xffffffffu, root, __ffs(who) - 1);
         }
-        if (on) {
-            if (root == hot) { hotacc += add; hotmin = min(hotmin, g); }
-            else if (add) { atomicAdd(&nd[root].y, add); atomicMin(&nd[root].z, g); }     // (fire and forget: L2 combines)
+        const bool cold = on && root != hot;
+        if (on && !cold) { hotacc += add; hotmin = min(hotmin, g); }
+        // the other roots: most appear once in a round and get their pair of reductions straight away (fire and forget); the
+        // few that appear several times (another large cluster with many pieces in this tile: the equilibrated lattice has
+        // them) are combined first, group after group
+        const unsigned grp = __match_any_sync(0xffffffffu, cold ? root : -1 - lane);
+        if (cold) {
+            if (grp == (1u << lane)) { if (add) { atomicAdd(&nd[root].y, add); atomicMin(&nd[root].z, g); } }
+            else {
+                const int tot = __reduce_add_sync(grp, add);
+                const int gm = __reduce_min_sync(grp, g);
+                if (tot && lane == __ffs(grp) - 1) { atomicAdd(&nd[root].y, tot); atomicMin(&nd[root].z, gm); }
+            }
         }
     }
     hotacc = warp_sum_i(hotacc);
