@@ -198,6 +198,19 @@ typedef struct { double tau_int; int64_t window, tmax; double c0; } sw_taustat;
 int        sw_bins(sw_handle* h, int32_t which, int64_t bin_len, double* bin_means, int64_t cap, sw_binstat* out);
 int        sw_autocorr(sw_handle* h, int32_t which, int64_t tmax, double c, double* rho, sw_taustat* out);
 
+/* sw_bins for callers that cannot allocate (code under CUDA graph capture, serving loops, harnesses that forbid
+ * cudaMalloc): the same binning, the same kernels, no cudaMalloc / cudaFree / host copy / synchronisation.  The bin means
+ * -- scratch between the two kernels -- live in a static device array of SW_BINS_NOALLOC_MAX doubles (512 KiB that every
+ * GPU which loads the library holds until the process exits), so nb * floor(n / bin_len) may not exceed
+ * SW_BINS_NOALLOC_MAX: beyond it the call returns SW_EINVAL and says so in sw_last_error (take a longer bin_len, or sw_bins).
+ * out_dev: DEVICE, nb records (n_bins, mean, err), written asynchronously on the handle's stream -- the caller orders its
+ * reads after it on that stream.  All calls on a GPU share the scratch array: calls that overlap on the GPU (handles on
+ * different streams) race on it; calls on one stream do not.  It keeps the last call's contents; nothing in it has to be
+ * cleared (every entry read is written first).  The first call on a device resolves the array's address
+ * (cudaGetSymbolAddress, no allocation): make one call before starting a graph capture.  Errors as sw_bins. */
+#define SW_BINS_NOALLOC_MAX 65536
+int        sw_bins_noalloc(sw_handle* h, int32_t which, int64_t bin_len, sw_binstat* out_dev);
+
 /* Per-stage device time in ms, summed over the sweeps of the last sw_sweep call that ran with stage
  * timing on: out = {bond, label, flip, observe}.  Stage timing brackets each stage with CUDA events
  * (it serialises nothing but adds event records; off by default).  BASELINE config 3. */

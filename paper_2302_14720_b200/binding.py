@@ -84,6 +84,7 @@ PROTOTYPES = {
     "sw_moments_reset": (C.c_int, [_VP]),
     "sw_bins": (C.c_int, [_VP, _I32, C.c_int64, C.POINTER(C.c_double), C.c_int64, C.POINTER(sw_binstat)]),
     "sw_autocorr": (C.c_int, [_VP, _I32, C.c_int64, C.c_double, C.POINTER(C.c_double), C.POINTER(sw_taustat)]),
+    "sw_bins_noalloc": (C.c_int, [_VP, _I32, C.c_int64, _VP]),
     "sw_set_stage_timing": (C.c_int, [_VP, C.c_int]),
     "sw_stage_ms": (C.c_int, [_VP, C.POINTER(C.c_float)]),
     "sw_kernel_ms": (C.c_int, [_VP, C.POINTER(C.c_float), _I32]),
@@ -247,6 +248,13 @@ def sw_bins(h, which: int, bin_len: int, want_means: bool = True):
     if want_means and nbins > 0:
         _check(lib().sw_bins(h, which, bin_len, means.ctypes.data_as(C.POINTER(C.c_double)), means.shape[1], out))
     return [{"n_bins": int(o.n_bins), "mean": o.mean, "err": o.err, "bin_means": means[b, :nbins].copy()} for b, o in enumerate(out)]
+
+SW_BINS_NOALLOC_MAX = 65536              # include/sw.h
+
+def sw_bins_noalloc(h, which: int, bin_len: int, out_dev_ptr: int) -> None:
+    """sw_bins without any allocation: nb records (int64 n_bins, double mean, double err) into DEVICE memory at
+    out_dev_ptr, asynchronously on the handle's stream (argument marshalling only)."""
+    _check(lib().sw_bins_noalloc(h, which, bin_len, C.c_void_p(out_dev_ptr)))
 
 def sw_autocorr(h, which: int, tmax: int, c: float = 6.0):
     """Normalised autocorrelation rho(0 .. tmax) of the last call's series and the windowed tau_int, per lattice."""
@@ -444,6 +452,11 @@ class SwendsenWang:
 
     def bins(self, which: int, bin_len: int):
         return sw_bins(self.h, which, bin_len)
+
+    def bins_noalloc(self, which: int, bin_len: int, out):
+        """`out`: a device tensor of nb * 3 float64 (= nb records of 24 bytes: n_bins as int64 bits, mean, err)."""
+        assert out.is_cuda and out.is_contiguous() and out.element_size() * out.numel() >= 24 * self.nb
+        sw_bins_noalloc(self.h, which, bin_len, out.data_ptr())
 
     def autocorr(self, which: int, tmax: int, c: float = 6.0):
         return sw_autocorr(self.h, which, tmax, c)

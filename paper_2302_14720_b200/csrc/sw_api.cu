@@ -732,6 +732,28 @@ void fill_obs(const sw_handle* h, const Rec& r, uint64_t sweep, sw_obs* o) {
 } // namespace
 
 // =================================================================================================
+// ---- sw_bins_noalloc: binning with no allocation (include/sw.h) ------------------------------------------
+// The bin means -- scratch between k_series_bins and k_series_binerr, which sw_bins takes from cudaMalloc -- live in a
+// file-scope device array: every GPU that loads the library holds these 512 KiB until the process exits.  In host code the
+// array's NAME is a host-side stand-in, not a device address (a kernel given it would fault or, where the GPU can reach
+// host memory, silently use the wrong memory): the address comes from cudaGetSymbolAddress, once per device, with that
+// device current.  Every call shares the array; calls that overlap on a GPU race on it.
+static __device__ __align__(256) double g_bins_scratch[SW_BINS_NOALLOC_MAX];
+namespace {
+double* g_bins_scratch_ptr[MAX_DEV];   // per device; written once (a race between two first calls stores the same value)
+int bins_scratch(int dev, double** out) {
+    if (dev < 0 || dev >= MAX_DEV) { set_err("sw_bins_noalloc: device %d is outside the per-device table (0 .. %d)", dev, MAX_DEV - 1); return SW_EINVAL; }
+    if (!g_bins_scratch_ptr[dev]) {
+        double* p = nullptr;
+        SW_CUDA(cudaGetSymbolAddress((void**)&p, g_bins_scratch));     // (the current device is `dev`: DevGuard of the caller)
+        if (!p) { set_err("sw_bins_noalloc: cudaGetSymbolAddress returned a null address"); return SW_ECUDA; }
+        g_bins_scratch_ptr[dev] = p;
+    }
+    *out = g_bins_scratch_ptr[dev];
+    return SW_OK;
+}
+} // namespace
+
 extern "C" {
 
 const char* sw_last_error(void) { return g_err.c_str(); }
@@ -1340,6 +1362,28 @@ int sw_test_label(sw_handle* h, const uint32_t* bondE, const uint32_t* bondS, in
     SW_CUDA(cudaMemcpyAsync(labels_out, h->label, (size_t)h->N * 4, cudaMemcpyDeviceToHost, h->stream));
     SW_CUDA(cudaStreamSynchronize(h->stream));
     h->have_sweep = false; h->rec_valid = false;
+    return SW_OK;
+}
+
+int sw_bins_noalloc(sw_handle* h, int32_t which, int64_t bin_len, sw_binstat* out_dev) {
+    if (!h || !out_dev || (which != 0 && which != 1) || bin_len < 1) { set_err("sw_bins_noalloc: invalid argument"); return SW_EINVAL; }
+    static_assert(sizeof(BinStat) == sizeof(sw_binstat), "the kernel's record is the header's");
+    DevGuard dg(h->dev);
+    SeriesView v;
+    if (!series_view(h, which, &v)) { set_err("sw_bins_noalloc: no series (no sw_sweep since the last state change)"); return SW_ESTATE; }
+    const long long nbins = v.n / bin_len;
+    if ((long long)h->nb * nbins > (long long)SW_BINS_NOALLOC_MAX) {
+        set_err("sw_bins_noalloc: %d lattices x %lld bins = %lld bin means exceed the static scratch of SW_BINS_NOALLOC_MAX = %d; "
+                "use a longer bin_len, or sw_bins", h->nb, nbins, (long long)h->nb * nbins, (int)SW_BINS_NOALLOC_MAX);
+        return SW_EINVAL;
+    }
+    double* scratch = nullptr;
+    { const int rc = bins_scratch(h->dev, &scratch); if (rc) return rc; }
+    // (nothing in the scratch has to start at zero: k_series_bins writes every entry k_series_binerr reads)
+    if (nbins > 0)
+        k_series_bins<<<grid1((size_t)nbins, 256, h->nb), 256, 0, h->stream>>>(v, scratch, bin_len, nbins, h->N);
+    k_series_binerr<<<(h->nb + 63) / 64, 64, 0, h->stream>>>(scratch, reinterpret_cast<BinStat*>(out_dev), nbins, h->nb);
+    SW_CUDA(cudaGetLastError());
     return SW_OK;
 }
 
