@@ -231,7 +231,8 @@ def profile_numbers():
         return {}
     return {"source": j.get("_source"), "sites": j.get("_sites", 268435456),
             "dram_bytes_per_launch": {k: v for k, v in j.items() if not k.startswith("_")},
-            "issue_active_pct": j.get("_issue_active_pct"), "thread_instr_slots_per_site": j.get("_thread_instr_slots_per_site")}
+            "issue_active_pct": j.get("_issue_active_pct"), "thread_instr_slots_per_site": j.get("_thread_instr_slots_per_site"),
+            "ncu_ms": j.get("_ncu_ms"), "ncu_ms_source": j.get("_ncu_ms_source")}
 
 
 def _timed_sweeps(sw, n):
@@ -430,7 +431,7 @@ def block_phi4(dev):
                        "state_after": {"link_per_link": o.link_per_link, "abs_m_per_site": o.abs_m_per_site,
                                        "n_clusters": int(o.n_clusters), "largest_cluster": int(o.largest_cluster)}}
     out["note"] = ("paper_*: PAPER.md:152-156 (another machine: context, not a target); the update is the cluster step only (Eq. 2-3), "
-                   "double precision, 6 launches per update replayed from a CUDA graph")
+                   "double precision, 4 launches per update replayed from a CUDA graph")
     return out
 
 
@@ -608,7 +609,8 @@ def main():
                 "traffic_source": prof.get("source"), "peak_source": peak_src,
                 "note": "achieved = ALGORITHMIC bytes (SURVEY.md 8(d) model, bytes_per_site x sites) / live CUDA-event time; traffic = "
                         "DRAM bytes of one launch from the committed ncu capture (real_* below are computed from it): the kernel moves "
-                        "less than the model charges (bit-packed spins, 16-bit roots) and is bound by instruction issue, not by HBM",
+                        "less than the model charges (bit-packed spins, 16-bit roots) and is bound by the shared-memory data pipe "
+                        "and instruction issue (profiles/r2_ncu_full.md), not by HBM",
                 "bytes_per_site": kb.get(dom), "ms_per_launch": dom_ms,
                 "share_of_step": kms[dom] / max(1e-9, sum(kms.values())),
                 "issue_active_pct": (prof.get("issue_active_pct") or {}).get(dom),
@@ -663,7 +665,13 @@ def main():
         e.update(real(k, v / timed))
         if k == "energy":                           # (see stages.observe: once per call, amortised)
             e.update({"model_GBps": None, "model_frac_of_peak": None, "amortised_over_sweeps": timed})
+        if (prof.get("ncu_ms") or {}).get(k) is not None:   # the same kernel in the committed ncu launch list (serialised, cold caches)
+            e["ncu_ms"] = prof["ncu_ms"][k]
         kernels[k] = e
+    kernels_note = ("ms: CUDA events around every launch of the K sweeps after the timed call (no graph, no programmatic dependent "
+                    "launch, flip bits on the main stream): they add up to ms_per_step_with_kernel_events, not to ms_per_step; "
+                    "k_roots_nodes in particular reads longer between events than in the ncu launch list (ncu_ms: "
+                    + str(prof.get("ncu_ms_source")) + "), and the graph-replayed sweep agrees with ncu")
     sweep_gbs = SWEEP_MODEL_BYTES_PER_SITE * N / (ms / K * 1e-3) / 1e9
     real_sweep = sum(v for v in (prof.get("dram_bytes_per_launch") or {}).values() if isinstance(v, (int, float)))
     sweep_model = {"bytes_per_site": SWEEP_MODEL_BYTES_PER_SITE, "achieved_GBps": sweep_gbs,
@@ -718,7 +726,7 @@ def main():
         "gpu_launches": int(launches),
         "roofline": roofline, "roofline_alu": roofline_alu,
         "sweep_model": sweep_model,
-        "per_sweep": per_sweep, "stages": stages, "kernels": kernels,
+        "per_sweep": per_sweep, "stages": stages, "kernels": kernels, "kernels_note": kernels_note,
         "cpu_baseline": cpu,
         "paper_context": "paper: 17x (SW) / 90x (Wolff) over serial, Haswell E5-2695 vs Tesla P100; "
                          "SW GPU rate 1.25e8 site-updates/s at L=4096 (PAPER.md:127,142)",
