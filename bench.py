@@ -403,6 +403,13 @@ def block_paper_sizes(B, dev):
         sw.close()
         out[str(L)] = {"us_per_sweep": 1e3 * ms, "site_updates_per_s": L * L / (ms * 1e-3),
                        "paper_gpu_us_per_sweep": paper_gpu_min[L] * 60e6 / 1e4, "paper_cpu_us_per_sweep": paper_cpu_min[L] * 60e6 / 1e4}
+        if L == 128:                                 # the whole call inside one cluster kernel (default) against the kernels one by one
+            sw = B.SwendsenWang(L, 2.5, 10 + L, device=str(dev))
+            B.sw_set_cluster(sw.h, False)
+            sw.sweep(100)
+            out[str(L)]["us_per_sweep_kernels_one_by_one"] = 1e3 * _timed_sweeps(sw, 400)
+            out[str(L)]["path"] = "k_sweeps_cluster: 8 tiles of 64 x 32, one thread-block cluster, all sweeps of the call inside one kernel"
+            sw.close()
     out["note"] = "paper_*: PAPER.md:137-142 (another machine: context, not a target); ours: 400 sweeps after 100, one sw_sweep call"
     return out
 

@@ -248,6 +248,13 @@ int        sw_set_path(sw_handle* h, int path);
  * lattices of fewer than 8 tiles).  Same results. */
 int        sw_set_tma(sw_handle* h, int on);
 
+/* Default 1: a lattice of at most 8 tiles of 64 x 32 sites (L = 64, 128) runs a whole
+ * sw_sweep(h, n) call inside ONE kernel, one thread-block cluster per lattice of the batch, the steps of a sweep separated
+ * by the cluster's hardware barrier instead of by kernel boundaries (k_sweeps_cluster; the paper's own sizes,
+ * PAPER.md:133-142).  0: the kernels of the fast path one by one, as for larger lattices (also taken with per-kernel
+ * timing, eager labels, path 6, and when the cluster launch fails).  Same results. */
+int        sw_set_cluster(sw_handle* h, int on);
+
 /* Path 11 only: number of passes (scans, including the last one that formed no reference) the label-equivalence
  * iteration of the last sweep / sw_test_label took -- a deterministic function of the bond graph (PAPER.md:53
  * reports "5 or 6" for 512 x 512).  Synchronises.  SW_ESTATE on another path, before any labelling, or if the

@@ -91,6 +91,7 @@ PROTOTYPES = {
     "sw_kernel_name": (C.c_char_p, [_I32]),
     "sw_set_path": (C.c_int, [_VP, C.c_int]),
     "sw_set_tma": (C.c_int, [_VP, C.c_int]),
+    "sw_set_cluster": (C.c_int, [_VP, C.c_int]),
     "sw_label_passes": (C.c_int, [_VP, C.POINTER(C.c_int32)]),
     "sw_sweep_ms": (C.c_int64, [_VP, C.POINTER(C.c_float), C.c_int64]),
     "sw_create_potts": (_VP, [C.c_int32, C.c_int32, C.c_double, C.c_uint64]),
@@ -320,6 +321,9 @@ def sw_sweep_ms(h) -> np.ndarray:
 
 def sw_set_tma(h, on: bool) -> None:
     _check(lib().sw_set_tma(_ptr(h), 1 if on else 0))
+
+def sw_set_cluster(h, on: bool) -> None:
+    _check(lib().sw_set_cluster(_ptr(h), 1 if on else 0))
 
 def sw_set_path(h, path: int) -> None:
     _check(lib().sw_set_path(_ptr(h), path))

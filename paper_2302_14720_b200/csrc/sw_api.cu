@@ -6,6 +6,7 @@
 #include "sw_tiled.cuh"
 #include "sw_scan.cuh"
 #include "sw_flip_tma.cuh"
+#include "sw_cluster.cuh"
 #include "sw_equiv.cuh"
 #include "sw_potts.cuh"
 #include "sw_series.cuh"
@@ -179,6 +180,8 @@ struct sw_handle {
     // TMA staging of the 16-bit root plane in the assignment kernel (sw_flip_tma.cuh): tensor map of lab16, made on first use
     CUtensorMap tmap, tmap_d; int tmap_state = 0;   // 0: not tried, 1: ready, -1: unavailable (k_flip16 is used)
     bool use_tma = true;
+    // lattices of at most 8 tiles: the whole sw_sweep call inside one kernel, one thread-block cluster per lattice (sw_cluster.cuh)
+    bool use_cluster = true, cluster_failed = false;
     // side branch of the sweep: the decision plane depends on nothing but the sweep index, so k_flipbits runs beside the labelling
     cudaStream_t side = nullptr; cudaEvent_t ev_fork = nullptr, ev_join = nullptr; bool side_failed = false;
 };
@@ -557,6 +560,32 @@ int launch_sweep_potts(sw_handle* h, int64_t k) {
     return SW_OK;
 }
 
+// Small lattices (sw_cluster.cuh): tiles per lattice when the whole call can run inside k_sweeps_cluster, else 0.  Not with
+// per-kernel timing or eager labels (they need the kernels apart), nor on the unfused path.
+constexpr int CLUSTER_MAX_TILES = 8;                // (the portable cluster size)
+int cluster_tiles(const sw_handle* h) {
+    if (!h->use_cluster || h->cluster_failed || !sweeps_on_bits(h) || h->timing || h->eager_labels) return 0;
+    if (scan_nw(h->tile) != 2) return 0;            // (64 x 32 tiles: L = 64 -> 2 tiles, L = 128 -> 8)
+    const int tiles = h->N / (64 * 32);
+    return tiles <= CLUSTER_MAX_TILES ? tiles : 0;
+}
+template <int NW, int TH, int BAND_T>
+cudaError_t launch_sweeps_cluster(sw_handle* h, int64_t n, int tiles) {
+    constexpr int THREADS = NW * TH * (32 / BAND_T);
+    constexpr size_t smem = (size_t)32 * NW * TH * sizeof(uint32_t);
+    static bool done[MAX_DEV];
+    if (opt_in_smem(k_sweeps_cluster<NW, TH, BAND_T>, smem, done, h->dev)) return cudaErrorUnknown;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(tiles, h->nb); cfg.blockDim = dim3(THREADS); cfg.dynamicSmemBytes = smem; cfg.stream = h->stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = tiles; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, k_sweeps_cluster<NW, TH, BAND_T>, h->sbits, h->bondE, h->bondS, h->lab16, h->nodes, h->ocount, h->bslot,
+                              h->series, (const Lat*)h->lat, h->mom, (unsigned long long)h->t, (uint32_t)h->ring(), (long long)n, 0,
+                              make_div(h->L), h->L, h->N, h->words, h->nb);
+}
+
 // one full sweep on h->stream; the sweep index and series slot are read on the device from h->ctl
 int launch_sweep(sw_handle* h, int64_t k) {
     if (h->q) return launch_sweep_potts(h, k);
@@ -857,7 +886,8 @@ int sw_sweep(sw_handle* h, int64_t n) {
             h->stream = user;
         }
     } stream_back{h, user};
-    bool graphs = h->use_graphs && !h->graph_failed && !h->timing && scan_nw(h->tile) && n >= 4 && !h->q;
+    int ctiles = cluster_tiles(h);
+    bool graphs = h->use_graphs && !h->graph_failed && !h->timing && scan_nw(h->tile) && n >= 4 && !h->q && !ctiles;
     if (graphs) {
         if (!h->gstream) {
             if (cudaStreamCreateWithFlags(&h->gstream, cudaStreamNonBlocking) != cudaSuccess ||
@@ -883,13 +913,25 @@ int sw_sweep(sw_handle* h, int64_t n) {
         h->ev_seq.clear();
     }
     SW_CUDA(cudaMemsetAsync(h->series, 0, (size_t)h->nb * sizeof(Rec), h->stream));
-    k_set_ctl<<<1, 1, 0, h->stream>>>(h->ctl, (unsigned long long)h->t, 0u, (uint32_t)h->ring());
-    h->launches += 1;
-    {
+    int64_t k = 0;
+    if (ctiles) {                                       // the whole call inside one kernel, a cluster per lattice
+        const cudaError_t e = launch_sweeps_cluster<2, 32, 8>(h, n, ctiles);
+        if (e != cudaSuccess) { (void)cudaGetLastError(); h->cluster_failed = true; ctiles = 0; }   // (nothing ran: take the kernels one by one)
+        else {
+            // Ctl as the sweeps below would have left it: the next sweep index, the slot after the last sweep (cleared)
+            k_set_ctl<<<1, 1, 0, h->stream>>>(h->ctl, (unsigned long long)h->t + (unsigned long long)n, (uint32_t)(n % h->ring()), (uint32_t)h->ring());
+            h->launches += 2;
+            h->labels_flat = false; h->lab_tile = h->tile;
+            k = n;
+        }
+    }
+    if (!ctiles) {
+        k_set_ctl<<<1, 1, 0, h->stream>>>(h->ctl, (unsigned long long)h->t, 0u, (uint32_t)h->ring());
+        h->launches += 1;
         int rc = launch_sweep(h, 0);                    // (also sets the kernels' attributes before any capture)
         if (rc) return rc;
+        k = 1;
     }
-    int64_t k = 1;
     if (graphs && !build_graphs(h)) { h->graph_failed = true; graphs = false; }
     if (graphs) {
         for (; k + GRAPH_UNROLL <= n; k += GRAPH_UNROLL) {
@@ -1280,6 +1322,12 @@ int sw_set_tma(sw_handle* h, int on) {
     if (!h) { set_err("sw_set_tma: null handle"); return SW_EINVAL; }
     h->use_tma = on != 0;
     h->gkey_path = -1;                              // (the captured sweep holds the other kernel: capture again)
+    return SW_OK;
+}
+
+int sw_set_cluster(sw_handle* h, int on) {
+    if (!h) { set_err("sw_set_cluster: null handle"); return SW_EINVAL; }
+    h->use_cluster = on != 0;
     return SW_OK;
 }
 

@@ -148,384 +148,15 @@ k_bond_label(const uint32_t* __restrict__ sbits, uint32_t* bondE, uint32_t* bond
              Rec* __restrict__ rec, const Lat* __restrict__ lat, const Ctl* __restrict__ ctl,
              int L, int N, int words, int nb, int obs_prev) {
     pdl_wait();
-    constexpr int BAND = BAND_T;                // (shadows the default: rows per warp block in this instantiation)
-    constexpr int TPW = 32 / BAND;              // threads per 32-site word (one warp per 32 x BAND block)
-    constexpr int TW = 32 * NW, SITES = TW * TH, WORDS = NW * TH, THREADS = WORDS * TPW;
-    constexpr int CAP = 2 * (TW + TH);
-    static_assert(TPW == 1 || TPW == 2 || TPW == 4, "threads per word");
-    constexpr int HKCAP = 1024;                 // hooked nodes the tile can list (~250 at T_c)
-    static_assert(TH % BAND == 0 && TH <= 64 && SITES <= 8192 && CAP < 0x3FFF, "tile shape");
-    extern __shared__ __align__(16) uint32_t par[];  // [SITES] (see above); dynamic: 32 KB at 128 x 64
-    __shared__ uint2 es[TH * NW];              // [row][strip] = (East word, South word)
-    __shared__ uint16_t hkitems[HKCAP];        // nodes hooked in phases 2 and 3
-    __shared__ uint32_t nIn[NW];               // South bonds entering from the tile above, per strip
-    __shared__ uint32_t wIn[2];                // East bonds entering from the tile to the West, bit = row
-    __shared__ int s_nopen, s_max, s_nlab, s_nhook, s_obs[2];
-
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const uint32_t lanebit = 1u << lane, lt = lanebit - 1u;
-    const int tilesX = L / TW;
-    const int ty = blockIdx.x / tilesX, tx = blockIdx.x - ty * tilesX;
-    const int y0 = ty * TH, x0 = tx * TW;
-    const int wprL = L >> 5;
-    // FUSE: the spins come bit-packed (bit 1 = +1; word w = sites 32w .. 32w+31), 1/8 of the int8 plane's bytes
-    const uint32_t* sb = sbits + (size_t)blockIdx.y * words;
-    const int8_t* col = reinterpret_cast<const int8_t*>(sbits) + (size_t)blockIdx.y * N;   // (POTTS)
-    const Lat la = lat[blockIdx.y];
-    const unsigned long long t = ctl->t;
-    const uint32_t tlo = (uint32_t)t, thi = (uint32_t)(t >> 32);
-
-    if (tid < NW) nIn[tid] = 0;
-    if (tid == 0) { wIn[0] = 0; wIn[1] = 0; s_nopen = 0; s_max = 0; s_nlab = 0; s_nhook = 0; s_obs[0] = 0; s_obs[1] = 0; }
-    uint32_t par_s = (uint32_t)__cvta_generic_to_shared(par);        // shared-window address of word 0
-    asm volatile("mov.u32 %0, %0;" : "+r"(par_s));                   // (opaque: kept in a register, not recomputed at every use)
-    const HookList hk = { (uint32_t)__cvta_generic_to_shared(hkitems), (uint32_t)__cvta_generic_to_shared(&s_nhook), HKCAP, (uint32_t)(L > -tid) };   // (1, but neither constant nor warp-uniform for ptxas)
-#pragma unroll
-    for (int k = 0; k < SITES / 4 / THREADS; ++k)                    // counts start at 0 (the scan stores parents only)
-        sts_u128(par_s + 16u * (k * THREADS + tid), make_uint4(0u, 0u, 0u, 0u));
-    __syncthreads();
-
-    // ---- phase 1: bonds of the tile, PAPER.md:37-39 (section 2.1) --------------------------------------
-    if (!FUSE) {
-        const uint32_t* bE = bondE + (size_t)blockIdx.y * words;
-        const uint32_t* bS = bondS + (size_t)blockIdx.y * words;
-        if (tid < WORDS) {
-            const int row = tid / NW, wx = tid - row * NW;
-            const size_t gw = (size_t)(y0 + row) * wprL + (x0 >> 5) + wx;
-            es[tid] = make_uint2(bE[gw], bS[gw]);
-        }
-        if (tid < NW) nIn[tid] = bS[(size_t)(y0 == 0 ? L - 1 : y0 - 1) * wprL + (x0 >> 5) + tid];
-        if (tid < TH) {
-            const int wl = (x0 >> 5) == 0 ? wprL - 1 : (x0 >> 5) - 1;
-            if (bE[(size_t)(y0 + tid) * wprL + wl] >> 31) atomicOr(&wIn[tid >> 5], 1u << (tid & 31));
-        }
-    } else {
-        const PhiloxKey key(la.key0, la.key1);
-        {
-            const int wid = tid / TPW, part = tid - wid * TPW;      // this thread's 32-site word (and which part of its draws)
-            const int row = wid / NW, wx = wid - row * NW;
-            const int y = y0 + row;
-            const int xw = (x0 >> 5) + wx;
-            const int w = y * wprL + xw;                              // word index within the lattice
-            uint32_t own = 0, eqE = 0, eqS = 0;
-            if (POTTS) {
-                const int8_t* r0 = col + (size_t)y * L + xw * 32;
-                const int8_t* r1 = col + (size_t)(y + 1 == L ? 0 : y + 1) * L + xw * 32;
-                const uint4 a0 = *reinterpret_cast<const uint4*>(r0), a1 = *reinterpret_cast<const uint4*>(r0 + 16);
-                const uint4 b0 = *reinterpret_cast<const uint4*>(r1), b1 = *reinterpret_cast<const uint4*>(r1 + 16);
-                const uint32_t nx = (uint8_t)col[(size_t)y * L + (xw + 1 == wprL ? 0 : (xw + 1) * 32)];
-                const uint32_t a[9] = { a0.x, a0.y, a0.z, a0.w, a1.x, a1.y, a1.z, a1.w, nx };
-                const uint32_t b[8] = { b0.x, b0.y, b0.z, b0.w, b1.x, b1.y, b1.z, b1.w };
-#pragma unroll
-                for (int k = 0; k < 8; ++k) {
-                    eqE |= neg_nibble(__vcmpeq4(a[k], __funnelshift_r(a[k], a[k + 1], 8))) << (4 * k);
-                    eqS |= neg_nibble(__vcmpeq4(a[k], b[k])) << (4 * k);
-                }
-            } else {
-                own = ~sb[w];                                            // bit = 1: spin -1
-                const uint32_t south = ~sb[(y + 1 == L ? 0 : y + 1) * wprL + xw];
-                const uint32_t nxw = sb[y * wprL + (xw + 1 == wprL ? 0 : xw + 1)];
-                const uint32_t eastm = (own >> 1) | ((~nxw & 1u) << 31);
-                eqE = ~(own ^ eastm); eqS = ~(own ^ south);
-            }
-            if (POTTS && obs_prev) {
-                // Potts: E = -#(equal East / South pairs) of the configuration the previous sweep left (M comes from the colour
-                // counts of the assignment kernel)
-                const int eo = warp_sum_i(-(__popc(eqE) + __popc(eqS)));
-                if (lane == 0) atomicAdd(&s_obs[0], eo);
-            }
-            if (!POTTS && obs_prev) {
-                // a7 for free: the equal-pair masks of the bond test are the energy of the
-                // configuration the previous sweep left: E = (#edges) - 2 (#equal pairs), M = N - 2 (#down)
-                const int eo = warp_sum_i(part == 0 ? 64 - 2 * (__popc(eqE) + __popc(eqS)) : 0);
-                const int mo = warp_sum_i(part == 0 ? 32 - 2 * __popc(own) : 0);
-                if (lane == 0) { atomicAdd(&s_obs[0], eo); atomicAdd(&s_obs[1], mo); }
-            }
-            uint32_t dE = 0, dS = 0;
-#pragma unroll
-            for (int cc = 0; cc < 16 / TPW; ++cc) {
-                const int c = part * (16 / TPW) + cc;
-                const uint4 r = philox4x32_10((uint32_t)w * 16u + c, tlo, thi, TAG_BOND, key);
-                if (r.x < la.thr) dE |= 1u << (2 * c);               // (a compare and a predicated OR per word)
-                if (r.z < la.thr) dE |= 2u << (2 * c);
-                if (r.y < la.thr) dS |= 1u << (2 * c);
-                if (r.w < la.thr) dS |= 2u << (2 * c);
-            }
-#pragma unroll
-            for (int o = 1; o < TPW; o <<= 1) {                      // the word's TPW threads are neighbouring lanes
-                dE |= __shfl_xor_sync(0xffffffffu, dE, o);
-                dS |= __shfl_xor_sync(0xffffffffu, dS, o);
-            }
-            const uint32_t e = eqE & dE, so = eqS & dS;
-            if (part == 0) {
-                es[wid] = make_uint2(e, so);
-                bondE[(size_t)blockIdx.y * words + w] = e;
-                bondS[(size_t)blockIdx.y * words + w] = so;
-            }
-        }
-        // bonds entering the tile: South bonds of the row above (TW / 2 calls), East bonds of the column to
-        // the West (32 calls).  They are owned by the neighbouring tiles; recomputed here from the same draws.
-        for (int j = tid; j < TW / 2 + TH; j += THREADS) {
-            if (j < TW / 2) {
-                const int yn = y0 == 0 ? L - 1 : y0 - 1;
-                const int x = x0 + 2 * j;
-                const int i = yn * L + x;                                  // even site; call covers i, i + 1
-                const uint4 r = philox4x32_10((uint32_t)(i >> 1), tlo, thi, TAG_BOND, key);
-                const int id = y0 * L + x;                                 // (x is even: both sites in one word)
-                const uint32_t eq = POTTS ? ((col[i] == col[id] ? 1u : 0u) | (col[i + 1] == col[id + 1] ? 2u : 0u))
-                                          : ~((sb[i >> 5] >> (i & 31)) ^ (sb[id >> 5] >> (id & 31)));
-                const uint32_t bits = (eq & ((r.y < la.thr ? 1u : 0u) | (r.w < la.thr ? 2u : 0u))) & 3u;
-                if (bits) atomicOr(&nIn[(2 * j) >> 5], bits << ((2 * j) & 31));
-            } else {
-                const int row = j - TW / 2;
-                const int xwst = x0 == 0 ? L - 1 : x0 - 1;                 // odd column
-                const int i = (y0 + row) * L + xwst;
-                const uint4 r = philox4x32_10((uint32_t)(i >> 1), tlo, thi, TAG_BOND, key);
-                const int ie = (y0 + row) * L + x0;
-                const bool same = POTTS ? col[i] == col[ie] : !(((sb[i >> 5] >> (i & 31)) ^ (sb[ie >> 5] >> (ie & 31))) & 1u);
-                if (same && r.z < la.thr)
-                    atomicOr(&wIn[row >> 5], 1u << (row & 31));
-            }
-        }
-    }
-    __syncthreads();
-
-    // ---- phase 2: scan-line labelling of this warp's block (32 columns x 32 rows), PAPER.md:49-51 -------
-    // Lane = column, the block's rows in sequence, uniform control flow.  A run of East bonds takes the label of the
-    // first of its sites that has a South bond from the row above (one shuffle), or opens a new label = its head's
-    // own index (a root).  Where another site of the run is bonded to a different label above, the two labels are
-    // equivalent: the lane notes the row in a bit mask (no divergent work in the loop, no list) and unites the pairs of
-    // its column once the block is scanned.  Labels are never refreshed on the way down, so the only loop-carried
-    // dependency of a row is the shuffle.
-    {
-        const int strip = warp % NW, yb = (warp / NW) * BAND;
-        int rowbase = yb * TW + strip * 32;                          // first site of the row in this strip
-        uint32_t rowaddr = par_s + 4u * (rowbase + lane) + 2u;       // my site's parent field in this row
-        uint32_t prev = 0;                                           // label of the site above
-        uint32_t s_up = 0;                                           // (a band's first row adopts nothing: seams come later)
-        uint32_t mymeet = 0;                                         // rows of the block where two labels met at my column
-#pragma unroll SCAN_UNROLL
-        for (int y = yb; y < yb + BAND; ++y, rowbase += TW, rowaddr += 4u * TW) {
-            const uint2 w = es[y * NW + strip];
-            const uint32_t nz = ~w.x | 0x80000000u;                  // bit k: no bond between columns k, k + 1 of the strip
-            const uint32_t below = nz & lt, above = nz & ~lt;        // run boundaries left of me / at or right of me
-            const int h = bfind_u32(below) + 1;                      // head column of my run
-            // my run: bits h .. tail, tail = lowest set bit of `above` (bit 31 is always set)
-            const uint32_t runmask = (above ^ (above - 1u)) & ~((1u << h) - 1u);
-            const uint32_t upm = s_up & runmask;                     // sites of my run bonded to the row above
-            const uint32_t got = __shfl_sync(0xffffffffu, prev, __ffs(upm) - 1);   // (source lane is taken mod 32)
-            const uint32_t c = upm ? got : (uint32_t)(rowbase + h);  // a new label: the head's own index (its own root)
-            sts_u16(rowaddr, c);
-            const bool meet = (s_up & lanebit) && prev != c;         // two labels meet at my site: the one above, my run's
-            mymeet = (mymeet >> 1) | (meet ? 0x80000000u : 0u);
-            prev = c;
-            s_up = w.y;
-        }
-        __syncwarp();                                                // the block's parents are written
-        // The meetings (~2.5 per lane at T_c, up to ~7) are united by all lanes, 32 at a time: every lane writes the sites of
-        // its column into the warp's list at the positions a prefix sum gives it.  The list lives in the (still unused)
-        // count fields of the warp's own block: entry k in the low half of the block's word (k >> 5, k & 31) -- no memory of
-        // its own (6 CTAs per SM), no capacity to overflow (a block has fewer meetings than sites).
-        mymeet >>= 32 - BAND;                                        // bit r: row yb + r
-        const uint32_t pl_s = par_s + 4u * (uint32_t)(yb * TW + strip * 32);
-        const int cnt = __popc(mymeet);
-        int pos = cnt;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const int v = __shfl_up_sync(0xffffffffu, pos, o);
-            if (lane >= o) pos += v;
-        }
-        const int npend = __shfl_sync(0xffffffffu, pos, 31);
-        pos -= cnt;
-        const int colbase = yb * TW + strip * 32 + lane;
-        while (mymeet) {
-            const int i = colbase + (__ffs(mymeet) - 1) * TW;
-            mymeet &= mymeet - 1u;
-            sts_u16(pl_s + 4u * (uint32_t)((pos >> 5) * TW + (pos & 31)), (uint32_t)i);
-            ++pos;
-        }
-        // An entry is read and its field cleared (the counts start at 0 in phase 3) while no union of this warp is in
-        // flight: a hook wipes the low half of the word it replaces and adds it back, and only this warp's unions touch
-        // this block's words before the barrier below.
-        for (int j0 = 0; j0 < npend; j0 += 32) {
-            __syncwarp();
-            const int j = j0 + lane;
-            const uint32_t slot = pl_s + 4u * (uint32_t)((j >> 5) * TW + (j & 31));
-            uint32_t i = 0;
-            if (j < npend) { i = lds_u16(slot); sts_u16(slot, 0u); }
-            __syncwarp();
-            if (j < npend) {
-                const int a = (int)lds_u16(par_s + 4u * (i - TW) + 2u), c = (int)lds_u16(par_s + 4u * i + 2u);
-                hooked(hk, sc_union(par_s, a, c));                   // (labels are mostly still roots: sc_union takes any nodes)
-            }
-        }
-    }
-    __syncthreads();
-
-    // ---- phase 3: seams between the warps' blocks: East bonds across strip edges, South bonds across bands
-    for (int j = tid; j < (NW - 1) * TH + (TH / BAND - 1) * TW; j += THREADS) {
-        if (j < (NW - 1) * TH) {
-            const int row = j / (NW - 1), st = j - row * (NW - 1);
-            if (es[row * NW + st].x >> 31) {
-                const int i = row * TW + st * 32 + 31;
-                hooked(hk, sc_union(par_s, (int)lds_u16(par_s + 4u * i + 2u), (int)lds_u16(par_s + 4u * i + 6u)));   // the two sites' labels
-            }
-        } else {
-            const int k = j - (NW - 1) * TH;
-            const int row = (k / TW + 1) * BAND - 1, c = k % TW;
-            if ((es[row * NW + (c >> 5)].y >> (c & 31)) & 1u) {
-                const int i = row * TW + c;
-                hooked(hk, sc_union(par_s, (int)lds_u16(par_s + 4u * i + 2u), (int)lds_u16(par_s + 4u * (i + TW) + 2u)));
-            }
-        }
-    }
-    // ... and, in the same phase, every site is counted at its label (any node of its tree will do: the flatten
-    // moves the counts to the roots); four consecutive sites per thread, one add where they share the label
-#pragma unroll 2
-    for (int k = 0; k < SITES / 4 / THREADS; ++k) {
-        const uint4 v = lds_u128(par_s + 16u * (k * THREADS + tid));
-        const uint32_t n0 = v.x >> 16, n1 = v.y >> 16, n2 = v.z >> 16, n3 = v.w >> 16;
-        if (n0 == n1 && n2 == n3 && n0 == n2) red_add_s(par_s + 4u * n0, 4u);
-        else {
-            red_add_s(par_s + 4u * n0, 1u); red_add_s(par_s + 4u * n1, 1u);
-            red_add_s(par_s + 4u * n2, 1u); red_add_s(par_s + 4u * n3, 1u);
-        }
-    }
-    // (the label nodes are counted here, in front of the barrier: bit tricks on the bond words only)
-    uint32_t o;                                                      // heads of runs without an uplink in this thread's word
-    int mybase;
-    {
-        const int wd = tid < WORDS ? tid : 0;                        // (with several threads per word the first WORDS threads count)
-        mybase = (wd / NW) * TW + (wd % NW) * 32;
-        const uint32_t ew = es[wd].x & 0x7FFFFFFFu;
-        uint32_t up = (wd / NW) % BAND ? es[wd - NW].y : 0u;         // South bonds of the row above, within the band
-        uint32_t m = ew;                                             // OR of the run's uplinks, gathered at its head
-        up |= (up >> 1) & m;  m &= m >> 1;
-        up |= (up >> 2) & m;  m &= m >> 2;
-        up |= (up >> 4) & m;  m &= m >> 4;
-        up |= (up >> 8) & m;  m &= m >> 8;
-        up |= (up >> 16) & m;
-        o = ~(ew << 1) & ~up;
-        if (tid >= WORDS) o = 0;
-        const int nl = warp_sum_i(__popc(o));
-        if (lane == 0) atomicAdd(&s_nlab, nl);
-    }
-    __syncthreads();
-
-    // ---- phase 3b: flatten ---------------------------------------------------------------------------
-    // The scan gave every site of a run the run's label = a root at that time; the only nodes that ever were
-    // roots are the heads of runs with no bond from the row above ("label nodes", ~0.2 per site at T_c), and
-    // the only ones that no longer are were hooked (~0.03 per site): each of those is pointed at its root and hands
-    // it its count, so that afterwards root(site) = parent(parent(site)) for every site, without a loop, and a
-    // root's count is the size of its tile-local cluster.  The label nodes themselves are only COUNTED (bit tricks
-    // on the bond words): roots = label nodes - hooked nodes.
-    {
-        const int nh = s_nhook;                                      // (complete: the barrier above)
-        if (nh <= HKCAP) {
-            for (int j = tid; j < nh; j += THREADS) sc_flatten(par_s, hkitems[j]);
-        } else {                                                     // more hooks than the list holds: visit every label node
-            while (o) {
-                const int n = mybase + __ffs(o) - 1;
-                o &= o - 1;
-                if ((int)lds_u16(par_s + 4u * n + 2u) != n) sc_flatten(par_s, n);
-            }
-        }
-    }
-    __syncthreads();
-
-    // ---- phase 4: the root of every site -> 16-bit tile-local label; the largest count of the tile ---------
-    constexpr int QSTEPS = SITES / 4 / THREADS;                      // = 8
-    constexpr int LOG_TW = ilog2_c(TW);
-    static_assert((1 << LOG_TW) == TW, "tile width is a power of two");
-    const int tilebase = y0 * L + x0;
-    {
-        // the tile-local 16-bit root of every site is all the sweep stores per site (2 B); the int32 labels
-        // of the C ABI are derived from it on demand (k_labels16)
-        uint16_t* out = lab16 + (size_t)blockIdx.y * N + (size_t)(y0 + ((4 * tid) >> LOG_TW)) * L + x0 + ((4 * tid) & (TW - 1));
-        const size_t step = (size_t)(4 * THREADS / TW) * L;          // rows a step of the CTA covers
-        uint32_t mx = 0;
-#pragma unroll
-        for (int k = 0; k < QSTEPS; ++k) {
-            const uint4 v = lds_u128(par_s + 16u * (k * THREADS + tid));
-            // site -> its label node -> root (label nodes are flat)
-            const uint32_t r0 = lds_u16(par_s + 4u * (v.x >> 16) + 2u), r1 = lds_u16(par_s + 4u * (v.y >> 16) + 2u),
-                           r2 = lds_u16(par_s + 4u * (v.z >> 16) + 2u), r3 = lds_u16(par_s + 4u * (v.w >> 16) + 2u);
-            *reinterpret_cast<uint2*>(out + k * step) = make_uint2(r0 | (r1 << 16), r2 | (r3 << 16));
-            // counts sit at label nodes only (0 elsewhere); a root holds its cluster's size, a hooked node a part of
-            // one: the maximum over all words is the largest tile-local cluster (a piece of a cluster that spans
-            // tiles may enter: its total, which k_flip16 maximises, is no smaller)
-            mx = max(max(mx, v.x & CNT16), max(v.y & CNT16, max(v.z & CNT16, v.w & CNT16)));
-        }
-        mx = (uint32_t)warp_max_i((int)mx);
-        if (lane == 0) atomicMax(&s_max, (int)mx);
-    }
-    __syncthreads();
-
-    // ---- phase 5: a root with a bond across the tile edge becomes a node of the global union-find --------
-    // (order of the border sites: North row, South row, West column, East column).  The first border site to
-    // reach a root claims it: slot in the tile's list, node, and the slot in place of the count in the root's word.
-    // Dense node arrays of CAP entries per tile (L2-resident at L = 16384) instead of the N-entry label array.
-    {
-        const int nodebase = blockIdx.x * CAP;                       // node ids are local to the lattice
-        const size_t lb = (size_t)blockIdx.y * gridDim.x * CAP;
-        int4* mynodes = nodes + lb + nodebase;
-        for (int j = tid; j < 2 * (TW + TH); j += THREADS) {
-            int site; bool open;
-            if (j < TW)               { site = j;                              open = (nIn[j >> 5] >> (j & 31)) & 1u; }
-            else if (j < 2 * TW)      { const int c = j - TW; site = (TH - 1) * TW + c;
-                                        open = (es[(TH - 1) * NW + (c >> 5)].y >> (c & 31)) & 1u; }
-            else if (j < 2 * TW + TH) { const int r = j - 2 * TW; site = r * TW; open = (wIn[r >> 5] >> (r & 31)) & 1u; }
-            else                      { const int r = j - 2 * TW - TH; site = r * TW + TW - 1;
-                                        open = es[r * NW + NW - 1].x >> 31; }
-            if (open) {
-                const uint32_t l = lds_u16(par_s + 4u * lds_u16(par_s + 4u * site + 2u) + 2u);   // site -> label node -> root
-                const uint32_t old = atom_or_s(par_s + 4u * l, CLAIMED16);
-                if (!(old & CLAIMED16)) {
-                    const int pos = atomicAdd(&s_nopen, 1);
-                    const int cnt = (int)(old & CNT16);
-                    const int g = tilebase + (int)(l >> LOG_TW) * L + (int)(l & (TW - 1));
-                    // node = (parent: its own root, size of the cluster rooted here: so far this piece,
-                    //         minimum site index of the cluster rooted here, site index of this tile root)
-                    mynodes[pos] = make_int4(nodebase + pos, cnt, g, g);
-                    red_add_s(par_s + 4u * l, (uint32_t)(pos - cnt));     // the root's word now carries its slot
-                }
-            }
-        }
-    }
-    __syncthreads();
-    if (tid == 0) {
-        ocount[(size_t)blockIdx.y * gridDim.x + blockIdx.x] = s_nopen;
-        Rec* rc = rec + (size_t)ctl->slot * nb + blockIdx.y;
-        const int nclosed = s_nlab - s_nhook - s_nopen;              // roots = label nodes - hooked nodes; closed = not claimed
-        if (s_max) atomic_max_ll(&rc->maxcl, s_max);
-        if (nclosed) atomic_add_ll(&rc->ncl, nclosed);               // a closed tile root is a cluster root
-        if (FUSE && obs_prev) {                                      // E, M of the previous sweep's configuration
-            Rec* rp = rec + (size_t)(ctl->slot == 0 ? ctl->cap - 1 : ctl->slot - 1) * nb + blockIdx.y;
-            if (s_obs[0]) atomic_add_ll(&rp->E, s_obs[0]);
-            if (s_obs[1]) atomic_add_ll(&rp->M, s_obs[1]);
-        }
-    }
-
-    // ---- phase 6: slot of the root of every border site with a bond across the tile edge ----------------
-    // (what k_merge_nodes reads instead of label[])
-    {
-        uint16_t* myb = bslot + ((size_t)blockIdx.y * gridDim.x + blockIdx.x) * CAP;
-        for (int j = tid; j < 2 * (TW + TH); j += THREADS) {
-            int site; bool open;
-            if (j < TW)               { site = j;                              open = (nIn[j >> 5] >> (j & 31)) & 1u; }
-            else if (j < 2 * TW)      { const int c = j - TW; site = (TH - 1) * TW + c;
-                                        open = (es[(TH - 1) * NW + (c >> 5)].y >> (c & 31)) & 1u; }
-            else if (j < 2 * TW + TH) { const int r = j - 2 * TW; site = r * TW; open = (wIn[r >> 5] >> (r & 31)) & 1u; }
-            else                      { const int r = j - 2 * TW - TH; site = r * TW + TW - 1;
-                                        open = es[r * NW + NW - 1].x >> 31; }
-            uint32_t slot = 0xFFFFu;
-            if (open) {
-                const uint32_t l = lds_u16(par_s + 4u * lds_u16(par_s + 4u * site + 2u) + 2u);
-                slot = lds_u32(par_s + 4u * l) & CNT16;
-            }
-            myb[j] = (uint16_t)slot;
-        }
-    }
+#define BL_LDSPIN(p, i) (p)[i]
+#define BL_T ctl->t
+#define BL_SLOT ctl->slot
+#define BL_CAP ctl->cap
+#include "sw_bond_label_body.inc"
+#undef BL_LDSPIN
+#undef BL_T
+#undef BL_SLOT
+#undef BL_CAP
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -537,13 +168,16 @@ k_bond_label(const uint32_t* __restrict__ sbits, uint32_t* bondE, uint32_t* bond
 // ---------------------------------------------------------------------------------------------------
 // union-find on the node array: the parent is field x of the node.  Walks go through L1 (a stale line shows an
 // older parent = still an ancestor); the atomicMin in L2 decides whether a node still is a root.
+// (CG -- k_sweeps_cluster, where the node array is rewritten sweep after sweep inside one kernel: every walk goes to L2)
+template <bool CG = false>
 __device__ __forceinline__ int nd_find(const int4* nodes, int x) {
-    int p = ld_ca(&nodes[x].x);
-    while (p != x) { x = p; p = ld_ca(&nodes[x].x); }
+    int p = CG ? ld_cg(&nodes[x].x) : ld_ca(&nodes[x].x);
+    while (p != x) { x = p; p = CG ? ld_cg(&nodes[x].x) : ld_ca(&nodes[x].x); }
     return x;
 }
+template <bool CG = false>
 __device__ __forceinline__ void nd_union(int4* nodes, int a, int b) {
-    a = nd_find(nodes, a); b = nd_find(nodes, b);
+    a = nd_find<CG>(nodes, a); b = nd_find<CG>(nodes, b);
     while (a != b) {
         if (a < b) { const int s = a; a = b; b = s; }      // a is the larger
         const int old = atomicMin(&nodes[a].x, b);
@@ -581,16 +215,12 @@ k_merge_nodes(int4* nodes, const uint16_t* __restrict__ bslot, int tilesX, int t
 // this kernel's time; combining none is fastest on the young lattice of the bench, 1.270 ms per sweep, but loses on
 // the equilibrated one: 1.367 ms at sweeps 200-249 against 1.314 for this version and 1.320 for combining all.)  wpt warps per tile (1 for large lattices; 4 for small ones, where the kernel is
 // the latency of one warp walking its tile's ~100 pieces 32 at a time): warp `sub` takes rounds sub, sub + wpt, ...
-template <int CAP>
-__global__ void __launch_bounds__(256)
-k_roots_nodes(int4* nodes, const int* __restrict__ ocount, int tiles, int wpt) {
-    pdl_wait();
-    const int gw = blockIdx.x * 8 + (threadIdx.x >> 5);
-    const int tile = gw / wpt, sub = gw - tile * wpt;
-    const int lane = threadIdx.x & 31;
-    if (tile >= tiles) return;                              // (warp-uniform)
-    int4* nd = nodes + (size_t)blockIdx.y * tiles * CAP;
-    const int n = ocount[(size_t)blockIdx.y * tiles + tile];
+__device__ __forceinline__ int4 ld_cg_int4(const int4* p) {
+    int4 v; asm volatile("ld.global.cg.v4.s32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p) : "memory"); return v;
+}
+// one warp: the pieces sub * 32 .., (sub + wpt) * 32 .. of `tile` (n of them) on the lattice's node array nd
+template <int CAP, bool CG>
+__device__ __forceinline__ void roots_warp(int4* nd, const int n, const int tile, const int sub, const int wpt, const int lane) {
     int hot = -1, hotacc = 0, hotmin = 0x7fffffff;
     for (int e0 = 32 * sub; e0 < n; e0 += 32 * wpt) {
         const int e = e0 + lane;
@@ -598,10 +228,10 @@ k_roots_nodes(int4* nodes, const int* __restrict__ ocount, int tiles, int wpt) {
         int root = -1 - lane, add = 0, g = 0x7fffffff;      // idle lanes: distinct keys, nothing to add
         if (on) {
             const int id = tile * CAP + e;
-            const int4 me = nd[id];
+            const int4 me = CG ? ld_cg_int4(nd + id) : nd[id];
             root = me.x;
             if (root != id) {                               // hooked: (no root changes during this kernel)
-                root = nd_find(nd, root);
+                root = nd_find<CG>(nd, root);
                 if (root != me.x) nd[id].x = root;          // only ever an ancestor: safe while others walk
                 add = me.y;                                 // a root's own piece is already in its size / min
             }
@@ -630,6 +260,15 @@ k_roots_nodes(int4* nodes, const int* __restrict__ ocount, int tiles, int wpt) {
     hotacc = warp_sum_i(hotacc);
     hotmin = __reduce_min_sync(0xffffffffu, hotmin);
     if (lane == 0 && hotacc) { atomicAdd(&nd[hot].y, hotacc); atomicMin(&nd[hot].z, hotmin); }
+}
+template <int CAP>
+__global__ void __launch_bounds__(256)
+k_roots_nodes(int4* nodes, const int* __restrict__ ocount, int tiles, int wpt) {
+    pdl_wait();
+    const int gw = blockIdx.x * 8 + (threadIdx.x >> 5);
+    const int tile = gw / wpt, sub = gw - tile * wpt;
+    if (tile >= tiles) return;                              // (warp-uniform)
+    roots_warp<CAP, false>(nodes + (size_t)blockIdx.y * tiles * CAP, ocount[(size_t)blockIdx.y * tiles + tile], tile, sub, wpt, threadIdx.x & 31);
 }
 
 // a4 on demand (sw_labels; every sweep with sw_set_eager_labels): flat int32 labels from the 16-bit tile-local

@@ -625,6 +625,7 @@ def test_many_sweeps_per_call_with_and_without_graphs(B, L, path, n):
     for graphs in (True, False):
         sw = B.SwendsenWang(L, T, seed, path=path)
         sw.set_graphs(graphs)
+        B.sw_set_cluster(sw.h, False)                # (L = 64, 128 would otherwise run the whole call inside k_sweeps_cluster)
         sw.sweep(n)
         assert np.array_equal(sw.series()[:, 0, :], ser_ref), f"series differ (graphs={graphs})"
         assert np.array_equal(sw.spins_host()[0], s_ref)
@@ -635,6 +636,38 @@ def test_many_sweeps_per_call_with_and_without_graphs(B, L, path, n):
         assert np.array_equal(sw.series()[:, 0, :], ser2)
         assert np.array_equal(sw.labels_host()[0], oracle.sweep(L, T, seed, n + 4, oracle.run(L, T, seed, 4, spins=s_ref, t0=n)[0])[3])
         sw.close()
+
+
+# lattices of at most 8 tiles: the whole call inside one kernel, a thread-block cluster per lattice (sw_cluster.cuh, default)
+# against the kernels of the fast path one by one (sw_set_cluster(h, 0)); the oracle decides which is right
+@pytest.mark.parametrize("L,nb,cap", [(64, 1, None), (128, 1, None), (128, 3, 16), (64, 5, 7), (128, 8, None)])
+def test_cluster_kernel_and_separate_kernels_agree(B, L, nb, cap):
+    Ts = [1.8 + 0.25 * b for b in range(nb)]
+    seeds = [500 + L + b for b in range(nb)]
+    a, k = B.SwendsenWang(L, Ts, seeds), B.SwendsenWang(L, Ts, seeds)
+    B.sw_set_cluster(k.h, False)
+    if cap:
+        B.sw_set_series_capacity(a.h, cap); B.sw_set_series_capacity(k.h, cap)      # the ring wraps inside the kernel
+    s = [oracle.init_random(L, sd) for sd in seeds]
+    t = 0
+    for n in (1, 2, 37, 5, 1):
+        a.sweep(n); k.sweep(n)
+        for b in range(nb):
+            for _ in range(n):
+                s[b], bE, bS, lab, obs = oracle.sweep(L, Ts[b], seeds[b], t + _, s[b])
+            assert np.array_equal(a.spins_host()[b], s[b]) and np.array_equal(a.labels_host()[b], lab), (n, b)
+            assert _obs_tuple(a.observables()[b]) == obs
+        t += n
+        assert np.array_equal(a.spins_host(), k.spins_host()) and np.array_equal(a.labels_host(), k.labels_host())
+        ga, gk = a.bonds_host(), k.bonds_host()
+        assert np.array_equal(ga[0], gk[0]) and np.array_equal(ga[1], gk[1])
+        assert np.array_equal(a.series(), k.series())
+        ma, mk = a.moments(), k.moments()
+        for b in range(nb):
+            assert _obs_tuple(a.observables()[b]) == _obs_tuple(k.observables()[b])
+            assert ma[b] == mk[b] and ma[b]["n"] == t                 # (dicts of the nine fields: the same sums in the same order)
+    assert a.sweep_index == k.sweep_index == t
+    a.close(); k.close()
 
 
 # ------------------------------------------------------------------------------------------------
