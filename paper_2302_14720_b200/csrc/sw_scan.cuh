@@ -8,7 +8,7 @@
 //                bit-planes; E, M of the previous sweep's configuration from the same equal-pair masks; the bonds that enter
 //                the tile from its North and West neighbours are recomputed (TW/2 + TH extra calls)
 //       phase 2  scan-line labelling, lane = column, the block's rows in sequence, uniform control flow: runs of East bonds
-//                from bit tricks on the row's bond word; a run takes the label of the first of its sites that has a South
+//                from bit tricks on the row's bond word; a run takes the label of the last of its sites that has a South
 //                bond from the row above (one shuffle), or opens a new label (its head's index); where another site of the
 //                run is bonded to a different label above, the lane notes the row in a bit mask; after the block every lane
 //                unites the pairs of its column (atomicMin hooking; hooked nodes go into a tile-wide list)
