@@ -101,6 +101,16 @@ def test_tiled_path_every_sweep(B, L, path):
         _compare_sweeps(B, L, T, seed + L, 6, path=path)
 
 
+# the bond threshold at its ends: T = 1e11 -> threshold 0 (no bond at all), T = 1e9 -> 8, T = 0.01 -> 2^32 - 1 (the draw bits
+# come out of the carry of word + (2^32 - threshold), k_bond_label); both tile shapes, the cluster kernel and the generic path
+@pytest.mark.parametrize("L,path", [(64, 0), (128, 0), (256, 0), (2048, 0), (20, 1)])
+def test_bond_threshold_at_its_ends(B, L, path):
+    for T in (1e11, 1e9, 0.01):
+        assert oracle.threshold(T) == {1e11: 0, 1e9: 8, 0.01: 2 ** 32 - 1}[T]
+        _compare_sweeps(B, L, T, 40 + L, 2, path=path)
+        _compare_sweeps(B, L, T, 41 + L, 2, path=path, start=np.ones(L * L, dtype=np.int8))
+
+
 def test_config1_L64_many_sweeps(B):
     # BASELINE configs[0]: L = 64, T = 2.26919, seed 2024 -- every one of the 1000 sweeps, in full
     _compare_sweeps(B, 64, wl.T_C_PRINTED, 2024, 1000)
