@@ -2,7 +2,7 @@
 //
 // Stage map; one CTA per tile of TW x TH sites, TW = 32 * NW; the tile is NW x TH / BAND blocks of
 // 32 x BAND sites, one warp each (BAND = 32: one thread per 32-site word; BAND = 8: four threads per word -- small lattices).
-//   a1+a2 k_bond_label<NW, TH, FUSE, POTTS, BAND>
+//   a1+a2 k_bond_label<NW, TH, FUSE, POTTS, BAND>   (body: sw_bond_label_body.inc, shared with k_sweeps_cluster, sw_cluster.cuh)
 //       phase 1  per 32-site word: the word's spins from the BIT-PACKED plane (FUSE; bit 1 = +1; the int8 plane is derived
 //                on demand, sw_spins), 16 Philox4x32-10 calls, bond words to shared memory and to the canonical global
 //                bit-planes; E, M of the previous sweep's configuration from the same equal-pair masks; the bonds that enter
@@ -10,8 +10,9 @@
 //       phase 2  scan-line labelling, lane = column, the block's rows in sequence, uniform control flow: runs of East bonds
 //                from bit tricks on the row's bond word; a run takes the label of the last of its sites that has a South
 //                bond from the row above (one shuffle), or opens a new label (its head's index); where another site of the
-//                run is bonded to a different label above, the lane notes the row in a bit mask; after the block every lane
-//                unites the pairs of its column (atomicMin hooking; hooked nodes go into a tile-wide list)
+//                run is bonded to a different label above, the lane notes the row in a bit mask; after the block the masks
+//                become one list (prefix sum; it lives in the unused count fields of the block's own words) and the warp
+//                unites the pairs 32 at a time (atomicMin hooking; hooked nodes go into a tile-wide list)
 //       phase 3  seams between blocks (East bonds across strips, South bonds across band seams); every site counted at its label
 //       phase 3b the label nodes (heads of runs with no bond from above) are counted; the hooked ones point at their roots and
 //                hand them their counts
@@ -44,9 +45,10 @@ __host__ __device__ constexpr int ilog2_c(int v) { return v <= 1 ? 0 : 1 + ilog2
 // ---- the shared parent array of k_bond_label -------------------------------------------------------------
 // One 32-bit word per site of the tile:
 //   bits 16 .. 29  parent (tile-local index); a root points at itself
-//   bits  0 .. 13  sites counted at this node: every run adds its length to the label it takes (phase 2); the
-//                  flatten (phase 3b) moves the counts of the nodes that were hooked to their roots, so that a
-//                  root ends up with the size of its tile-local cluster
+//   bits  0 .. 13  sites counted at this node: 0 from the scan's store, then every site is counted at its label (phase 3);
+//                  the flatten (phase 3b) moves the counts of the nodes that were hooked to their roots, so that a
+//                  root ends up with the size of its tile-local cluster.  (Between the scan of a block and its unions the
+//                  fields of the block's first words hold the warp's list of meetings.)
 //   bit  14        CLAIMED (roots with a bond across the tile edge, phase 5): the low 14 bits now hold the root's
 //                  slot in the tile's node list instead of the count
 // The parent sits in the HIGH half so that hooking "larger under smaller" stays one atomicMin on the whole
