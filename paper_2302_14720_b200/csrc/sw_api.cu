@@ -312,7 +312,7 @@ int launch_bond_label_scan(sw_handle* h, bool fused, bool obs_prev) {
     const size_t nedge = (size_t)h->L * (h->L / TW + h->L / TH);
     SW_MARK(h, K_MERGE);
     SW_CUDA(launch_pdl(k_merge_nodes<TW, TH>, grid1(nedge, 256, h->nb), dim3(256), 0, h->stream,
-        h->nodes, h->bslot, h->L / TW, h->L / TH));
+        h->nodes, h->bslot, h->L / TW, h->L / TH, make_div(h->L / TW)));
     SW_MARK(h, K_SIZES);
     const int wpt = roots_warps_per_tile(h, tiles);
     SW_CUDA(launch_pdl(k_roots_nodes<CAP>, grid1((size_t)tiles * wpt * 32, 256, h->nb), dim3(256), 0, h->stream,
@@ -502,7 +502,7 @@ int launch_bond_label_potts(sw_handle* h, bool obs_prev) {
         h->series, h->lat, h->ctl, h->L, h->N, h->words, h->nb, obs_prev ? 1 : 0);
     const size_t nedge = (size_t)h->L * (h->L / TW + h->L / TH);
     SW_MARK(h, K_MERGE);
-    k_merge_nodes<TW, TH><<<grid1(nedge, 256, h->nb), 256, 0, h->stream>>>(h->nodes, h->bslot, h->L / TW, h->L / TH);
+    k_merge_nodes<TW, TH><<<grid1(nedge, 256, h->nb), 256, 0, h->stream>>>(h->nodes, h->bslot, h->L / TW, h->L / TH, make_div(h->L / TW));
     SW_MARK(h, K_SIZES);
     const int wpt = roots_warps_per_tile(h, tiles);
     k_roots_nodes<CAP><<<grid1((size_t)tiles * wpt * 32, 256, h->nb), 256, 0, h->stream>>>(h->nodes, h->ocount, tiles, wpt);

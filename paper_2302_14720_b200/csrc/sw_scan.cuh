@@ -199,7 +199,7 @@ __device__ __forceinline__ void nd_union(int4* nodes, int a, int b) {
 
 template <int TW, int TH>
 __global__ void __launch_bounds__(256)
-k_merge_nodes(int4* nodes, const uint16_t* __restrict__ bslot, int tilesX, int tilesY) {
+k_merge_nodes(int4* nodes, const uint16_t* __restrict__ bslot, int tilesX, int tilesY, DivL dx) {   // dx: division by tilesX
     pdl_wait();
     constexpr int CAP = 2 * (TW + TH), PER = TW + TH;       // per tile: TW South-row sites, TH East-column sites
     const int idx = blockIdx.x * 256 + threadIdx.x;
@@ -208,13 +208,23 @@ k_merge_nodes(int4* nodes, const uint16_t* __restrict__ bslot, int tilesX, int t
     const size_t lb = (size_t)blockIdx.y * tiles * CAP;
     const uint16_t* bs = bslot + lb;
     const int ta = idx / PER, j = idx - ta * PER;
-    const int r = ta / tilesX, c = ta - r * tilesX;
+    const int r = div_l(ta, dx), c = ta - r * tilesX;
     int ka, tb, kb;
     if (j < TW) { ka = TW + j;                tb = (r + 1 == tilesY ? 0 : r + 1) * tilesX + c; kb = j; }            // South row -> North row below
     else        { ka = 2 * TW + TH + (j - TW); tb = r * tilesX + (c + 1 == tilesX ? 0 : c + 1); kb = 2 * TW + (j - TW); }  // East column -> West column
     const int sa = bs[(size_t)ta * CAP + ka], sb = bs[(size_t)tb * CAP + kb];   // (both loads in flight before the test)
     if (sa == 0xFFFF) return;                               // no bond across the edge here
-    nd_union(nodes + lb, ta * CAP + sa, tb * CAP + sb);
+    int4* nd = nodes + lb;
+    int a = ta * CAP + sa, b = tb * CAP + sb;
+    int pa = ld_ca(&nd[a].x), pb = ld_ca(&nd[b].x);         // the first hops of both walks in flight together
+    while (pa != a) { a = pa; pa = ld_ca(&nd[a].x); }
+    while (pb != b) { b = pb; pb = ld_ca(&nd[b].x); }
+    while (a != b) {
+        if (a < b) { const int s = a; a = b; b = s; }      // a is the larger
+        const int old = atomicMin(&nd[a].x, b);
+        if (old == a) break;
+        a = old;
+    }
 }
 
 // After the merge: every open piece adds its size and its site index to the node it hangs under (sum -> cluster
