@@ -191,10 +191,13 @@ k_flip16_tma(const __grid_constant__ CUtensorMap tm_lab, const __grid_constant__
             const uint4 v = lds_u128(base + 2u * l);                       // (the box is row-major: site l at byte 2 l)
             const uint32_t w4[4] = { v.x, v.y, v.z, v.w };
             uint32_t b8 = 0;                                               // bit u: site l + u goes up
+            uint32_t pr = 0xFFFFFFFFu, pb = 0;                             // (a site often has its left neighbour's root: no second lookup)
 #pragma unroll
             for (int u = 0; u < 8; ++u) {
                 const uint32_t r = (u & 1) ? (w4[u >> 1] >> 16) : (w4[u >> 1] & 0xFFFFu);
-                b8 += lds_u8(dc_s + r) << u;
+                if (r != pr) pb = lds_u8(dc_s + r);
+                pr = r;
+                b8 += pb << u;
             }
             const size_t gsite = (size_t)blockIdx.y * N + (size_t)(y0 + (l >> LOG_TW)) * L + x0 + (l & (TW - 1));
             reinterpret_cast<uint8_t*>(sbits)[gsite >> 3] = (uint8_t)b8;
