@@ -680,6 +680,30 @@ def test_cluster_kernel_and_separate_kernels_agree(B, L, nb, cap):
     a.close(); k.close()
 
 
+def test_cluster_kernels_of_two_handles_on_two_streams(B):
+    """Two lattices, each swept by its own cluster kernel on its own stream, launched back to back with no synchronisation in
+    between: nothing is shared between handles, so both must land where the oracle does."""
+    import torch
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    with torch.cuda.stream(s1):
+        a = B.SwendsenWang(128, T_C, 71)
+    with torch.cuda.stream(s2):
+        b = B.SwendsenWang(64, 2.0, 72)
+    for n in (30, 1, 12):
+        with torch.cuda.stream(s1):
+            a.use_current_stream(); a.sweep(n)
+        with torch.cuda.stream(s2):
+            b.use_current_stream(); b.sweep(n)
+    torch.cuda.synchronize()
+    sa, sera = oracle.run(128, T_C, 71, 43)
+    sb, serb = oracle.run(64, 2.0, 72, 43)
+    assert np.array_equal(a.spins_host()[0], sa) and np.array_equal(b.spins_host()[0], sb)
+    assert _obs_tuple(a.observables()[0]) == tuple(int(v) for v in sera[-1])
+    assert _obs_tuple(b.observables()[0]) == tuple(int(v) for v in serb[-1])
+    assert np.array_equal(a.series()[:, 0, :], sera[-12:]) and np.array_equal(b.series()[:, 0, :], serb[-12:])
+    a.close(); b.close()
+
+
 # ------------------------------------------------------------------------------------------------
 # SURVEY.md 8(f) NEXT-2: the paper's own labelling (PAPER.md:49-53) as path 11.  Labels are the same canonical
 # minimum-index labels (bit-exact with the definition), and the number of passes is a deterministic function of
