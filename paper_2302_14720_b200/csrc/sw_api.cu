@@ -292,7 +292,7 @@ template <int NW, int TH, int BAND_T = 32>
 int launch_bond_label_scan(sw_handle* h, bool fused, bool obs_prev) {
     constexpr int TW = 32 * NW, CAP = 2 * (TW + TH), THREADS = NW * TH * (32 / BAND_T);
     const int tiles = h->N / (TW * TH);
-    constexpr size_t smem = (size_t)TW * TH * sizeof(uint32_t);      // the parent array (dynamic: 32 KB at 128 x 64)
+    constexpr size_t smem = bond_label_smem(TW * TH);                 // the parent array + the list of hooked nodes (dynamic: 34 KB at 128 x 64)
     static bool done[2][MAX_DEV];
     { int rc = opt_in_smem(k_bond_label<NW, TH, true, false, BAND_T>, smem, done[0], h->dev); if (rc) return rc; }
     { int rc = opt_in_smem(k_bond_label<NW, TH, false, false, BAND_T>, smem, done[1], h->dev); if (rc) return rc; }
@@ -493,7 +493,7 @@ bool potts_folded(const sw_handle* h) { return h->q && h->q <= 8 && h->tile == S
 int launch_bond_label_potts(sw_handle* h, bool obs_prev) {
     constexpr int NW = 4, TH = 64, TW = 32 * NW, CAP = 2 * (TW + TH);
     const int tiles = h->N / (TW * TH);
-    constexpr size_t smem = (size_t)TW * TH * sizeof(uint32_t);
+    constexpr size_t smem = bond_label_smem(TW * TH);
     static bool done[MAX_DEV];
     { int rc = opt_in_smem(k_bond_label<NW, TH, true, true>, smem, done, h->dev); if (rc) return rc; }
     SW_MARK(h, K_BONDLABEL);
@@ -572,7 +572,7 @@ int cluster_tiles(const sw_handle* h) {
 template <int NW, int TH, int BAND_T>
 cudaError_t launch_sweeps_cluster(sw_handle* h, int64_t n, int tiles) {
     constexpr int THREADS = NW * TH * (32 / BAND_T);
-    constexpr size_t smem = (size_t)32 * NW * TH * sizeof(uint32_t);
+    constexpr size_t smem = bond_label_smem(32 * NW * TH);
     static bool done[MAX_DEV];
     if (opt_in_smem(k_sweeps_cluster<NW, TH, BAND_T>, smem, done, h->dev)) return cudaErrorUnknown;
     cudaLaunchConfig_t cfg = {};

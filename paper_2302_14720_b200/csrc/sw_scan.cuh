@@ -109,6 +109,10 @@ __device__ __forceinline__ uint32_t atom_add_s(uint32_t a, uint32_t v) {
 // the tile's list of hooked nodes (phase 3b flattens from it with all threads); the counter runs on past the capacity
 // (it also gives the number of roots), and phase 3b then visits every label node instead
 struct HookList { uint32_t items_s, count_s; int cap; uint32_t one; };     // (shared-window addresses; one = 1)
+// The list and its counter sit behind the parent array in the kernel's DYNAMIC shared memory, so that their addresses are
+// the parent array's (kept in a register) plus a constant.  Bytes of dynamic shared memory k_bond_label needs:
+constexpr int BL_HKCAP = 1024;                  // hooked nodes a tile can list (~250 at T_c)
+__host__ __device__ constexpr size_t bond_label_smem(int sites) { return (size_t)sites * 4 + (size_t)BL_HKCAP * 2 + 16; }
 __device__ __forceinline__ void hooked(const HookList& hk, int node) {
     if (node == NO_NODE) return;
     // (the increment is a 1 that ptxas cannot prove to be one -- `one` comes from a kernel argument: it would otherwise
